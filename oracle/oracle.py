@@ -1,0 +1,134 @@
+"""ctypes binding of the CPU oracle (oracle/tpc_oracle.cpp).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs.  The product (paper_1905_05515_b200) never imports this module.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtpc_oracle.so")
+_SRC = os.path.join(_HERE, "tpc_oracle.cpp")
+_KINDS = {0: (C.c_int32, np.int32), 1: (C.c_int64, np.int64), 2: (C.c_double, np.float64), 3: (C.c_float, np.float32)}
+
+STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6}
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off: every fp32 product is rounded before it is added (no FMA)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", _SRC, "-o", _SO])
+    return _SO
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        lib.orc_create.restype = C.c_void_p
+        lib.orc_create.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float)] + [C.c_double] * 7
+        lib.orc_destroy.argtypes = [C.c_void_p]
+        lib.orc_set_param.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
+        lib.orc_load.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        lib.orc_run.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        lib.orc_get.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_void_p), C.POINTER(C.c_int64), C.POINTER(C.c_int)]
+        lib.orc_propagate.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
+        lib.orc_update.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, C.c_double,
+                                   C.POINTER(C.c_double)]
+        lib.orc_set_tracklets.argtypes = [C.c_void_p, C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                          C.POINTER(C.c_double), C.POINTER(C.c_int32)]
+        _lib = lib
+    return _lib
+
+
+def _fp(a, ct):
+    return a.ctypes.data_as(C.POINTER(ct))
+
+
+class Oracle:
+    """One oracle context.  `double=False` is the fp32 parity reference, `double=True` the fp64 pin instance."""
+
+    def __init__(self, n_sectors, n_rows, row_x, sector_dphi, z_max, t_frame, sigma_y, sigma_z, bz, vdrift,
+                 double=False, **params):
+        self.lib = _load()
+        self.n_sectors, self.n_rows = int(n_sectors), int(n_rows)
+        self.row_x = np.ascontiguousarray(row_x, dtype=np.float32)
+        self.h = self.lib.orc_create(int(double), self.n_sectors, self.n_rows, _fp(self.row_x, C.c_float),
+                                     float(sector_dphi), float(z_max), float(t_frame), float(sigma_y), float(sigma_z),
+                                     float(bz), float(vdrift))
+        for k, v in params.items():
+            self.set_param(k, v)
+
+    @classmethod
+    def for_workload(cls, w, double=False, **params):
+        o = cls(double=double, **w.geometry(), **params)
+        o.load(w.unit_off, w.y, w.t)
+        return o
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.orc_destroy(self.h)
+            self.h = None
+
+    def set_param(self, name, value):
+        if self.lib.orc_set_param(self.h, name.encode(), float(value)) != 0:
+            raise KeyError(name)
+
+    def load(self, unit_off, y, t):
+        self.unit_off = np.ascontiguousarray(unit_off, dtype=np.int64)
+        y = np.ascontiguousarray(y, dtype=np.float32)
+        t = np.ascontiguousarray(t, dtype=np.float32)
+        assert self.unit_off.shape[0] == self.n_sectors * self.n_rows + 1 and y.shape[0] == self.unit_off[-1] == t.shape[0]
+        self.lib.orc_load(self.h, _fp(self.unit_off, C.c_int64), _fp(y, C.c_float), _fp(t, C.c_float))
+
+    def run(self, upto="s6", brute_links=False, brute_pickup=False):
+        self.lib.orc_run(self.h, STAGES[upto], int(brute_links) | (int(brute_pickup) << 1))
+        return self
+
+    def get(self, name):
+        p, n, k = C.c_void_p(), C.c_int64(), C.c_int()
+        if self.lib.orc_get(self.h, name.encode(), C.byref(p), C.byref(n), C.byref(k)) != 0:
+            raise KeyError(name)
+        ct, dt = _KINDS[k.value]
+        if n.value == 0:
+            return np.zeros(0, dtype=dt)
+        return np.ctypeslib.as_array(C.cast(p, C.POINTER(ct)), shape=(n.value,)).copy()
+
+    # ---- single-step entry points for the closed-form pins ----
+    def propagate(self, par, cov, dx):
+        par = np.array(par, dtype=np.float64); cov = np.array(cov, dtype=np.float64)
+        rc = self.lib.orc_propagate(self.h, _fp(par, C.c_double), _fp(cov, C.c_double), float(dx))
+        return rc == 0, par, cov
+
+    def update(self, par, cov, ym, zm):
+        par = np.array(par, dtype=np.float64); cov = np.array(cov, dtype=np.float64); chi2 = C.c_double()
+        self.lib.orc_update(self.h, _fp(par, C.c_double), _fp(cov, C.c_double), float(ym), float(zm), C.byref(chi2))
+        return par, cov, chi2.value
+
+    def select(self, sector, n_hits, chi2, rowhit):
+        """S6 alone on hand-built tracklets (S1 must have run)."""
+        sector = np.ascontiguousarray(sector, dtype=np.int32); n_hits = np.ascontiguousarray(n_hits, dtype=np.int32)
+        chi2 = np.ascontiguousarray(chi2, dtype=np.float64); rowhit = np.ascontiguousarray(rowhit, dtype=np.int32)
+        assert rowhit.shape == (sector.shape[0], self.n_rows)
+        self.lib.orc_set_tracklets(self.h, sector.shape[0], _fp(sector, C.c_int32), _fp(n_hits, C.c_int32),
+                                   _fp(chi2, C.c_double), _fp(rowhit, C.c_int32))
+        return self.tracks()
+
+    def tracks(self):
+        d = {k: self.get("trk_" + k) for k in ("sector", "ndf", "tracklet", "cl_begin", "cl_row", "cl_index", "x", "par",
+                                                "cov", "chi2")}
+        d["par"] = d["par"].reshape(-1, 5); d["cov"] = d["cov"].reshape(-1, 15)
+        return d
+
+    def tracklets(self):
+        d = {k: self.get("tl_" + k) for k in ("n", "first", "last", "rowhit", "sector", "chi2", "x", "par", "cov", "zref")}
+        d["par"] = d["par"].reshape(-1, 5); d["cov"] = d["cov"].reshape(-1, 15); d["rowhit"] = d["rowhit"].reshape(-1, self.n_rows)
+        return d

@@ -1,0 +1,522 @@
+/*
+ * tpc_oracle.cpp -- plain, slow, single-threaded CPU ORACLE of the TPC sector track finding.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this file.  It shares no code with the CUDA library
+ * (paper_1905_05515_b200/csrc) and neither includes the other.
+ *
+ * What it computes: PAPER.md:27-30 (section 2: time scaled to z with the average drift velocity, all
+ * tracks assumed primary from the origin, a first preliminary fit used to find the full track) and
+ * PAPER.md:37-41 (section 3: Cellular-Automaton seeding, then single-hypothesis Kalman track following).
+ * The paper gives no formula for any step (it defers to its refs [6]-[9], not available), so every
+ * step below follows the readings listed in DESIGN.md section 4 (S0..S6, A1..A33), in that order and
+ * notation; each function names the step it implements.
+ *
+ * Two instances: Real=float (the parity reference: decisions are taken in fp32, the kernel's
+ * precision, with contraction off) and Real=double (closed-form pins).
+ * Build: g++ -O2 -ffp-contract=off -shared -fPIC oracle/tpc_oracle.cpp -o oracle/libtpc_oracle.so
+ *
+ * Pins (tests/test_oracle_*.py): S0 closed form; S1 invariants; S2 brute force O(N^2) + bin-size and
+ * permutation invariance + straight lines; S3/S4 invariants; S5 propagate vs closed-form circle,
+ * composition, round trip, Jacobian vs finite differences; S5 fit: noise-free helix recovery 1e-5,
+ * Bz=0 exact, chi2/ndf = 1 and pulls on smeared tracks; S6 hand-built sharing cases, order invariance.
+ * Absolute efficiency / resolution versus the paper: parity unpinned (PAPER.md:49 gives no number).
+ */
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <string>
+#include <vector>
+#include <algorithm>
+#include <limits>
+
+namespace {
+
+struct Tunables {            // DESIGN.md table T (all are readings; the paper is silent)
+  double wy = 1.5, wz = 1.5, dzdx_max = 1.5, wz0 = 0.75, cut2 = 1.75;
+  int min_seed = 3;
+  double c0[5] = {1.0, 2.25, 1.0, 1.0, 100.0};
+  double s_max = 0.95, n_sigma = 4.0, w_max = 3.0;
+  int max_gap = 4;
+  double edge_margin = 1.0;
+  int min_hits = 10;
+  double grid_min = 1.0, grid_max = 64.0, grid_scale = 1.0;   // S1 bin size clamp; scale is a test knob
+};
+
+struct OracleBase {
+  virtual ~OracleBase() {}
+  virtual int load(const int64_t* unit_off, const float* y, const float* t) = 0;
+  virtual int run(int upto, int brute) = 0;
+  virtual int get(const char* name, const void** p, int64_t* n, int* kind) = 0;
+  virtual int propagate(double* par, double* cov, double dx) = 0;
+  virtual int update(double* par, double* cov, double ym, double zm, double* chi2) = 0;
+  virtual int set_tracklets(int64_t n, const int32_t* sector, const int32_t* nh, const double* chi2, const int32_t* rowhit) = 0;
+  Tunables T;
+  std::string err;
+};
+
+template <class Real>
+struct Oracle : OracleBase {
+  // geometry
+  int NS, R; std::vector<float> row_x; double dphi, z_max, t_frame, sigma_y, sigma_z, bz, vdrift;
+  bool continuous;
+  // per-row constants (double -> Real once)
+  std::vector<Real> X, tu, td, ar, br, thr, wzu, wzd, yedge;
+  Real cB;
+  // clusters
+  int64_t N = 0; std::vector<int64_t> off;           // [U+1]
+  std::vector<float> in_y, in_t;
+  std::vector<Real> z;                                // S0, input order
+  // S1
+  std::vector<Real> ys, zs; std::vector<int32_t> perm; std::vector<int64_t> bin_off; std::vector<int32_t> bin_start;
+  std::vector<int32_t> g_ny, g_nz; std::vector<Real> g_ylo, g_zlo, g_invs;
+  std::vector<double> g_ylo_d, g_zlo_d, g_invs_d;
+  // S2/S3
+  std::vector<int32_t> link_up, link_dn, clean_up, clean_dn;
+  // S4
+  std::vector<int32_t> start_unit, start_pos;
+  // S5
+  std::vector<int32_t> tl_n, tl_first, tl_last, tl_rowhit, tl_sector; std::vector<double> tl_chi2, tl_x, tl_par, tl_cov, tl_zref;
+  // S6
+  std::vector<int32_t> trk_sector, trk_ndf, trk_tracklet, trk_cl_row, trk_cl_index; std::vector<int64_t> trk_cl_begin;
+  std::vector<double> trk_x, trk_par, trk_cov, trk_chi2;
+  std::vector<double> z_d, ys_d, zs_d;   // export copies
+
+  Oracle(int ns, int nr, const float* rx, double dphi_, double zmax, double tframe, double sy, double sz, double bz_, double vd)
+      : NS(ns), R(nr), row_x(rx, rx + nr), dphi(dphi_), z_max(zmax), t_frame(tframe), sigma_y(sy), sigma_z(sz), bz(bz_), vdrift(vd) {
+    continuous = t_frame > 0;
+  }
+
+  // ---- per-row constant table: formulas of DESIGN.md section 4 "per-row constants", double -> Real once ----
+  void make_tables() {
+    X.assign(R, 0); tu.assign(R, 0); td.assign(R, 0); ar.assign(R, 0); br.assign(R, 0); thr.assign(R, 0);
+    wzu.assign(R, 0); wzd.assign(R, 0); yedge.assign(R, 0);
+    for (int r = 0; r < R; r++) {
+      double x = row_x[r], xu = r + 1 < R ? row_x[r + 1] : x, xd = r > 0 ? row_x[r - 1] : x;
+      double a = xu - x, b = x - xd;
+      X[r] = (Real)x; tu[r] = (Real)(xu / x); td[r] = (Real)(xd / x); ar[r] = (Real)a; br[r] = (Real)b;
+      thr[r] = (Real)(T.cut2 * 0.5 * (a * a + b * b));
+      wzu[r] = (Real)(T.dzdx_max * a + T.wz0); wzd[r] = (Real)(T.dzdx_max * b + T.wz0);
+      yedge[r] = (Real)(x * std::tan(0.5 * dphi));
+    }
+    cB = (Real)(-0.00299792458 * bz);
+  }
+
+  int load(const int64_t* unit_off, const float* y, const float* t) override {
+    int U = NS * R; off.assign(unit_off, unit_off + U + 1); N = off[U];
+    in_y.assign(y, y + N); in_t.assign(t, t + N);
+    return 0;
+  }
+
+  // ---- S0: z = z_max - vdrift * t ("scales the time to z linearly using the average drift velocity") ----
+  void s0_time_to_z() {
+    z.resize(N);
+    const Real zm = (Real)z_max, vd = (Real)vdrift;
+    for (int64_t i = 0; i < N; i++) { Real prod = vd * (Real)in_t[i]; z[i] = zm - prod; }
+  }
+
+  // ---- S1: per (sector,row) 2-D grid, stable counting sort ----
+  static int bin_of(Real v, Real lo, Real inv, int nb) {
+    Real f = (v - lo) * inv;
+    if (!(f > (Real)0)) return 0;            // negative or NaN -> bin 0
+    if (f >= (Real)nb) return nb - 1;
+    int b = (int)f; return b > nb - 1 ? nb - 1 : b;
+  }
+  void s1_grid() {
+    int U = NS * R;
+    g_ny.assign(U, 1); g_nz.assign(U, 1); g_ylo.assign(U, 0); g_zlo.assign(U, 0); g_invs.assign(U, 1);
+    g_ylo_d.assign(U, 0); g_zlo_d.assign(U, 0); g_invs_d.assign(U, 0);
+    bin_off.assign(U + 1, 0);
+    for (int u = 0; u < U; u++) {
+      int r = u % R; int64_t n = off[u + 1] - off[u];
+      double ye = (double)row_x[r] * std::tan(0.5 * dphi);
+      double y_lo = -ye - 1.0, y_hi = ye + 1.0, z_lo = -vdrift * t_frame - 1.0, z_hi = z_max + 1.0;
+      double s = std::sqrt((y_hi - y_lo) * (z_hi - z_lo) / (double)std::max<int64_t>(n, 1)) * T.grid_scale;
+      s = std::min(std::max(s, T.grid_min), T.grid_max);
+      int ny = std::max(1, (int)std::ceil((y_hi - y_lo) / s)), nz = std::max(1, (int)std::ceil((z_hi - z_lo) / s));
+      g_ny[u] = ny; g_nz[u] = nz;
+      g_ylo[u] = (Real)(float)y_lo; g_zlo[u] = (Real)(float)z_lo; g_invs[u] = (Real)(float)(1.0 / s);
+      g_ylo_d[u] = (double)g_ylo[u]; g_zlo_d[u] = (double)g_zlo[u]; g_invs_d[u] = (double)g_invs[u];
+      bin_off[u + 1] = bin_off[u] + (int64_t)ny * nz + 1;
+    }
+    bin_start.assign(bin_off[U], 0); ys.resize(N); zs.resize(N); perm.resize(N);
+    std::vector<int32_t> b;
+    for (int u = 0; u < U; u++) {
+      int64_t o = off[u], n = off[u + 1] - o; int ny = g_ny[u], nz = g_nz[u], nb = ny * nz;
+      int32_t* bs = &bin_start[bin_off[u]];
+      b.resize(n);
+      for (int64_t i = 0; i < n; i++) {
+        int by = bin_of((Real)in_y[o + i], g_ylo[u], g_invs[u], ny), bz_ = bin_of(z[o + i], g_zlo[u], g_invs[u], nz);
+        b[i] = bz_ * ny + by; bs[b[i] + 1]++;
+      }
+      for (int k = 0; k < nb; k++) bs[k + 1] += bs[k];
+      std::vector<int32_t> cur(bs, bs + nb);
+      for (int64_t i = 0; i < n; i++) {      // ascending original index inside each bin
+        int32_t p = cur[b[i]]++; ys[o + p] = (Real)in_y[o + i]; zs[o + p] = z[o + i]; perm[o + p] = (int32_t)i;
+      }
+    }
+  }
+
+  // hits of unit u (sorted positions) inside [ylo,yhi]x[zlo,zhi] bins; brute: every hit of the unit
+  template <class F> void for_bins(int u, Real ylo, Real yhi, Real zlo, Real zhi, bool brute, F&& f) const {
+    int64_t n = off[u + 1] - off[u];
+    if (n == 0) return;
+    if (brute) { for (int32_t p = 0; p < n; p++) f(p); return; }
+    int ny = g_ny[u], nz = g_nz[u]; const int32_t* bs = &bin_start[bin_off[u]];
+    int by0 = bin_of(ylo, g_ylo[u], g_invs[u], ny), by1 = bin_of(yhi, g_ylo[u], g_invs[u], ny);
+    int bz0 = bin_of(zlo, g_zlo[u], g_invs[u], nz), bz1 = bin_of(zhi, g_zlo[u], g_invs[u], nz);
+    for (int bz_ = bz0; bz_ <= bz1; bz_++)
+      for (int32_t p = bs[bz_ * ny + by0]; p < bs[bz_ * ny + by1 + 1]; p++) f(p);
+  }
+
+  // ---- S2: neighbour finder -- best (up,down) pair by collinearity, window centred on the from-origin projection ----
+  void s2_neighbours(bool brute) {
+    link_up.assign(N, -1); link_dn.assign(N, -1);
+    const Real wy = (Real)T.wy, wz = (Real)T.wz;
+    std::vector<int32_t> cu, cd;
+    for (int sec = 0; sec < NS; sec++)
+      for (int r = 1; r <= R - 2; r++) {
+        int u = sec * R + r, uu = u + 1, ud = u - 1; int64_t o = off[u], ou = off[uu], od = off[ud], n = off[u + 1] - o;
+        for (int64_t h = 0; h < n; h++) {
+          Real y = ys[o + h], zz = zs[o + h];
+          cu.clear(); cd.clear();
+          { Real yc = y * tu[r], zc = continuous ? zz : zz * tu[r], hw = continuous ? wzu[r] : wz;
+            Real ylo = yc - wy, yhi = yc + wy, zlo = zc - hw, zhi = zc + hw;
+            for_bins(uu, ylo, yhi, zlo, zhi, brute, [&](int32_t p) {
+              Real yu = ys[ou + p], zu = zs[ou + p];
+              if (yu >= ylo && yu <= yhi && zu >= zlo && zu <= zhi) cu.push_back(p); }); }
+          if (cu.empty()) continue;
+          { Real yc = y * td[r], zc = continuous ? zz : zz * td[r], hw = continuous ? wzd[r] : wz;
+            Real ylo = yc - wy, yhi = yc + wy, zlo = zc - hw, zhi = zc + hw;
+            for_bins(ud, ylo, yhi, zlo, zhi, brute, [&](int32_t p) {
+              Real yd = ys[od + p], zd = zs[od + p];
+              if (yd >= ylo && yd <= yhi && zd >= zlo && zd <= zhi) cd.push_back(p); }); }
+          if (cd.empty()) continue;
+          bool have = false; Real bestD = 0; int32_t bu = -1, bd = -1, bpu = 0, bpd = 0;
+          for (int32_t pu : cu)
+            for (int32_t pd : cd) {
+              Real dyu = ys[ou + pu] - y, dyd = y - ys[od + pd]; Real m1 = br[r] * dyu, m2 = ar[r] * dyd; Real ey = m1 - m2;
+              Real dzu = zs[ou + pu] - zz, dzd = zz - zs[od + pd]; Real m3 = br[r] * dzu, m4 = ar[r] * dzd; Real ez = m3 - m4;
+              Real e1 = ey * ey, e2 = ez * ez; Real D = e1 + e2;
+              int32_t iu = perm[ou + pu], id = perm[od + pd];
+              if (!have || D < bestD || (D == bestD && (iu < bpu || (iu == bpu && id < bpd)))) {
+                have = true; bestD = D; bu = pu; bd = pd; bpu = iu; bpd = id; }
+            }
+          if (have && bestD < thr[r]) { link_up[o + h] = bu; link_dn[o + h] = bd; }
+        }
+      }
+  }
+
+  // ---- S3: mutual-link cleaner (double-buffered definition) ----
+  void s3_clean() {
+    clean_up.assign(N, -1); clean_dn.assign(N, -1);
+    for (int sec = 0; sec < NS; sec++)
+      for (int r = 0; r < R; r++) {
+        int u = sec * R + r; int64_t o = off[u], n = off[u + 1] - o;
+        for (int64_t h = 0; h < n; h++) {
+          int32_t up = link_up[o + h], dn = link_dn[o + h];
+          if (up >= 0 && r + 1 < R && link_dn[off[u + 1] + up] == (int32_t)h) clean_up[o + h] = up;
+          if (dn >= 0 && r > 0 && link_up[off[u - 1] + dn] == (int32_t)h) clean_dn[o + h] = dn;
+        }
+      }
+  }
+
+  // ---- S4: start hits = chain beginnings with >= min_seed hits, ascending (sector,row,sorted pos) ----
+  void s4_start_hits() {
+    start_unit.clear(); start_pos.clear();
+    for (int u = 0; u < NS * R; u++) {
+      int64_t o = off[u], n = off[u + 1] - o;
+      for (int64_t h = 0; h < n; h++) {
+        if (!(clean_dn[o + h] < 0 && clean_up[o + h] >= 0)) continue;
+        int len = 1; int uu = u; int32_t p = (int32_t)h;
+        while (len < T.min_seed) { int32_t nx = clean_up[off[uu] + p]; if (nx < 0) break; p = nx; uu++; len++; }
+        if (len >= T.min_seed) { start_unit.push_back(u); start_pos.push_back((int32_t)h); }
+      }
+    }
+  }
+
+  // ---- S5 building blocks ----
+  struct State { Real p[5]; Real C[5][5]; };
+
+  // propagate the state from its x to x+dx on the helix in uniform Bz; false = |sin(phi)| leaves [-s_max, s_max]
+  bool propagate_state(State& st, Real dx) const {
+    const Real smax = (Real)T.s_max;
+    Real y = st.p[0], zz = st.p[1], s = st.p[2], t = st.p[3], q = st.p[4];
+    Real k = cB * q;
+    Real kdx = k * dx;
+    Real s1 = s + kdx;
+    if (!(std::fabs(s) <= smax) || !(std::fabs(s1) <= smax)) return false;
+    Real c = std::sqrt((Real)1 - s * s), c1 = std::sqrt((Real)1 - s1 * s1);
+    Real cc = c + c1, ss = s + s1, tq = ss / cc;
+    Real g = (Real)1 + tq * tq;
+    Real L = dx * std::sqrt(g);
+    Real h = ((Real)0.5 * k) * L, h2 = h * h;
+    const Real hthr = sizeof(Real) == 4 ? (Real)0.25 : (Real)1e-3;
+    Real S;
+    if (std::fabs(h) < hthr) {   // asin(h)/h = 1 + h^2/6 + 3h^4/40 + 15h^6/336 + 105h^8/3456 + ...
+      Real poly = (Real)(105.0 / 3456.0);
+      poly = (Real)(15.0 / 336.0) + h2 * poly;
+      poly = (Real)(3.0 / 40.0) + h2 * poly;
+      poly = (Real)(1.0 / 6.0) + h2 * poly;
+      poly = (Real)1 + h2 * poly;
+      S = L * poly;
+    } else S = ((Real)2 / k) * std::asin(h);
+    Real dSdk;
+    const Real kthr = sizeof(Real) == 4 ? (Real)1e-2 : (Real)1e-3;
+    if (std::fabs(kdx) >= kthr) dSdk = (dx / c1 - S) / k;
+    else { Real sm = (s + (Real)2 * s1) / (Real)3; Real cm2 = (Real)1 - sm * sm; Real cm = std::sqrt(cm2);
+      dSdk = ((dx * dx) * sm) / ((Real)2 * (cm2 * cm)); }
+    Real cc1 = c * c1;
+    Real F[5][5]; for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) F[i][j] = i == j ? (Real)1 : (Real)0;
+    F[0][2] = ((dx * g) * cc) / ((Real)2 * cc1);
+    F[0][4] = (((dx * dx) * cB) * g) / ((Real)2 * c1);
+    F[1][2] = ((t * dx) * tq) / cc1;
+    F[1][3] = S;
+    F[1][4] = (t * cB) * dSdk;
+    F[2][4] = cB * dx;
+    st.p[0] = y + dx * tq; st.p[1] = zz + t * S; st.p[2] = s1;
+    Real Tm[5][5], Cn[5][5];
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = a + F[i][m] * st.C[m][j]; Tm[i][j] = a; }
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = a + Tm[i][m] * F[j][m]; Cn[i][j] = a; }
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = Cn[i][j]; st.C[j][i] = Cn[i][j]; }   // symmetrise: lower triangle mirrored
+    return true;
+  }
+
+  // Kalman update with the joint 2-D measurement (ym, zm), R = diag(sigma_y^2, sigma_z^2); returns chi2 increment
+  Real update_state(State& st, Real ym, Real zm) const {
+    const Real ry = (Real)sigma_y * (Real)sigma_y, rz = (Real)sigma_z * (Real)sigma_z;
+    Real s00 = st.C[0][0] + ry, s10 = st.C[1][0], s11 = st.C[1][1] + rz;
+    Real det = s00 * s11 - s10 * s10;
+    Real i00 = s11 / det, i11 = s00 / det, i10 = -s10 / det;
+    Real r0 = ym - st.p[0], r1 = zm - st.p[1];
+    Real K0[5], K1[5];
+    for (int i = 0; i < 5; i++) { K0[i] = st.C[i][0] * i00 + st.C[i][1] * i10; K1[i] = st.C[i][0] * i10 + st.C[i][1] * i11; }
+    Real Cn[5][5];
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) Cn[i][j] = st.C[i][j] - (K0[i] * st.C[0][j] + K1[i] * st.C[1][j]);
+    for (int i = 0; i < 5; i++) st.p[i] = st.p[i] + (K0[i] * r0 + K1[i] * r1);
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = Cn[i][j]; st.C[j][i] = Cn[i][j]; }
+    return r0 * (i00 * r0 + i10 * r1) + r1 * (i10 * r0 + i11 * r1);
+  }
+
+  void reset_cov(State& st) const { for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) st.C[i][j] = i == j ? (Real)T.c0[i] : (Real)0; }
+
+  // cluster pick-up on row r of a sector: nearest hit inside min(w_max, n_sigma*sqrt(C+sigma^2)); -1 = none
+  int32_t pickup(int sec, int r, const State& st, Real zref, bool brute) const {
+    int u = sec * R + r; int64_t o = off[u];
+    const Real wmax = (Real)T.w_max, ns = (Real)T.n_sigma;
+    Real wy = ns * std::sqrt(st.C[0][0] + (Real)sigma_y * (Real)sigma_y); if (!(wy <= wmax)) wy = wmax;
+    Real wz = ns * std::sqrt(st.C[1][1] + (Real)sigma_z * (Real)sigma_z); if (!(wz <= wmax)) wz = wmax;
+    Real y = st.p[0], zr = st.p[1];
+    Real ylo = y - wy, yhi = y + wy, zlo = zr - wz, zhi = zr + wz;
+    const Real margin = (Real)0.05;   // the bin range only has to be a superset of the z_rel window
+    int32_t best = -1; Real bestd = 0; int32_t besti = 0;
+    for_bins(u, ylo, yhi, (zlo + zref) - margin, (zhi + zref) + margin, brute, [&](int32_t p) {
+      Real yc = ys[o + p], zc = zs[o + p] - zref;
+      if (!(yc >= ylo && yc <= yhi && zc >= zlo && zc <= zhi)) return;
+      Real dy = yc - y, dz = zc - zr; Real d = dy * dy + dz * dz; int32_t ip = perm[o + p];
+      if (best < 0 || d < bestd || (d == bestd && ip < besti)) { best = p; bestd = d; besti = ip; } });
+    return best;
+  }
+
+  // ---- S5: tracklet constructor, one hypothesis per start hit ----
+  void s5_tracklets(bool brute) {
+    int64_t M = (int64_t)start_unit.size();
+    tl_n.assign(M, 0); tl_first.assign(M, -1); tl_last.assign(M, -1); tl_rowhit.assign(M * R, -1); tl_sector.assign(M, 0);
+    tl_chi2.assign(M, 0); tl_x.assign(M, 0); tl_par.assign(M * 5, 0); tl_cov.assign(M * 15, 0); tl_zref.assign(M, 0);
+    for (int64_t i = 0; i < M; i++) {
+      int u0 = start_unit[i], sec = u0 / R, r0 = u0 % R; int32_t h0 = start_pos[i];
+      int32_t* rowhit = &tl_rowhit[i * R];
+      auto Y = [&](int r, int32_t p) { return ys[off[sec * R + r] + p]; };
+      auto Z = [&](int r, int32_t p) { return zs[off[sec * R + r] + p]; };
+      const Real zref = Z(r0, h0);
+      State st;
+      { // Phase A init: direction from the origin
+        Real x = X[r0], y = Y(r0, h0); Real rr = std::sqrt(x * x + y * y);
+        st.p[0] = y; st.p[1] = 0; st.p[2] = y / rr; st.p[3] = continuous ? (Real)0 : zref / rr; st.p[4] = 0; reset_cov(st);
+      }
+      update_state(st, Y(r0, h0), (Real)0); rowhit[r0] = h0;
+      int r = r0; int32_t h = h0; bool ok = true;
+      State saved = st; int r_out = r0;
+      for (;;) {   // Phase A: follow the cleaned up-links, no gate
+        int32_t up = clean_up[off[sec * R + r] + h]; if (up < 0) break;
+        if (!propagate_state(st, X[r + 1] - X[r])) { ok = false; break; }
+        r++; h = up; update_state(st, Y(r, h), Z(r, h) - zref); rowhit[r] = h; saved = st; r_out = r;
+      }
+      if (ok) {    // Phase B: extrapolate outward with pick-up
+        int gap = 0;
+        for (int rr = r + 1; rr < R; rr++) {
+          if (!propagate_state(st, X[rr] - X[rr - 1])) break;
+          if (std::fabs(st.p[0]) > yedge[rr] + (Real)T.edge_margin) break;
+          int32_t p = pickup(sec, rr, st, zref, brute);
+          if (p >= 0) { update_state(st, Y(rr, p), Z(rr, p) - zref); rowhit[rr] = p; gap = 0; saved = st; r_out = rr; }
+          else { gap++; if (gap > T.max_gap) break; }
+        }
+      }
+      // Phase C: inward refit from the outermost assigned hit, then extrapolate inward
+      st = saved; reset_cov(st);
+      Real chi2 = 0; int n = 0;
+      chi2 = chi2 + update_state(st, Y(r_out, rowhit[r_out]), Z(r_out, rowhit[r_out]) - zref); n = 1;
+      State snap = st; int r_snap = r_out; int first_assigned = r0; int gap = 0; int stop_row = -1;
+      for (int rr = r_out - 1; rr >= 0; rr--) {
+        if (!propagate_state(st, X[rr] - X[rr + 1])) { stop_row = rr; break; }
+        if (rowhit[rr] >= 0) { chi2 = chi2 + update_state(st, Y(rr, rowhit[rr]), Z(rr, rowhit[rr]) - zref); n++; snap = st; r_snap = rr; continue; }
+        if (std::fabs(st.p[0]) > yedge[rr] + (Real)T.edge_margin) { if (rr < first_assigned) break; else continue; }
+        int32_t p = pickup(sec, rr, st, zref, brute);
+        if (p >= 0) { chi2 = chi2 + update_state(st, Y(rr, p), Z(rr, p) - zref); n++; rowhit[rr] = p; snap = st; r_snap = rr;
+          if (rr < first_assigned) { first_assigned = rr; gap = 0; } }
+        else if (rr < first_assigned) { gap++; if (gap > T.max_gap) break; }
+      }
+      for (int rr = 0; rr <= stop_row; rr++) rowhit[rr] = -1;   // hits never reached by the refit are not part of the tracklet
+      tl_sector[i] = sec; tl_n[i] = n; tl_chi2[i] = (double)chi2; tl_first[i] = r_snap; tl_last[i] = r_out; tl_x[i] = (double)X[r_snap]; tl_zref[i] = (double)zref;
+      for (int k = 0; k < 5; k++) tl_par[i * 5 + k] = (double)snap.p[k];
+      tl_par[i * 5 + 1] = (double)(snap.p[1] + zref);
+      int c = 0; for (int a = 0; a < 5; a++) for (int b = 0; b <= a; b++) tl_cov[i * 15 + c++] = (double)snap.C[a][b];
+    }
+  }
+
+  bool tracklet_kept(int64_t i) const { return tl_n[i] >= T.min_hits && std::isfinite(tl_chi2[i]); }
+  Real quality(int64_t i) const { return (Real)tl_chi2[i] / (Real)(2 * tl_n[i] - 5); }
+  // true if tracklet a beats tracklet b for a shared cluster: more hits, then lower chi2/ndf, then lower index
+  bool beats(int64_t a, int64_t b) const {
+    if (tl_n[a] != tl_n[b]) return tl_n[a] > tl_n[b];
+    Real qa = quality(a), qb = quality(b);
+    if (qa != qb) return qa < qb;
+    return a < b;
+  }
+
+  // ---- S6: selector -- winner takes the cluster; a track = a tracklet with >= min_hits owned clusters ----
+  void s6_select() {
+    int64_t M = (int64_t)tl_n.size();
+    std::vector<int64_t> owner(N, -1);
+    for (int64_t i = 0; i < M; i++) {
+      if (!tracklet_kept(i)) continue;
+      int sec = tl_sector[i];
+      for (int r = 0; r < R; r++) { int32_t p = tl_rowhit[i * R + r]; if (p < 0) continue;
+        int64_t g = off[sec * R + r] + p; if (owner[g] < 0 || beats(i, owner[g])) owner[g] = i; }
+    }
+    trk_sector.clear(); trk_ndf.clear(); trk_tracklet.clear(); trk_cl_row.clear(); trk_cl_index.clear(); trk_cl_begin.assign(1, 0);
+    trk_x.clear(); trk_par.clear(); trk_cov.clear(); trk_chi2.clear();
+    for (int64_t i = 0; i < M; i++) {
+      if (!tracklet_kept(i)) continue;
+      int sec = tl_sector[i]; int owned = 0;
+      for (int r = 0; r < R; r++) { int32_t p = tl_rowhit[i * R + r]; if (p >= 0 && owner[off[sec * R + r] + p] == i) owned++; }
+      if (owned < T.min_hits) continue;
+      for (int r = 0; r < R; r++) { int32_t p = tl_rowhit[i * R + r]; if (p >= 0 && owner[off[sec * R + r] + p] == i) {
+        trk_cl_row.push_back(r); trk_cl_index.push_back(perm[off[sec * R + r] + p]); } }
+      trk_cl_begin.push_back((int64_t)trk_cl_row.size());
+      trk_sector.push_back(sec); trk_ndf.push_back(2 * tl_n[i] - 5); trk_tracklet.push_back((int32_t)i);
+      trk_x.push_back(tl_x[i]); trk_chi2.push_back(tl_chi2[i]);
+      for (int k = 0; k < 5; k++) trk_par.push_back(tl_par[i * 5 + k]);
+      for (int k = 0; k < 15; k++) trk_cov.push_back(tl_cov[i * 15 + k]);
+    }
+  }
+
+  int run(int upto, int brute) override {
+    make_tables();
+    s0_time_to_z(); if (upto <= 0) return 0;
+    s1_grid(); if (upto <= 1) return 0;
+    s2_neighbours(brute & 1); if (upto <= 2) return 0;
+    s3_clean(); if (upto <= 3) return 0;
+    s4_start_hits(); if (upto <= 4) return 0;
+    s5_tracklets((brute & 2) != 0); if (upto <= 5) return 0;
+    s6_select();
+    return 0;
+  }
+
+  // hand-built tracklets for S6 pins (requires S1 to have run so that perm/off exist)
+  int set_tracklets(int64_t n, const int32_t* sector, const int32_t* nh, const double* chi2, const int32_t* rowhit) override {
+    tl_n.assign(nh, nh + n); tl_sector.assign(sector, sector + n); tl_chi2.assign(chi2, chi2 + n);
+    tl_rowhit.assign(rowhit, rowhit + n * R); tl_first.assign(n, 0); tl_last.assign(n, 0); tl_x.assign(n, 0);
+    tl_par.assign(n * 5, 0); tl_cov.assign(n * 15, 0); tl_zref.assign(n, 0);
+    s6_select(); return 0;
+  }
+
+  static void to_state(State& st, const double* par, const double* cov) {
+    for (int i = 0; i < 5; i++) st.p[i] = (Real)par[i];
+    int c = 0; for (int a = 0; a < 5; a++) for (int b = 0; b <= a; b++) { st.C[a][b] = (Real)cov[c]; st.C[b][a] = (Real)cov[c]; c++; }
+  }
+  static void from_state(const State& st, double* par, double* cov) {
+    for (int i = 0; i < 5; i++) par[i] = (double)st.p[i];
+    int c = 0; for (int a = 0; a < 5; a++) for (int b = 0; b <= a; b++) cov[c++] = (double)st.C[a][b];
+  }
+  int propagate(double* par, double* cov, double dx) override {
+    make_tables(); State st; to_state(st, par, cov); bool ok = propagate_state(st, (Real)dx); from_state(st, par, cov); return ok ? 0 : 1; }
+  int update(double* par, double* cov, double ym, double zm, double* chi2) override {
+    make_tables(); State st; to_state(st, par, cov); *chi2 = (double)update_state(st, (Real)ym, (Real)zm); from_state(st, par, cov); return 0; }
+
+  // kind: 0 int32, 1 int64, 2 double, 3 float
+  template <class V> static void dcopy(const std::vector<V>& a, std::vector<double>& d) { d.assign(a.begin(), a.end()); }
+  int get(const char* name, const void** p, int64_t* n, int* kind) override {
+    std::string s(name);
+#define RET(vec, k) { *p = (vec).data(); *n = (int64_t)(vec).size(); *kind = (k); return 0; }
+    if (s == "z") { dcopy(z, z_d); RET(z_d, 2) }
+    if (s == "ys") { dcopy(ys, ys_d); RET(ys_d, 2) }
+    if (s == "zs") { dcopy(zs, zs_d); RET(zs_d, 2) }
+    if (s == "perm") RET(perm, 0)
+    if (s == "bin_off") RET(bin_off, 1)
+    if (s == "bin_start") RET(bin_start, 0)
+    if (s == "grid_ny") RET(g_ny, 0)
+    if (s == "grid_nz") RET(g_nz, 0)
+    if (s == "grid_ylo") RET(g_ylo_d, 2)
+    if (s == "grid_zlo") RET(g_zlo_d, 2)
+    if (s == "grid_invs") RET(g_invs_d, 2)
+    if (s == "link_up") RET(link_up, 0)
+    if (s == "link_dn") RET(link_dn, 0)
+    if (s == "clean_up") RET(clean_up, 0)
+    if (s == "clean_dn") RET(clean_dn, 0)
+    if (s == "start_unit") RET(start_unit, 0)
+    if (s == "start_pos") RET(start_pos, 0)
+    if (s == "tl_n") RET(tl_n, 0)
+    if (s == "tl_first") RET(tl_first, 0)
+    if (s == "tl_last") RET(tl_last, 0)
+    if (s == "tl_rowhit") RET(tl_rowhit, 0)
+    if (s == "tl_sector") RET(tl_sector, 0)
+    if (s == "tl_chi2") RET(tl_chi2, 2)
+    if (s == "tl_x") RET(tl_x, 2)
+    if (s == "tl_par") RET(tl_par, 2)
+    if (s == "tl_cov") RET(tl_cov, 2)
+    if (s == "tl_zref") RET(tl_zref, 2)
+    if (s == "trk_sector") RET(trk_sector, 0)
+    if (s == "trk_ndf") RET(trk_ndf, 0)
+    if (s == "trk_tracklet") RET(trk_tracklet, 0)
+    if (s == "trk_cl_begin") RET(trk_cl_begin, 1)
+    if (s == "trk_cl_row") RET(trk_cl_row, 0)
+    if (s == "trk_cl_index") RET(trk_cl_index, 0)
+    if (s == "trk_x") RET(trk_x, 2)
+    if (s == "trk_par") RET(trk_par, 2)
+    if (s == "trk_cov") RET(trk_cov, 2)
+    if (s == "trk_chi2") RET(trk_chi2, 2)
+#undef RET
+    return -1;
+  }
+};
+
+}  // namespace
+
+extern "C" {
+void* orc_create(int use_double, int n_sectors, int n_rows, const float* row_x, double dphi, double z_max, double t_frame,
+                 double sigma_y, double sigma_z, double bz, double vdrift) {
+  if (use_double) return new Oracle<double>(n_sectors, n_rows, row_x, dphi, z_max, t_frame, sigma_y, sigma_z, bz, vdrift);
+  return new Oracle<float>(n_sectors, n_rows, row_x, dphi, z_max, t_frame, sigma_y, sigma_z, bz, vdrift);
+}
+void orc_destroy(void* h) { delete (OracleBase*)h; }
+int orc_set_param(void* h, const char* name, double v) {
+  Tunables& T = ((OracleBase*)h)->T; std::string s(name);
+  if (s == "wy") T.wy = v; else if (s == "wz") T.wz = v; else if (s == "dzdx_max") T.dzdx_max = v; else if (s == "wz0") T.wz0 = v;
+  else if (s == "cut2") T.cut2 = v; else if (s == "min_seed") T.min_seed = (int)v; else if (s == "s_max") T.s_max = v;
+  else if (s == "n_sigma") T.n_sigma = v; else if (s == "w_max") T.w_max = v; else if (s == "max_gap") T.max_gap = (int)v;
+  else if (s == "edge_margin") T.edge_margin = v; else if (s == "min_hits") T.min_hits = (int)v;
+  else if (s == "c0_y") T.c0[0] = v; else if (s == "c0_z") T.c0[1] = v; else if (s == "c0_sinphi") T.c0[2] = v;
+  else if (s == "c0_dzds") T.c0[3] = v; else if (s == "c0_qpt") T.c0[4] = v;
+  else if (s == "grid_scale") T.grid_scale = v;
+  else return -1;
+  return 0;
+}
+int orc_load(void* h, const int64_t* unit_off, const float* y, const float* t) { return ((OracleBase*)h)->load(unit_off, y, t); }
+int orc_run(void* h, int upto, int brute) { return ((OracleBase*)h)->run(upto, brute); }
+int orc_get(void* h, const char* name, const void** p, int64_t* n, int* kind) { return ((OracleBase*)h)->get(name, p, n, kind); }
+int orc_propagate(void* h, double* par, double* cov, double dx) { return ((OracleBase*)h)->propagate(par, cov, dx); }
+int orc_update(void* h, double* par, double* cov, double ym, double zm, double* chi2) { return ((OracleBase*)h)->update(par, cov, ym, zm, chi2); }
+int orc_set_tracklets(void* h, int64_t n, const int32_t* sector, const int32_t* nh, const double* chi2, const int32_t* rowhit) {
+  return ((OracleBase*)h)->set_tracklets(n, sector, nh, chi2, rowhit); }
+}
