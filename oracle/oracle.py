@@ -69,7 +69,11 @@ class Oracle:
 
     @classmethod
     def for_workload(cls, w, double=False, **params):
-        o = cls(double=double, **w.geometry(), **params)
+        geo = w.geometry()
+        for k in list(params):          # a geometry field given explicitly overrides the workload's (e.g. sigma_y for noise-free input)
+            if k in geo:
+                geo[k] = params.pop(k)
+        o = cls(double=double, **geo, **params)
         o.load(w.unit_off, w.y, w.t)
         return o
 
