@@ -1,0 +1,125 @@
+// k1_grid.cu -- K1: S0 (time -> z) fused with S1 (per-row 2-D grid, stable counting sort).
+//
+// One CTA per (sector,row) unit.  The bin counters / cursors of the unit live in shared memory (global scratch for units
+// whose grid does not fit).  Passes over the unit's clusters:
+//   B  count      : float4-vectorised, coalesced loads of pad-y and time; z = z_max - vdrift*t; bin; shared-memory atomicAdd
+//   C  scan       : block exclusive scan of the counters -> bin_start (global) and cursors (shared)
+//   D  scatter    : same loads again (L2 hits: a unit is <= a few hundred KB), pos = atomicAdd(cursor[bin]); perm[pos] = i
+//   E1 canonical  : one thread per bin sorts the (about one) entries of its bin by original index -> the order inside a bin is
+//                   ascending original index, i.e. the counting sort is stable and independent of the atomic order
+//   E2 gather     : one thread per sorted position writes float2 (y, z), coalesced
+// Algorithmic HBM bytes per cluster: 8 read (y,t) + 8 (yz) + 4 (perm) + ~4 (bin_start) written = 24.
+#include "tpc_internal.cuh"
+
+namespace tpc {
+namespace {
+
+// Calls f(i, y, t) for every cluster i in [0,n) of a unit whose arrays start at element offset `src` (float4 body when aligned).
+template <class F>
+__device__ __forceinline__ void for_each_cluster(const float* __restrict__ in_y, const float* __restrict__ in_t, long long src, int n,
+                                                 F&& f) {
+  const float* py = in_y + src;
+  const float* pt = in_t + src;
+  int head = (int)((4 - (src & 3)) & 3);
+  if (head > n) head = n;
+  const int nvec = (n - head) >> 2;
+  const int tail0 = head + (nvec << 2);
+  if ((int)threadIdx.x < head) f((int)threadIdx.x, py[threadIdx.x], pt[threadIdx.x]);
+  const float4* vy = reinterpret_cast<const float4*>(py + head);
+  const float4* vt = reinterpret_cast<const float4*>(pt + head);
+  for (int v = threadIdx.x; v < nvec; v += blockDim.x) {
+    float4 a = __ldg(vy + v), b = __ldg(vt + v);
+    int i = head + (v << 2);
+    f(i, a.x, b.x); f(i + 1, a.y, b.y); f(i + 2, a.z, b.z); f(i + 3, a.w, b.w);
+  }
+  int i = tail0 + threadIdx.x;
+  if (i < n) f(i, py[i], pt[i]);
+}
+
+__global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict__ units, const float* __restrict__ in_y,
+                                                       const float* __restrict__ in_t, float2* __restrict__ yz,
+                                                       int* __restrict__ perm, int* __restrict__ bin_start, int* __restrict__ cursor_g,
+                                                       const float zmax, const float vdrift) {
+  extern __shared__ int s_cnt[];
+  __shared__ int s_warp[33];
+  const UnitDesc d = units[blockIdx.x];
+  const int n = d.n, ny = d.ny, nz = d.nz, nb = ny * nz;
+  int* __restrict__ bs = bin_start + d.bin_off;
+  if (n == 0) {
+    for (int b = threadIdx.x; b <= nb; b += blockDim.x) bs[b] = 0;
+    return;
+  }
+  int* cnt = d.cur_off >= 0 ? cursor_g + d.cur_off : s_cnt;
+  for (int b = threadIdx.x; b < nb; b += blockDim.x) cnt[b] = 0;
+  __syncthreads();
+
+  // B: count.  S0: product rounded, then subtracted (no FMA).
+  for_each_cluster(in_y, in_t, d.src, n, [&](int, float y, float t) {
+    float z = __fsub_rn(zmax, __fmul_rn(vdrift, t));
+    int b = bin_of(z, d.zlo, d.invs, nz) * ny + bin_of(y, d.ylo, d.invs, ny);
+    atomicAdd(&cnt[b], 1);
+  });
+  __syncthreads();
+
+  // C: exclusive scan of the counters; bin_start[b] (global) and cursor[b] (cnt) both get the start of bin b.
+  int carry = 0;
+  for (int base = 0; base < nb; base += blockDim.x) {
+    int b = base + threadIdx.x;
+    int v = b < nb ? cnt[b] : 0;
+    int total;
+    int ex = block_excl_scan(v, s_warp, &total) + carry;
+    if (b < nb) { cnt[b] = ex; bs[b] = ex; }
+    carry += total;
+  }
+  if (threadIdx.x == 0) bs[nb] = n;
+  __syncthreads();
+
+  // D: scatter original indices to their bins (order inside a bin arbitrary here).
+  int* __restrict__ pm = perm + d.off;
+  for_each_cluster(in_y, in_t, d.src, n, [&](int i, float y, float t) {
+    float z = __fsub_rn(zmax, __fmul_rn(vdrift, t));
+    int b = bin_of(z, d.zlo, d.invs, nz) * ny + bin_of(y, d.ylo, d.invs, ny);
+    int pos = atomicAdd(&cnt[b], 1);
+    pm[pos] = i;
+  });
+  __syncthreads();
+
+  // E1: canonical order inside each bin = ascending original index (insertion sort; bins hold about one cluster).
+  for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+    const int lo = b ? cnt[b - 1] : 0, hi = cnt[b];   // after D, cursor[b] = end of bin b
+    for (int i = lo + 1; i < hi; i++) {
+      int v = pm[i], j = i - 1;
+      while (j >= lo && pm[j] > v) { pm[j + 1] = pm[j]; j--; }
+      pm[j + 1] = v;
+    }
+  }
+  __syncthreads();
+
+  // E2: sorted payload, coalesced writes.
+  float2* __restrict__ out = yz + d.off;
+  const float* py = in_y + d.src;
+  const float* pt = in_t + d.src;
+  for (int p = threadIdx.x; p < n; p += blockDim.x) {
+    int i = pm[p];
+    out[p] = make_float2(py[i], __fsub_rn(zmax, __fmul_rn(vdrift, pt[i])));
+  }
+}
+
+}  // namespace
+
+int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float* d_in_y, const float* d_in_t, float2* d_yz,
+                   int* d_perm, int* d_bin_start, int* d_cursor, const Params& P, int max_cursor_ints_smem, int max_n) {
+  if (U <= 0) return 0;
+  int threads = 128;
+  while (threads < 1024 && threads * 8 < max_n) threads <<= 1;   // about 8 clusters per thread and pass
+  size_t smem = (size_t)max_cursor_ints_smem * sizeof(int);
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(k1_grid_build, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return -(int)e;
+  }
+  k1_grid_build<<<U, threads, smem, L.stream>>>(d_units, d_in_y, d_in_t, d_yz, d_perm, d_bin_start, d_cursor, P.zmax, P.vdrift);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? 1 : -(int)e;
+}
+
+}  // namespace tpc

@@ -1,0 +1,145 @@
+// k6_selector.cu -- K6: S6 tracklet selector, resolves shared clusters (BASELINE north_star; definition in DESIGN.md section 4).
+//
+// Every cluster referenced by a kept tracklet (n >= min_hits, finite chi2) goes to the tracklet with the maximum key
+// (n, -chi2/ndf, -tracklet index).  The key is packed into 64 bits so that one atomicMax per reference resolves the owner:
+//   bits 63..56  n (<= 255 rows)
+//   bits 55..24  bitwise NOT of the order-preserving image of the fp32 quality chi2/ndf (lower quality wins)
+//   bits 23..0   0xFFFFFF - tracklet index (lower index wins)                       -> at most 2^24 tracklets per call
+// k6_owner : atomicMax of the key on owner[cluster]          k6_count : owned clusters per tracklet, track flag
+// scan     : exclusive prefix sum of (flag << 40 | owned)     k6_emit  : compacted tracks + CSR cluster lists, in tracklet order
+#include "tpc_internal.cuh"
+
+namespace tpc {
+namespace {
+
+constexpr int K6_THREADS = 128;
+constexpr unsigned long long REF_MASK = (1ull << 40) - 1ull;
+
+__device__ __forceinline__ unsigned long long make_key(int n, float chi2, int idx) {
+  const float q = chi2 / (float)(2 * n - 5);
+  unsigned b = __float_as_uint(q);
+  b = (b & 0x80000000u) ? ~b : (b | 0x80000000u);   // monotone map float -> unsigned
+  return ((unsigned long long)(unsigned)n << 56) | ((unsigned long long)(~b) << 24) | (unsigned long long)(0xFFFFFFu - (unsigned)idx);
+}
+
+__global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const long long Mpad, const int R, const int min_hits,
+                                                       const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
+                                                       const int* __restrict__ rowhit, const int* __restrict__ tl_n,
+                                                       const int* __restrict__ tl_first, const int* __restrict__ tl_last,
+                                                       const float* __restrict__ tl_chi2, unsigned long long* __restrict__ owner,
+                                                       unsigned long long* __restrict__ tl_key) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  const int n = tl_n[i];
+  const float chi2 = tl_chi2[i];
+  const bool kept = n >= min_hits && isfinite(chi2);
+  const unsigned long long key = kept ? make_key(n, chi2, i) : 0ull;
+  tl_key[i] = key;
+  if (!kept) return;
+  const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
+  const int r1 = tl_last[i];
+  for (int r = tl_first[i]; r <= r1; r++) {
+    const int p = rowhit[(long long)r * Mpad + i];
+    if (p >= 0) atomicMax(&owner[su[r].off + p], key);
+  }
+}
+
+__global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const long long Mpad, const int R, const int min_hits,
+                                                       const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
+                                                       const int* __restrict__ rowhit, const int* __restrict__ tl_first,
+                                                       const int* __restrict__ tl_last, const unsigned long long* __restrict__ owner,
+                                                       const unsigned long long* __restrict__ tl_key,
+                                                       unsigned long long* __restrict__ scan_in) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  const unsigned long long key = tl_key[i];
+  int owned = 0;
+  if (key) {
+    const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
+    const int r1 = tl_last[i];
+    for (int r = tl_first[i]; r <= r1; r++) {
+      const int p = rowhit[(long long)r * Mpad + i];
+      if (p >= 0 && owner[su[r].off + p] == key) owned++;
+    }
+  }
+  scan_in[i] = owned >= min_hits && key ? ((1ull << 40) | (unsigned long long)owned) : 0ull;
+}
+
+__global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const long long Mpad, const int R, const int* __restrict__ start_unit,
+                                                      const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
+                                                      const int* __restrict__ perm, const int* __restrict__ rowhit,
+                                                      const int* __restrict__ tl_n, const int* __restrict__ tl_first,
+                                                      const int* __restrict__ tl_last, const float* __restrict__ tl_chi2,
+                                                      const float* __restrict__ tl_par, const float* __restrict__ tl_cov,
+                                                      const unsigned long long* __restrict__ owner,
+                                                      const unsigned long long* __restrict__ tl_key,
+                                                      const unsigned long long* __restrict__ scan_in,
+                                                      const unsigned long long* __restrict__ scan_out, int* __restrict__ o_sector,
+                                                      float* __restrict__ o_x, float* __restrict__ o_par, float* __restrict__ o_cov,
+                                                      float* __restrict__ o_chi2, int* __restrict__ o_ndf, int* __restrict__ o_tracklet,
+                                                      long long* __restrict__ o_cl_begin, int* __restrict__ o_cl_row,
+                                                      int* __restrict__ o_cl_index, const long long n_tracks, const long long n_refs) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) o_cl_begin[n_tracks] = n_refs;
+  if (i >= M || scan_in[i] == 0ull) return;
+  const unsigned long long so = scan_out[i];
+  const long long t = (long long)(so >> 40);
+  long long k = (long long)(so & REF_MASK);
+  const int sec = start_unit[i] / R;
+  const UnitDesc* __restrict__ su = units + (long long)sec * R;
+  const unsigned long long key = tl_key[i];
+  const int r0 = tl_first[i], r1 = tl_last[i];
+  o_sector[t] = sec; o_x[t] = rows[r0].x; o_chi2[t] = tl_chi2[i]; o_ndf[t] = 2 * tl_n[i] - 5; o_tracklet[t] = i; o_cl_begin[t] = k;
+#pragma unroll
+  for (int j = 0; j < 5; j++) o_par[t * 5 + j] = tl_par[(long long)i * 5 + j];
+#pragma unroll
+  for (int j = 0; j < 15; j++) o_cov[t * 15 + j] = tl_cov[(long long)i * 15 + j];
+  for (int r = r0; r <= r1; r++) {
+    const int p = rowhit[(long long)r * Mpad + i];
+    if (p < 0) continue;
+    const long long g = su[r].off + p;
+    if (owner[g] == key) { o_cl_row[k] = r; o_cl_index[k] = perm[g]; k++; }
+  }
+}
+
+}  // namespace
+
+int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const int* d_start_unit, const UnitDesc* d_units,
+                     const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
+                     const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
+                     unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
+                     unsigned long long* d_total, const Params& P) {
+  (void)d_rows; (void)d_perm;
+  if (M <= 0) {
+    cudaError_t e = cudaMemsetAsync(d_total, 0, sizeof(unsigned long long), L.stream);
+    return e == cudaSuccess ? 0 : -(int)e;
+  }
+  cudaError_t e = cudaMemsetAsync(d_owner, 0, (size_t)N * sizeof(unsigned long long), L.stream);
+  if (e != cudaSuccess) return -(int)e;
+  const int blocks = (M + K6_THREADS - 1) / K6_THREADS;
+  k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M, Mpad, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first, d_tl_last,
+                                                 d_tl_chi2, d_owner, d_tl_key);
+  k6_count<<<blocks, K6_THREADS, 0, L.stream>>>(M, Mpad, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_first, d_tl_last, d_owner,
+                                                 d_tl_key, d_scan_in);
+  int rc = launch_scan_u64(L, d_scan_in, d_scan_out, M, d_scan_tmp, d_total);
+  if (rc < 0) return rc;
+  e = cudaGetLastError();
+  return e == cudaSuccess ? 2 + rc : -(int)e;
+}
+
+int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
+                   const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
+                   const float* d_tl_chi2, const float* d_tl_par, const float* d_tl_cov, const unsigned long long* d_owner,
+                   const unsigned long long* d_tl_key, const unsigned long long* d_scan_in, const unsigned long long* d_scan_out,
+                   int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,
+                   long long* o_cl_begin, int* o_cl_row, int* o_cl_index, long long n_tracks, long long n_refs, const Params& P) {
+  const int blocks = M > 0 ? (M + K6_THREADS - 1) / K6_THREADS : 1;
+  k6_emit<<<blocks, K6_THREADS, 0, L.stream>>>(M, Mpad, P.R, d_start_unit, d_units, d_rows, d_perm, d_rowhit, d_tl_n, d_tl_first,
+                                                d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out,
+                                                o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row, o_cl_index,
+                                                n_tracks, n_refs);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? 1 : -(int)e;
+}
+
+}  // namespace tpc

@@ -1,0 +1,124 @@
+// tpc_internal.cuh -- shared declarations of the CUDA path (context layout, per-row / per-unit tables, device helpers).
+// Product code: shares nothing with oracle/.  Definitions follow DESIGN.md section 4 (S0..S6).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tpc {
+
+// Per-row constants, computed on the host in double and rounded once to float ("per-row constants").
+struct RowConst {
+  float x;       // local x of the row
+  float tu, td;  // x_{r+1}/x_r, x_{r-1}/x_r : from-origin projection factors
+  float a, b;    // x_{r+1}-x_r, x_r-x_{r-1}
+  float thr;     // cut2 * 0.5 * (a^2+b^2)
+  float wzu, wzd;// continuous-mode z half-widths up / down
+  float yedge;   // x_r * tan(dphi/2)
+  float pad[3];
+};
+
+// One (sector,row) unit: where its clusters come from, where its sorted copy lives, and its S1 grid.
+struct UnitDesc {
+  long long off;      // offset of the unit in the sorted arrays (CSR over units)
+  long long src;      // offset of the unit's clusters in the input arena
+  long long bin_off;  // offset of the unit's bin_start table (ny*nz+1 entries)
+  long long cur_off;  // K1: offset into the global cursor scratch, or -1 when the cursors fit shared memory
+  int n, ny, nz;
+  float ylo, zlo, invs;
+  int pad[2];
+};
+
+// Scalar parameters passed by value to every kernel (table T of DESIGN.md, rounded to float exactly once on the host).
+struct Params {
+  int NS, R, continuous;
+  float zmax, vdrift;             // S0
+  float wy, wz;                   // S2
+  int min_seed;                   // S4
+  float cB;                       // curvature constant -0.00299792458*Bz
+  float c0[5];                    // S5 initial covariance diagonal
+  float ry, rz;                   // sigma_y^2, sigma_z^2
+  float smax, nsigma, wmax, edge_margin;
+  int max_gap, min_hits;
+};
+
+// Work item of K2/K3: a chunk of consecutive sorted hits of one unit.
+struct Item { int unit; int start; };
+
+// ---- device helpers ------------------------------------------------------------------------------------------------
+// S1 bin of a coordinate: fp32 subtract, fp32 multiply (no FMA), negative / NaN -> 0, clamp to nb-1.
+__device__ __forceinline__ int bin_of(float v, float lo, float inv, int nb) {
+  float f = __fmul_rn(__fsub_rn(v, lo), inv);
+  if (!(f > 0.0f)) return 0;
+  if (f >= (float)nb) return nb - 1;
+  int b = (int)f;
+  return b > nb - 1 ? nb - 1 : b;
+}
+
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) { int t = __shfl_up_sync(0xffffffffu, v, d); if (lane >= d) v += t; }
+  return v;
+}
+
+// Exclusive scan of one value per thread over the block (blockDim.x multiple of 32, <= 1024).  s_warp: 33 ints of shared memory.
+// Returns the exclusive prefix; *total receives the block total.  Contains three __syncthreads.
+__device__ __forceinline__ int block_excl_scan(int v, int* s_warp, int* total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  int inc = warp_incl_scan(v, lane);
+  if (lane == 31) s_warp[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    int t = lane < nw ? s_warp[lane] : 0;
+    int ti = warp_incl_scan(t, lane);
+    s_warp[lane] = ti - t;
+    if (lane == 31) s_warp[32] = ti;
+  }
+  __syncthreads();
+  int res = inc - v + s_warp[w];
+  *total = s_warp[32];
+  __syncthreads();   // s_warp may be reused right away by the caller's next round
+  return res;
+}
+
+// ---- kernel launchers (one per step; each returns the number of kernels it launched, or a negative cudaError) --------
+struct Launch {
+  cudaStream_t stream;
+  int sm_count;
+};
+
+int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float* d_in_y, const float* d_in_t, float2* d_yz,
+                   int* d_perm, int* d_bin_start, int* d_cursor, const Params& P, int max_cursor_ints_smem, int max_n);
+
+int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units,
+                         const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up,
+                         int* d_link_dn, const Params& P);
+
+int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, int* d_link_up,
+                          int* d_link_dn, unsigned* d_mask, int* d_item_count, int* d_item_base, int* d_scan_tmp,
+                          int* d_start_unit, int* d_start_pos, int* d_total, const Params& P);
+
+int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
+                        const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, const int* d_link_up,
+                        int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2, float* d_tl_par,
+                        float* d_tl_cov, const Params& P);
+
+int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const int* d_start_unit, const UnitDesc* d_units,
+                     const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
+                     const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
+                     unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
+                     unsigned long long* d_total, const Params& P);
+
+int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
+                   const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
+                   const float* d_tl_chi2, const float* d_tl_par, const float* d_tl_cov, const unsigned long long* d_owner,
+                   const unsigned long long* d_tl_key, const unsigned long long* d_scan_in, const unsigned long long* d_scan_out,
+                   int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,
+                   long long* o_cl_begin, int* o_cl_row, int* o_cl_index, long long n_tracks, long long n_refs, const Params& P);
+
+// device-wide exclusive scans (own kernels; three launches each)
+int launch_scan_i32(const Launch& L, const int* d_in, int* d_out, int n, int* d_tmp, int* d_total);
+int launch_scan_u64(const Launch& L, const unsigned long long* d_in, unsigned long long* d_out, int n, unsigned long long* d_tmp,
+                    unsigned long long* d_total);
+constexpr int SCAN_TILE = 4096;   // elements per CTA in the scans; tmp needs ceil(n/SCAN_TILE)+1 entries
+
+}  // namespace tpc
