@@ -1,0 +1,645 @@
+// tpc_abi.cu -- the C ABI of include/tpc.h: context, staging of clusters, host-side tables, kernel sequence, result export.
+// Everything the path computes runs in the kernels of k1..k6; the host code here only sizes buffers, computes the per-row
+// and per-unit constant tables (double -> float once) and moves bytes.  No CPU fallback exists.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <string>
+#include <vector>
+#include <algorithm>
+
+#include "../../include/tpc.h"
+#include "tpc_internal.cuh"
+
+using namespace tpc;
+
+namespace {
+
+std::string g_create_error = "";
+
+// grow-only device buffer
+struct DevBuf {
+  void* p = nullptr; size_t cap = 0;
+  cudaError_t ensure(size_t bytes) {
+    if (bytes <= cap) return cudaSuccess;
+    size_t want = std::max(bytes, cap + cap / 2);
+    want = (want + 255) & ~(size_t)255;
+    if (p) { cudaError_t e = cudaFree(p); p = nullptr; cap = 0; if (e != cudaSuccess) return e; }
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e != cudaSuccess) { p = nullptr; return e; }
+    cap = want; return cudaSuccess;
+  }
+  // grow keeping the first keep_bytes (device-to-device copy on the stream)
+  cudaError_t ensure_keep(size_t bytes, size_t keep_bytes, cudaStream_t s) {
+    if (bytes <= cap) return cudaSuccess;
+    size_t want = std::max(bytes, cap * 2);
+    want = (want + 255) & ~(size_t)255;
+    void* np = nullptr;
+    cudaError_t e = cudaMalloc(&np, want);
+    if (e != cudaSuccess) return e;
+    if (p && keep_bytes) { e = cudaMemcpyAsync(np, p, keep_bytes, cudaMemcpyDeviceToDevice, s); if (e != cudaSuccess) { cudaFree(np); return e; } }
+    if (p) { cudaStreamSynchronize(s); cudaFree(p); }
+    p = np; cap = want; return cudaSuccess;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+  template <class T> T* as() const { return (T*)p; }
+};
+
+// grow-only pinned host buffer
+struct PinBuf {
+  void* p = nullptr; size_t cap = 0;
+  cudaError_t ensure_keep(size_t bytes, size_t keep_bytes) {
+    if (bytes <= cap) return cudaSuccess;
+    size_t want = std::max(bytes, cap * 2);
+    void* np = nullptr;
+    cudaError_t e = cudaMallocHost(&np, want);
+    if (e != cudaSuccess) return e;
+    if (p && keep_bytes) memcpy(np, p, keep_bytes);
+    if (p) cudaFreeHost(p);
+    p = np; cap = want; return cudaSuccess;
+  }
+  cudaError_t ensure(size_t bytes) { return ensure_keep(bytes, 0); }
+  void release() { if (p) cudaFreeHost(p); p = nullptr; cap = 0; }
+  template <class T> T* as() const { return (T*)p; }
+};
+
+struct Tunables {   // DESIGN.md table T
+  double wy = 1.5, wz = 1.5, dzdx_max = 1.5, wz0 = 0.75, cut2 = 1.75;
+  int min_seed = 3;
+  double c0[5] = {1.0, 2.25, 1.0, 1.0, 100.0};
+  double s_max = 0.95, n_sigma = 4.0, w_max = 3.0;
+  int max_gap = 4;
+  double edge_margin = 1.0;
+  int min_hits = 10;
+  double grid_min = 1.0, grid_max = 64.0, grid_scale = 1.0;
+  int debug_keep = 0;
+  int chunk = 512;            // clusters per K2/K3 work item (multiple of 32)
+};
+
+struct UnitSrc { long long src = 0; int n = 0; };
+
+constexpr int K1_SMEM_CURSOR_MAX = 50 * 1024;   // ints (200 KB) of shared-memory bin cursors per CTA; larger grids use global scratch
+
+}  // namespace
+
+struct tpc_ctx {
+  // geometry / physics
+  int NS = 0, R = 0;
+  std::vector<float> row_x;
+  float dphi = 0, z_max = 0, t_frame = 0, sigma_y = 0, sigma_z = 0, bz = 0, vdrift = 0;
+  Tunables T;
+  int device = 0, sm_count = 148;
+  cudaStream_t stream = nullptr;
+  std::string err;
+  bool loaded_any = false;       // a load happened since create/clear (freezes tpc_set_param)
+  bool have_result = false;
+
+  // input staging: one logical arena; host loads land in h_y/h_t (pinned) and are uploaded at find time
+  std::vector<UnitSrc> usrc;     // [U]
+  long long arena_pos = 0;
+  PinBuf h_y, h_t;
+  DevBuf d_in_y, d_in_t;
+  std::vector<std::pair<long long, long long>> dirty;   // host ranges [a,b) not yet uploaded
+
+  // tables
+  std::vector<UnitDesc> h_units; std::vector<Item> h_items;
+  PinBuf p_units, p_items, p_small;
+  DevBuf d_rows, d_units, d_items;
+  bool rows_valid = false;
+  Params P;
+
+  // S1..S4
+  long long N = 0, n_bins = 0; int n_items = 0;
+  DevBuf d_yz, d_perm, d_bin_start, d_cursor, d_link_up, d_link_dn, d_raw_up, d_raw_dn, d_mask, d_item_count, d_item_base, d_scan_tmp;
+  DevBuf d_start_unit, d_start_pos, d_counters;
+  // S5/S6
+  int M = 0; long long Mpad = 0;
+  DevBuf d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out, d_scan_tmp64;
+  // outputs (device)
+  long long n_tracks = 0, n_refs = 0;
+  DevBuf o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row, o_cl_index;
+  // outputs / debug copies (host)
+  std::vector<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; std::vector<float> ho_x, ho_par, ho_cov, ho_chi2;
+  std::vector<int64_t> ho_cl_begin;
+  std::vector<float> dbg_yz; std::vector<int32_t> dbg_perm, dbg_bins, dbg_up, dbg_dn, dbg_su, dbg_sp;
+  std::vector<int32_t> dbg_tl_sector, dbg_tl_row, dbg_tl_n, dbg_tl_first, dbg_tl_last, dbg_rowhit; std::vector<float> dbg_tl_chi2, dbg_tl_x, dbg_tl_par, dbg_tl_cov;
+
+  cudaEvent_t ev[10] = {};
+  tpc_timings timings = {};
+};
+
+namespace {
+
+int fail(tpc_ctx* c, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof(buf), fmt, ap); va_end(ap);
+  if (c) c->err = buf; else g_create_error = buf;
+  return code;
+}
+#define CUDA_TRY(c, expr)                                                                                         \
+  do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return fail((c), e_ == cudaErrorMemoryAllocation ? TPC_E_NOMEM : TPC_E_CUDA, \
+                                                                   "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+#define LAUNCH_TRY(c, expr, counter)                                                                              \
+  do { int rc_ = (expr); if (rc_ < 0) return fail((c), TPC_E_CUDA, "%s: %s", #expr, cudaGetErrorString((cudaError_t)(-rc_))); (counter) += rc_; } while (0)
+
+// 0 = unregistered host, 1 = pinned host, 2 = device / managed
+int pointer_kind(const void* p) {
+  cudaPointerAttributes a;
+  cudaError_t e = cudaPointerGetAttributes(&a, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return 0; }
+  if (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) return 2;
+  if (a.type == cudaMemoryTypeHost) return 1;
+  return 0;
+}
+
+void add_dirty(tpc_ctx* c, long long a, long long b) {
+  if (!c->dirty.empty() && c->dirty.back().second == a) c->dirty.back().second = b;
+  else c->dirty.emplace_back(a, b);
+}
+
+}  // namespace
+
+// =====================================================================================================================
+extern "C" {
+
+int tpc_abi_version(void) { return 1; }
+
+const char* tpc_last_error(const tpc_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int tpc_create(const tpc_geometry* g, float bz, float vdrift, tpc_ctx** out) {
+  if (out) *out = nullptr;
+  if (!g || !out) return fail(nullptr, TPC_E_ARG, "tpc_create: null argument");
+  if (g->n_sectors < 1 || g->n_rows < 3 || !g->row_x) return fail(nullptr, TPC_E_ARG, "tpc_create: need n_sectors >= 1, n_rows >= 3 and row_x");
+  if (g->n_rows > 255) return fail(nullptr, TPC_E_CAPACITY, "tpc_create: n_rows > 255 does not fit the selector key");
+  if ((long long)g->n_sectors * g->n_rows > (1 << 24)) return fail(nullptr, TPC_E_CAPACITY, "tpc_create: too many (sector,row) units");
+  for (int r = 0; r < g->n_rows; r++) {
+    if (!std::isfinite(g->row_x[r]) || !(g->row_x[r] > 0) || (r && !(g->row_x[r] > g->row_x[r - 1])))
+      return fail(nullptr, TPC_E_ARG, "tpc_create: row_x must be finite, positive and strictly increasing (row %d)", r);
+  }
+  if (!std::isfinite(bz) || !std::isfinite(vdrift) || !(vdrift > 0)) return fail(nullptr, TPC_E_ARG, "tpc_create: Bz must be finite and vdrift finite and > 0");
+  if (!(g->sector_dphi > 0) || !(g->sector_dphi < 3.14159f) || !(g->z_max > 0) || !(g->t_frame >= 0) || !(g->sigma_y > 0) || !(g->sigma_z > 0) ||
+      !std::isfinite(g->z_max) || !std::isfinite(g->t_frame))
+    return fail(nullptr, TPC_E_ARG, "tpc_create: sector_dphi in (0,pi), z_max > 0, t_frame >= 0, sigma_y/z > 0 required");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(nullptr, TPC_E_CUDA, "tpc_create: no CUDA device (%s); this library has no CPU fallback", e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+  }
+  tpc_ctx* c = new (std::nothrow) tpc_ctx();
+  if (!c) return fail(nullptr, TPC_E_NOMEM, "tpc_create: out of host memory");
+  c->NS = g->n_sectors; c->R = g->n_rows; c->row_x.assign(g->row_x, g->row_x + g->n_rows);
+  c->dphi = g->sector_dphi; c->z_max = g->z_max; c->t_frame = g->t_frame; c->sigma_y = g->sigma_y; c->sigma_z = g->sigma_z;
+  c->bz = bz; c->vdrift = vdrift;
+  c->usrc.assign((size_t)c->NS * c->R, UnitSrc());
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&c->device) != cudaSuccess || cudaGetDeviceProperties(&prop, c->device) != cudaSuccess) {
+    int rc = fail(nullptr, TPC_E_CUDA, "tpc_create: cannot query the CUDA device: %s", cudaGetErrorString(cudaGetLastError()));
+    delete c; return rc;
+  }
+  c->sm_count = prop.multiProcessorCount;
+  for (auto& ev : c->ev) {
+    if (cudaEventCreate(&ev) != cudaSuccess) { int rc = fail(nullptr, TPC_E_CUDA, "tpc_create: cudaEventCreate failed"); delete c; return rc; }
+  }
+  *out = c;
+  return TPC_OK;
+}
+
+void tpc_destroy(tpc_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  DevBuf* bufs[] = {&c->d_in_y, &c->d_in_t, &c->d_rows, &c->d_units, &c->d_items, &c->d_yz, &c->d_perm, &c->d_bin_start, &c->d_cursor,
+                    &c->d_link_up, &c->d_link_dn, &c->d_raw_up, &c->d_raw_dn, &c->d_mask, &c->d_item_count, &c->d_item_base, &c->d_scan_tmp,
+                    &c->d_start_unit, &c->d_start_pos, &c->d_counters, &c->d_rowhit, &c->d_tl_n, &c->d_tl_first, &c->d_tl_last, &c->d_tl_chi2,
+                    &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
+                    &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index};
+  for (DevBuf* b : bufs) b->release();
+  c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
+  for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
+  delete c;
+}
+
+int tpc_set_stream(tpc_ctx* c, void* s) {
+  if (!c) return TPC_E_ARG;
+  c->stream = (cudaStream_t)s;
+  return TPC_OK;
+}
+
+int tpc_set_param(tpc_ctx* c, const char* name, double v) {
+  if (!c || !name) return fail(c, TPC_E_ARG, "tpc_set_param: null argument");
+  if (c->loaded_any) return fail(c, TPC_E_STATE, "tpc_set_param(%s): only before the first load after tpc_create / tpc_clear", name);
+  if (!std::isfinite(v)) return fail(c, TPC_E_ARG, "tpc_set_param(%s): value must be finite", name);
+  Tunables& T = c->T; std::string s(name);
+  auto pos = [&](double& f) { if (!(v > 0)) return fail(c, TPC_E_ARG, "tpc_set_param(%s): must be > 0", name); f = v; return (int)TPC_OK; };
+  auto nonneg = [&](double& f) { if (!(v >= 0)) return fail(c, TPC_E_ARG, "tpc_set_param(%s): must be >= 0", name); f = v; return (int)TPC_OK; };
+  int rc = TPC_OK;
+  if (s == "wy") rc = pos(T.wy); else if (s == "wz") rc = pos(T.wz); else if (s == "dzdx_max") rc = nonneg(T.dzdx_max);
+  else if (s == "wz0") rc = nonneg(T.wz0); else if (s == "cut2") rc = pos(T.cut2);
+  else if (s == "min_seed") { if (v < 1 || v > 255) return fail(c, TPC_E_ARG, "min_seed must be in 1..255"); T.min_seed = (int)v; }
+  else if (s == "c0_y") rc = pos(T.c0[0]); else if (s == "c0_z") rc = pos(T.c0[1]); else if (s == "c0_sinphi") rc = pos(T.c0[2]);
+  else if (s == "c0_dzds") rc = pos(T.c0[3]); else if (s == "c0_qpt") rc = pos(T.c0[4]);
+  else if (s == "s_max") { if (!(v > 0 && v < 1)) return fail(c, TPC_E_ARG, "s_max must be in (0,1)"); T.s_max = v; }
+  else if (s == "n_sigma") rc = pos(T.n_sigma); else if (s == "w_max") rc = pos(T.w_max);
+  else if (s == "max_gap") { if (v < 0 || v > 255) return fail(c, TPC_E_ARG, "max_gap must be in 0..255"); T.max_gap = (int)v; }
+  else if (s == "edge_margin") rc = nonneg(T.edge_margin);
+  else if (s == "min_hits") { if (v < 3 || v > 255) return fail(c, TPC_E_ARG, "min_hits must be in 3..255 (ndf = 2n-5 > 0)"); T.min_hits = (int)v; }
+  else if (s == "grid_scale") rc = pos(T.grid_scale);
+  else if (s == "debug_keep") T.debug_keep = v != 0;
+  else if (s == "chunk") { int k = (int)v; if (k < 32 || k > 4096 || (k & 31)) return fail(c, TPC_E_ARG, "chunk must be a multiple of 32 in 32..4096"); T.chunk = k; }
+  else return fail(c, TPC_E_ARG, "tpc_set_param: unknown parameter '%s'", name);
+  if (rc == TPC_OK) c->rows_valid = false;
+  return rc;
+}
+
+int tpc_clear(tpc_ctx* c) {
+  if (!c) return TPC_E_ARG;
+  cudaStreamSynchronize(c->stream);   // staged device copies may still read caller memory; outputs are about to be invalidated
+  std::fill(c->usrc.begin(), c->usrc.end(), UnitSrc());
+  c->arena_pos = 0; c->dirty.clear(); c->loaded_any = false; c->have_result = false;
+  c->N = 0; c->M = 0; c->n_tracks = 0; c->n_refs = 0;
+  return TPC_OK;
+}
+
+// append n floats per array at the arena position (rounded up to a multiple of 4 elements for 16-byte vector loads)
+static int stage_append(tpc_ctx* c, const float* y, const float* t, long long n, long long* pos_out) {
+  long long pos = (c->arena_pos + 3) & ~3LL;
+  *pos_out = pos;
+  if (n == 0) return TPC_OK;
+  const int ky = pointer_kind(y), kt = pointer_kind(t);
+  if ((ky == 2) != (kt == 2)) return fail(c, TPC_E_ARG, "tpc_load_clusters: pad_y and time must both be host or both be device pointers");
+  const size_t bytes = (size_t)n * sizeof(float), end_bytes = (size_t)(pos + n) * sizeof(float);
+  const bool direct = ky == 2 || (ky == 1 && kt == 1 && n >= (1 << 16));
+  if (direct) {   // device source (D2D) or large pinned source (DMA straight from the caller's buffer), async on the stream
+    const cudaMemcpyKind kind = ky == 2 ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CUDA_TRY(c, c->d_in_y.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4, c->stream));
+    CUDA_TRY(c, c->d_in_t.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_in_y.as<float>() + pos, y, bytes, kind, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_in_t.as<float>() + pos, t, bytes, kind, c->stream));
+  } else {        // pageable (or small) host source: copy into the pinned arena now, upload at tpc_find_tracks
+    CUDA_TRY(c, c->h_y.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4));
+    CUDA_TRY(c, c->h_t.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4));
+    memcpy(c->h_y.as<float>() + pos, y, bytes);
+    memcpy(c->h_t.as<float>() + pos, t, bytes);
+    add_dirty(c, pos, pos + n);
+  }
+  c->arena_pos = pos + n;
+  return TPC_OK;
+}
+
+int tpc_load_clusters(tpc_ctx* c, int sector, int row, const float* pad_y, const float* time, const float* charge, int n) {
+  (void)charge;   // carried by the interface, never read on this path (S0)
+  if (!c) return TPC_E_ARG;
+  if (sector < 0 || sector >= c->NS || row < 0 || row >= c->R) return fail(c, TPC_E_ARG, "tpc_load_clusters: sector %d / row %d out of range", sector, row);
+  if (n < 0 || (n > 0 && (!pad_y || !time))) return fail(c, TPC_E_ARG, "tpc_load_clusters: n < 0 or null array with n > 0");
+  long long pos = 0;
+  int rc = stage_append(c, pad_y, time, n, &pos);
+  if (rc != TPC_OK) return rc;
+  UnitSrc& u = c->usrc[(size_t)sector * c->R + row];
+  u.src = pos; u.n = n;
+  c->loaded_any = true; c->have_result = false;
+  return TPC_OK;
+}
+
+int tpc_load_clusters_batch(tpc_ctx* c, const int64_t* unit_off, const float* pad_y, const float* time, const float* charge) {
+  (void)charge;
+  if (!c) return TPC_E_ARG;
+  if (!unit_off) return fail(c, TPC_E_ARG, "tpc_load_clusters_batch: null unit_off");
+  const int U = c->NS * c->R;
+  if (unit_off[0] < 0) return fail(c, TPC_E_ARG, "tpc_load_clusters_batch: negative offset");
+  for (int u = 0; u < U; u++) {
+    if (unit_off[u + 1] < unit_off[u]) return fail(c, TPC_E_ARG, "tpc_load_clusters_batch: unit_off must be ascending (unit %d)", u);
+    if (unit_off[u + 1] - unit_off[u] > 0x7fffffffLL) return fail(c, TPC_E_CAPACITY, "tpc_load_clusters_batch: more than 2^31-1 clusters in unit %d", u);
+  }
+  const long long n = unit_off[U] - unit_off[0];
+  if (n > 0 && (!pad_y || !time)) return fail(c, TPC_E_ARG, "tpc_load_clusters_batch: null array");
+  std::fill(c->usrc.begin(), c->usrc.end(), UnitSrc());   // replaces everything loaded before
+  c->arena_pos = 0; c->dirty.clear();
+  long long pos = 0;
+  int rc = stage_append(c, pad_y ? pad_y + unit_off[0] : nullptr, time ? time + unit_off[0] : nullptr, n, &pos);
+  if (rc != TPC_OK) return rc;
+  for (int u = 0; u < U; u++) { c->usrc[u].src = pos + (unit_off[u] - unit_off[0]); c->usrc[u].n = (int)(unit_off[u + 1] - unit_off[u]); }
+  c->loaded_any = true; c->have_result = false;
+  return TPC_OK;
+}
+
+}  // extern "C"
+
+// =====================================================================================================================
+// Host-side tables: formulas evaluated in double, rounded to float once.
+namespace {
+
+void make_params_and_rows(tpc_ctx* c, std::vector<RowConst>& rows) {
+  const Tunables& T = c->T; const int R = c->R;
+  rows.assign(R, RowConst());
+  const double dphi = (double)c->dphi;
+  for (int r = 0; r < R; r++) {
+    const double x = c->row_x[r], xu = r + 1 < R ? (double)c->row_x[r + 1] : x, xd = r > 0 ? (double)c->row_x[r - 1] : x;
+    const double a = xu - x, b = x - xd;
+    RowConst& k = rows[r];
+    k.x = (float)x; k.tu = (float)(xu / x); k.td = (float)(xd / x); k.a = (float)a; k.b = (float)b;
+    k.thr = (float)(T.cut2 * 0.5 * (a * a + b * b));
+    k.wzu = (float)(T.dzdx_max * a + T.wz0); k.wzd = (float)(T.dzdx_max * b + T.wz0);
+    k.yedge = (float)(x * tan(0.5 * dphi));
+    k.pad[0] = k.pad[1] = k.pad[2] = 0.f;
+  }
+  Params& P = c->P;
+  P.NS = c->NS; P.R = R; P.continuous = c->t_frame > 0 ? 1 : 0;
+  P.zmax = c->z_max; P.vdrift = c->vdrift;
+  P.wy = (float)T.wy; P.wz = (float)T.wz; P.min_seed = T.min_seed;
+  P.cB = (float)(-0.00299792458 * (double)c->bz);
+  for (int i = 0; i < 5; i++) P.c0[i] = (float)T.c0[i];
+  P.ry = c->sigma_y * c->sigma_y; P.rz = c->sigma_z * c->sigma_z;
+  P.smax = (float)T.s_max; P.nsigma = (float)T.n_sigma; P.wmax = (float)T.w_max; P.edge_margin = (float)T.edge_margin;
+  P.max_gap = T.max_gap; P.min_hits = T.min_hits;
+}
+
+// S1 grid descriptor of every unit + CSR offsets + K2/K3 work items.  Returns a tpc_status.
+int make_units(tpc_ctx* c, int* max_smem_cursor, long long* cursor_total, int* max_n) {
+  const Tunables& T = c->T; const int R = c->R, U = c->NS * R;
+  c->h_units.resize(U); c->h_items.clear();
+  const double dphi = (double)c->dphi, vd = (double)c->vdrift, tf = (double)c->t_frame, zmax = (double)c->z_max;
+  long long off = 0, boff = 0, coff = 0; int msm = 0, mn = 0;
+  for (int u = 0; u < U; u++) {
+    const int r = u % R; const int n = c->usrc[u].n;
+    const double ye = (double)c->row_x[r] * tan(0.5 * dphi);
+    const double y_lo = -ye - 1.0, y_hi = ye + 1.0, z_lo = -vd * tf - 1.0, z_hi = zmax + 1.0;
+    double s = sqrt((y_hi - y_lo) * (z_hi - z_lo) / (double)std::max(n, 1)) * T.grid_scale;
+    s = std::min(std::max(s, T.grid_min), T.grid_max);
+    const double fy = ceil((y_hi - y_lo) / s), fz = ceil((z_hi - z_lo) / s);
+    if (fy * fz > 2.0e9) return fail(c, TPC_E_CAPACITY, "grid of unit %d has more than 2e9 bins", u);
+    UnitDesc& d = c->h_units[u];
+    d.ny = std::max(1, (int)fy); d.nz = std::max(1, (int)fz);
+    d.ylo = (float)y_lo; d.zlo = (float)z_lo; d.invs = (float)(1.0 / s);
+    d.n = n; d.off = off; d.src = c->usrc[u].src; d.bin_off = boff; d.pad[0] = d.pad[1] = 0;
+    const long long nb = (long long)d.ny * d.nz;
+    if (nb + 1 <= K1_SMEM_CURSOR_MAX) { d.cur_off = -1; if (n > 0) msm = std::max(msm, (int)nb + 1); }
+    else { d.cur_off = coff; coff += nb + 1; }
+    for (int s0 = 0; s0 < n; s0 += T.chunk) c->h_items.push_back(Item{u, s0});
+    off += n; boff += nb + 1; mn = std::max(mn, n);
+  }
+  c->N = off; c->n_bins = boff; c->n_items = (int)c->h_items.size();
+  *max_smem_cursor = msm; *cursor_total = coff; *max_n = mn;
+  return TPC_OK;
+}
+
+int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_find_tracks: null argument");
+  memset(out, 0, sizeof(*out));
+  const int R = c->R, U = c->NS * R;
+  cudaStream_t st = c->stream;
+  Launch L{st, c->sm_count};
+  long long launches = 0;
+  c->have_result = false;
+  tpc_timings& tm = c->timings; memset(&tm, 0, sizeof(tm));
+
+  // ---- host tables
+  std::vector<RowConst> rows;
+  make_params_and_rows(c, rows);
+  int msm = 0, max_n = 0; long long cursor_total = 0;
+  int rc = make_units(c, &msm, &cursor_total, &max_n);
+  if (rc != TPC_OK) return rc;
+  const long long N = c->N; const int n_items = c->n_items; const int chunk = c->T.chunk;
+  const Params& P = c->P;
+
+  CUDA_TRY(c, cudaEventRecord(c->ev[0], st));
+  // ---- upload: staged host clusters + tables
+  CUDA_TRY(c, c->d_in_y.ensure_keep((size_t)(c->arena_pos + 16) * 4, (size_t)c->arena_pos * 4, st));
+  CUDA_TRY(c, c->d_in_t.ensure_keep((size_t)(c->arena_pos + 16) * 4, (size_t)c->arena_pos * 4, st));
+  for (auto& rg : c->dirty) {
+    const size_t b = (size_t)(rg.second - rg.first) * 4;
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_in_y.as<float>() + rg.first, c->h_y.as<float>() + rg.first, b, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_in_t.as<float>() + rg.first, c->h_t.as<float>() + rg.first, b, cudaMemcpyHostToDevice, st));
+  }
+  c->dirty.clear();
+  CUDA_TRY(c, c->d_rows.ensure(rows.size() * sizeof(RowConst)));
+  CUDA_TRY(c, c->d_units.ensure((size_t)U * sizeof(UnitDesc)));
+  CUDA_TRY(c, c->d_items.ensure((size_t)std::max(n_items, 1) * sizeof(Item)));
+  CUDA_TRY(c, c->p_units.ensure((size_t)U * sizeof(UnitDesc) + rows.size() * sizeof(RowConst)));
+  CUDA_TRY(c, c->p_items.ensure((size_t)std::max(n_items, 1) * sizeof(Item)));
+  CUDA_TRY(c, c->p_small.ensure(256));
+  memcpy(c->p_units.p, c->h_units.data(), (size_t)U * sizeof(UnitDesc));
+  memcpy((char*)c->p_units.p + (size_t)U * sizeof(UnitDesc), rows.data(), rows.size() * sizeof(RowConst));
+  if (n_items) memcpy(c->p_items.p, c->h_items.data(), (size_t)n_items * sizeof(Item));
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_units.p, c->p_units.p, (size_t)U * sizeof(UnitDesc), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_rows.p, (char*)c->p_units.p + (size_t)U * sizeof(UnitDesc), rows.size() * sizeof(RowConst), cudaMemcpyHostToDevice, st));
+  if (n_items) CUDA_TRY(c, cudaMemcpyAsync(c->d_items.p, c->p_items.p, (size_t)n_items * sizeof(Item), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(c, cudaEventRecord(c->ev[1], st));
+
+  // ---- buffers of S1..S4
+  CUDA_TRY(c, c->d_yz.ensure((size_t)(N + 4) * sizeof(float2)));
+  CUDA_TRY(c, c->d_perm.ensure((size_t)(N + 4) * 4));
+  CUDA_TRY(c, c->d_bin_start.ensure((size_t)(c->n_bins + 8) * 4));
+  CUDA_TRY(c, c->d_cursor.ensure((size_t)(cursor_total + 4) * 4));
+  CUDA_TRY(c, c->d_link_up.ensure((size_t)(N + 4) * 4));
+  CUDA_TRY(c, c->d_link_dn.ensure((size_t)(N + 4) * 4));
+  CUDA_TRY(c, c->d_mask.ensure((size_t)std::max(n_items, 1) * (chunk / 32) * 4));
+  CUDA_TRY(c, c->d_item_count.ensure((size_t)std::max(n_items, 1) * 4));
+  CUDA_TRY(c, c->d_item_base.ensure((size_t)std::max(n_items, 1) * 4));
+  CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(n_items / SCAN_TILE + 4) * 4));
+  const long long start_cap = N / std::max(1, c->T.min_seed) + 4;
+  CUDA_TRY(c, c->d_start_unit.ensure((size_t)start_cap * 4));
+  CUDA_TRY(c, c->d_start_pos.ensure((size_t)start_cap * 4));
+  CUDA_TRY(c, c->d_counters.ensure(256));
+
+  // ---- K1: S0 + S1
+  LAUNCH_TRY(c, launch_k1_grid(L, U, c->d_units.as<UnitDesc>(), c->d_in_y.as<float>(), c->d_in_t.as<float>(), c->d_yz.as<float2>(),
+                               c->d_perm.as<int>(), c->d_bin_start.as<int>(), c->d_cursor.as<int>(), P, std::max(msm, 1), max_n), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[2], st));
+  // ---- K2: S2
+  LAUNCH_TRY(c, launch_k2_neighbours(L, n_items, c->d_items.as<Item>(), chunk, c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
+                                     c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(),
+                                     c->d_link_dn.as<int>(), P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[3], st));
+  if (c->T.debug_keep && N > 0) {
+    CUDA_TRY(c, c->d_raw_up.ensure((size_t)N * 4)); CUDA_TRY(c, c->d_raw_dn.ensure((size_t)N * 4));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_raw_up.p, c->d_link_up.p, (size_t)N * 4, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_raw_dn.p, c->d_link_dn.p, (size_t)N * 4, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(c, cudaEventRecord(c->ev[3], st));
+  }
+  // ---- K3: S3 + S4
+  int* d_nstart = c->d_counters.as<int>();
+  unsigned long long* d_total64 = (unsigned long long*)(c->d_counters.as<char>() + 64);
+  LAUNCH_TRY(c, launch_k3_clean_start(L, n_items, c->d_items.as<Item>(), chunk, c->d_units.as<UnitDesc>(), c->d_link_up.as<int>(),
+                                      c->d_link_dn.as<int>(), c->d_mask.as<unsigned>(), c->d_item_count.as<int>(), c->d_item_base.as<int>(),
+                                      c->d_scan_tmp.as<int>(), c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), d_nstart, P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[4], st));
+  CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  const int M = *c->p_small.as<int>();
+  if (M < 0 || M > start_cap) return fail(c, TPC_E_CUDA, "start-hit count %d out of range", M);
+  if (M > (1 << 24)) return fail(c, TPC_E_CAPACITY, "%d tracklets exceed the 2^24 capacity of the selector key", M);
+  const long long Mpad = ((long long)M + 31) & ~31LL;
+  c->M = M; c->Mpad = Mpad;
+
+  // ---- K5: S5
+  const size_t Mz = (size_t)std::max(M, 1);
+  CUDA_TRY(c, c->d_rowhit.ensure((size_t)std::max(Mpad, 32LL) * R * 4));
+  CUDA_TRY(c, c->d_tl_n.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_first.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_last.ensure(Mz * 4));
+  CUDA_TRY(c, c->d_tl_chi2.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_par.ensure(Mz * 20)); CUDA_TRY(c, c->d_tl_cov.ensure(Mz * 60));
+  CUDA_TRY(c, c->d_owner.ensure((size_t)(N + 4) * 8)); CUDA_TRY(c, c->d_tl_key.ensure(Mz * 8));
+  CUDA_TRY(c, c->d_scan_in.ensure(Mz * 8)); CUDA_TRY(c, c->d_scan_out.ensure(Mz * 8));
+  CUDA_TRY(c, c->d_scan_tmp64.ensure((size_t)(M / SCAN_TILE + 4) * 8));
+  LAUNCH_TRY(c, launch_k5_tracklets(L, M, Mpad, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
+                                    c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
+                                    c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
+                                    c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[5], st));
+
+  // ---- K6: S6
+  typedef unsigned long long u64;
+  LAUNCH_TRY(c, launch_k6_select(L, M, Mpad, N, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
+                                 c->d_perm.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(),
+                                 c->d_tl_chi2.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
+                                 c->d_scan_out.as<u64>(), c->d_scan_tmp64.as<u64>(), d_total64, P), launches);
+  CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 64, d_total64, 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  const u64 total = *(u64*)(c->p_small.as<char>() + 64);
+  const long long nt = (long long)(total >> 40), nr = (long long)(total & ((1ull << 40) - 1ull));
+  c->n_tracks = nt; c->n_refs = nr;
+  const size_t ntz = (size_t)std::max(nt, 1LL), nrz = (size_t)std::max(nr, 1LL);
+  CUDA_TRY(c, c->o_sector.ensure(ntz * 4)); CUDA_TRY(c, c->o_x.ensure(ntz * 4)); CUDA_TRY(c, c->o_par.ensure(ntz * 20));
+  CUDA_TRY(c, c->o_cov.ensure(ntz * 60)); CUDA_TRY(c, c->o_chi2.ensure(ntz * 4)); CUDA_TRY(c, c->o_ndf.ensure(ntz * 4));
+  CUDA_TRY(c, c->o_tracklet.ensure(ntz * 4)); CUDA_TRY(c, c->o_cl_begin.ensure((ntz + 1) * 8));
+  CUDA_TRY(c, c->o_cl_row.ensure(nrz * 4)); CUDA_TRY(c, c->o_cl_index.ensure(nrz * 4));
+  LAUNCH_TRY(c, launch_k6_emit(L, M, Mpad, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_perm.as<int>(),
+                               c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(),
+                               c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
+                               c->d_scan_out.as<u64>(), c->o_sector.as<int>(), c->o_x.as<float>(), c->o_par.as<float>(), c->o_cov.as<float>(),
+                               c->o_chi2.as<float>(), c->o_ndf.as<int>(), c->o_tracklet.as<int>(), c->o_cl_begin.as<long long>(),
+                               c->o_cl_row.as<int>(), c->o_cl_index.as<int>(), nt, nr, P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[6], st));
+
+  // ---- result
+  out->n_tracks = nt; out->n_cluster_refs = nr;
+  if (to_host) {
+    c->ho_sector.resize(ntz); c->ho_x.resize(ntz); c->ho_par.resize(ntz * 5); c->ho_cov.resize(ntz * 15); c->ho_chi2.resize(ntz);
+    c->ho_ndf.resize(ntz); c->ho_tracklet.resize(ntz); c->ho_cl_begin.resize(ntz + 1); c->ho_cl_row.resize(nrz); c->ho_cl_index.resize(nrz);
+    if (nt > 0) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_sector.data(), c->o_sector.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_x.data(), c->o_x.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_par.data(), c->o_par.p, nt * 20, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_cov.data(), c->o_cov.p, nt * 60, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_chi2.data(), c->o_chi2.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_ndf.data(), c->o_ndf.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_tracklet.data(), c->o_tracklet.p, nt * 4, cudaMemcpyDeviceToHost, st));
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(c->ho_cl_begin.data(), c->o_cl_begin.p, (nt + 1) * 8, cudaMemcpyDeviceToHost, st));
+    if (nr > 0) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_cl_row.data(), c->o_cl_row.p, nr * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->ho_cl_index.data(), c->o_cl_index.p, nr * 4, cudaMemcpyDeviceToHost, st));
+    }
+    out->sector = c->ho_sector.data(); out->x = c->ho_x.data(); out->par = c->ho_par.data(); out->cov = c->ho_cov.data();
+    out->chi2 = c->ho_chi2.data(); out->ndf = c->ho_ndf.data(); out->tracklet = c->ho_tracklet.data();
+    out->cl_begin = c->ho_cl_begin.data(); out->cl_row = c->ho_cl_row.data(); out->cl_index = c->ho_cl_index.data();
+  } else {
+    out->sector = c->o_sector.as<int32_t>(); out->x = c->o_x.as<float>(); out->par = c->o_par.as<float>(); out->cov = c->o_cov.as<float>();
+    out->chi2 = c->o_chi2.as<float>(); out->ndf = c->o_ndf.as<int32_t>(); out->tracklet = c->o_tracklet.as<int32_t>();
+    out->cl_begin = c->o_cl_begin.as<int64_t>(); out->cl_row = c->o_cl_row.as<int32_t>(); out->cl_index = c->o_cl_index.as<int32_t>();
+  }
+  CUDA_TRY(c, cudaEventRecord(c->ev[7], st));
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  float* ms[7] = {&tm.ms_upload, &tm.ms_grid, &tm.ms_neighbours, &tm.ms_clean_start, &tm.ms_tracklets, &tm.ms_selector, &tm.ms_download};
+  for (int i = 0; i < 7; i++) CUDA_TRY(c, cudaEventElapsedTime(ms[i], c->ev[i], c->ev[i + 1]));
+  CUDA_TRY(c, cudaEventElapsedTime(&tm.ms_total, c->ev[0], c->ev[7]));
+  tm.n_clusters = N; tm.n_bins = c->n_bins; tm.n_start_hits = M; tm.n_tracks = nt; tm.n_cluster_refs = nr; tm.launches = launches;
+  tm.n_tracklets_kept = -1;
+  c->have_result = true;
+  return TPC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+int tpc_find_tracks(tpc_ctx* c, tpc_tracks* out) { return find_tracks_impl(c, out, true); }
+int tpc_find_tracks_device(tpc_ctx* c, tpc_tracks* out) { return find_tracks_impl(c, out, false); }
+int tpc_get_timings(tpc_ctx* c, tpc_timings* out) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_get_timings: null argument");
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_get_timings: no tpc_find_tracks call has completed");
+  *out = c->timings; return TPC_OK;
+}
+}
+
+// =====================================================================================================================
+// Parity / debug exports: synchronous device -> host copies of intermediate tables of the last call.
+extern "C" {
+
+int tpc_debug_get_grid(tpc_ctx* c, int sector, int row, tpc_grid_view* out) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_debug_get_grid: null argument");
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_debug_get_grid: call tpc_find_tracks first");
+  if (sector < 0 || sector >= c->NS || row < 0 || row >= c->R) return fail(c, TPC_E_ARG, "tpc_debug_get_grid: sector/row out of range");
+  const UnitDesc& d = c->h_units[(size_t)sector * c->R + row];
+  const int nb = d.ny * d.nz;
+  c->dbg_yz.resize((size_t)std::max(d.n, 1) * 2); c->dbg_perm.resize(std::max(d.n, 1)); c->dbg_bins.resize(nb + 1);
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (d.n) {
+    CUDA_TRY(c, cudaMemcpy(c->dbg_yz.data(), c->d_yz.as<float2>() + d.off, (size_t)d.n * 8, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_perm.data(), c->d_perm.as<int>() + d.off, (size_t)d.n * 4, cudaMemcpyDeviceToHost));
+  }
+  CUDA_TRY(c, cudaMemcpy(c->dbg_bins.data(), c->d_bin_start.as<int>() + d.bin_off, (size_t)(nb + 1) * 4, cudaMemcpyDeviceToHost));
+  out->n = d.n; out->ny = d.ny; out->nz = d.nz; out->y_lo = d.ylo; out->z_lo = d.zlo; out->inv_s = d.invs;
+  out->yz = c->dbg_yz.data(); out->perm = c->dbg_perm.data(); out->bin_start = c->dbg_bins.data();
+  return TPC_OK;
+}
+
+int tpc_debug_get_links(tpc_ctx* c, int sector, int row, int cleaned, const int32_t** up, const int32_t** dn, int32_t* n) {
+  if (!c || !up || !dn || !n) return fail(c, TPC_E_ARG, "tpc_debug_get_links: null argument");
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_debug_get_links: call tpc_find_tracks first");
+  if (sector < 0 || sector >= c->NS || row < 0 || row >= c->R) return fail(c, TPC_E_ARG, "tpc_debug_get_links: sector/row out of range");
+  if (!cleaned && !c->T.debug_keep) return fail(c, TPC_E_STATE, "tpc_debug_get_links: pre-cleaning tables need tpc_set_param(debug_keep, 1)");
+  const UnitDesc& d = c->h_units[(size_t)sector * c->R + row];
+  c->dbg_up.resize(std::max(d.n, 1)); c->dbg_dn.resize(std::max(d.n, 1));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (d.n) {
+    const int* su = cleaned ? c->d_link_up.as<int>() : c->d_raw_up.as<int>();
+    const int* sd = cleaned ? c->d_link_dn.as<int>() : c->d_raw_dn.as<int>();
+    CUDA_TRY(c, cudaMemcpy(c->dbg_up.data(), su + d.off, (size_t)d.n * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_dn.data(), sd + d.off, (size_t)d.n * 4, cudaMemcpyDeviceToHost));
+  }
+  *up = c->dbg_up.data(); *dn = c->dbg_dn.data(); *n = d.n;
+  return TPC_OK;
+}
+
+int tpc_debug_get_start_hits(tpc_ctx* c, const int32_t** unit, const int32_t** pos, int64_t* n) {
+  if (!c || !unit || !pos || !n) return fail(c, TPC_E_ARG, "tpc_debug_get_start_hits: null argument");
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_debug_get_start_hits: call tpc_find_tracks first");
+  c->dbg_su.resize(std::max(c->M, 1)); c->dbg_sp.resize(std::max(c->M, 1));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (c->M) {
+    CUDA_TRY(c, cudaMemcpy(c->dbg_su.data(), c->d_start_unit.p, (size_t)c->M * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_sp.data(), c->d_start_pos.p, (size_t)c->M * 4, cudaMemcpyDeviceToHost));
+  }
+  *unit = c->dbg_su.data(); *pos = c->dbg_sp.data(); *n = c->M;
+  return TPC_OK;
+}
+
+int tpc_debug_get_tracklets(tpc_ctx* c, tpc_tracklet_view* out) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_debug_get_tracklets: null argument");
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_debug_get_tracklets: call tpc_find_tracks first");
+  const int M = c->M, R = c->R; const size_t Mz = std::max(M, 1);
+  c->dbg_tl_sector.resize(Mz); c->dbg_tl_row.resize(Mz); c->dbg_tl_n.resize(Mz); c->dbg_tl_first.resize(Mz); c->dbg_tl_last.resize(Mz);
+  c->dbg_tl_chi2.resize(Mz); c->dbg_tl_x.resize(Mz); c->dbg_tl_par.resize(Mz * 5); c->dbg_tl_cov.resize(Mz * 15); c->dbg_rowhit.assign(Mz * R, -1);
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (M) {
+    std::vector<int32_t> su(M), raw((size_t)c->Mpad * R);
+    CUDA_TRY(c, cudaMemcpy(su.data(), c->d_start_unit.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_tl_n.data(), c->d_tl_n.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_tl_first.data(), c->d_tl_first.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_tl_last.data(), c->d_tl_last.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_tl_chi2.data(), c->d_tl_chi2.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_tl_par.data(), c->d_tl_par.p, (size_t)M * 20, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(c->dbg_tl_cov.data(), c->d_tl_cov.p, (size_t)M * 60, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(raw.data(), c->d_rowhit.p, raw.size() * 4, cudaMemcpyDeviceToHost));
+    for (int i = 0; i < M; i++) {
+      c->dbg_tl_sector[i] = su[i] / R; c->dbg_tl_row[i] = su[i] % R; c->dbg_tl_x[i] = c->row_x[c->dbg_tl_first[i]];
+      for (int r = c->dbg_tl_first[i]; r <= c->dbg_tl_last[i]; r++) c->dbg_rowhit[(size_t)r * M + i] = raw[(size_t)r * c->Mpad + i];
+    }
+  }
+  out->n_tracklets = M; out->sector = c->dbg_tl_sector.data(); out->start_row = c->dbg_tl_row.data(); out->n_hits = c->dbg_tl_n.data();
+  out->first_row = c->dbg_tl_first.data(); out->last_row = c->dbg_tl_last.data(); out->chi2 = c->dbg_tl_chi2.data(); out->x = c->dbg_tl_x.data();
+  out->par = c->dbg_tl_par.data(); out->cov = c->dbg_tl_cov.data(); out->rowhit = c->dbg_rowhit.data();
+  return TPC_OK;
+}
+
+}  // extern "C"
