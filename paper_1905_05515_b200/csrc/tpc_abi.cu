@@ -39,6 +39,7 @@ struct DevBuf {
     void* np = nullptr;
     cudaError_t e = cudaMalloc(&np, want);
     if (e != cudaSuccess) return e;
+    keep_bytes = std::min(keep_bytes, cap);
     if (p && keep_bytes) { e = cudaMemcpyAsync(np, p, keep_bytes, cudaMemcpyDeviceToDevice, s); if (e != cudaSuccess) { cudaFree(np); return e; } }
     if (p) { cudaStreamSynchronize(s); cudaFree(p); }
     p = np; cap = want; return cudaSuccess;
@@ -56,6 +57,7 @@ struct PinBuf {
     void* np = nullptr;
     cudaError_t e = cudaMallocHost(&np, want);
     if (e != cudaSuccess) return e;
+    keep_bytes = std::min(keep_bytes, cap);
     if (p && keep_bytes) memcpy(np, p, keep_bytes);
     if (p) cudaFreeHost(p);
     p = np; cap = want; return cudaSuccess;

@@ -1,0 +1,103 @@
+"""GPU-vs-oracle comparison helpers (used by tests/test_gpu_parity.py and __graft_entry__.smoke()).
+
+The oracle gets exactly the values the C ABI carries (geometry scalars rounded to fp32), so that both sides start from
+identical numbers; tunables are doubles on both sides.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from oracle.oracle import Oracle
+
+F32_KEYS = ("sector_dphi", "z_max", "t_frame", "sigma_y", "sigma_z", "bz", "vdrift")
+
+
+def abi_geometry(w) -> dict:
+    """Workload geometry with every scalar rounded to fp32, as tpc_create receives it."""
+    g = dict(w.geometry())
+    for k in F32_KEYS:
+        g[k] = float(np.float32(g[k]))
+    return g
+
+
+def make_oracle(w, **params) -> Oracle:
+    o = Oracle(double=False, **abi_geometry(w), **params)
+    o.load(w.unit_off, w.y, w.t)
+    return o
+
+
+def compare_grid(w, o, trk, units=None) -> int:
+    """Bit-exact S0/S1 tables: grid descriptor, bin_start, perm, sorted (y,z).  Returns the number of units compared."""
+    R = w.n_rows
+    ys, zs, perm = o.get("ys"), o.get("zs"), o.get("perm")
+    bin_off, bin_start = o.get("bin_off"), o.get("bin_start")
+    ny, nz, ylo, zlo, invs = o.get("grid_ny"), o.get("grid_nz"), o.get("grid_ylo"), o.get("grid_zlo"), o.get("grid_invs")
+    units = range(w.n_sectors * R) if units is None else units
+    k = 0
+    for u in units:
+        g = trk.grid(u // R, u % R)
+        a, b = int(w.unit_off[u]), int(w.unit_off[u + 1])
+        assert g["n"] == b - a and g["ny"] == ny[u] and g["nz"] == nz[u], (u, g["n"], g["ny"], g["nz"])
+        assert np.float32(ylo[u]) == g["y_lo"] and np.float32(zlo[u]) == g["z_lo"] and np.float32(invs[u]) == g["inv_s"], u
+        assert np.array_equal(g["bin_start"], bin_start[bin_off[u]:bin_off[u + 1]]), u
+        assert np.array_equal(g["perm"], perm[a:b]), u
+        assert np.array_equal(g["yz"][:, 0], ys[a:b].astype(np.float32)), u
+        assert np.array_equal(g["yz"][:, 1], zs[a:b].astype(np.float32)), u
+        k += 1
+    return k
+
+
+def gather_links(w, trk, cleaned):
+    up = np.full(w.n_clusters, -2, np.int32)
+    dn = np.full(w.n_clusters, -2, np.int32)
+    R = w.n_rows
+    for u in range(w.n_sectors * R):
+        a, b = int(w.unit_off[u]), int(w.unit_off[u + 1])
+        if b > a:
+            up[a:b], dn[a:b] = trk.links(u // R, u % R, cleaned)
+    return up, dn
+
+
+def compare_links(w, o, trk) -> dict:
+    """Raw (S2) and cleaned (S3) link tables and the S4 start list; returns the differing-hit counts (bar: 0)."""
+    out = {}
+    for cleaned, (nu, nd) in ((False, ("link_up", "link_dn")), (True, ("clean_up", "clean_dn"))):
+        up, dn = gather_links(w, trk, cleaned)
+        diff = (up != o.get(nu)) | (dn != o.get(nd))
+        out["cleaned" if cleaned else "raw"] = int(diff.sum())
+    su, sp = trk.start_hits()
+    out["start_equal"] = bool(np.array_equal(su, o.get("start_unit")) and np.array_equal(sp, o.get("start_pos")))
+    out["n_start"] = int(len(su))
+    return out
+
+
+def track_sets(tr) -> dict:
+    """(sector, frozenset of (row, cluster index)) -> track index."""
+    d = {}
+    for i in range(len(tr["sector"])):
+        a, b = int(tr["cl_begin"][i]), int(tr["cl_begin"][i + 1])
+        key = (int(tr["sector"][i]), tuple(zip(tr["cl_row"][a:b].tolist(), tr["cl_index"][a:b].tolist())))
+        d[key] = i
+    return d
+
+
+def compare_tracks(otr, gtr, rel=1e-4, sig=1e-3) -> dict:
+    """Reading A31/A19: pair tracks by (sector, exact cluster set); parameters within rel*|oracle| or sig*sqrt(C_ii)."""
+    so, sg = track_sets(otr), track_sets(gtr)
+    common = [k for k in so if k in sg]
+    n_bad = 0
+    worst = 0.0
+    dcov = np.array([0, 2, 5, 9, 14])
+    for k in common:
+        i, j = so[k], sg[k]
+        po, pg = otr["par"][i].astype(np.float64), np.asarray(gtr["par"][j], dtype=np.float64)
+        so_ = np.sqrt(np.abs(otr["cov"][i][dcov].astype(np.float64)))
+        d = np.abs(po - pg)
+        ok = (d <= rel * np.abs(po)) | (d <= sig * so_)
+        worst = max(worst, float(np.max(d / np.maximum(rel * np.abs(po), sig * so_ + 1e-300))))
+        c2o, c2g = float(otr["chi2"][i]), float(gtr["chi2"][j])
+        if not ok.all() or abs(c2o - c2g) > 1e-3 * max(1.0, abs(c2o)) or int(otr["ndf"][i]) != int(gtr["ndf"][j]) or \
+                float(otr["x"][i]) != float(gtr["x"][j]):
+            n_bad += 1
+    return dict(n_oracle=len(so), n_gpu=len(sg), identical_sets=len(common), frac_identical=len(common) / max(1, len(so)),
+                param_mismatch=n_bad, worst_ratio=worst)

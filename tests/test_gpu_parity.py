@@ -1,0 +1,102 @@
+"""Parity of the CUDA path (through the C ABI) against the fp32 oracle on the same seeded inputs.  All tests need a B200.
+
+Bars (BASELINE.json north_star): S0-S4 tables bit-exact; >= 99.9 % of oracle tracks with an identical
+cluster set on the GPU side; parameters of paired tracks within 1e-4 relative (or 1e-3 sigma near zero, reading A19);
+efficiency / fake rate versus generator truth within 0.1 %.
+"""
+import numpy as np
+import pytest
+
+from gen import workloads as W
+from tests import helpers as H
+from tests import parity as P
+
+pytestmark = pytest.mark.gpu
+
+
+def _tracker(w, **params):
+    import paper_1905_05515_b200 as T
+    return T.Tracker(**P.abi_geometry(w), **params)
+
+
+def _full_parity(w, grid_units=None, per_unit=False, **params):
+    o = P.make_oracle(w, **params).run("s6")
+    with _tracker(w, debug_keep=1, **params) as trk:
+        trk.load_workload(w, per_unit=per_unit)
+        gtr = trk.find_tracks().as_dict()
+        ng = P.compare_grid(w, o, trk, grid_units)
+        lk = P.compare_links(w, o, trk)
+        tm = trk.timings()
+    assert ng > 0
+    assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
+    otr = o.tracks()
+    res = P.compare_tracks(otr, gtr)
+    assert res["frac_identical"] >= 0.999, res
+    assert res["n_gpu"] - res["identical_sets"] <= max(1, 0.001 * res["n_oracle"]), res
+    assert res["param_mismatch"] <= 0.001 * res["n_oracle"], res
+    assert tm["n_clusters"] == w.n_clusters and tm["n_start_hits"] == lk["n_start"] and tm["launches"] >= 10
+    return o, otr, gtr, res
+
+
+def test_c1_full_parity_and_truth():
+    w = W.config(1)
+    o, otr, gtr, res = _full_parity(w)
+    mo, mg = H.truth_metrics(w, otr), H.truth_metrics(w, gtr)
+    assert abs(mo["eff"] - mg["eff"]) <= 1e-3 and abs(mo["fake_rate"] - mg["fake_rate"]) <= 1e-3
+    assert mg["eff"] > 0.95
+
+
+def test_c1_per_unit_loads_equal_batch():
+    w = W.config(1)
+    _full_parity(w, per_unit=True)
+
+
+def test_c2_full_parity():
+    w = W.config(2)
+    rng = np.random.default_rng(0)
+    units = rng.choice(w.n_sectors * w.n_rows, 300, replace=False)
+    o, otr, gtr, res = _full_parity(w, grid_units=units)
+    mo, mg = H.truth_metrics(w, otr), H.truth_metrics(w, gtr)
+    assert abs(mo["eff"] - mg["eff"]) <= 1e-3 and abs(mo["fake_rate"] - mg["fake_rate"]) <= 1e-3
+
+
+def test_c3_scaled_continuous_parity():
+    w = W.config(3, scale=0.1)     # 200 us frame, ~1.2 M clusters, z down to -516 cm
+    rng = np.random.default_rng(1)
+    _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, 200, replace=False))
+
+
+def test_c4_loopers_parity():
+    w = W.config(4)
+    rng = np.random.default_rng(2)
+    _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, 200, replace=False))
+
+
+def test_empty_and_tiny_inputs():
+    w = W.config(1, scale=0.05)
+    with _tracker(w) as trk:
+        r = trk.find_tracks()            # nothing loaded
+        assert r.n_tracks == 0 and r.n_cluster_refs == 0 and len(r.cl_begin) == 1
+        trk.load(0, 5, np.array([1.0], np.float32), np.array([10.0], np.float32))
+        r = trk.find_tracks()
+        assert r.n_tracks == 0
+        trk.clear()
+        trk.load_workload(w)
+        r1 = trk.find_tracks().as_dict()
+        r2 = trk.find_tracks().as_dict()   # same clusters again: identical result (buffers reused)
+        for k in r1:
+            assert np.array_equal(r1[k], r2[k]), k
+
+
+def test_device_inputs_and_device_outputs_match_host_path():
+    import torch
+    w = W.config(1)
+    with _tracker(w) as trk:
+        trk.load_workload(w)
+        host = trk.find_tracks().as_dict()
+    with _tracker(w) as trk:
+        trk.set_stream(torch.cuda.current_stream().cuda_stream)
+        trk.load_batch(w.unit_off, torch.from_numpy(w.y).cuda(), torch.from_numpy(w.t).cuda())
+        dev = trk.find_tracks_device()
+        for k, v in dev.as_dict().items():
+            assert np.array_equal(v.cpu().numpy(), host[k]), k
