@@ -81,6 +81,7 @@ typedef struct {
   float ms_total;           /* first event to last event */
   int64_t n_clusters, n_bins, n_start_hits, n_tracklets_kept, n_tracks, n_cluster_refs;
   int64_t launches;         /* number of kernels of this library launched by the call */
+  int64_t n_propagations, n_updates, n_pickups;   /* S5 work counters: helix transports, Kalman updates, grid pick-ups */
 } tpc_timings;
 
 /* One (sector,row) of the S1 grid, host copies (library-owned), for parity tests. */

@@ -45,7 +45,7 @@ class _Timings(C.Structure):
     _fields_ = [(k, C.c_float) for k in ("ms_upload", "ms_grid", "ms_neighbours", "ms_clean_start", "ms_tracklets",
                                          "ms_selector", "ms_download", "ms_total")] + \
                [(k, C.c_int64) for k in ("n_clusters", "n_bins", "n_start_hits", "n_tracklets_kept", "n_tracks",
-                                         "n_cluster_refs", "launches")]
+                                         "n_cluster_refs", "launches", "n_propagations", "n_updates", "n_pickups")]
 
 
 class _GridView(C.Structure):

@@ -185,9 +185,11 @@ __global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const lo
                                                            const int* __restrict__ link_up, int* __restrict__ rowhit,
                                                            int* __restrict__ tl_n, int* __restrict__ tl_first,
                                                            int* __restrict__ tl_last, float* __restrict__ tl_chi2,
-                                                           float* __restrict__ tl_par, float* __restrict__ tl_cov, const Params P) {
+                                                           float* __restrict__ tl_par, float* __restrict__ tl_cov,
+                                                           unsigned long long* __restrict__ counters, const Params P) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= M) return;
+  int n_prop = 0, n_upd = 1, n_pick = 0;   // work counters (bench: algorithmic flop count of the launch)
   const int R = P.R;
   const int u0 = start_unit[i], h0 = start_pos[i];
   const int sec = u0 / R, r0 = u0 - sec * R;
@@ -212,10 +214,11 @@ __global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const lo
   for (;;) {
     const int up = link_up[su[r].off + h];
     if (up < 0) break;
+    n_prop++;
     if (!propagate(st, rows[r + 1].x - rows[r].x, P)) { ok = false; break; }
     r++; h = up;
     const float2 c = yz[su[r].off + h];
-    update(st, c.x, c.y - zref, P);
+    update(st, c.x, c.y - zref, P); n_upd++;
     rh[(long long)r * Mpad] = h;
     sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = r; c_out = c;
   }
@@ -223,13 +226,14 @@ __global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const lo
   if (ok) {
     int gap = 0;
     for (int rr = r + 1; rr < R; rr++) {
+      n_prop++;
       if (!propagate(st, rows[rr].x - rows[rr - 1].x, P)) break;
       if (fabsf(st.y) > rows[rr].yedge + P.edge_margin) break;
       float2 c;
-      const int p = pickup(su[rr], yz, perm, bin_start, st, zref, P, &c);
+      const int p = pickup(su[rr], yz, perm, bin_start, st, zref, P, &c); n_pick++;
       rh[(long long)rr * Mpad] = p;
       if (p >= 0) {
-        update(st, c.x, c.y - zref, P);
+        update(st, c.x, c.y - zref, P); n_upd++;
         gap = 0; sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = rr; c_out = c;
       } else if (++gap > P.max_gap) break;
     }
@@ -241,6 +245,7 @@ __global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const lo
   chi2 = chi2 + update(st, c_out.x, c_out.y - zref, P); n = 1;
   State snap = st; int r_snap = r_out; int first_assigned = r0; int gap = 0;
   for (int rr = r_out - 1; rr >= 0; rr--) {
+    n_prop++;
     if (!propagate(st, rows[rr].x - rows[rr + 1].x, P)) break;
     const int a = rr >= r0 ? rh[(long long)rr * Mpad] : -1;   // rows below r0 were never visited before
     if (a >= 0) {
@@ -254,7 +259,7 @@ __global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const lo
       continue;
     }
     float2 c;
-    const int p = pickup(su[rr], yz, perm, bin_start, st, zref, P, &c);
+    const int p = pickup(su[rr], yz, perm, bin_start, st, zref, P, &c); n_pick++;
     if (rr < r0 || p >= 0) rh[(long long)rr * Mpad] = p;
     if (p >= 0) {
       chi2 = chi2 + update(st, c.x, c.y - zref, P); n++; snap = st; r_snap = rr;
@@ -271,6 +276,10 @@ __global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const lo
   oc[0] = snap.c00; oc[1] = snap.c10; oc[2] = snap.c11; oc[3] = snap.c20; oc[4] = snap.c21; oc[5] = snap.c22; oc[6] = snap.c30;
   oc[7] = snap.c31; oc[8] = snap.c32; oc[9] = snap.c33; oc[10] = snap.c40; oc[11] = snap.c41; oc[12] = snap.c42; oc[13] = snap.c43;
   oc[14] = snap.c44;
+  n_upd += n;   // phase C updates
+  atomicAdd(&counters[0], (unsigned long long)n_prop);
+  atomicAdd(&counters[1], (unsigned long long)n_upd);
+  atomicAdd(&counters[2], (unsigned long long)n_pick);
 }
 
 }  // namespace
@@ -278,11 +287,11 @@ __global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const lo
 int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
                         const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, const int* d_link_up,
                         int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2, float* d_tl_par,
-                        float* d_tl_cov, const Params& P) {
+                        float* d_tl_cov, unsigned long long* d_counters, const Params& P) {
   if (M <= 0) return 0;
   k5_tracklets<<<(M + K5_THREADS - 1) / K5_THREADS, K5_THREADS, 0, L.stream>>>(M, Mpad, d_start_unit, d_start_pos, d_units, d_rows, d_yz,
                                                                                 d_perm, d_bin_start, d_link_up, d_rowhit, d_tl_n,
-                                                                                d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, P);
+                                                                                d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_counters, P);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }

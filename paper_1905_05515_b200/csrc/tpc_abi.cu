@@ -483,10 +483,12 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, c->d_owner.ensure((size_t)(N + 4) * 8)); CUDA_TRY(c, c->d_tl_key.ensure(Mz * 8));
   CUDA_TRY(c, c->d_scan_in.ensure(Mz * 8)); CUDA_TRY(c, c->d_scan_out.ensure(Mz * 8));
   CUDA_TRY(c, c->d_scan_tmp64.ensure((size_t)(M / SCAN_TILE + 4) * 8));
+  unsigned long long* d_k5cnt = (unsigned long long*)(c->d_counters.as<char>() + 128);
+  CUDA_TRY(c, cudaMemsetAsync(d_k5cnt, 0, 24, st));
   LAUNCH_TRY(c, launch_k5_tracklets(L, M, Mpad, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
                                     c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
                                     c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
-                                    c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), P), launches);
+                                    c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt, P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[5], st));
 
   // ---- K6: S6
@@ -496,6 +498,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
                                  c->d_tl_chi2.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
                                  c->d_scan_out.as<u64>(), c->d_scan_tmp64.as<u64>(), d_total64, P), launches);
   CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 64, d_total64, 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 128, d_k5cnt, 24, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(c, cudaStreamSynchronize(st));
   const u64 total = *(u64*)(c->p_small.as<char>() + 64);
   const long long nt = (long long)(total >> 40), nr = (long long)(total & ((1ull << 40) - 1ull));
@@ -547,6 +550,8 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, cudaEventElapsedTime(&tm.ms_total, c->ev[0], c->ev[7]));
   tm.n_clusters = N; tm.n_bins = c->n_bins; tm.n_start_hits = M; tm.n_tracks = nt; tm.n_cluster_refs = nr; tm.launches = launches;
   tm.n_tracklets_kept = -1;
+  { const unsigned long long* k5 = (const unsigned long long*)(c->p_small.as<char>() + 128);
+    tm.n_propagations = (int64_t)k5[0]; tm.n_updates = (int64_t)k5[1]; tm.n_pickups = (int64_t)k5[2]; }
   c->have_result = true;
   return TPC_OK;
 }

@@ -100,7 +100,7 @@ int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int
 int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
                         const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, const int* d_link_up,
                         int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2, float* d_tl_par,
-                        float* d_tl_cov, const Params& P);
+                        float* d_tl_cov, unsigned long long* d_counters, const Params& P);
 
 int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const int* d_start_unit, const UnitDesc* d_units,
                      const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
