@@ -1,0 +1,249 @@
+"""bench.py -- TPC clusters/s and Pb-Pb collisions/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl reference]
+
+A step = one pass of the whole hot path (S0..S6: K1 grid, K2 neighbours, K3 clean/start, K5 tracklets, K6 selector) over one
+synthetic time frame.  Default workload: config C3 (2 ms continuous frame at 50 kHz, ~12.5 M clusters, ~93 collisions).
+`value`: clusters/s with the clusters already resident in HBM (tpc_find_tracks_device, results stay on the device).
+`e2e`:   same metric through the C ABI with HOST buffers: pinned host -> device copy of (pad-y, time), all kernels, and the
+         device -> host copy of the tracks, every step.
+N > 1 (torchrun): every rank processes its own time frame (seed 3+rank) -- independent units, no data-path collective, weak
+scaling; time = max over ranks.  --impl reference: the CPU oracle (oracle/), as it stands, on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "tpc_clusters_per_s"
+UNIT = "clusters/s"
+# algorithmic HBM bytes per cluster
+BYTES_PER_CLUSTER = {"grid": 24.0, "neighbours": 20.0, "clean_start": 24.0}
+# fp32 operations (no FMA: one flop per instruction) per S5 primitive, counted from k5_tracklets.cu
+FLOP_PROPAGATE, FLOP_UPDATE, FLOP_PICKUP = 170.0, 132.0, 28.0
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_ev = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_ev.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self._stop_ev.wait(0.1)
+
+    def stop(self):
+        self._stop_ev.set()
+        self.join(timeout=6)
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+def oracle_run(w, sectors):
+    """The oracle as it stands on a sector sample of the workload; returns (seconds, clusters, cores)."""
+    from tests import parity as P
+    ws = w.sector_slice(sectors)
+    o = P.make_oracle(ws)
+    t0 = time.perf_counter()
+    o.run("s6")
+    return time.perf_counter() - t0, ws.n_clusters, 1
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    from gen import workloads as W
+    w = W.config(args.config, seed=args.config)
+    sectors = list(range(args.ref_sectors))
+    times, n = [], 0
+    for i in range(args.warmup + args.steps):
+        dt, n, cores = oracle_run(w, sectors)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    v = n / (ms * 1e-3)
+    sample = f"sectors 0..{args.ref_sectors - 1} of C{args.config} ({n} clusters) per step, full S0..S6, fp32 oracle instance"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "f32", "data": "synthetic", "config": {"workload": f"C{args.config}", "sample": sample},
+                      "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+def run_gpu(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    import paper_1905_05515_b200 as T
+    from gen import workloads as W
+
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    w = W.config(args.config, seed=args.config + rank)          # every rank its own time frame (weak scaling)
+    N = w.n_clusters
+    stream = torch.cuda.current_stream()
+    trk = T.Tracker(**w.geometry())
+    trk.set_stream(stream.cuda_stream)
+    y_d, t_d = torch.from_numpy(w.y).cuda(), torch.from_numpy(w.t).cuda()
+    y_h, t_h = torch.from_numpy(w.y).pin_memory(), torch.from_numpy(w.t).pin_memory()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    # ---- device-resident arm: `value`
+    trk.load_batch(w.unit_off, y_d, t_d)
+    for _ in range(args.warmup):
+        res = trk.find_tracks_device()
+    keys = ("ms_grid", "ms_neighbours", "ms_clean_start", "ms_tracklets", "ms_selector")
+    acc = {k: 0.0 for k in keys}
+    barrier()
+    sampler = ClockSampler(local_rank); sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    launches = 0
+    for _ in range(args.steps):
+        res = trk.find_tracks_device()
+        tm = trk.timings()
+        launches += tm["launches"]
+        for k in keys:
+            acc[k] += tm[k]
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    total_clusters = sum_over_ranks(float(N))
+    total_colls = sum_over_ranks(float(w.n_collisions))
+    value = total_clusters / (ms * 1e-3)
+    kern = {k: acc[k] / args.steps for k in keys}
+    n_tracks, n_refs = res.n_tracks, res.n_cluster_refs
+
+    # ---- end-to-end arm: host buffers in, host tracks out, every step
+    for _ in range(min(args.warmup, 3)):
+        trk.load_batch(w.unit_off, y_h, t_h); trk.find_tracks()
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        trk.load_batch(w.unit_off, y_h, t_h)
+        hres = trk.find_tracks()
+    e1.record(stream)
+    barrier()
+    ms_e2e = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    h2d = 2 * 4 * N
+    d2h = hres.n_tracks * (4 + 4 + 20 + 60 + 4 + 4 + 4) + (hres.n_tracks + 1) * 8 + hres.n_cluster_refs * 8
+    trk.close()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of every kernel; the dominant one goes into "roofline"
+    hbm_peak, peak_src, sm_max = _peaks()
+    alu_peak = 148 * 128 * sm_max * 1e6 / 1e12      # TFLOP/s, one fp32 op per lane per clock (FMA contraction is off)
+    traffic = {}
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp))
+    roofs = {}
+    for name, key in (("grid", "ms_grid"), ("neighbours", "ms_neighbours"), ("clean_start", "ms_clean_start")):
+        a = BYTES_PER_CLUSTER[name] * N / (kern[key] * 1e-3) / 1e9
+        roofs[name] = {"bound": "hbm", "achieved": a, "peak": hbm_peak, "unit": "GB/s", "frac": a / hbm_peak, "peak_source": peak_src,
+                       "ms": kern[key], "traffic": traffic.get(name)}
+    flops = FLOP_PROPAGATE * tm["n_propagations"] + FLOP_UPDATE * tm["n_updates"] + FLOP_PICKUP * tm["n_pickups"]
+    a = flops / (kern["ms_tracklets"] * 1e-3) / 1e12
+    roofs["tracklets"] = {"bound": "alu", "achieved": a, "peak": alu_peak, "unit": "TFLOP/s", "frac": a / alu_peak,
+                          "peak_source": "148 SM x 128 fp32 lanes x sm_max_mhz, no FMA (DESIGN.md section 8)", "ms": kern["ms_tracklets"],
+                          "traffic": traffic.get("tracklets")}
+    roofs["selector"] = {"bound": "hbm", "achieved": None, "peak": hbm_peak, "unit": "GB/s", "frac": None, "ms": kern["ms_selector"],
+                         "traffic": traffic.get("selector")}
+    dominant = max(("grid", "neighbours", "clean_start", "tracklets"), key=lambda k: roofs[k]["ms"])
+    roofline = dict(roofs[dominant]); roofline["kernel"] = dominant
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        dt, n, cores = oracle_run(w, list(range(args.ref_sectors)))
+        cpu = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": f"sectors 0..{args.ref_sectors - 1} of C{args.config} ({n} clusters), full S0..S6, fp32 oracle instance, 1 thread"}
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": f"C{args.config}: {w.params.t_frame:g} us frame, {N} clusters, {w.n_collisions} collisions per GPU",
+                      "l2": "inputs+tables larger than L2 (no flush needed)" if N * 40 > 126e6 else "working set fits L2",
+                      "parallelism": f"{world} independent time frames"},
+           "collisions_per_s": total_colls / (ms * 1e-3), "tracks_per_step": n_tracks, "cluster_refs_per_step": n_refs,
+           "realtime_factor": (w.params.t_frame * 1e-3 * world) / ms if w.params.t_frame > 0 else None,
+           "e2e": {"value": total_clusters / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d,
+                   "d2h_bytes_per_step": d2h},
+           "gpu_launches": int(launches), "kernel_ms": kern, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
+           "clocks": clocks}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="workload preset C1..C5 (default C3, the 50 kHz time frame)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-sectors", type=int, default=4, help="sectors of the workload the CPU oracle is timed on")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+    run_gpu(args, rank, world, local)
+
+
+if __name__ == "__main__":
+    main()
