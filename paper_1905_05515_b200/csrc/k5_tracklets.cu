@@ -1,14 +1,15 @@
 // k5_tracklets.cu -- K5: S5 Kalman-filter tracklet constructor ("first preliminary fit, used to find the full track";
 // PAPER.md:41 single hypothesis per seed, linear in the event size; definition in DESIGN.md section 4).
 //
-// One thread per tracklet (= start hit).  The 5-parameter state (y, z_rel, sin phi, dz/ds, q/pT) and the 15 covariance
+// One lane per tracklet (= start hit) at a time, persistent CTAs with a global work queue.  The 5-parameter state (y, z_rel, sin phi, dz/ds, q/pT) and the 15 covariance
 // entries live in registers, fp32.  Phases: A seed fit along the cleaned up-links, B outward extrapolation row by row in the
 // uniform Bz helix with cluster pick-up from the S1 grid, C inward refit + inward extrapolation.  z is carried relative to the
 // start hit (z_rel = z - z_ref, formed in fp32 before use) so that long continuous time frames (|z| up to 2.6e4 cm) keep
 // full fp32 resolution.  Arithmetic is written term by term in the documented order and compiled without FMA contraction,
 // so pick-up decisions agree with the fp32 definition.
-// rowhit layout: [row][tracklet] (Mpad columns) -> a warp working on one row writes one coalesced line.  Only rows between the
-// first and the last row a tracklet visits are written; tl_first / tl_last delimit the valid range (no memset of the table).
+// rowhit layout: [tracklet][row]: a lane writes and re-reads consecutive rows of its own tracklet (L2-resident while the tracklet
+// is alive).  Only rows between the first and the last row a tracklet visits are written; tl_first / tl_last delimit the valid
+// range (no memset of the table).
 #include "tpc_internal.cuh"
 
 namespace tpc {
@@ -178,108 +179,164 @@ __device__ __forceinline__ int pickup(const UnitDesc& d, const float2* __restric
   return best;
 }
 
-__global__ void __launch_bounds__(K5_THREADS) k5_tracklets(const int M, const long long Mpad, const int* __restrict__ start_unit,
-                                                           const int* __restrict__ start_pos, const UnitDesc* __restrict__ units,
-                                                           const RowConst* __restrict__ rows, const float2* __restrict__ yz,
-                                                           const int* __restrict__ perm, const int* __restrict__ bin_start,
-                                                           const int* __restrict__ link_up, int* __restrict__ rowhit,
-                                                           int* __restrict__ tl_n, int* __restrict__ tl_first,
-                                                           int* __restrict__ tl_last, float* __restrict__ tl_chi2,
-                                                           float* __restrict__ tl_par, float* __restrict__ tl_cov,
-                                                           unsigned long long* __restrict__ counters, const Params P) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= M) return;
-  int n_prop = 0, n_upd = 1, n_pick = 0;   // work counters (bench: algorithmic flop count of the launch)
-  const int R = P.R;
-  const int u0 = start_unit[i], h0 = start_pos[i];
-  const int sec = u0 / R, r0 = u0 - sec * R;
-  const UnitDesc* __restrict__ su = units + (long long)sec * R;   // units of this sector, indexed by row
-  int* __restrict__ rh = rowhit + i;                              // rh[r * Mpad]
 
-  const float2 c0 = yz[su[r0].off + h0];
-  const float zref = c0.y;
-  State st;
-  {
-    const float x = rows[r0].x, y = c0.x;
-    const float rr = sqrtf(x * x + y * y);
-    st.y = y; st.z = 0.0f; st.s = y / rr; st.t = P.continuous ? 0.0f : zref / rr; st.q = 0.0f;
-    reset_cov(st, P);
-  }
-  update(st, c0.x, 0.0f, P);
-  rh[(long long)r0 * Mpad] = h0;
-  int r = r0, h = h0; bool ok = true;
-  float sv_y = st.y, sv_z = st.z, sv_s = st.s, sv_t = st.t, sv_q = st.q;   // state after the last update (covariance is reset in C)
-  int r_out = r0; float2 c_out = c0;
-  // ---- Phase A: follow the cleaned up-links, no gate
+// Per-lane modes of the row-step state machine.  Every loop iteration of a warp is ONE row step for every lane: (maybe) transport,
+// select the measurement for the row, (maybe) Kalman update, bookkeeping.  Lanes in different phases of different tracklets
+// therefore execute the same transport / update instruction streams together; a lane that finishes a tracklet pulls the next
+// one from a global work queue (persistent CTAs), so short and long tracklets balance out.
+enum : int { MD_FETCH = 0, MD_INIT, MD_A, MD_B, MD_TRANS, MD_C, MD_EXIT };
+
+__global__ void __launch_bounds__(K5_THREADS, 4) k5_tracklets(const int M, const int* __restrict__ start_unit,
+                                                              const int* __restrict__ start_pos, const UnitDesc* __restrict__ units,
+                                                              const RowConst* __restrict__ rows, const float2* __restrict__ yz,
+                                                              const int* __restrict__ perm, const int* __restrict__ bin_start,
+                                                              const int* __restrict__ link_up, int* __restrict__ rowhit,
+                                                              int* __restrict__ tl_n, int* __restrict__ tl_first,
+                                                              int* __restrict__ tl_last, float* __restrict__ tl_chi2,
+                                                              float* __restrict__ tl_par, float* __restrict__ tl_cov,
+                                                              unsigned long long* __restrict__ counters, int* __restrict__ queue,
+                                                              const Params P) {
+  const unsigned FULL = 0xffffffffu;
+  const int R = P.R, lane = threadIdx.x & 31;
+  int mode = MD_FETCH;
+  int i = -1, r0 = 0, h0 = 0, r = 0, nxt = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
+  float zref = 0.0f, chi2 = 0.0f;
+  float2 c0 = make_float2(0.f, 0.f), c_out = c0;
+  float sv_y = 0.f, sv_z = 0.f, sv_s = 0.f, sv_t = 0.f, sv_q = 0.f;
+  State st = {}, snap = {};
+  const UnitDesc* __restrict__ su = units;
+  int* __restrict__ rh = rowhit;
+  unsigned n_prop = 0, n_upd = 0, n_pick = 0;
+
   for (;;) {
-    const int up = link_up[su[r].off + h];
-    if (up < 0) break;
-    n_prop++;
-    if (!propagate(st, rows[r + 1].x - rows[r].x, P)) { ok = false; break; }
-    r++; h = up;
-    const float2 c = yz[su[r].off + h];
-    update(st, c.x, c.y - zref, P); n_upd++;
-    rh[(long long)r * Mpad] = h;
-    sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = r; c_out = c;
-  }
-  // ---- Phase B: extrapolate outward with pick-up
-  if (ok) {
-    int gap = 0;
-    for (int rr = r + 1; rr < R; rr++) {
-      n_prop++;
-      if (!propagate(st, rows[rr].x - rows[rr - 1].x, P)) break;
-      if (fabsf(st.y) > rows[rr].yedge + P.edge_margin) break;
-      float2 c;
-      const int p = pickup(su[rr], yz, perm, bin_start, st, zref, P, &c); n_pick++;
-      rh[(long long)rr * Mpad] = p;
-      if (p >= 0) {
-        update(st, c.x, c.y - zref, P); n_upd++;
-        gap = 0; sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = rr; c_out = c;
-      } else if (++gap > P.max_gap) break;
+    // ---- work queue: lanes without a tracklet take the next start hits (one atomic per warp)
+    const unsigned need = __ballot_sync(FULL, mode == MD_FETCH);
+    if (need) {
+      const int leader = __ffs(need) - 1;
+      int base = 0;
+      if (lane == leader) base = atomicAdd(queue, __popc(need));
+      base = __shfl_sync(FULL, base, leader);
+      if (mode == MD_FETCH) {
+        i = base + __popc(need & ((1u << lane) - 1u));
+        if (i < M) {
+          const int u0 = start_unit[i];
+          h0 = start_pos[i];
+          const int sec = u0 / R;
+          r0 = u0 - sec * R;
+          su = units + (long long)sec * R;
+          rh = rowhit + (long long)i * R;
+          c0 = yz[su[r0].off + h0];
+          zref = c0.y;
+          mode = MD_INIT;
+        } else {
+          mode = MD_EXIT;
+        }
+      }
+    }
+    if (__all_sync(FULL, mode == MD_EXIT)) break;
+
+    // ---- 1. transport to the next row (phases A, B outward; C inward)
+    const bool moving = mode == MD_A || mode == MD_B || mode == MD_C;
+    const int rn = mode == MD_C ? r - 1 : r + 1;
+    bool prop_ok = true;
+    if (moving) { n_prop++; prop_ok = propagate(st, rows[rn].x - rows[r].x, P); }
+
+    // ---- 2. measurement for this step
+    bool have = false, finish = false;
+    float2 c = c0;
+    int hit = -1, row = rn;
+    if (mode == MD_INIT) {          // Phase A start: direction from the origin, first update with the start hit
+      const float x = rows[r0].x, y = c0.x;
+      const float rr = sqrtf(x * x + y * y);
+      st.y = y; st.z = 0.0f; st.s = y / rr; st.t = P.continuous ? 0.0f : zref / rr; st.q = 0.0f;
+      reset_cov(st, P);
+      have = true; hit = h0; row = r0;
+    } else if (mode == MD_A) {      // follow the cleaned up-link, no gate
+      if (!prop_ok) mode = MD_TRANS;
+      else { hit = nxt; c = yz[su[rn].off + hit]; have = true; }
+    } else if (mode == MD_B) {      // outward extrapolation with pick-up
+      if (!prop_ok || fabsf(st.y) > rows[rn].yedge + P.edge_margin) mode = MD_TRANS;
+      else {
+        n_pick++;
+        hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c);
+        rh[rn] = hit;
+        have = hit >= 0;
+        r = rn;
+        if (!have && ++gap > P.max_gap) mode = MD_TRANS;
+      }
+    } else if (mode == MD_TRANS) {  // Phase C start: state after the outermost update, fresh covariance, refit inward
+      st.y = sv_y; st.z = sv_z; st.s = sv_s; st.t = sv_t; st.q = sv_q;
+      reset_cov(st, P);
+      chi2 = 0.0f; n = 0; first_assigned = r0; gap = 0;
+      c = c_out; have = true; row = r_out; r = r_out;
+    } else if (mode == MD_C) {
+      if (!prop_ok) finish = true;
+      else {
+        const int a = rn >= r0 ? rh[rn] : -1;   // rows below r0 were never visited before
+        r = rn;
+        if (a >= 0) { hit = a; c = yz[su[rn].off + a]; have = true; }
+        else if (fabsf(st.y) > rows[rn].yedge + P.edge_margin) {
+          if (rn < first_assigned) finish = true;
+          else if (rn < r0) rh[rn] = -1;       // skipped row inside the tracklet's range: reads as "no cluster"
+        } else {
+          n_pick++;
+          hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c);
+          if (rn < r0 || hit >= 0) rh[rn] = hit;
+          have = hit >= 0;
+          if (have) { if (rn < first_assigned) { first_assigned = rn; gap = 0; } }
+          else if (rn < first_assigned && ++gap > P.max_gap) finish = true;
+        }
+      }
+    }
+
+    // ---- 3. Kalman update (all lanes that have a measurement, whatever their phase)
+    float dchi = 0.0f;
+    if (have) { n_upd++; dchi = update(st, c.x, c.y - zref, P); }
+
+    // ---- 4. bookkeeping and phase transitions
+    if (mode == MD_INIT) {
+      rh[r0] = h0; r = r0;
+      sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = r0; c_out = c0;
+      nxt = link_up[su[r0].off + h0];
+      gap = 0;
+      mode = nxt >= 0 ? MD_A : (r0 + 1 < R ? MD_B : MD_TRANS);
+    } else if (mode == MD_A) {      // (a failed transport already switched the lane to MD_TRANS)
+      r = rn; rh[rn] = hit;
+      sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = rn; c_out = c;
+      nxt = link_up[su[rn].off + hit];
+      if (nxt < 0) { gap = 0; mode = rn + 1 < R ? MD_B : MD_TRANS; }
+    } else if (mode == MD_B) {
+      if (have) { gap = 0; sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = rn; c_out = c; }
+      if (rn + 1 >= R) mode = MD_TRANS;
+    } else if (mode == MD_TRANS) {
+      if (have) {                   // (have is false only for lanes that switched to MD_TRANS in step 2 of this iteration)
+        chi2 = chi2 + dchi; n = 1; snap = st; r_snap = r_out;
+        if (r_out - 1 >= 0) mode = MD_C; else finish = true;
+      }
+    } else if (mode == MD_C) {
+      if (have) { chi2 = chi2 + dchi; n++; snap = st; r_snap = rn; }
+      if (!finish && rn == 0) finish = true;
+    }
+
+    if (finish) {   // tracklet complete: hits exist exactly on the rows [r_snap, r_out] that carry a non-negative rowhit
+      tl_n[i] = n; tl_first[i] = r_snap; tl_last[i] = r_out; tl_chi2[i] = chi2;
+      float* __restrict__ op = tl_par + (long long)i * 5;
+      op[0] = snap.y; op[1] = snap.z + zref; op[2] = snap.s; op[3] = snap.t; op[4] = snap.q;
+      float* __restrict__ oc = tl_cov + (long long)i * 15;
+      oc[0] = snap.c00; oc[1] = snap.c10; oc[2] = snap.c11; oc[3] = snap.c20; oc[4] = snap.c21; oc[5] = snap.c22; oc[6] = snap.c30;
+      oc[7] = snap.c31; oc[8] = snap.c32; oc[9] = snap.c33; oc[10] = snap.c40; oc[11] = snap.c41; oc[12] = snap.c42; oc[13] = snap.c43;
+      oc[14] = snap.c44;
+      mode = MD_FETCH;
     }
   }
-  // ---- Phase C: inward refit from the outermost assigned hit, then extrapolate inward
-  st.y = sv_y; st.z = sv_z; st.s = sv_s; st.t = sv_t; st.q = sv_q;
-  reset_cov(st, P);
-  float chi2 = 0.0f; int n = 0;
-  chi2 = chi2 + update(st, c_out.x, c_out.y - zref, P); n = 1;
-  State snap = st; int r_snap = r_out; int first_assigned = r0; int gap = 0;
-  for (int rr = r_out - 1; rr >= 0; rr--) {
-    n_prop++;
-    if (!propagate(st, rows[rr].x - rows[rr + 1].x, P)) break;
-    const int a = rr >= r0 ? rh[(long long)rr * Mpad] : -1;   // rows below r0 were never visited before
-    if (a >= 0) {
-      const float2 c = yz[su[rr].off + a];
-      chi2 = chi2 + update(st, c.x, c.y - zref, P); n++; snap = st; r_snap = rr;
-      continue;
-    }
-    if (fabsf(st.y) > rows[rr].yedge + P.edge_margin) {
-      if (rr < first_assigned) break;
-      if (rr < r0) rh[(long long)rr * Mpad] = -1;   // skipped row inside the tracklet's range: must read as "no cluster"
-      continue;
-    }
-    float2 c;
-    const int p = pickup(su[rr], yz, perm, bin_start, st, zref, P, &c); n_pick++;
-    if (rr < r0 || p >= 0) rh[(long long)rr * Mpad] = p;
-    if (p >= 0) {
-      chi2 = chi2 + update(st, c.x, c.y - zref, P); n++; snap = st; r_snap = rr;
-      if (rr < first_assigned) { first_assigned = rr; gap = 0; }
-    } else if (rr < first_assigned) {
-      if (++gap > P.max_gap) break;
-    }
+  // work counters: one atomic per warp
+  for (int d = 16; d > 0; d >>= 1) {
+    n_prop += __shfl_down_sync(FULL, n_prop, d); n_upd += __shfl_down_sync(FULL, n_upd, d); n_pick += __shfl_down_sync(FULL, n_pick, d);
   }
-  // hits exist only in [r_snap, r_out]: every visited row carrying a hit produced an update, rows never reached are outside.
-  tl_n[i] = n; tl_first[i] = r_snap; tl_last[i] = r_out; tl_chi2[i] = chi2;
-  float* __restrict__ op = tl_par + (long long)i * 5;
-  op[0] = snap.y; op[1] = snap.z + zref; op[2] = snap.s; op[3] = snap.t; op[4] = snap.q;
-  float* __restrict__ oc = tl_cov + (long long)i * 15;
-  oc[0] = snap.c00; oc[1] = snap.c10; oc[2] = snap.c11; oc[3] = snap.c20; oc[4] = snap.c21; oc[5] = snap.c22; oc[6] = snap.c30;
-  oc[7] = snap.c31; oc[8] = snap.c32; oc[9] = snap.c33; oc[10] = snap.c40; oc[11] = snap.c41; oc[12] = snap.c42; oc[13] = snap.c43;
-  oc[14] = snap.c44;
-  n_upd += n;   // phase C updates
-  atomicAdd(&counters[0], (unsigned long long)n_prop);
-  atomicAdd(&counters[1], (unsigned long long)n_upd);
-  atomicAdd(&counters[2], (unsigned long long)n_pick);
+  if (lane == 0) {
+    atomicAdd(&counters[0], (unsigned long long)n_prop); atomicAdd(&counters[1], (unsigned long long)n_upd);
+    atomicAdd(&counters[2], (unsigned long long)n_pick);
+  }
 }
 
 }  // namespace
@@ -288,11 +345,20 @@ int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_sta
                         const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, const int* d_link_up,
                         int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2, float* d_tl_par,
                         float* d_tl_cov, unsigned long long* d_counters, const Params& P) {
+  (void)Mpad;
   if (M <= 0) return 0;
-  k5_tracklets<<<(M + K5_THREADS - 1) / K5_THREADS, K5_THREADS, 0, L.stream>>>(M, Mpad, d_start_unit, d_start_pos, d_units, d_rows, d_yz,
-                                                                                d_perm, d_bin_start, d_link_up, d_rowhit, d_tl_n,
-                                                                                d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_counters, P);
-  cudaError_t e = cudaGetLastError();
+  int* d_queue = reinterpret_cast<int*>(d_counters + 3);   // work-queue head, zeroed with the counters by the caller
+  int per_sm = 0;
+  cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k5_tracklets, K5_THREADS, 0);
+  if (e != cudaSuccess) return -(int)e;
+  if (per_sm < 1) per_sm = 1;
+  int blocks = L.sm_count * per_sm;                         // persistent CTAs: one resident wave
+  const int need = (M + K5_THREADS - 1) / K5_THREADS;
+  if (blocks > need) blocks = need;
+  k5_tracklets<<<blocks, K5_THREADS, 0, L.stream>>>(M, d_start_unit, d_start_pos, d_units, d_rows, d_yz, d_perm, d_bin_start, d_link_up,
+                                                    d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_counters,
+                                                    d_queue, P);
+  e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }
 

@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const long l
   const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
   const int r1 = tl_last[i];
   for (int r = tl_first[i]; r <= r1; r++) {
-    const int p = rowhit[(long long)r * Mpad + i];
+    const int p = rowhit[(long long)i * R + r];
     if (p >= 0) atomicMax(&owner[su[r].off + p], key);
   }
 }
@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const long l
     const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
     const int r1 = tl_last[i];
     for (int r = tl_first[i]; r <= r1; r++) {
-      const int p = rowhit[(long long)r * Mpad + i];
+      const int p = rowhit[(long long)i * R + r];
       if (p >= 0 && owner[su[r].off + p] == key) owned++;
     }
   }
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const long lo
 #pragma unroll
   for (int j = 0; j < 15; j++) o_cov[t * 15 + j] = tl_cov[(long long)i * 15 + j];
   for (int r = r0; r <= r1; r++) {
-    const int p = rowhit[(long long)r * Mpad + i];
+    const int p = rowhit[(long long)i * R + r];
     if (p < 0) continue;
     const long long g = su[r].off + p;
     if (owner[g] == key) { o_cl_row[k] = r; o_cl_index[k] = perm[g]; k++; }

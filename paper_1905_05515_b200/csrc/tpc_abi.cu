@@ -484,7 +484,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, c->d_scan_in.ensure(Mz * 8)); CUDA_TRY(c, c->d_scan_out.ensure(Mz * 8));
   CUDA_TRY(c, c->d_scan_tmp64.ensure((size_t)(M / SCAN_TILE + 4) * 8));
   unsigned long long* d_k5cnt = (unsigned long long*)(c->d_counters.as<char>() + 128);
-  CUDA_TRY(c, cudaMemsetAsync(d_k5cnt, 0, 24, st));
+  CUDA_TRY(c, cudaMemsetAsync(d_k5cnt, 0, 32, st));
   LAUNCH_TRY(c, launch_k5_tracklets(L, M, Mpad, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
                                     c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
                                     c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
@@ -640,7 +640,7 @@ int tpc_debug_get_tracklets(tpc_ctx* c, tpc_tracklet_view* out) {
     CUDA_TRY(c, cudaMemcpy(raw.data(), c->d_rowhit.p, raw.size() * 4, cudaMemcpyDeviceToHost));
     for (int i = 0; i < M; i++) {
       c->dbg_tl_sector[i] = su[i] / R; c->dbg_tl_row[i] = su[i] % R; c->dbg_tl_x[i] = c->row_x[c->dbg_tl_first[i]];
-      for (int r = c->dbg_tl_first[i]; r <= c->dbg_tl_last[i]; r++) c->dbg_rowhit[(size_t)r * M + i] = raw[(size_t)r * c->Mpad + i];
+      for (int r = c->dbg_tl_first[i]; r <= c->dbg_tl_last[i]; r++) c->dbg_rowhit[(size_t)r * M + i] = raw[(size_t)i * R + r];
     }
   }
   out->n_tracklets = M; out->sector = c->dbg_tl_sector.data(); out->start_row = c->dbg_tl_row.data(); out->n_hits = c->dbg_tl_n.data();
