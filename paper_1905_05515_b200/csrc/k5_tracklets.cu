@@ -235,63 +235,69 @@ __global__ void __launch_bounds__(K5_THREADS, 4) k5_tracklets(const int M, const
     }
     if (__all_sync(FULL, mode == MD_EXIT)) break;
 
-    // ---- 1. transport to the next row (phases A, B outward; C inward)
+    // ---- 1. transport to the next row (phases A, B outward; C inward).  __syncwarp() before each shared stage makes the
+    //         lanes of all phases reconverge, so the transport / pick-up / update code runs once per warp and step.
     const bool moving = mode == MD_A || mode == MD_B || mode == MD_C;
     const int rn = mode == MD_C ? r - 1 : r + 1;
     bool prop_ok = true;
+    __syncwarp();
     if (moving) { n_prop++; prop_ok = propagate(st, rows[rn].x - rows[r].x, P); }
 
-    // ---- 2. measurement for this step
-    bool have = false, finish = false;
+    // ---- 2a. per-phase decision: which measurement this step uses (a linked / assigned hit, a pick-up, or none)
+    bool have = false, finish = false, do_pick = false, load_hit = false;
     float2 c = c0;
-    int hit = -1, row = rn;
+    int hit = -1;
     if (mode == MD_INIT) {          // Phase A start: direction from the origin, first update with the start hit
       const float x = rows[r0].x, y = c0.x;
       const float rr = sqrtf(x * x + y * y);
       st.y = y; st.z = 0.0f; st.s = y / rr; st.t = P.continuous ? 0.0f : zref / rr; st.q = 0.0f;
       reset_cov(st, P);
-      have = true; hit = h0; row = r0;
+      have = true; hit = h0;
     } else if (mode == MD_A) {      // follow the cleaned up-link, no gate
       if (!prop_ok) mode = MD_TRANS;
-      else { hit = nxt; c = yz[su[rn].off + hit]; have = true; }
+      else { hit = nxt; load_hit = true; have = true; }
     } else if (mode == MD_B) {      // outward extrapolation with pick-up
       if (!prop_ok || fabsf(st.y) > rows[rn].yedge + P.edge_margin) mode = MD_TRANS;
-      else {
-        n_pick++;
-        hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c);
-        rh[rn] = hit;
-        have = hit >= 0;
-        r = rn;
-        if (!have && ++gap > P.max_gap) mode = MD_TRANS;
-      }
+      else { do_pick = true; r = rn; }
     } else if (mode == MD_TRANS) {  // Phase C start: state after the outermost update, fresh covariance, refit inward
       st.y = sv_y; st.z = sv_z; st.s = sv_s; st.t = sv_t; st.q = sv_q;
       reset_cov(st, P);
       chi2 = 0.0f; n = 0; first_assigned = r0; gap = 0;
-      c = c_out; have = true; row = r_out; r = r_out;
+      c = c_out; have = true; r = r_out;
     } else if (mode == MD_C) {
       if (!prop_ok) finish = true;
       else {
         const int a = rn >= r0 ? rh[rn] : -1;   // rows below r0 were never visited before
         r = rn;
-        if (a >= 0) { hit = a; c = yz[su[rn].off + a]; have = true; }
+        if (a >= 0) { hit = a; load_hit = true; have = true; }
         else if (fabsf(st.y) > rows[rn].yedge + P.edge_margin) {
           if (rn < first_assigned) finish = true;
           else if (rn < r0) rh[rn] = -1;       // skipped row inside the tracklet's range: reads as "no cluster"
-        } else {
-          n_pick++;
-          hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c);
-          if (rn < r0 || hit >= 0) rh[rn] = hit;
-          have = hit >= 0;
-          if (have) { if (rn < first_assigned) { first_assigned = rn; gap = 0; } }
-          else if (rn < first_assigned && ++gap > P.max_gap) finish = true;
-        }
+        } else do_pick = true;
       }
     }
+    // ---- 2b. cluster pick-up from the grid (phase B and phase C lanes together)
+    __syncwarp();
+    if (do_pick) { n_pick++; hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c); }
+    __syncwarp();
+    if (do_pick) {
+      have = hit >= 0;
+      if (mode == MD_B) {
+        rh[rn] = hit;
+        if (!have && ++gap > P.max_gap) mode = MD_TRANS;
+      } else {
+        if (rn < r0 || have) rh[rn] = hit;
+        if (have) { if (rn < first_assigned) { first_assigned = rn; gap = 0; } }
+        else if (rn < first_assigned && ++gap > P.max_gap) finish = true;
+      }
+    }
+    if (load_hit) c = yz[su[rn].off + hit];
 
     // ---- 3. Kalman update (all lanes that have a measurement, whatever their phase)
     float dchi = 0.0f;
+    __syncwarp();
     if (have) { n_upd++; dchi = update(st, c.x, c.y - zref, P); }
+    __syncwarp();
 
     // ---- 4. bookkeeping and phase transitions
     if (mode == MD_INIT) {
