@@ -163,9 +163,17 @@ __device__ __forceinline__ int pickup(const UnitDesc& d, const float2* __restric
   const int* __restrict__ bs = bin_start + d.bin_off;
   const float2* __restrict__ hits = yz + d.off;
   int best = -1; float bestd = 0.0f;
-  for (int bz = bz0; bz <= bz1; bz++) {
-    const int pa = bs[bz * d.ny + by0], pb = bs[bz * d.ny + by1 + 1];
-    for (int p = pa; p < pb; p++) {
+  // Two bin rows per round (the window is at most 2*w_max + margin wide, so one round is the rule): the four bin_start
+  // reads are issued together, then ONE flat loop runs over the candidates of both rows, so that lanes with different
+  // candidate counts share the loop instead of diverging in a nest.  Any visiting order gives the same argmin (total order).
+  for (int bz = bz0; bz <= bz1; bz += 2) {
+    const int ra = bz * d.ny, rb = ra + d.ny;
+    const bool two = bz + 1 <= bz1;
+    const int pa0 = bs[ra + by0], pb0 = bs[ra + by1 + 1];
+    const int pa1 = two ? bs[rb + by0] : 0, pb1 = two ? bs[rb + by1 + 1] : 0;
+    const int n0 = pb0 - pa0, total = n0 + (pb1 - pa1);
+    for (int k = 0; k < total; k++) {
+      const int p = k < n0 ? pa0 + k : pa1 + (k - n0);
       const float2 c = hits[p];
       const float yc = c.x, zc = c.y - zref;
       if (!(yc >= ylo && yc <= yhi && zc >= zlo && zc <= zhi)) continue;
