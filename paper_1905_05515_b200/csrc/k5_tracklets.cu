@@ -194,7 +194,7 @@ __device__ __forceinline__ int pickup(const UnitDesc& d, const float2* __restric
 // one from a global work queue (persistent CTAs), so short and long tracklets balance out.
 enum : int { MD_FETCH = 0, MD_INIT, MD_A, MD_B, MD_TRANS, MD_C, MD_EXIT };
 
-__global__ void __launch_bounds__(K5_THREADS, 4) k5_tracklets(const int M, const int* __restrict__ start_unit,
+__global__ void __launch_bounds__(K5_THREADS, 5) k5_tracklets(const int M, const int* __restrict__ start_unit,
                                                               const int* __restrict__ start_pos, const UnitDesc* __restrict__ units,
                                                               const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                               const int* __restrict__ perm, const int* __restrict__ bin_start,
@@ -211,7 +211,9 @@ __global__ void __launch_bounds__(K5_THREADS, 4) k5_tracklets(const int M, const
   float zref = 0.0f, chi2 = 0.0f;
   float2 c0 = make_float2(0.f, 0.f), c_out = c0;
   float sv_y = 0.f, sv_z = 0.f, sv_s = 0.f, sv_t = 0.f, sv_q = 0.f;
-  State st = {}, snap = {};
+  State st = {};
+  __shared__ float s_snap[20][K5_THREADS];   // state after the last Phase-C update, per lane (written often, read once)
+  const int tx = threadIdx.x;
   const UnitDesc* __restrict__ su = units;
   int* __restrict__ rh = rowhit;
   unsigned n_prop = 0, n_upd = 0, n_pick = 0;
@@ -308,6 +310,7 @@ __global__ void __launch_bounds__(K5_THREADS, 4) k5_tracklets(const int M, const
     __syncwarp();
 
     // ---- 4. bookkeeping and phase transitions
+    bool save_snap = false;
     if (mode == MD_INIT) {
       rh[r0] = h0; r = r0;
       sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = r0; c_out = c0;
@@ -324,22 +327,26 @@ __global__ void __launch_bounds__(K5_THREADS, 4) k5_tracklets(const int M, const
       if (rn + 1 >= R) mode = MD_TRANS;
     } else if (mode == MD_TRANS) {
       if (have) {                   // (have is false only for lanes that switched to MD_TRANS in step 2 of this iteration)
-        chi2 = chi2 + dchi; n = 1; snap = st; r_snap = r_out;
+        chi2 = chi2 + dchi; n = 1; r_snap = r_out; save_snap = true;
         if (r_out - 1 >= 0) mode = MD_C; else finish = true;
       }
     } else if (mode == MD_C) {
-      if (have) { chi2 = chi2 + dchi; n++; snap = st; r_snap = rn; }
+      if (have) { chi2 = chi2 + dchi; n++; r_snap = rn; save_snap = true; }
       if (!finish && rn == 0) finish = true;
     }
+
+    if (save_snap) { s_snap[0][tx] = st.y; s_snap[1][tx] = st.z; s_snap[2][tx] = st.s; s_snap[3][tx] = st.t; s_snap[4][tx] = st.q;
+          s_snap[5][tx] = st.c00; s_snap[6][tx] = st.c10; s_snap[7][tx] = st.c11; s_snap[8][tx] = st.c20; s_snap[9][tx] = st.c21;
+          s_snap[10][tx] = st.c22; s_snap[11][tx] = st.c30; s_snap[12][tx] = st.c31; s_snap[13][tx] = st.c32; s_snap[14][tx] = st.c33;
+          s_snap[15][tx] = st.c40; s_snap[16][tx] = st.c41; s_snap[17][tx] = st.c42; s_snap[18][tx] = st.c43; s_snap[19][tx] = st.c44; }
 
     if (finish) {   // tracklet complete: hits exist exactly on the rows [r_snap, r_out] that carry a non-negative rowhit
       tl_n[i] = n; tl_first[i] = r_snap; tl_last[i] = r_out; tl_chi2[i] = chi2;
       float* __restrict__ op = tl_par + (long long)i * 5;
-      op[0] = snap.y; op[1] = snap.z + zref; op[2] = snap.s; op[3] = snap.t; op[4] = snap.q;
+      op[0] = s_snap[0][tx]; op[1] = s_snap[1][tx] + zref; op[2] = s_snap[2][tx]; op[3] = s_snap[3][tx]; op[4] = s_snap[4][tx];
       float* __restrict__ oc = tl_cov + (long long)i * 15;
-      oc[0] = snap.c00; oc[1] = snap.c10; oc[2] = snap.c11; oc[3] = snap.c20; oc[4] = snap.c21; oc[5] = snap.c22; oc[6] = snap.c30;
-      oc[7] = snap.c31; oc[8] = snap.c32; oc[9] = snap.c33; oc[10] = snap.c40; oc[11] = snap.c41; oc[12] = snap.c42; oc[13] = snap.c43;
-      oc[14] = snap.c44;
+#pragma unroll
+      for (int k = 0; k < 15; k++) oc[k] = s_snap[5 + k][tx];
       mode = MD_FETCH;
     }
   }
