@@ -194,7 +194,7 @@ __device__ __forceinline__ int pickup(const UnitDesc& d, const float2* __restric
 // one from a global work queue (persistent CTAs), so short and long tracklets balance out.
 enum : int { MD_FETCH = 0, MD_INIT, MD_A, MD_B, MD_TRANS, MD_C, MD_EXIT };
 
-__global__ void __launch_bounds__(K5_THREADS, 5) k5_tracklets(const int M, const int* __restrict__ start_unit,
+__global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const int* __restrict__ start_unit,
                                                               const int* __restrict__ start_pos, const UnitDesc* __restrict__ units,
                                                               const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                               const int* __restrict__ perm, const int* __restrict__ bin_start,
@@ -209,11 +209,11 @@ __global__ void __launch_bounds__(K5_THREADS, 5) k5_tracklets(const int M, const
   int mode = MD_FETCH;
   int i = -1, r0 = 0, h0 = 0, r = 0, nxt = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
   float zref = 0.0f, chi2 = 0.0f;
-  float2 c0 = make_float2(0.f, 0.f), c_out = c0;
-  float sv_y = 0.f, sv_z = 0.f, sv_s = 0.f, sv_t = 0.f, sv_q = 0.f;
+  float2 c0 = make_float2(0.f, 0.f);
   State st = {};
   __shared__ float s_snap[20][K5_THREADS];   // state after the last Phase-C update, per lane (written often, read once)
   const int tx = threadIdx.x;
+  __shared__ float s_sv[7][K5_THREADS];       // state after the outermost update (5 parameters) + that cluster (y, z)
   const UnitDesc* __restrict__ su = units;
   int* __restrict__ rh = rowhit;
   unsigned n_prop = 0, n_upd = 0, n_pick = 0;
@@ -270,10 +270,10 @@ __global__ void __launch_bounds__(K5_THREADS, 5) k5_tracklets(const int M, const
       if (!prop_ok || fabsf(st.y) > rows[rn].yedge + P.edge_margin) mode = MD_TRANS;
       else { do_pick = true; r = rn; }
     } else if (mode == MD_TRANS) {  // Phase C start: state after the outermost update, fresh covariance, refit inward
-      st.y = sv_y; st.z = sv_z; st.s = sv_s; st.t = sv_t; st.q = sv_q;
+      st.y = s_sv[0][tx]; st.z = s_sv[1][tx]; st.s = s_sv[2][tx]; st.t = s_sv[3][tx]; st.q = s_sv[4][tx];
       reset_cov(st, P);
       chi2 = 0.0f; n = 0; first_assigned = r0; gap = 0;
-      c = c_out; have = true; r = r_out;
+      c = make_float2(s_sv[5][tx], s_sv[6][tx]); have = true; r = r_out;
     } else if (mode == MD_C) {
       if (!prop_ok) finish = true;
       else {
@@ -313,17 +313,17 @@ __global__ void __launch_bounds__(K5_THREADS, 5) k5_tracklets(const int M, const
     bool save_snap = false;
     if (mode == MD_INIT) {
       rh[r0] = h0; r = r0;
-      sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = r0; c_out = c0;
+      s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = r0; s_sv[5][tx] = c0.x; s_sv[6][tx] = c0.y;
       nxt = link_up[su[r0].off + h0];
       gap = 0;
       mode = nxt >= 0 ? MD_A : (r0 + 1 < R ? MD_B : MD_TRANS);
     } else if (mode == MD_A) {      // (a failed transport already switched the lane to MD_TRANS)
       r = rn; rh[rn] = hit;
-      sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = rn; c_out = c;
+      s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = rn; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y;
       nxt = link_up[su[rn].off + hit];
       if (nxt < 0) { gap = 0; mode = rn + 1 < R ? MD_B : MD_TRANS; }
     } else if (mode == MD_B) {
-      if (have) { gap = 0; sv_y = st.y; sv_z = st.z; sv_s = st.s; sv_t = st.t; sv_q = st.q; r_out = rn; c_out = c; }
+      if (have) { gap = 0; s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = rn; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y; }
       if (rn + 1 >= R) mode = MD_TRANS;
     } else if (mode == MD_TRANS) {
       if (have) {                   // (have is false only for lanes that switched to MD_TRANS in step 2 of this iteration)
