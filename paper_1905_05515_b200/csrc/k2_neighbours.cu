@@ -5,9 +5,12 @@
 //
 // One CTA per work item = a chunk of consecutive sorted clusters of one (sector,row).  Because the S1 order is z-major, the
 // clusters and bins of rows r+1 / r-1 that any window of the chunk can touch are ONE contiguous slab of each row's sorted
-// arrays.  Phase 1 finds the slab (block min/max of the window bin rows), thread 0 issues up to four 1-D TMA bulk copies
-// (cp.async.bulk, mbarrier complete_tx) that stage the slabs (float2 clusters + bin_start) in shared memory, phase 2 runs
-// the window scan and the pair search out of shared memory.  A slab that does not fit falls back to global (L2) reads.
+// arrays.  Thread 0 bounds the slab in O(1) from the bin rows of the first and last cluster of the chunk (one bin row of
+// safety margin; a superset is all that staging needs), issues up to four 1-D TMA bulk copies (cp.async.bulk, mbarrier
+// complete_tx) that stage the slabs (float2 clusters + bin_start) in shared memory, and every thread then runs the window
+// scan and the pair search for its clusters out of shared memory.  A slab that does not fit falls back to global (L2) reads.
+// The scan is flat: the candidates of the (at most two) bin rows of a window are visited by ONE loop that records the
+// in-window ones in a bit mask; the pair search then walks the set bits of the up and down masks (about one each).
 // All decision arithmetic (window bounds, membership, ey, ez, D, D < thr, argmin with index tie-break) is spelled with
 // explicit round-to-nearest intrinsics: no FMA contraction, same operation order as the definition -> bit-exact link tables.
 // Algorithmic HBM bytes per cluster: 8 (own float2) + 4 (bin table) + 8 (two links written) = 20, rows r+-1 reused from L2/smem.
@@ -18,7 +21,7 @@ namespace tpc {
 namespace {
 
 constexpr int K2_THREADS = 256;
-constexpr int K2_STAGE_BYTES = 64 * 1024;
+constexpr int K2_STAGE_BYTES = 40 * 1024;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -48,11 +51,23 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
 }
 
+
 struct Stage {          // written by thread 0, read by all
   int staged;
   int pshift_u, pshift_d, bshift_u, bshift_d;
   int hoff_d, boff_u, boff_d;   // byte offsets of the four regions in the staging buffer (hits_u at 0)
 };
+
+// One search window on a neighbour row: candidate ranges of its (at most two) bin rows.
+struct Win {
+  float ylo, yhi, zlo, zhi;
+  int a0, n0, a1, n;   // row 0: positions a0 .. a0+n0-1, row 1: a1 .. ; n = total candidates to test
+  bool wide;           // window spans more than two bin rows (tiny bins): generic path
+};
+
+__device__ __forceinline__ bool in_win(const float2 c, const Win& w) {
+  return c.x >= w.ylo && c.x <= w.yhi && c.y >= w.zlo && c.y <= w.zhi;
+}
 
 __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restrict__ items, const int chunk,
                                                             const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
@@ -61,7 +76,6 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
                                                             int* __restrict__ link_dn, const Params P) {
   extern __shared__ __align__(128) unsigned char s_stage[];
   __shared__ __align__(8) uint64_t s_bar;
-  __shared__ int s_red[4];
   __shared__ Stage s_st;
 
   const Item it = items[blockIdx.x];
@@ -82,36 +96,21 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
   const RowConst rc = rows[r];
   const float hw_u = P.continuous ? rc.wzu : P.wz, hw_d = P.continuous ? rc.wzd : P.wz;
 
+  // ---- staging: thread 0 bounds the slabs of rows r+1 / r-1 and issues the TMA bulk copies
   if (threadIdx.x == 0) {
-    s_red[0] = INT_MAX; s_red[1] = -1; s_red[2] = INT_MAX; s_red[3] = -1;
     mbar_init(&s_bar, 1);
     mbar_fence_init();
-  }
-  __syncthreads();
-
-  // ---- phase 1: bin rows of rows r+1 / r-1 touched by any window of this chunk
-  {
-    int mnu = INT_MAX, mxu = -1, mnd = INT_MAX, mxd = -1;
-    for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
-      const float z = own[k].y;
-      const float zcu = P.continuous ? z : __fmul_rn(z, rc.tu), zcd = P.continuous ? z : __fmul_rn(z, rc.td);
-      mnu = min(mnu, bin_of(__fsub_rn(zcu, hw_u), du.zlo, du.invs, du.nz));
-      mxu = max(mxu, bin_of(__fadd_rn(zcu, hw_u), du.zlo, du.invs, du.nz));
-      mnd = min(mnd, bin_of(__fsub_rn(zcd, hw_d), dd.zlo, dd.invs, dd.nz));
-      mxd = max(mxd, bin_of(__fadd_rn(zcd, hw_d), dd.zlo, dd.invs, dd.nz));
-    }
-    mnu = __reduce_min_sync(0xffffffffu, mnu); mxu = __reduce_max_sync(0xffffffffu, mxu);
-    mnd = __reduce_min_sync(0xffffffffu, mnd); mxd = __reduce_max_sync(0xffffffffu, mxd);
-    if ((threadIdx.x & 31) == 0) {
-      atomicMin(&s_red[0], mnu); atomicMax(&s_red[1], mxu); atomicMin(&s_red[2], mnd); atomicMax(&s_red[3], mxd);
-    }
-  }
-  __syncthreads();
-
-  // ---- staging: thread 0 sizes the two slabs and issues the TMA bulk copies
-  if (threadIdx.x == 0) {
+    // The chunk is sorted by bin (z-major): its clusters lie in the bin rows [bzf, bzl] of this row's grid, hence
+    // z in [zA, zB] with one bin row of margin (open-ended at the clamped first / last bin row, which also hold NaN / inf).
+    const int bzf = bin_of(own[0].y, d.zlo, d.invs, d.nz), bzl = bin_of(own[cnt - 1].y, d.zlo, d.invs, d.nz);
+    const float s = 1.0f / d.invs, inf = __int_as_float(0x7f800000);
+    const float zA = bzf <= 0 ? -inf : d.zlo + (float)(bzf - 1) * s;
+    const float zB = bzl >= d.nz - 1 ? inf : d.zlo + (float)(bzl + 2) * s;
+    const float zAu = P.continuous ? zA : fminf(zA * rc.tu, zA), zBu = P.continuous ? zB : fmaxf(zB * rc.tu, zB);
+    const float zAd = P.continuous ? zA : fminf(zA * rc.td, zA), zBd = P.continuous ? zB : fmaxf(zB * rc.td, zB);
     Stage st;
-    const int bz0u = s_red[0], bz1u = max(s_red[1], s_red[0]), bz0d = s_red[2], bz1d = max(s_red[3], s_red[2]);
+    const int bz0u = bin_of(zAu - hw_u, du.zlo, du.invs, du.nz), bz1u = bin_of(zBu + hw_u, du.zlo, du.invs, du.nz);
+    const int bz0d = bin_of(zAd - hw_d, dd.zlo, dd.invs, dd.nz), bz1d = bin_of(zBd + hw_d, dd.zlo, dd.invs, dd.nz);
     const long long gbu = du.bin_off + (long long)bz0u * du.ny, gbd = dd.bin_off + (long long)bz0d * dd.ny;
     const int nbu = (bz1u - bz0u + 1) * du.ny + 1, nbd = (bz1d - bz0d + 1) * dd.ny + 1;
     const int p0u = bin_start[gbu], p1u = bin_start[gbu + nbu - 1], p0d = bin_start[gbd], p1d = bin_start[gbd + nbd - 1];
@@ -144,49 +143,76 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
   } else {
     yzu = yz + du.off; yzd = yz + dd.off; bsu = bin_start + du.bin_off; bsd = bin_start + dd.bin_off;
   }
-  const int psu = st.pshift_u, psd = st.pshift_d, bsu_s = st.bshift_u, bsd_s = st.bshift_d;
+  yzu -= st.pshift_u; yzd -= st.pshift_d; bsu -= st.bshift_u; bsd -= st.bshift_d;   // index by row position / row bin directly
   const int* __restrict__ permu = perm + du.off;
   const int* __restrict__ permd = perm + dd.off;
 
-  // ---- phase 2: window scan + best pair, one thread per cluster
+  // window on a neighbour row: bounds (one fp32 op each) and the candidate ranges of its bin rows
+  auto make_win = [&](const float yc, const float zc, const float hw, const UnitDesc& g, const int* bs) {
+    Win w;
+    w.ylo = __fsub_rn(yc, P.wy); w.yhi = __fadd_rn(yc, P.wy); w.zlo = __fsub_rn(zc, hw); w.zhi = __fadd_rn(zc, hw);
+    const int by0 = bin_of(w.ylo, g.ylo, g.invs, g.ny), by1 = bin_of(w.yhi, g.ylo, g.invs, g.ny);
+    const int bz0 = bin_of(w.zlo, g.zlo, g.invs, g.nz), bz1 = bin_of(w.zhi, g.zlo, g.invs, g.nz);
+    w.wide = bz1 - bz0 > 1;
+    const int ra = bz0 * g.ny;
+    w.a0 = bs[ra + by0]; w.n0 = bs[ra + by1 + 1] - w.a0;
+    w.a1 = 0; w.n = w.n0;
+    if (bz1 > bz0) { const int rb = ra + g.ny; w.a1 = bs[rb + by0]; w.n += bs[rb + by1 + 1] - w.a1; }
+    return w;
+  };
+
+  // ---- window scan + best pair, one thread per cluster
   for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
     const float2 h = own[k];
     const float y = h.x, z = h.y;
-    // up window (row r+1)
-    const float ycu = __fmul_rn(y, rc.tu), zcu = P.continuous ? z : __fmul_rn(z, rc.tu);
-    const float ylou = __fsub_rn(ycu, P.wy), yhiu = __fadd_rn(ycu, P.wy), zlou = __fsub_rn(zcu, hw_u), zhiu = __fadd_rn(zcu, hw_u);
-    const int by0u = bin_of(ylou, du.ylo, du.invs, du.ny), by1u = bin_of(yhiu, du.ylo, du.invs, du.ny);
-    const int bz0u = bin_of(zlou, du.zlo, du.invs, du.nz), bz1u = bin_of(zhiu, du.zlo, du.invs, du.nz);
-    // down window (row r-1)
-    const float ycd = __fmul_rn(y, rc.td), zcd = P.continuous ? z : __fmul_rn(z, rc.td);
-    const float ylod = __fsub_rn(ycd, P.wy), yhid = __fadd_rn(ycd, P.wy), zlod = __fsub_rn(zcd, hw_d), zhid = __fadd_rn(zcd, hw_d);
-    const int by0d = bin_of(ylod, dd.ylo, dd.invs, dd.ny), by1d = bin_of(yhid, dd.ylo, dd.invs, dd.ny);
-    const int bz0d = bin_of(zlod, dd.zlo, dd.invs, dd.nz), bz1d = bin_of(zhid, dd.zlo, dd.invs, dd.nz);
+    const Win wu = make_win(__fmul_rn(y, rc.tu), P.continuous ? z : __fmul_rn(z, rc.tu), hw_u, du, bsu);
+    const Win wd = make_win(__fmul_rn(y, rc.td), P.continuous ? z : __fmul_rn(z, rc.td), hw_d, dd, bsd);
 
     bool have = false; float bestD = 0.0f; int bu = -1, bd = -1;
-    for (int bz = bz0u; bz <= bz1u; bz++) {
-      const int pa = bsu[bz * du.ny + by0u - bsu_s], pb = bsu[bz * du.ny + by1u + 1 - bsu_s];
-      for (int p = pa; p < pb; p++) {
-        const float2 cu = yzu[p - psu];
-        if (!(cu.x >= ylou && cu.x <= yhiu && cu.y >= zlou && cu.y <= zhiu)) continue;
-        const float m1 = __fmul_rn(rc.b, __fsub_rn(cu.x, y)), m3 = __fmul_rn(rc.b, __fsub_rn(cu.y, z));
-        for (int bzd = bz0d; bzd <= bz1d; bzd++) {
-          const int qa = bsd[bzd * dd.ny + by0d - bsd_s], qb = bsd[bzd * dd.ny + by1d + 1 - bsd_s];
-          for (int q = qa; q < qb; q++) {
-            const float2 cd = yzd[q - psd];
-            if (!(cd.x >= ylod && cd.x <= yhid && cd.y >= zlod && cd.y <= zhid)) continue;
-            const float ey = __fsub_rn(m1, __fmul_rn(rc.a, __fsub_rn(y, cd.x)));
-            const float ez = __fsub_rn(m3, __fmul_rn(rc.a, __fsub_rn(z, cd.y)));
-            const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-            bool better = !have || D < bestD;
-            if (have && D == bestD) {   // tie: lower original index of the up cluster, then of the down cluster (rare: global reads)
-              const int iu = permu[p], ib = permu[bu];
-              better = iu < ib || (iu == ib && permd[q] < permd[bd]);
-            }
-            if (better) { have = true; bestD = D; bu = p; bd = q; }
-          }
+    auto pair = [&](const int p, const float2 cu, const int q, const float2 cd) {
+      const float ey = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.x, y)), __fmul_rn(rc.a, __fsub_rn(y, cd.x)));
+      const float ez = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.y, z)), __fmul_rn(rc.a, __fsub_rn(z, cd.y)));
+      const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+      bool better = !have || D < bestD;
+      if (have && D == bestD) {   // tie: lower original index of the up cluster, then of the down cluster (rare: global reads)
+        const int iu = permu[p], ib = permu[bu];
+        better = iu < ib || (iu == ib && permd[q] < permd[bd]);
+      }
+      if (better) { have = true; bestD = D; bu = p; bd = q; }
+    };
+
+    if (!wu.wide && !wd.wide && wu.n <= 32 && wd.n <= 32) {
+      // flat scan: one loop per side marks the in-window candidates, then the pair search walks the set bits
+      unsigned mu = 0u, md = 0u;
+      for (int j = 0; j < wd.n; j++) { const int q = j < wd.n0 ? wd.a0 + j : wd.a1 + (j - wd.n0); if (in_win(yzd[q], wd)) md |= 1u << j; }
+      if (md) for (int j = 0; j < wu.n; j++) { const int p = j < wu.n0 ? wu.a0 + j : wu.a1 + (j - wu.n0); if (in_win(yzu[p], wu)) mu |= 1u << j; }
+      while (mu) {
+        const int j = __ffs(mu) - 1; mu &= mu - 1u;
+        const int p = j < wu.n0 ? wu.a0 + j : wu.a1 + (j - wu.n0);
+        const float2 cu = yzu[p];
+        unsigned m = md;
+        while (m) {
+          const int i = __ffs(m) - 1; m &= m - 1u;
+          const int q = i < wd.n0 ? wd.a0 + i : wd.a1 + (i - wd.n0);
+          pair(p, cu, q, yzd[q]);
         }
       }
+    } else {
+      // generic path (bins smaller than the window, or very dense rows): nested scan over all bin rows of both windows
+      const int by0u = bin_of(wu.ylo, du.ylo, du.invs, du.ny), by1u = bin_of(wu.yhi, du.ylo, du.invs, du.ny);
+      const int bz0u = bin_of(wu.zlo, du.zlo, du.invs, du.nz), bz1u = bin_of(wu.zhi, du.zlo, du.invs, du.nz);
+      const int by0d = bin_of(wd.ylo, dd.ylo, dd.invs, dd.ny), by1d = bin_of(wd.yhi, dd.ylo, dd.invs, dd.ny);
+      const int bz0d = bin_of(wd.zlo, dd.zlo, dd.invs, dd.nz), bz1d = bin_of(wd.zhi, dd.zlo, dd.invs, dd.nz);
+      for (int bz = bz0u; bz <= bz1u; bz++)
+        for (int p = bsu[bz * du.ny + by0u]; p < bsu[bz * du.ny + by1u + 1]; p++) {
+          const float2 cu = yzu[p];
+          if (!in_win(cu, wu)) continue;
+          for (int bzd = bz0d; bzd <= bz1d; bzd++)
+            for (int q = bsd[bzd * dd.ny + by0d]; q < bsd[bzd * dd.ny + by1d + 1]; q++) {
+              const float2 cd = yzd[q];
+              if (in_win(cd, wd)) pair(p, cu, q, cd);
+            }
+        }
     }
     const bool ok = have && bestD < rc.thr;
     lup[k] = ok ? bu : -1;
