@@ -174,7 +174,8 @@ def tpc_get_timings(h) -> dict:
 
 @dataclass
 class Tracks:
-    """Result of tpc_find_tracks (numpy arrays, copied out) or tpc_find_tracks_device (torch CUDA tensors, library-owned views)."""
+    """Result of tpc_find_tracks (numpy views of library-owned pinned host arrays) or tpc_find_tracks_device (torch CUDA tensors,
+    library-owned views).  Both stay valid until the next tpc_find_tracks* / tpc_clear / tpc_destroy on the context; use copy() to keep them."""
     n_tracks: int
     n_cluster_refs: int
     sector: object
@@ -188,6 +189,11 @@ class Tracks:
     cl_row: object
     cl_index: object
 
+    def copy(self):
+        """Owning copy (the arrays of a result are library-owned views and are overwritten by the next call)."""
+        d = {k: (v.copy() if isinstance(v, np.ndarray) else v.clone()) for k, v in self.as_dict().items()}
+        return Tracks(self.n_tracks, self.n_cluster_refs, **d)
+
     def as_dict(self):
         return {k: getattr(self, k) for k in ("sector", "x", "par", "cov", "chi2", "ndf", "tracklet", "cl_begin", "cl_row", "cl_index")}
 
@@ -197,10 +203,11 @@ _FIELDS = [("sector", np.int32, 1), ("x", np.float32, 1), ("par", np.float32, 5)
 
 
 def _host_array(addr, n, dtype):
+    """Zero-copy numpy view of a library-owned host array (valid until the next tpc_find_tracks* / tpc_clear / tpc_destroy)."""
     if n == 0 or not addr:
         return np.zeros(0, dtype=dtype)
     ct = {np.int32: C.c_int32, np.float32: C.c_float, np.int64: C.c_int64}[dtype]
-    return np.ctypeslib.as_array(C.cast(addr, C.POINTER(ct)), shape=(n,)).copy()
+    return np.ctypeslib.as_array(C.cast(addr, C.POINTER(ct)), shape=(n,))
 
 
 class _DevView:

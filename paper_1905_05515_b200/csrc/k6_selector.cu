@@ -5,6 +5,7 @@
 //   bits 63..56  n (<= 255 rows)
 //   bits 55..24  bitwise NOT of the order-preserving image of the fp32 quality chi2/ndf (lower quality wins)
 //   bits 23..0   0xFFFFFF - tracklet index (lower index wins)                       -> at most 2^24 tracklets per call
+// One warp per tracklet in all three kernels.
 // k6_owner : atomicMax of the key on owner[cluster]          k6_count : owned clusters per tracklet, track flag
 // scan     : exclusive prefix sum of (flag << 40 | owned)     k6_emit  : compacted tracks + CSR cluster lists, in tracklet order
 #include "tpc_internal.cuh"
@@ -22,50 +23,55 @@ __device__ __forceinline__ unsigned long long make_key(int n, float chi2, int id
   return ((unsigned long long)(unsigned)n << 56) | ((unsigned long long)(~b) << 24) | (unsigned long long)(0xFFFFFFu - (unsigned)idx);
 }
 
-__global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const long long Mpad, const int R, const int min_hits,
+// All three kernels map ONE WARP to one tracklet: the lanes read 32 consecutive rows of its rowhit line (coalesced) and issue
+// their owner-key atomics / owner reads in parallel.
+__global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const int R, const int min_hits,
                                                        const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
                                                        const int* __restrict__ rowhit, const int* __restrict__ tl_n,
                                                        const int* __restrict__ tl_first, const int* __restrict__ tl_last,
                                                        const float* __restrict__ tl_chi2, unsigned long long* __restrict__ owner,
                                                        unsigned long long* __restrict__ tl_key) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
   if (i >= M) return;
   const int n = tl_n[i];
   const float chi2 = tl_chi2[i];
   const bool kept = n >= min_hits && isfinite(chi2);
   const unsigned long long key = kept ? make_key(n, chi2, i) : 0ull;
-  tl_key[i] = key;
+  if (lane == 0) tl_key[i] = key;
   if (!kept) return;
   const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
+  const int* __restrict__ rh = rowhit + (long long)i * R;
   const int r1 = tl_last[i];
-  for (int r = tl_first[i]; r <= r1; r++) {
-    const int p = rowhit[(long long)i * R + r];
+  for (int r = tl_first[i] + lane; r <= r1; r += 32) {
+    const int p = rh[r];
     if (p >= 0) atomicMax(&owner[su[r].off + p], key);
   }
 }
 
-__global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const long long Mpad, const int R, const int min_hits,
+__global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const int R, const int min_hits,
                                                        const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
                                                        const int* __restrict__ rowhit, const int* __restrict__ tl_first,
                                                        const int* __restrict__ tl_last, const unsigned long long* __restrict__ owner,
                                                        const unsigned long long* __restrict__ tl_key,
                                                        unsigned long long* __restrict__ scan_in) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
   if (i >= M) return;
   const unsigned long long key = tl_key[i];
   int owned = 0;
   if (key) {
     const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
+    const int* __restrict__ rh = rowhit + (long long)i * R;
     const int r1 = tl_last[i];
-    for (int r = tl_first[i]; r <= r1; r++) {
-      const int p = rowhit[(long long)i * R + r];
+    for (int r = tl_first[i] + lane; r <= r1; r += 32) {
+      const int p = rh[r];
       if (p >= 0 && owner[su[r].off + p] == key) owned++;
     }
   }
-  scan_in[i] = owned >= min_hits && key ? ((1ull << 40) | (unsigned long long)owned) : 0ull;
+  owned = __reduce_add_sync(0xffffffffu, owned);
+  if (lane == 0) scan_in[i] = owned >= min_hits && key ? ((1ull << 40) | (unsigned long long)owned) : 0ull;
 }
 
-__global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const long long Mpad, const int R, const int* __restrict__ start_unit,
+__global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const int R, const int* __restrict__ start_unit,
                                                       const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
                                                       const int* __restrict__ perm, const int* __restrict__ rowhit,
                                                       const int* __restrict__ tl_n, const int* __restrict__ tl_first,
@@ -79,26 +85,31 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const long lo
                                                       float* __restrict__ o_chi2, int* __restrict__ o_ndf, int* __restrict__ o_tracklet,
                                                       long long* __restrict__ o_cl_begin, int* __restrict__ o_cl_row,
                                                       int* __restrict__ o_cl_index, const long long n_tracks, const long long n_refs) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i == 0) o_cl_begin[n_tracks] = n_refs;
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = (int)(gt >> 5), lane = threadIdx.x & 31;
+  if (gt == 0) o_cl_begin[n_tracks] = n_refs;
   if (i >= M || scan_in[i] == 0ull) return;
   const unsigned long long so = scan_out[i];
   const long long t = (long long)(so >> 40);
   long long k = (long long)(so & REF_MASK);
   const int sec = start_unit[i] / R;
   const UnitDesc* __restrict__ su = units + (long long)sec * R;
+  const int* __restrict__ rh = rowhit + (long long)i * R;
   const unsigned long long key = tl_key[i];
   const int r0 = tl_first[i], r1 = tl_last[i];
-  o_sector[t] = sec; o_x[t] = rows[r0].x; o_chi2[t] = tl_chi2[i]; o_ndf[t] = 2 * tl_n[i] - 5; o_tracklet[t] = i; o_cl_begin[t] = k;
-#pragma unroll
-  for (int j = 0; j < 5; j++) o_par[t * 5 + j] = tl_par[(long long)i * 5 + j];
-#pragma unroll
-  for (int j = 0; j < 15; j++) o_cov[t * 15 + j] = tl_cov[(long long)i * 15 + j];
-  for (int r = r0; r <= r1; r++) {
-    const int p = rowhit[(long long)i * R + r];
-    if (p < 0) continue;
-    const long long g = su[r].off + p;
-    if (owner[g] == key) { o_cl_row[k] = r; o_cl_index[k] = perm[g]; k++; }
+  if (lane == 0) {
+    o_sector[t] = sec; o_x[t] = rows[r0].x; o_chi2[t] = tl_chi2[i]; o_ndf[t] = 2 * tl_n[i] - 5; o_tracklet[t] = i; o_cl_begin[t] = k;
+  }
+  if (lane < 5) o_par[t * 5 + lane] = tl_par[(long long)i * 5 + lane];
+  if (lane < 15) o_cov[t * 15 + lane] = tl_cov[(long long)i * 15 + lane];
+  for (int rb = r0; rb <= r1; rb += 32) {       // ascending rows: ballot + prefix popcount keeps the list ordered
+    const int r = rb + lane;
+    long long g = 0;
+    bool own = false;
+    if (r <= r1) { const int p = rh[r]; if (p >= 0) { g = su[r].off + p; own = owner[g] == key; } }
+    const unsigned m = __ballot_sync(0xffffffffu, own);
+    if (own) { const long long o = k + __popc(m & ((1u << lane) - 1u)); o_cl_row[o] = r; o_cl_index[o] = perm[g]; }
+    k += __popc(m);
   }
 }
 
@@ -116,10 +127,11 @@ int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const 
   }
   cudaError_t e = cudaMemsetAsync(d_owner, 0, (size_t)N * sizeof(unsigned long long), L.stream);
   if (e != cudaSuccess) return -(int)e;
-  const int blocks = (M + K6_THREADS - 1) / K6_THREADS;
-  k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M, Mpad, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first, d_tl_last,
+  (void)Mpad;
+  const int blocks = (int)(((long long)M * 32 + K6_THREADS - 1) / K6_THREADS);
+  k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first, d_tl_last,
                                                  d_tl_chi2, d_owner, d_tl_key);
-  k6_count<<<blocks, K6_THREADS, 0, L.stream>>>(M, Mpad, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_first, d_tl_last, d_owner,
+  k6_count<<<blocks, K6_THREADS, 0, L.stream>>>(M, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_first, d_tl_last, d_owner,
                                                  d_tl_key, d_scan_in);
   int rc = launch_scan_u64(L, d_scan_in, d_scan_out, M, d_scan_tmp, d_total);
   if (rc < 0) return rc;
@@ -133,8 +145,9 @@ int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_un
                    const unsigned long long* d_tl_key, const unsigned long long* d_scan_in, const unsigned long long* d_scan_out,
                    int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,
                    long long* o_cl_begin, int* o_cl_row, int* o_cl_index, long long n_tracks, long long n_refs, const Params& P) {
-  const int blocks = M > 0 ? (M + K6_THREADS - 1) / K6_THREADS : 1;
-  k6_emit<<<blocks, K6_THREADS, 0, L.stream>>>(M, Mpad, P.R, d_start_unit, d_units, d_rows, d_perm, d_rowhit, d_tl_n, d_tl_first,
+  (void)Mpad;
+  const int blocks = M > 0 ? (int)(((long long)M * 32 + K6_THREADS - 1) / K6_THREADS) : 1;
+  k6_emit<<<blocks, K6_THREADS, 0, L.stream>>>(M, P.R, d_start_unit, d_units, d_rows, d_perm, d_rowhit, d_tl_n, d_tl_first,
                                                 d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out,
                                                 o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row, o_cl_index,
                                                 n_tracks, n_refs);

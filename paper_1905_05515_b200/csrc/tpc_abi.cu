@@ -67,6 +67,14 @@ struct PinBuf {
   template <class T> T* as() const { return (T*)p; }
 };
 
+// grow-only pinned host array (result arrays: the device -> host copy is then a true asynchronous DMA)
+template <class T> struct PinVec {
+  PinBuf b;
+  cudaError_t resize(size_t n) { return b.ensure(std::max<size_t>(n, 1) * sizeof(T)); }
+  T* data() const { return (T*)b.p; }
+  void release() { b.release(); }
+};
+
 struct Tunables {   // DESIGN.md table T
   double wy = 1.5, wz = 1.5, dzdx_max = 1.5, wz0 = 0.75, cut2 = 1.75;
   int min_seed = 3;
@@ -123,8 +131,8 @@ struct tpc_ctx {
   long long n_tracks = 0, n_refs = 0;
   DevBuf o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row, o_cl_index;
   // outputs / debug copies (host)
-  std::vector<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; std::vector<float> ho_x, ho_par, ho_cov, ho_chi2;
-  std::vector<int64_t> ho_cl_begin;
+  PinVec<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; PinVec<float> ho_x, ho_par, ho_cov, ho_chi2;
+  PinVec<int64_t> ho_cl_begin;
   std::vector<float> dbg_yz; std::vector<int32_t> dbg_perm, dbg_bins, dbg_up, dbg_dn, dbg_su, dbg_sp;
   std::vector<int32_t> dbg_tl_sector, dbg_tl_row, dbg_tl_n, dbg_tl_first, dbg_tl_last, dbg_rowhit; std::vector<float> dbg_tl_chi2, dbg_tl_x, dbg_tl_par, dbg_tl_cov;
 
@@ -219,6 +227,8 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
+  c->ho_sector.release(); c->ho_ndf.release(); c->ho_tracklet.release(); c->ho_cl_row.release(); c->ho_cl_index.release();
+  c->ho_x.release(); c->ho_par.release(); c->ho_cov.release(); c->ho_chi2.release(); c->ho_cl_begin.release();
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
   delete c;
 }
@@ -519,8 +529,10 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   // ---- result
   out->n_tracks = nt; out->n_cluster_refs = nr;
   if (to_host) {
-    c->ho_sector.resize(ntz); c->ho_x.resize(ntz); c->ho_par.resize(ntz * 5); c->ho_cov.resize(ntz * 15); c->ho_chi2.resize(ntz);
-    c->ho_ndf.resize(ntz); c->ho_tracklet.resize(ntz); c->ho_cl_begin.resize(ntz + 1); c->ho_cl_row.resize(nrz); c->ho_cl_index.resize(nrz);
+    CUDA_TRY(c, c->ho_sector.resize(ntz)); CUDA_TRY(c, c->ho_x.resize(ntz)); CUDA_TRY(c, c->ho_par.resize(ntz * 5));
+    CUDA_TRY(c, c->ho_cov.resize(ntz * 15)); CUDA_TRY(c, c->ho_chi2.resize(ntz)); CUDA_TRY(c, c->ho_ndf.resize(ntz));
+    CUDA_TRY(c, c->ho_tracklet.resize(ntz)); CUDA_TRY(c, c->ho_cl_begin.resize(ntz + 1)); CUDA_TRY(c, c->ho_cl_row.resize(nrz));
+    CUDA_TRY(c, c->ho_cl_index.resize(nrz));
     if (nt > 0) {
       CUDA_TRY(c, cudaMemcpyAsync(c->ho_sector.data(), c->o_sector.p, nt * 4, cudaMemcpyDeviceToHost, st));
       CUDA_TRY(c, cudaMemcpyAsync(c->ho_x.data(), c->o_x.p, nt * 4, cudaMemcpyDeviceToHost, st));

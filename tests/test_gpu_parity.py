@@ -23,7 +23,7 @@ def _full_parity(w, grid_units=None, per_unit=False, **params):
     o = P.make_oracle(w, **params).run("s6")
     with _tracker(w, debug_keep=1, **params) as trk:
         trk.load_workload(w, per_unit=per_unit)
-        gtr = trk.find_tracks().as_dict()
+        gtr = trk.find_tracks().copy().as_dict()
         ng = P.compare_grid(w, o, trk, grid_units)
         lk = P.compare_links(w, o, trk)
         tm = trk.timings()
@@ -82,7 +82,7 @@ def test_empty_and_tiny_inputs():
         assert r.n_tracks == 0
         trk.clear()
         trk.load_workload(w)
-        r1 = trk.find_tracks().as_dict()
+        r1 = trk.find_tracks().copy().as_dict()
         r2 = trk.find_tracks().as_dict()   # same clusters again: identical result (buffers reused)
         for k in r1:
             assert np.array_equal(r1[k], r2[k]), k
@@ -93,7 +93,7 @@ def test_device_inputs_and_device_outputs_match_host_path():
     w = W.config(1)
     with _tracker(w) as trk:
         trk.load_workload(w)
-        host = trk.find_tracks().as_dict()
+        host = trk.find_tracks().copy().as_dict()
     with _tracker(w) as trk:
         trk.set_stream(torch.cuda.current_stream().cuda_stream)
         trk.load_batch(w.unit_off, torch.from_numpy(w.y).cuda(), torch.from_numpy(w.t).cuda())
