@@ -100,3 +100,39 @@ def test_device_inputs_and_device_outputs_match_host_path():
         dev = trk.find_tracks_device()
         for k, v in dev.as_dict().items():
             assert np.array_equal(v.cpu().numpy(), host[k]), k
+
+
+def test_c3_full_size_parity():
+    """BASELINE.json configs[2] at full size (2 ms frame, ~12.5 M clusters), the configuration bench.py times."""
+    w = W.config(3)
+    rng = np.random.default_rng(3)
+    o, otr, gtr, res = _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, 150, replace=False))
+    assert res["n_oracle"] > 100000
+    mo, mg = H.truth_metrics(w, otr), H.truth_metrics(w, gtr)
+    assert abs(mo["eff"] - mg["eff"]) <= 1e-3 and abs(mo["fake_rate"] - mg["fake_rate"]) <= 1e-3
+
+
+def test_c5_scaled_large_frame_invariants():
+    """10 ms frame shape (configs[4]) at 30 % length (~23 M clusters): properties that hold at any size, no oracle run."""
+    w = W.config(5, scale=0.3)
+    with _tracker(w) as trk:
+        trk.load_workload(w)
+        r = trk.find_tracks()
+        tm = trk.timings()
+        assert tm["n_clusters"] == w.n_clusters and r.n_tracks > 100000
+        cb = r.cl_begin
+        assert cb[0] == 0 and cb[-1] == r.n_cluster_refs and np.all(np.diff(cb) >= 10)          # every track has >= min_hits clusters
+        g = w.unit_off[r.sector.astype(np.int64).repeat(np.diff(cb)) * w.n_rows + r.cl_row] + r.cl_index
+        assert len(np.unique(g)) == len(g)                                                       # every cluster in at most one track
+        assert np.all(r.cl_index >= 0) and np.all(g < w.n_clusters)
+        rows_sorted = np.ones(len(g), bool); rows_sorted[1:] = np.diff(r.cl_row) > 0; rows_sorted[cb[:-1]] = True
+        assert rows_sorted.all()                                                                 # ascending rows inside a track
+        assert np.all(np.isfinite(r.par)) and np.all(np.isfinite(r.cov)) and np.all(r.ndf == 2 * (r.ndf + 5) // 2 - 5)
+        # grid invariants of a few units at this size
+        for u in (7, 1000, 4000):
+            gr = trk.grid(u // w.n_rows, u % w.n_rows)
+            bs = gr["bin_start"]
+            assert bs[0] == 0 and bs[-1] == gr["n"] and np.all(np.diff(bs) >= 0)
+            assert np.array_equal(np.sort(gr["perm"]), np.arange(gr["n"]))
+        mg = H.truth_metrics(w, r.as_dict())
+        assert mg["eff_primary"] > 0.95 and mg["fake_rate"] < 0.02
