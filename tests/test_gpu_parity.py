@@ -136,3 +136,40 @@ def test_c5_scaled_large_frame_invariants():
             assert np.array_equal(np.sort(gr["perm"]), np.arange(gr["n"]))
         mg = H.truth_metrics(w, r.as_dict())
         assert mg["eff_primary"] > 0.95 and mg["fake_rate"] < 0.02
+
+
+def _inject(w, unit, y_extra, t_extra):
+    """Copy of workload w with extra clusters appended to one (sector,row) unit (labels -1)."""
+    import copy
+    a = int(w.unit_off[unit + 1])
+    w2 = copy.copy(w)
+    k = len(y_extra)
+    w2.y = np.concatenate([w.y[:a], y_extra.astype(np.float32), w.y[a:]])
+    w2.t = np.concatenate([w.t[:a], t_extra.astype(np.float32), w.t[a:]])
+    w2.q = np.concatenate([w.q[:a], np.ones(k, np.float32), w.q[a:]])
+    w2.label = np.concatenate([w.label[:a], -np.ones(k, np.int32), w.label[a:]])
+    w2.leg0 = np.concatenate([w.leg0[:a], np.zeros(k, np.uint8), w.leg0[a:]])
+    off = w.unit_off.copy(); off[unit + 1:] += k
+    w2.unit_off = off
+    return w2
+
+
+def test_degenerate_units_dense_overflow_and_nonfinite():
+    """Maximum-size / degenerate grids: a unit with more bins than fit shared memory (global-cursor path), a bin holding
+    more than 255 identical clusters (rank overflow path), NaN / inf coordinates (clamped into bin 0 / last bin, never linked)."""
+    w = W.config(1, scale=0.2)
+    rng = np.random.default_rng(5)
+    tmax = w.params.z_max / w.params.vdrift
+    u_dense, u_same, u_bad = 40, 60, 80
+    w = _inject(w, u_dense, rng.uniform(-20, 20, 70000), rng.uniform(0, tmax, 70000))      # > 50 k bins
+    w = _inject(w, u_same, np.full(400, 3.25), np.full(400, 17.5))                          # 400 clusters in one bin
+    w = _inject(w, u_bad, np.array([np.nan, np.inf, -np.inf, 1.0, 2.0]), np.array([5.0, 6.0, 7.0, np.nan, np.inf]))
+    o = P.make_oracle(w).run("s6")
+    with _tracker(w, debug_keep=1) as trk:
+        trk.load_workload(w)
+        gtr = trk.find_tracks().copy().as_dict()
+        P.compare_grid(w, o, trk, [u_dense - 1, u_dense, u_dense + 1, u_same, u_bad, 0, 151])
+        lk = P.compare_links(w, o, trk)
+    assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
+    res = P.compare_tracks(o.tracks(), gtr)
+    assert res["frac_identical"] >= 0.999 and res["param_mismatch"] == 0, res
