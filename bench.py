@@ -128,7 +128,7 @@ def run_gpu(args, rank, world, local_rank):
     w = W.config(args.config, seed=args.config + rank)          # every rank its own time frame (weak scaling)
     N = w.n_clusters
     stream = torch.cuda.current_stream()
-    trk = T.Tracker(**w.geometry())
+    trk = T.Tracker(**w.geometry(), **dict((kv.split("=")[0], float(kv.split("=")[1])) for kv in args.param))
     trk.set_stream(stream.cuda_stream)
     y_d, t_d = torch.from_numpy(w.y).cuda(), torch.from_numpy(w.t).cuda()
     y_h, t_h = torch.from_numpy(w.y).pin_memory(), torch.from_numpy(w.t).pin_memory()
@@ -250,6 +250,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-sectors", type=int, default=4, help="sectors of the workload the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--param", action="append", default=[], help="library tunable name=value (tpc_set_param), e.g. chunk=1024")
     args = ap.parse_args()
     rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
     if args.impl == "reference":

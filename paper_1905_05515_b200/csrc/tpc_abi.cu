@@ -85,7 +85,7 @@ struct Tunables {   // DESIGN.md table T
   int min_hits = 10;
   double grid_min = 1.0, grid_max = 64.0, grid_scale = 1.0;
   int debug_keep = 0;
-  int chunk = 512;            // clusters per K2/K3 work item (multiple of 32)
+  int chunk = 1024;           // clusters per K2/K3 work item (multiple of 32)
 };
 
 struct UnitSrc { long long src = 0; int n = 0; };

@@ -45,13 +45,11 @@ struct Params {
 struct Item { int unit; int start; };
 
 // ---- device helpers ------------------------------------------------------------------------------------------------
-// S1 bin of a coordinate: fp32 subtract, fp32 multiply (no FMA), negative / NaN -> 0, clamp to nb-1.
+// S1 bin of a coordinate: fp32 subtract, fp32 multiply (no FMA), negative / NaN -> 0, clamp to nb-1, truncate.
+// (fmaxf(NaN, 0) = 0; clamping before the truncation gives the same integer as truncating first: nb-1 < 2^24 is exact in fp32.)
 __device__ __forceinline__ int bin_of(float v, float lo, float inv, int nb) {
-  float f = __fmul_rn(__fsub_rn(v, lo), inv);
-  if (!(f > 0.0f)) return 0;
-  if (f >= (float)nb) return nb - 1;
-  int b = (int)f;
-  return b > nb - 1 ? nb - 1 : b;
+  const float f = __fmul_rn(__fsub_rn(v, lo), inv);
+  return __float2int_rz(fminf(fmaxf(f, 0.0f), (float)(nb - 1)));
 }
 
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
