@@ -184,8 +184,20 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
     if (!wu.wide && !wd.wide && wu.n <= 32 && wd.n <= 32) {
       // flat scan: one loop per side marks the in-window candidates, then the pair search walks the set bits
       unsigned mu = 0u, md = 0u;
-      for (int j = 0; j < wd.n; j++) { const int q = j < wd.n0 ? wd.a0 + j : wd.a1 + (j - wd.n0); if (in_win(yzd[q], wd)) md |= 1u << j; }
-      if (md) for (int j = 0; j < wu.n; j++) { const int p = j < wu.n0 ? wu.a0 + j : wu.a1 + (j - wu.n0); if (in_win(yzu[p], wu)) mu |= 1u << j; }
+      {   // down window first: without a down candidate there is no pair and the up scan is skipped
+        int j = 0;
+#pragma unroll 1
+        for (int q = wd.a0; j < wd.n0; q++, j++) if (in_win(yzd[q], wd)) md |= 1u << j;
+#pragma unroll 1
+        for (int q = wd.a1; j < wd.n; q++, j++) if (in_win(yzd[q], wd)) md |= 1u << j;
+      }
+      if (md) {
+        int j = 0;
+#pragma unroll 1
+        for (int p = wu.a0; j < wu.n0; p++, j++) if (in_win(yzu[p], wu)) mu |= 1u << j;
+#pragma unroll 1
+        for (int p = wu.a1; j < wu.n; p++, j++) if (in_win(yzu[p], wu)) mu |= 1u << j;
+      }
       while (mu) {
         const int j = __ffs(mu) - 1; mu &= mu - 1u;
         const int p = j < wu.n0 ? wu.a0 + j : wu.a1 + (j - wu.n0);
