@@ -172,6 +172,7 @@ __device__ __forceinline__ int pickup(const UnitDesc& d, const float2* __restric
     const int pa0 = bs[ra + by0], pb0 = bs[ra + by1 + 1];
     const int pa1 = two ? bs[rb + by0] : 0, pb1 = two ? bs[rb + by1 + 1] : 0;
     const int n0 = pb0 - pa0, total = n0 + (pb1 - pa1);
+#pragma unroll 1
     for (int k = 0; k < total; k++) {
       const int p = k < n0 ? pa0 + k : pa1 + (k - n0);
       const float2 c = hits[p];
