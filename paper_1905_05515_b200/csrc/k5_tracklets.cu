@@ -208,7 +208,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
   const unsigned FULL = 0xffffffffu;
   const int R = P.R, lane = threadIdx.x & 31;
   int mode = MD_FETCH;
-  int i = -1, r0 = 0, h0 = 0, r = 0, nxt = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
+  int i = -1, r0 = 0, h0 = 0, r = 0, nxt = -1, a_next = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
   float zref = 0.0f, chi2 = 0.0f;
   float2 c0 = make_float2(0.f, 0.f);
   State st = {};
@@ -251,11 +251,16 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     const bool moving = mode == MD_A || mode == MD_B || mode == MD_C;
     const int rn = mode == MD_C ? r - 1 : r + 1;
     bool prop_ok = true;
+    // measurement prefetch: a linked (phase A) or already assigned (phase C) cluster of the target row is known before the
+    // transport, so its load is issued here and its latency hides behind the transport arithmetic
+    const int hit_pref = mode == MD_A ? nxt : (mode == MD_C ? a_next : -1);
+    float2 c_pref = make_float2(0.f, 0.f);
+    if (hit_pref >= 0) c_pref = yz[su[rn].off + hit_pref];
     __syncwarp();
     if (moving) { n_prop++; prop_ok = propagate(st, rows[rn].x - rows[r].x, P); }
 
     // ---- 2a. per-phase decision: which measurement this step uses (a linked / assigned hit, a pick-up, or none)
-    bool have = false, finish = false, do_pick = false, load_hit = false;
+    bool have = false, finish = false, do_pick = false;
     float2 c = c0;
     int hit = -1;
     if (mode == MD_INIT) {          // Phase A start: direction from the origin, first update with the start hit
@@ -266,7 +271,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
       have = true; hit = h0;
     } else if (mode == MD_A) {      // follow the cleaned up-link, no gate
       if (!prop_ok) mode = MD_TRANS;
-      else { hit = nxt; load_hit = true; have = true; }
+      else { hit = nxt; c = c_pref; have = true; }
     } else if (mode == MD_B) {      // outward extrapolation with pick-up
       if (!prop_ok || fabsf(st.y) > rows[rn].yedge + P.edge_margin) mode = MD_TRANS;
       else { do_pick = true; r = rn; }
@@ -278,9 +283,9 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     } else if (mode == MD_C) {
       if (!prop_ok) finish = true;
       else {
-        const int a = rn >= r0 ? rh[rn] : -1;   // rows below r0 were never visited before
+        const int a = a_next;                   // rowhit of this row, read one step ahead (-1 below r0: never visited before)
         r = rn;
-        if (a >= 0) { hit = a; load_hit = true; have = true; }
+        if (a >= 0) { hit = a; c = c_pref; have = true; }
         else if (fabsf(st.y) > rows[rn].yedge + P.edge_margin) {
           if (rn < first_assigned) finish = true;
           else if (rn < r0) rh[rn] = -1;       // skipped row inside the tracklet's range: reads as "no cluster"
@@ -302,7 +307,6 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
         else if (rn < first_assigned && ++gap > P.max_gap) finish = true;
       }
     }
-    if (load_hit) c = yz[su[rn].off + hit];
 
     // ---- 3. Kalman update (all lanes that have a measurement, whatever their phase)
     float dchi = 0.0f;
@@ -329,11 +333,12 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     } else if (mode == MD_TRANS) {
       if (have) {                   // (have is false only for lanes that switched to MD_TRANS in step 2 of this iteration)
         chi2 = chi2 + dchi; n = 1; r_snap = r_out; save_snap = true;
-        if (r_out - 1 >= 0) mode = MD_C; else finish = true;
+        if (r_out - 1 >= 0) { mode = MD_C; a_next = r_out - 1 >= r0 ? rh[r_out - 1] : -1; } else finish = true;
       }
     } else if (mode == MD_C) {
       if (have) { chi2 = chi2 + dchi; n++; r_snap = rn; save_snap = true; }
       if (!finish && rn == 0) finish = true;
+      if (!finish) a_next = rn - 1 >= r0 ? rh[rn - 1] : -1;
     }
 
     if (save_snap) { s_snap[0][tx] = st.y; s_snap[1][tx] = st.z; s_snap[2][tx] = st.s; s_snap[3][tx] = st.t; s_snap[4][tx] = st.q;
