@@ -234,7 +234,8 @@ def run_gpu(args, rank, world, local_rank):
            "realtime_factor": (w.params.t_frame * 1e-3 * world) / ms if w.params.t_frame > 0 else None,
            "e2e": {"value": total_clusters / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h},
-           "gpu_launches": int(launches), "kernel_ms": kern, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
+           "gpu_launches": int(launches), "kernel_ms": kern,
+           "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
            "clocks": clocks}
     print(json.dumps(out))
     if world > 1:

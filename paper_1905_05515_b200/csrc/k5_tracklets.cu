@@ -173,16 +173,27 @@ __device__ __forceinline__ int pickup(const UnitDesc& d, const float2* __restric
     const int pa1 = two ? bs[rb + by0] : 0, pb1 = two ? bs[rb + by1 + 1] : 0;
     const int n0 = pb0 - pa0, total = n0 + (pb1 - pa1);
 #pragma unroll 1
-    for (int k = 0; k < total; k++) {
-      const int p = k < n0 ? pa0 + k : pa1 + (k - n0);
-      const float2 c = hits[p];
-      const float yc = c.x, zc = c.y - zref;
-      if (!(yc >= ylo && yc <= yhi && zc >= zlo && zc <= zhi)) continue;
-      const float dy = yc - y, dz = zc - zr;
-      const float dd = dy * dy + dz * dz;
-      bool better = best < 0 || dd < bestd;
-      if (best >= 0 && dd == bestd) better = perm[d.off + p] < perm[d.off + best];
-      if (better) { best = p; bestd = dd; *hit = c; }
+    for (int k0 = 0; k0 < total; k0 += 2) {   // two candidates per round: their loads are independent and issued together
+      float2 cc[2];
+#pragma unroll
+      for (int j = 0; j < 2; j++) {
+        const int k = k0 + j;
+        cc[j] = k < total ? hits[k < n0 ? pa0 + k : pa1 + (k - n0)] : make_float2(0.f, 0.f);
+      }
+#pragma unroll
+      for (int j = 0; j < 2; j++) {
+        const int k = k0 + j;
+        const float2 c = cc[j];
+        const float yc = c.x, zc = c.y - zref;
+        if (k < total && yc >= ylo && yc <= yhi && zc >= zlo && zc <= zhi) {
+          const int p = k < n0 ? pa0 + k : pa1 + (k - n0);
+          const float dy = yc - y, dz = zc - zr;
+          const float dd = dy * dy + dz * dz;
+          bool better = best < 0 || dd < bestd;
+          if (best >= 0 && dd == bestd) better = perm[d.off + p] < perm[d.off + best];
+          if (better) { best = p; bestd = dd; *hit = c; }
+        }
+      }
     }
   }
   return best;
@@ -208,7 +219,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
   const unsigned FULL = 0xffffffffu;
   const int R = P.R, lane = threadIdx.x & 31;
   int mode = MD_FETCH;
-  int i = -1, r0 = 0, h0 = 0, r = 0, nxt = -1, a_next = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
+  int i = -1, r0 = 0, h0 = 0, r = 0, nxt = -1, a_next = -1, a_next2 = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
   float zref = 0.0f, chi2 = 0.0f;
   float2 c0 = make_float2(0.f, 0.f);
   State st = {};
@@ -333,12 +344,13 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     } else if (mode == MD_TRANS) {
       if (have) {                   // (have is false only for lanes that switched to MD_TRANS in step 2 of this iteration)
         chi2 = chi2 + dchi; n = 1; r_snap = r_out; save_snap = true;
-        if (r_out - 1 >= 0) { mode = MD_C; a_next = r_out - 1 >= r0 ? rh[r_out - 1] : -1; } else finish = true;
+        if (r_out - 1 >= 0) { mode = MD_C; a_next = r_out - 1 >= r0 ? rh[r_out - 1] : -1; a_next2 = r_out - 2 >= r0 ? rh[r_out - 2] : -1; }
+        else finish = true;
       }
     } else if (mode == MD_C) {
       if (have) { chi2 = chi2 + dchi; n++; r_snap = rn; save_snap = true; }
       if (!finish && rn == 0) finish = true;
-      if (!finish) a_next = rn - 1 >= r0 ? rh[rn - 1] : -1;
+      if (!finish) { a_next = a_next2; a_next2 = rn - 2 >= r0 ? rh[rn - 2] : -1; }   // rowhit is read two rows ahead
     }
 
     if (save_snap) { s_snap[0][tx] = st.y; s_snap[1][tx] = st.z; s_snap[2][tx] = st.s; s_snap[3][tx] = st.t; s_snap[4][tx] = st.q;
