@@ -219,9 +219,8 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
   const unsigned FULL = 0xffffffffu;
   const int R = P.R, lane = threadIdx.x & 31;
   int mode = MD_FETCH;
-  int i = -1, r0 = 0, h0 = 0, r = 0, nxt = -1, a_next = -1, a_next2 = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
+  int i = -1, r0 = 0, r = 0, nxt = -1, a_next = -1, a_next2 = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
   float zref = 0.0f, chi2 = 0.0f;
-  float2 c0 = make_float2(0.f, 0.f);
   State st = {};
   __shared__ float s_snap[20][K5_THREADS];   // state after the last Phase-C update, per lane (written often, read once)
   const int tx = threadIdx.x;
@@ -242,13 +241,12 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
         i = base + __popc(need & ((1u << lane) - 1u));
         if (i < M) {
           const int u0 = start_unit[i];
-          h0 = start_pos[i];
+          const int h0 = start_pos[i];
           const int sec = u0 / R;
           r0 = u0 - sec * R;
           su = units + (long long)sec * R;
           rh = rowhit + (long long)i * R;
-          c0 = yz[su[r0].off + h0];
-          zref = c0.y;
+          zref = yz[su[r0].off + h0].y;
           mode = MD_INIT;
         } else {
           mode = MD_EXIT;
@@ -272,14 +270,17 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
 
     // ---- 2a. per-phase decision: which measurement this step uses (a linked / assigned hit, a pick-up, or none)
     bool have = false, finish = false, do_pick = false;
-    float2 c = c0;
+    float2 c = make_float2(0.f, 0.f);
     int hit = -1;
-    if (mode == MD_INIT) {          // Phase A start: direction from the origin, first update with the start hit
+    if (mode == MD_INIT) {
+      hit = start_pos[i];
+      c = yz[su[r0].off + hit];
+      const float2 c0 = c;          // Phase A start: direction from the origin, first update with the start hit
       const float x = rows[r0].x, y = c0.x;
       const float rr = sqrtf(x * x + y * y);
       st.y = y; st.z = 0.0f; st.s = y / rr; st.t = P.continuous ? 0.0f : zref / rr; st.q = 0.0f;
       reset_cov(st, P);
-      have = true; hit = h0;
+      have = true;
     } else if (mode == MD_A) {      // follow the cleaned up-link, no gate
       if (!prop_ok) mode = MD_TRANS;
       else { hit = nxt; c = c_pref; have = true; }
@@ -328,9 +329,9 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     // ---- 4. bookkeeping and phase transitions
     bool save_snap = false;
     if (mode == MD_INIT) {
-      rh[r0] = h0; r = r0;
-      s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = r0; s_sv[5][tx] = c0.x; s_sv[6][tx] = c0.y;
-      nxt = link_up[su[r0].off + h0];
+      rh[r0] = hit; r = r0;
+      s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = r0; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y;
+      nxt = link_up[su[r0].off + hit];
       gap = 0;
       mode = nxt >= 0 ? MD_A : (r0 + 1 < R ? MD_B : MD_TRANS);
     } else if (mode == MD_A) {      // (a failed transport already switched the lane to MD_TRANS)
