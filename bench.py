@@ -203,8 +203,10 @@ def run_gpu(args, rank, world, local_rank):
     alu_peak = 148 * 128 * sm_max * 1e6 / 1e12      # TFLOP/s, one fp32 op per lane per clock (FMA contraction is off)
     traffic = {}
     tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp))
+    if os.path.exists(tp):            # DRAM bytes per launch from the committed ncu --set full capture (only for its workload)
+        tj = json.load(open(tp))
+        if tj.get("workload") == f"C{args.config}":
+            traffic = tj.get("bytes_per_launch", {})
     roofs = {}
     for name, key in (("grid", "ms_grid"), ("neighbours", "ms_neighbours"), ("clean_start", "ms_clean_start")):
         a = BYTES_PER_CLUSTER[name] * N / (kern[key] * 1e-3) / 1e9
