@@ -202,11 +202,12 @@ def run_gpu(args, rank, world, local_rank):
     hbm_peak, peak_src, sm_max = _peaks()
     alu_peak = 148 * 128 * sm_max * 1e6 / 1e12      # TFLOP/s, one fp32 op per lane per clock (FMA contraction is off)
     traffic = {}
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):            # DRAM bytes per launch from the committed ncu --set full capture (only for its workload)
-        tj = json.load(open(tp))
-        if tj.get("workload") == f"C{args.config}":
-            traffic = tj.get("bytes_per_launch", {})
+    tp = os.path.join(ROOT, "profiles", f"traffic_c{args.config}.csv")   # DRAM bytes per launch from the committed ncu --set full capture
+    if os.path.exists(tp):
+        for line in open(tp):
+            f = line.strip().split(",")
+            if len(f) == 2 and f[1].isdigit():
+                traffic[f[0]] = int(f[1])
     roofs = {}
     for name, key in (("grid", "ms_grid"), ("neighbours", "ms_neighbours"), ("clean_start", "ms_clean_start")):
         a = BYTES_PER_CLUSTER[name] * N / (kern[key] * 1e-3) / 1e9
