@@ -179,7 +179,8 @@ def run_gpu(args, rank, world, local_rank):
     kern = {k: acc[k] / args.steps for k in keys}
     n_tracks, n_refs = res.n_tracks, res.n_cluster_refs
 
-    # ---- end-to-end arm: host buffers in, host tracks out, every step
+    # ---- end-to-end arm: host buffers in, host tracks out, every step.  Serial (one frame at a time: latency) and pipelined
+    #      (two contexts on two streams, one host thread each: the copies of one frame overlap the kernels of the other).
     for _ in range(min(args.warmup, 3)):
         trk.load_batch(w.unit_off, y_h, t_h); trk.find_tracks()
     barrier()
@@ -189,7 +190,41 @@ def run_gpu(args, rank, world, local_rank):
         hres = trk.find_tracks()
     e1.record(stream)
     barrier()
+    ms_e2e_serial = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    trks = [T.Tracker(**w.geometry(), **dict((kv.split("=")[0], float(kv.split("=")[1])) for kv in args.param)) for _ in streams]
+    for t_, s_ in zip(trks, streams):
+        t_.set_stream(s_.cuda_stream)
+        t_.load_batch(w.unit_off, y_h, t_h); t_.find_tracks()            # warm-up: buffers allocated
+    steps_of = [list(range(j, args.steps, 2)) for j in range(2)]
+    errs = []
+
+    def worker(j):
+        try:
+            torch.cuda.set_device(local_rank)
+            for _ in steps_of[j]:
+                trks[j].load_batch(w.unit_off, y_h, t_h)
+                trks[j].find_tracks()
+        except Exception as ex:      # noqa: BLE001
+            errs.append(ex)
+
+    barrier()
+    e0.record(stream)
+    for s_ in streams:
+        s_.wait_event(e0)
+    th = [threading.Thread(target=worker, args=(j,)) for j in range(2)]
+    [t_.start() for t_ in th]
+    [t_.join() for t_ in th]
+    for s_ in streams:
+        stream.wait_stream(s_)
+    e1.record(stream)
+    barrier()
+    if errs:
+        raise errs[0]
     ms_e2e = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    for t_ in trks:
+        t_.close()
     h2d = 2 * 4 * N
     d2h = hres.n_tracks * (4 + 4 + 20 + 60 + 4 + 4 + 4) + (hres.n_tracks + 1) * 8 + hres.n_cluster_refs * 8
     trk.close()
@@ -236,7 +271,8 @@ def run_gpu(args, rank, world, local_rank):
            "collisions_per_s": total_colls / (ms * 1e-3), "tracks_per_step": n_tracks, "cluster_refs_per_step": n_refs,
            "realtime_factor": (w.params.t_frame * 1e-3 * world) / ms if w.params.t_frame > 0 else None,
            "e2e": {"value": total_clusters / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d,
-                   "d2h_bytes_per_step": d2h},
+                   "d2h_bytes_per_step": d2h, "mode": "2 frames in flight (2 contexts, 2 streams): copies overlap kernels",
+                   "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
            "clocks": clocks}
