@@ -111,7 +111,7 @@ int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float*
                    int* d_perm, int* d_bin_start, int* d_cursor, const Params& P, int max_cursor_ints_smem, int max_n) {
   if (U <= 0) return 0;
   int threads = 128;
-  while (threads < 1024 && threads * 8 < max_n) threads <<= 1;   // about 8 clusters per thread and pass
+  while (threads < 1024 && threads * 16 < max_n) threads <<= 1;   // about 8-16 clusters per thread and pass: small CTAs, more of them per SM
   size_t smem = (size_t)max_cursor_ints_smem * sizeof(int);
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(k1_grid_build, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
