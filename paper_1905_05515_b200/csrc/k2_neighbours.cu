@@ -21,7 +21,7 @@ namespace tpc {
 namespace {
 
 constexpr int K2_THREADS = 256;
-constexpr int K2_STAGE_BYTES = 40 * 1024;
+constexpr int K2_STAGE_PER_CLUSTER = 40;   // staging bytes per cluster of the chunk: two neighbour slabs of (8 + 4) bytes + margin
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
                                                             const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
                                                             const float2* __restrict__ yz, const int* __restrict__ perm,
                                                             const int* __restrict__ bin_start, int* __restrict__ link_up,
-                                                            int* __restrict__ link_dn, const Params P) {
+                                                            int* __restrict__ link_dn, const Params P, const int stage_bytes) {
   extern __shared__ __align__(128) unsigned char s_stage[];
   __shared__ __align__(8) uint64_t s_bar;
   __shared__ Stage s_st;
@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
     const long long had0 = (dd.off + p0d) & ~1LL, had1 = (dd.off + p1d + 1) & ~1LL;
     const long long bau0 = gbu & ~3LL, bau1 = (gbu + nbu + 3) & ~3LL, bad0 = gbd & ~3LL, bad1 = (gbd + nbd + 3) & ~3LL;
     const long long hbu = (hau1 - hau0) * 8, hbd = (had1 - had0) * 8, bbu = (bau1 - bau0) * 4, bbd = (bad1 - bad0) * 4;
-    st.staged = hbu + hbd + bbu + bbd <= (long long)K2_STAGE_BYTES;
+    st.staged = hbu + hbd + bbu + bbd <= (long long)stage_bytes;
     if (st.staged) {
       st.pshift_u = (int)(hau0 - du.off); st.pshift_d = (int)(had0 - dd.off);
       st.bshift_u = (int)(bau0 - du.bin_off); st.bshift_d = (int)(bad0 - dd.bin_off);
@@ -238,13 +238,13 @@ int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int 
                          const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up,
                          int* d_link_dn, const Params& P) {
   if (n_items <= 0) return 0;
-  {
-    cudaError_t e = cudaFuncSetAttribute(k2_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, K2_STAGE_BYTES);
-    if (e != cudaSuccess) return -(int)e;
-  }
-  k2_neighbours<<<n_items, K2_THREADS, K2_STAGE_BYTES, L.stream>>>(d_items, chunk, d_units, d_rows, d_yz, d_perm, d_bin_start,
-                                                                    d_link_up, d_link_dn, P);
-  cudaError_t e = cudaGetLastError();
+  const int stage_bytes = ((chunk * K2_STAGE_PER_CLUSTER + 4096) + 127) & ~127;
+  const int threads = L.k2_threads > 0 ? L.k2_threads : K2_THREADS;
+  cudaError_t e = cudaFuncSetAttribute(k2_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, stage_bytes);
+  if (e != cudaSuccess) return -(int)e;
+  k2_neighbours<<<n_items, threads, stage_bytes, L.stream>>>(d_items, chunk, d_units, d_rows, d_yz, d_perm, d_bin_start, d_link_up,
+                                                           d_link_dn, P, stage_bytes);
+  e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }
 

@@ -86,6 +86,7 @@ struct Tunables {   // DESIGN.md table T
   double grid_min = 1.0, grid_max = 64.0, grid_scale = 1.0;
   int debug_keep = 0;
   int chunk = 1024;           // clusters per K2/K3 work item (multiple of 32)
+  int k2_threads = 0;         // K2 block size (0 = default 256); tuning knob
 };
 
 struct UnitSrc { long long src = 0; int n = 0; };
@@ -259,6 +260,7 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "min_hits") { if (v < 3 || v > 255) return fail(c, TPC_E_ARG, "min_hits must be in 3..255 (ndf = 2n-5 > 0)"); T.min_hits = (int)v; }
   else if (s == "grid_scale") rc = pos(T.grid_scale);
   else if (s == "debug_keep") T.debug_keep = v != 0;
+  else if (s == "k2_threads") { int k = (int)v; if (k < 32 || k > 256 || (k & 31)) return fail(c, TPC_E_ARG, "k2_threads must be a multiple of 32 in 32..256"); T.k2_threads = k; }
   else if (s == "chunk") { int k = (int)v; if (k < 32 || k > 4096 || (k & 31)) return fail(c, TPC_E_ARG, "chunk must be a multiple of 32 in 32..4096"); T.chunk = k; }
   else return fail(c, TPC_E_ARG, "tpc_set_param: unknown parameter '%s'", name);
   if (rc == TPC_OK) c->rows_valid = false;
@@ -401,7 +403,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   memset(out, 0, sizeof(*out));
   const int R = c->R, U = c->NS * R;
   cudaStream_t st = c->stream;
-  Launch L{st, c->sm_count};
+  Launch L{st, c->sm_count, c->T.k2_threads};
   long long launches = 0;
   c->have_result = false;
   tpc_timings& tm = c->timings; memset(&tm, 0, sizeof(tm));

@@ -82,6 +82,7 @@ __device__ __forceinline__ int block_excl_scan(int v, int* s_warp, int* total) {
 struct Launch {
   cudaStream_t stream;
   int sm_count;
+  int k2_threads;   // 0 = default
 };
 
 int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float* d_in_y, const float* d_in_t, float2* d_yz,
