@@ -173,3 +173,36 @@ def test_degenerate_units_dense_overflow_and_nonfinite():
     assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
     res = P.compare_tracks(o.tracks(), gtr)
     assert res["frac_identical"] >= 0.999 and res["param_mismatch"] == 0, res
+
+
+def test_abi_state_and_argument_errors_on_device():
+    import paper_1905_05515_b200 as T
+    w = W.config(1, scale=0.05)
+    with _tracker(w) as trk:
+        with pytest.raises(T.TpcError) as e:
+            trk.timings()                                    # nothing computed yet
+        assert e.value.code == -2
+        with pytest.raises(T.TpcError) as e:
+            trk.load(99, 0, np.zeros(1, np.float32), np.zeros(1, np.float32))
+        assert e.value.code == -1
+        with pytest.raises(T.TpcError) as e:
+            trk.load(0, 999, np.zeros(1, np.float32), np.zeros(1, np.float32))
+        assert e.value.code == -1
+        with pytest.raises(T.TpcError) as e:
+            trk.set_param("no_such_parameter", 1.0)
+        assert e.value.code == -1
+        trk.load_workload(w)
+        with pytest.raises(T.TpcError) as e:
+            trk.set_param("wy", 2.0)                         # tunables are frozen after the first load
+        assert e.value.code == -2
+        trk.find_tracks()
+        with pytest.raises(T.TpcError) as e:
+            trk.links(0, 5, cleaned=False)                   # raw links need debug_keep
+        assert e.value.code == -2
+        trk.clear()
+        trk.set_param("wy", 1.5)                             # allowed again after tpc_clear
+        # a second load of the same (sector,row) replaces the first
+        y = w.y[w.unit_off[7]:w.unit_off[8]]; t = w.t[w.unit_off[7]:w.unit_off[8]]
+        trk.load(0, 7, y[:3], t[:3]); trk.load(0, 7, y, t)
+        trk.find_tracks()
+        assert trk.grid(0, 7)["n"] == len(y)
