@@ -39,8 +39,8 @@ __device__ __forceinline__ void for_each_cluster(const float* __restrict__ in_y,
 __global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict__ units, const float* __restrict__ in_y,
                                                        const float* __restrict__ in_t, float2* __restrict__ yz,
                                                        int* __restrict__ perm, int* __restrict__ bin_start, int* __restrict__ cursor_g,
-                                                       const float zmax, const float vdrift) {
-  extern __shared__ int s_cnt[];
+                                                       const float zmax, const float vdrift, const int smem_ints) {
+  extern __shared__ __align__(16) int s_cnt[];
   __shared__ int s_warp[33];
   const UnitDesc d = units[blockIdx.x];
   const int n = d.n, ny = d.ny, nz = d.nz, nb = ny * nz;
@@ -49,14 +49,25 @@ __global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict
     for (int b = threadIdx.x; b <= nb; b += blockDim.x) bs[b] = 0;
     return;
   }
-  int* cnt = d.cur_off >= 0 ? cursor_g + d.cur_off : s_cnt;
+  // Shared-memory plan of this unit (ints): [0, nb) bin counters / cursors; then, when they fit, the sorted original
+  // indices (n) and the unit's (y, z) pairs (2n, 8-byte aligned).  Units too large for that keep them in global memory (L2).
+  const bool cnt_s = d.cur_off < 0;
+  const int perm_at = (nb + 1) & ~1;
+  const bool perm_s = cnt_s && perm_at + n <= smem_ints;
+  const int yz_at = (perm_at + n + 1) & ~1;
+  const bool yz_s = perm_s && yz_at + 2 * n <= smem_ints;
+  int* cnt = cnt_s ? s_cnt : cursor_g + d.cur_off;
+  int* __restrict__ pg = perm + d.off;
+  int* pm = perm_s ? s_cnt + perm_at : pg;
+  float2* syz = reinterpret_cast<float2*>(s_cnt + yz_at);
   for (int b = threadIdx.x; b < nb; b += blockDim.x) cnt[b] = 0;
   __syncthreads();
 
   // B: count.  S0: product rounded, then subtracted (no FMA).
-  for_each_cluster(in_y, in_t, d.src, n, [&](int, float y, float t) {
+  for_each_cluster(in_y, in_t, d.src, n, [&](int i, float y, float t) {
     float z = __fsub_rn(zmax, __fmul_rn(vdrift, t));
     int b = bin_of(z, d.zlo, d.invs, nz) * ny + bin_of(y, d.ylo, d.invs, ny);
+    if (yz_s) syz[i] = make_float2(y, z);
     atomicAdd(&cnt[b], 1);
   });
   __syncthreads();
@@ -75,13 +86,19 @@ __global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict
   __syncthreads();
 
   // D: scatter original indices to their bins (order inside a bin arbitrary here).
-  int* __restrict__ pm = perm + d.off;
-  for_each_cluster(in_y, in_t, d.src, n, [&](int i, float y, float t) {
-    float z = __fsub_rn(zmax, __fmul_rn(vdrift, t));
-    int b = bin_of(z, d.zlo, d.invs, nz) * ny + bin_of(y, d.ylo, d.invs, ny);
-    int pos = atomicAdd(&cnt[b], 1);
-    pm[pos] = i;
-  });
+  if (yz_s) {
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+      const float2 c = syz[i];
+      int b = bin_of(c.y, d.zlo, d.invs, nz) * ny + bin_of(c.x, d.ylo, d.invs, ny);
+      pm[atomicAdd(&cnt[b], 1)] = i;
+    }
+  } else {
+    for_each_cluster(in_y, in_t, d.src, n, [&](int i, float y, float t) {
+      float z = __fsub_rn(zmax, __fmul_rn(vdrift, t));
+      int b = bin_of(z, d.zlo, d.invs, nz) * ny + bin_of(y, d.ylo, d.invs, ny);
+      pm[atomicAdd(&cnt[b], 1)] = i;
+    });
+  }
   __syncthreads();
 
   // E1: canonical order inside each bin = ascending original index (insertion sort; bins hold about one cluster).
@@ -97,27 +114,38 @@ __global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict
 
   // E2: sorted payload, coalesced writes.
   float2* __restrict__ out = yz + d.off;
-  const float* py = in_y + d.src;
-  const float* pt = in_t + d.src;
-  for (int p = threadIdx.x; p < n; p += blockDim.x) {
-    int i = pm[p];
-    out[p] = make_float2(py[i], __fsub_rn(zmax, __fmul_rn(vdrift, pt[i])));
+  if (yz_s) {
+    for (int p = threadIdx.x; p < n; p += blockDim.x) { const int i = pm[p]; pg[p] = i; out[p] = syz[i]; }
+  } else {
+    const float* py = in_y + d.src;
+    const float* pt = in_t + d.src;
+    for (int p = threadIdx.x; p < n; p += blockDim.x) {
+      const int i = pm[p];
+      if (perm_s) pg[p] = i;
+      out[p] = make_float2(py[i], __fsub_rn(zmax, __fmul_rn(vdrift, pt[i])));
+    }
   }
 }
 
 }  // namespace
 
 int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float* d_in_y, const float* d_in_t, float2* d_yz,
-                   int* d_perm, int* d_bin_start, int* d_cursor, const Params& P, int max_cursor_ints_smem, int max_n) {
+                   int* d_perm, int* d_bin_start, int* d_cursor, const Params& P, int max_cursor_ints_smem, int max_n,
+                   int max_perm_ints, int max_yz_ints) {
   if (U <= 0) return 0;
   int threads = 128;
   while (threads < 1024 && threads * 16 < max_n) threads <<= 1;   // about 8-16 clusters per thread and pass: small CTAs, more of them per SM
-  size_t smem = (size_t)max_cursor_ints_smem * sizeof(int);
+  // Shared memory per CTA: the cursors always; the sorted indices and the (y, z) pairs too while that keeps >= 4 CTAs per SM
+  // (56 KB); the sorted indices alone up to 2 CTAs per SM (112 KB).
+  int ints = max_cursor_ints_smem;
+  if (max_yz_ints <= 14 * 1024) ints = ints > max_yz_ints ? ints : max_yz_ints;
+  else if (max_perm_ints <= 28 * 1024) ints = ints > max_perm_ints ? ints : max_perm_ints;
+  size_t smem = (size_t)ints * sizeof(int);
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(k1_grid_build, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return -(int)e;
   }
-  k1_grid_build<<<U, threads, smem, L.stream>>>(d_units, d_in_y, d_in_t, d_yz, d_perm, d_bin_start, d_cursor, P.zmax, P.vdrift);
+  k1_grid_build<<<U, threads, smem, L.stream>>>(d_units, d_in_y, d_in_t, d_yz, d_perm, d_bin_start, d_cursor, P.zmax, P.vdrift, ints);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }

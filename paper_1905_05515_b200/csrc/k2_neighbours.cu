@@ -61,12 +61,110 @@ struct Stage {          // written by thread 0, read by all
 // One search window on a neighbour row: candidate ranges of its (at most two) bin rows.
 struct Win {
   float ylo, yhi, zlo, zhi;
-  int a0, n0, a1, n;   // row 0: positions a0 .. a0+n0-1, row 1: a1 .. ; n = total candidates to test
+  int a0, n0, a1m, n;  // candidate j < n0 is position a0 + j (bin row 0), else a1m + j (bin row 1; a1m = start - n0); n = total
   bool wide;           // window spans more than two bin rows (tiny bins): generic path
 };
 
 __device__ __forceinline__ bool in_win(const float2 c, const Win& w) {
   return c.x >= w.ylo && c.x <= w.yhi && c.y >= w.zlo && c.y <= w.zhi;
+}
+__device__ __forceinline__ int win_pos(const Win& w, const int j) { return (j < w.n0 ? w.a0 : w.a1m) + j; }
+
+// Window scan + best pair for the `cnt` clusters `own[0..cnt)` of one chunk, one thread per cluster.  yzu / yzd / bsu / bsd are
+// indexed by row position / row bin; they point into the staging buffer (shared-memory instance) or into global memory
+// (fallback instance) -- the function is inlined at both call sites so that each instance knows its address space.
+__device__ __forceinline__ void search_chunk(const float2* __restrict__ yzu, const float2* __restrict__ yzd, const int* __restrict__ bsu,
+                                             const int* __restrict__ bsd, const float2* __restrict__ own, const int cnt,
+                                             int* __restrict__ lup, int* __restrict__ ldn, const UnitDesc& du, const UnitDesc& dd,
+                                             const RowConst& rc, const float hw_u, const float hw_d,
+                                             const int* __restrict__ permu, const int* __restrict__ permd, const Params& P) {
+  // window on a neighbour row: bounds (one fp32 op each) and the candidate ranges of its bin rows
+  auto make_win = [&](const float yc, const float zc, const float hw, const UnitDesc& g, const int* bs) {
+    Win w;
+    w.ylo = __fsub_rn(yc, P.wy); w.yhi = __fadd_rn(yc, P.wy); w.zlo = __fsub_rn(zc, hw); w.zhi = __fadd_rn(zc, hw);
+    const int by0 = bin_of(w.ylo, g.ylo, g.invs, g.ny), by1 = bin_of(w.yhi, g.ylo, g.invs, g.ny);
+    const int bz0 = bin_of(w.zlo, g.zlo, g.invs, g.nz), bz1 = bin_of(w.zhi, g.zlo, g.invs, g.nz);
+    w.wide = bz1 - bz0 > 1;
+    const int ra = bz0 * g.ny;
+    w.a0 = bs[ra + by0]; w.n0 = bs[ra + by1 + 1] - w.a0;
+    w.a1m = 0; w.n = w.n0;
+    if (bz1 > bz0) { const int rb = ra + g.ny; const int a1 = bs[rb + by0]; w.n += bs[rb + by1 + 1] - a1; w.a1m = a1 - w.n0; }
+    return w;
+  };
+  // one flat loop over the candidates of both bin rows of a window: bit j of the result = candidate j lies in the window
+  auto scan = [&](const float2* __restrict__ hits, const Win& w) {
+    unsigned m = 0u;
+#pragma unroll 1
+    for (int j = 0; j < w.n; j++) {
+      const float2 c = hits[win_pos(w, j)];
+      // m |= in_win(c, w) << j, as four chained ordered compares and one predicated OR (NaN compares false, as in in_win)
+      asm("{\n.reg .pred p;\n"
+          "setp.ge.f32 p, %1, %3;\n"
+          "setp.le.and.f32 p, %1, %4, p;\n"
+          "setp.ge.and.f32 p, %2, %5, p;\n"
+          "setp.le.and.f32 p, %2, %6, p;\n"
+          "@p or.b32 %0, %0, %7;\n}"
+          : "+r"(m) : "f"(c.x), "f"(c.y), "f"(w.ylo), "f"(w.yhi), "f"(w.zlo), "f"(w.zhi), "r"(1u << j));
+    }
+    return m;
+  };
+
+  for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
+    const float2 h = own[k];
+    const float y = h.x, z = h.y;
+    const Win wu = make_win(__fmul_rn(y, rc.tu), P.continuous ? z : __fmul_rn(z, rc.tu), hw_u, du, bsu);
+    const Win wd = make_win(__fmul_rn(y, rc.td), P.continuous ? z : __fmul_rn(z, rc.td), hw_d, dd, bsd);
+
+    bool have = false; float bestD = 0.0f; int bu = -1, bd = -1;
+    auto pair = [&](const int p, const float2 cu, const int q, const float2 cd) {
+      const float ey = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.x, y)), __fmul_rn(rc.a, __fsub_rn(y, cd.x)));
+      const float ez = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.y, z)), __fmul_rn(rc.a, __fsub_rn(z, cd.y)));
+      const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+      bool better = !have || D < bestD;
+      if (have && D == bestD) {   // tie: lower original index of the up cluster, then of the down cluster (rare: global reads)
+        const int iu = permu[p], ib = permu[bu];
+        better = iu < ib || (iu == ib && permd[q] < permd[bd]);
+      }
+      if (better) { have = true; bestD = D; bu = p; bd = q; }
+    };
+
+    if (!wu.wide && !wd.wide && wu.n <= 32 && wd.n <= 32) {
+      // flat scan per side marks the in-window candidates, then the pair search walks the set bits.
+      // Down window first: without a down candidate there is no pair and the up scan is skipped.
+      const unsigned md = scan(yzd, wd);
+      unsigned mu = md ? scan(yzu, wu) : 0u;
+      while (mu) {
+        const int j = __ffs(mu) - 1; mu &= mu - 1u;
+        const int p = win_pos(wu, j);
+        const float2 cu = yzu[p];
+        unsigned m = md;
+        while (m) {
+          const int i = __ffs(m) - 1; m &= m - 1u;
+          const int q = win_pos(wd, i);
+          pair(p, cu, q, yzd[q]);
+        }
+      }
+    } else {
+      // generic path (bins smaller than the window, or very dense rows): nested scan over all bin rows of both windows
+      const int by0u = bin_of(wu.ylo, du.ylo, du.invs, du.ny), by1u = bin_of(wu.yhi, du.ylo, du.invs, du.ny);
+      const int bz0u = bin_of(wu.zlo, du.zlo, du.invs, du.nz), bz1u = bin_of(wu.zhi, du.zlo, du.invs, du.nz);
+      const int by0d = bin_of(wd.ylo, dd.ylo, dd.invs, dd.ny), by1d = bin_of(wd.yhi, dd.ylo, dd.invs, dd.ny);
+      const int bz0d = bin_of(wd.zlo, dd.zlo, dd.invs, dd.nz), bz1d = bin_of(wd.zhi, dd.zlo, dd.invs, dd.nz);
+      for (int bz = bz0u; bz <= bz1u; bz++)
+        for (int p = bsu[bz * du.ny + by0u]; p < bsu[bz * du.ny + by1u + 1]; p++) {
+          const float2 cu = yzu[p];
+          if (!in_win(cu, wu)) continue;
+          for (int bzd = bz0d; bzd <= bz1d; bzd++)
+            for (int q = bsd[bzd * dd.ny + by0d]; q < bsd[bzd * dd.ny + by1d + 1]; q++) {
+              const float2 cd = yzd[q];
+              if (in_win(cd, wd)) pair(p, cu, q, cd);
+            }
+        }
+    }
+    const bool ok = have && bestD < rc.thr;
+    lup[k] = ok ? bu : -1;
+    ldn[k] = ok ? bd : -1;
+  }
 }
 
 __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restrict__ items, const int chunk,
@@ -135,100 +233,17 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
   }
   __syncthreads();
   const Stage st = s_st;
-  const float2* yzu; const float2* yzd; const int* bsu; const int* bsd;
-  if (st.staged) {
-    yzu = reinterpret_cast<const float2*>(s_stage); yzd = reinterpret_cast<const float2*>(s_stage + st.hoff_d);
-    bsu = reinterpret_cast<const int*>(s_stage + st.boff_u); bsd = reinterpret_cast<const int*>(s_stage + st.boff_d);
-    mbar_wait(&s_bar, 0);
-  } else {
-    yzu = yz + du.off; yzd = yz + dd.off; bsu = bin_start + du.bin_off; bsd = bin_start + dd.bin_off;
-  }
-  yzu -= st.pshift_u; yzd -= st.pshift_d; bsu -= st.bshift_u; bsd -= st.bshift_d;   // index by row position / row bin directly
   const int* __restrict__ permu = perm + du.off;
   const int* __restrict__ permd = perm + dd.off;
-
-  // window on a neighbour row: bounds (one fp32 op each) and the candidate ranges of its bin rows
-  auto make_win = [&](const float yc, const float zc, const float hw, const UnitDesc& g, const int* bs) {
-    Win w;
-    w.ylo = __fsub_rn(yc, P.wy); w.yhi = __fadd_rn(yc, P.wy); w.zlo = __fsub_rn(zc, hw); w.zhi = __fadd_rn(zc, hw);
-    const int by0 = bin_of(w.ylo, g.ylo, g.invs, g.ny), by1 = bin_of(w.yhi, g.ylo, g.invs, g.ny);
-    const int bz0 = bin_of(w.zlo, g.zlo, g.invs, g.nz), bz1 = bin_of(w.zhi, g.zlo, g.invs, g.nz);
-    w.wide = bz1 - bz0 > 1;
-    const int ra = bz0 * g.ny;
-    w.a0 = bs[ra + by0]; w.n0 = bs[ra + by1 + 1] - w.a0;
-    w.a1 = 0; w.n = w.n0;
-    if (bz1 > bz0) { const int rb = ra + g.ny; w.a1 = bs[rb + by0]; w.n += bs[rb + by1 + 1] - w.a1; }
-    return w;
-  };
-
-  // ---- window scan + best pair, one thread per cluster
-  for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
-    const float2 h = own[k];
-    const float y = h.x, z = h.y;
-    const Win wu = make_win(__fmul_rn(y, rc.tu), P.continuous ? z : __fmul_rn(z, rc.tu), hw_u, du, bsu);
-    const Win wd = make_win(__fmul_rn(y, rc.td), P.continuous ? z : __fmul_rn(z, rc.td), hw_d, dd, bsd);
-
-    bool have = false; float bestD = 0.0f; int bu = -1, bd = -1;
-    auto pair = [&](const int p, const float2 cu, const int q, const float2 cd) {
-      const float ey = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.x, y)), __fmul_rn(rc.a, __fsub_rn(y, cd.x)));
-      const float ez = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.y, z)), __fmul_rn(rc.a, __fsub_rn(z, cd.y)));
-      const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
-      bool better = !have || D < bestD;
-      if (have && D == bestD) {   // tie: lower original index of the up cluster, then of the down cluster (rare: global reads)
-        const int iu = permu[p], ib = permu[bu];
-        better = iu < ib || (iu == ib && permd[q] < permd[bd]);
-      }
-      if (better) { have = true; bestD = D; bu = p; bd = q; }
-    };
-
-    if (!wu.wide && !wd.wide && wu.n <= 32 && wd.n <= 32) {
-      // flat scan: one loop per side marks the in-window candidates, then the pair search walks the set bits
-      unsigned mu = 0u, md = 0u;
-      {   // down window first: without a down candidate there is no pair and the up scan is skipped
-        int j = 0;
-#pragma unroll 1
-        for (int q = wd.a0; j < wd.n0; q++, j++) if (in_win(yzd[q], wd)) md |= 1u << j;
-#pragma unroll 1
-        for (int q = wd.a1; j < wd.n; q++, j++) if (in_win(yzd[q], wd)) md |= 1u << j;
-      }
-      if (md) {
-        int j = 0;
-#pragma unroll 1
-        for (int p = wu.a0; j < wu.n0; p++, j++) if (in_win(yzu[p], wu)) mu |= 1u << j;
-#pragma unroll 1
-        for (int p = wu.a1; j < wu.n; p++, j++) if (in_win(yzu[p], wu)) mu |= 1u << j;
-      }
-      while (mu) {
-        const int j = __ffs(mu) - 1; mu &= mu - 1u;
-        const int p = j < wu.n0 ? wu.a0 + j : wu.a1 + (j - wu.n0);
-        const float2 cu = yzu[p];
-        unsigned m = md;
-        while (m) {
-          const int i = __ffs(m) - 1; m &= m - 1u;
-          const int q = i < wd.n0 ? wd.a0 + i : wd.a1 + (i - wd.n0);
-          pair(p, cu, q, yzd[q]);
-        }
-      }
-    } else {
-      // generic path (bins smaller than the window, or very dense rows): nested scan over all bin rows of both windows
-      const int by0u = bin_of(wu.ylo, du.ylo, du.invs, du.ny), by1u = bin_of(wu.yhi, du.ylo, du.invs, du.ny);
-      const int bz0u = bin_of(wu.zlo, du.zlo, du.invs, du.nz), bz1u = bin_of(wu.zhi, du.zlo, du.invs, du.nz);
-      const int by0d = bin_of(wd.ylo, dd.ylo, dd.invs, dd.ny), by1d = bin_of(wd.yhi, dd.ylo, dd.invs, dd.ny);
-      const int bz0d = bin_of(wd.zlo, dd.zlo, dd.invs, dd.nz), bz1d = bin_of(wd.zhi, dd.zlo, dd.invs, dd.nz);
-      for (int bz = bz0u; bz <= bz1u; bz++)
-        for (int p = bsu[bz * du.ny + by0u]; p < bsu[bz * du.ny + by1u + 1]; p++) {
-          const float2 cu = yzu[p];
-          if (!in_win(cu, wu)) continue;
-          for (int bzd = bz0d; bzd <= bz1d; bzd++)
-            for (int q = bsd[bzd * dd.ny + by0d]; q < bsd[bzd * dd.ny + by1d + 1]; q++) {
-              const float2 cd = yzd[q];
-              if (in_win(cd, wd)) pair(p, cu, q, cd);
-            }
-        }
-    }
-    const bool ok = have && bestD < rc.thr;
-    lup[k] = ok ? bu : -1;
-    ldn[k] = ok ? bd : -1;
+  if (st.staged) {
+    // shared-memory instance: the four regions are addressed from the staging buffer directly (LDS with 32-bit addresses)
+    mbar_wait(&s_bar, 0);
+    search_chunk(reinterpret_cast<const float2*>(s_stage) - st.pshift_u, reinterpret_cast<const float2*>(s_stage + st.hoff_d) - st.pshift_d,
+                 reinterpret_cast<const int*>(s_stage + st.boff_u) - st.bshift_u, reinterpret_cast<const int*>(s_stage + st.boff_d) - st.bshift_d,
+                 own, cnt, lup, ldn, du, dd, rc, hw_u, hw_d, permu, permd, P);
+  } else {
+    search_chunk(yz + du.off, yz + dd.off, bin_start + du.bin_off, bin_start + dd.bin_off, own, cnt, lup, ldn, du, dd, rc, hw_u, hw_d,
+                 permu, permd, P);
   }
 }
 

@@ -370,11 +370,11 @@ void make_params_and_rows(tpc_ctx* c, std::vector<RowConst>& rows) {
 }
 
 // S1 grid descriptor of every unit + CSR offsets + K2/K3 work items.  Returns a tpc_status.
-int make_units(tpc_ctx* c, int* max_smem_cursor, long long* cursor_total, int* max_n) {
+int make_units(tpc_ctx* c, int* max_smem_cursor, long long* cursor_total, int* max_n, int* max_perm, int* max_yz) {
   const Tunables& T = c->T; const int R = c->R, U = c->NS * R;
   c->h_units.resize(U); c->h_items.clear();
   const double dphi = (double)c->dphi, vd = (double)c->vdrift, tf = (double)c->t_frame, zmax = (double)c->z_max;
-  long long off = 0, boff = 0, coff = 0; int msm = 0, mn = 0;
+  long long off = 0, boff = 0, coff = 0; int msm = 0, mn = 0; long long mperm = 0, myz = 0;
   for (int u = 0; u < U; u++) {
     const int r = u % R; const int n = c->usrc[u].n;
     const double ye = (double)c->row_x[r] * tan(0.5 * dphi);
@@ -388,13 +388,21 @@ int make_units(tpc_ctx* c, int* max_smem_cursor, long long* cursor_total, int* m
     d.ylo = (float)y_lo; d.zlo = (float)z_lo; d.invs = (float)(1.0 / s);
     d.n = n; d.off = off; d.src = c->usrc[u].src; d.bin_off = boff; d.pad[0] = d.pad[1] = 0;
     const long long nb = (long long)d.ny * d.nz;
-    if (nb + 1 <= K1_SMEM_CURSOR_MAX) { d.cur_off = -1; if (n > 0) msm = std::max(msm, (int)nb + 1); }
+    if (nb + 1 <= K1_SMEM_CURSOR_MAX) {
+      d.cur_off = -1;
+      if (n > 0) {   // K1 shared-memory plan: cursors, then sorted indices, then (y, z) pairs (k1_grid.cu)
+        msm = std::max(msm, (int)nb + 1);
+        const long long pa = (nb + 1) & ~1LL, ya = (pa + n + 1) & ~1LL;
+        mperm = std::max(mperm, pa + n); myz = std::max(myz, ya + 2LL * n);
+      }
+    }
     else { d.cur_off = coff; coff += nb + 1; }
     for (int s0 = 0; s0 < n; s0 += T.chunk) c->h_items.push_back(Item{u, s0});
     off += n; boff += nb + 1; mn = std::max(mn, n);
   }
   c->N = off; c->n_bins = boff; c->n_items = (int)c->h_items.size();
   *max_smem_cursor = msm; *cursor_total = coff; *max_n = mn;
+  *max_perm = (int)std::min(mperm, 1LL << 30); *max_yz = (int)std::min(myz, 1LL << 30);
   return TPC_OK;
 }
 
@@ -411,8 +419,8 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   // ---- host tables
   std::vector<RowConst> rows;
   make_params_and_rows(c, rows);
-  int msm = 0, max_n = 0; long long cursor_total = 0;
-  int rc = make_units(c, &msm, &cursor_total, &max_n);
+  int msm = 0, max_n = 0, max_perm = 0, max_yz = 0; long long cursor_total = 0;
+  int rc = make_units(c, &msm, &cursor_total, &max_n, &max_perm, &max_yz);
   if (rc != TPC_OK) return rc;
   const long long N = c->N; const int n_items = c->n_items; const int chunk = c->T.chunk;
   const Params& P = c->P;
@@ -459,7 +467,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
 
   // ---- K1: S0 + S1
   LAUNCH_TRY(c, launch_k1_grid(L, U, c->d_units.as<UnitDesc>(), c->d_in_y.as<float>(), c->d_in_t.as<float>(), c->d_yz.as<float2>(),
-                               c->d_perm.as<int>(), c->d_bin_start.as<int>(), c->d_cursor.as<int>(), P, std::max(msm, 1), max_n), launches);
+                               c->d_perm.as<int>(), c->d_bin_start.as<int>(), c->d_cursor.as<int>(), P, std::max(msm, 1), max_n, max_perm, max_yz), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[2], st));
   // ---- K2: S2
   LAUNCH_TRY(c, launch_k2_neighbours(L, n_items, c->d_items.as<Item>(), chunk, c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),

@@ -86,7 +86,8 @@ struct Launch {
 };
 
 int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float* d_in_y, const float* d_in_t, float2* d_yz,
-                   int* d_perm, int* d_bin_start, int* d_cursor, const Params& P, int max_cursor_ints_smem, int max_n);
+                   int* d_perm, int* d_bin_start, int* d_cursor, const Params& P, int max_cursor_ints_smem, int max_n,
+                   int max_perm_ints, int max_yz_ints);
 
 int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units,
                          const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up,
