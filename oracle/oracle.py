@@ -16,7 +16,7 @@ _SO = os.path.join(_HERE, "libtpc_oracle.so")
 _SRC = os.path.join(_HERE, "tpc_oracle.cpp")
 _KINDS = {0: (C.c_int32, np.int32), 1: (C.c_int64, np.int64), 2: (C.c_double, np.float64), 3: (C.c_float, np.float32)}
 
-STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6}
+STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6, "s7": 7}
 
 
 def build(force: bool = False) -> str:
@@ -129,6 +129,12 @@ class Oracle:
     def tracks(self):
         d = {k: self.get("trk_" + k) for k in ("sector", "ndf", "tracklet", "cl_begin", "cl_row", "cl_index", "x", "par",
                                                 "cov", "chi2")}
+        d["par"] = d["par"].reshape(-1, 5); d["cov"] = d["cov"].reshape(-1, 15)
+        return d
+
+    def refit(self):
+        """S7 (NEXT-1): refitted state of every S6 track over its owned clusters + collision-time estimate (run("s7") first)."""
+        d = {k: self.get("rf_" + k) for k in ("n", "ndf", "x", "par", "cov", "chi2", "z0", "t0")}
         d["par"] = d["par"].reshape(-1, 5); d["cov"] = d["cov"].reshape(-1, 15)
         return d
 

@@ -20,6 +20,7 @@
  * permutation invariance + straight lines; S3/S4 invariants; S5 propagate vs closed-form circle,
  * composition, round trip, Jacobian vs finite differences; S5 fit: noise-free helix recovery 1e-5,
  * Bz=0 exact, chi2/ndf = 1 and pulls on smeared tracks; S6 hand-built sharing cases, order invariance.
+ * S7 (NEXT-1) refit + collision time: noise-free recovery, chi2/ndf = 1, t0 against the generator's collision times.
  * Absolute efficiency / resolution versus the paper: parity unpinned (PAPER.md:49 gives no number).
  */
 #include <cmath>
@@ -80,6 +81,8 @@ struct Oracle : OracleBase {
   // S6
   std::vector<int32_t> trk_sector, trk_ndf, trk_tracklet, trk_cl_row, trk_cl_index; std::vector<int64_t> trk_cl_begin;
   std::vector<double> trk_x, trk_par, trk_cov, trk_chi2;
+  // S7 (NEXT-1): refit of the owned clusters + collision-time estimate
+  std::vector<int32_t> rf_n, rf_ndf; std::vector<double> rf_x, rf_par, rf_cov, rf_chi2, rf_z0, rf_t0;
   std::vector<double> z_d, ys_d, zs_d;   // export copies
 
   Oracle(int ns, int nr, const float* rx, double dphi_, double zmax, double tframe, double sy, double sz, double bz_, double vd)
@@ -411,6 +414,66 @@ struct Oracle : OracleBase {
     }
   }
 
+  // ---- S7 (NEXT-1; "improve the z-estimation"): refit of the clusters a track OWNS after the
+  //      selection, so that state, covariance and chi2/ndf describe the returned cluster list (reading A17 -> A37), and the
+  //      collision time of a continuous-read-out track from its extrapolation to the beam line (reading A38).
+  //      Pass 1 outward over the owned clusters (seed direction from the origin, C0), pass 2 inward with a fresh C0.
+  void s7_refit() {
+    int64_t NT = (int64_t)trk_sector.size();
+    rf_n.assign(NT, 0); rf_ndf.assign(NT, 0); rf_x.assign(NT, 0); rf_par.assign(NT * 5, 0); rf_cov.assign(NT * 15, 0);
+    rf_chi2.assign(NT, 0); rf_z0.assign(NT, 0); rf_t0.assign(NT, 0);
+    for (int64_t i = 0; i < NT; i++) {
+      const int sec = trk_sector[i]; const int64_t a = trk_cl_begin[i], m = trk_cl_begin[i + 1] - a;
+      const int32_t T_ = trk_tracklet[i];
+      auto row = [&](int64_t k) { return (int)trk_cl_row[a + k]; };
+      auto pos = [&](int64_t k) { return off[sec * R + row(k)] + tl_rowhit[(int64_t)T_ * R + row(k)]; };
+      const Real zref = zs[pos(0)];
+      State st;
+      { Real x = X[row(0)], y = ys[pos(0)]; Real rr = std::sqrt(x * x + y * y);
+        st.p[0] = y; st.p[1] = 0; st.p[2] = y / rr; st.p[3] = continuous ? (Real)0 : zref / rr; st.p[4] = 0; reset_cov(st); }
+      update_state(st, ys[pos(0)], (Real)0);
+      int64_t last = 0;
+      for (int64_t k = 1; k < m; k++) {                       // pass 1: outward
+        if (!propagate_state(st, X[row(k)] - X[row(k - 1)])) break;
+        update_state(st, ys[pos(k)], zs[pos(k)] - zref); last = k;
+      }
+      reset_cov(st);                                          // pass 2: inward from the outermost cluster reached
+      Real chi2 = 0; int n = 0;
+      chi2 = chi2 + update_state(st, ys[pos(last)], zs[pos(last)] - zref); n = 1;
+      State snap = st; int64_t kin = last;
+      for (int64_t k = last - 1; k >= 0; k--) {
+        if (!propagate_state(st, X[row(k)] - X[row(k + 1)])) break;
+        chi2 = chi2 + update_state(st, ys[pos(k)], zs[pos(k)] - zref); n++; snap = st; kin = k;
+      }
+      rf_n[i] = n; rf_ndf[i] = 2 * n - 5; rf_chi2[i] = (double)chi2; rf_x[i] = (double)X[row(kin)];
+      for (int k = 0; k < 5; k++) rf_par[i * 5 + k] = (double)snap.p[k];
+      const Real zabs = snap.p[1] + zref;
+      rf_par[i * 5 + 1] = (double)zabs;
+      int c = 0; for (int u = 0; u < 5; u++) for (int v = 0; v <= u; v++) rf_cov[i * 15 + c++] = (double)snap.C[u][v];
+      // collision time (A38): a primary passes the beam line (x = y = 0); the chord from there to the state point has length
+      // L, the arc over it S = L * asin(h)/h with h = k L / 2 (same series / switch as propagate_state); z at the beam line
+      // z0 = z - (dz/ds) * S; a collision at time t0 shifts the scaled z rigidly by -vdrift * t0 (A6), hence t0 = -z0 / vdrift.
+      { Real x = X[row(kin)], y = snap.p[0]; Real L = std::sqrt(x * x + y * y); Real k = cB * snap.p[4];
+        Real h = ((Real)0.5 * k) * L, h2 = h * h;
+        const Real hthr = sizeof(Real) == 4 ? (Real)0.25 : (Real)1e-3;
+        Real S;
+        if (std::fabs(h) < hthr) {
+          Real poly = (Real)(105.0 / 3456.0);
+          poly = (Real)(15.0 / 336.0) + h2 * poly;
+          poly = (Real)(3.0 / 40.0) + h2 * poly;
+          poly = (Real)(1.0 / 6.0) + h2 * poly;
+          poly = (Real)1 + h2 * poly;
+          S = L * poly;
+        } else {
+          if (h > (Real)1) h = (Real)1; if (h < (Real)-1) h = (Real)-1;
+          S = ((Real)2 / k) * std::asin(h);
+        }
+        Real z0 = zabs - snap.p[3] * S;
+        rf_z0[i] = (double)z0;
+        rf_t0[i] = (double)(-z0 / (Real)vdrift); }
+    }
+  }
+
   int run(int upto, int brute) override {
     make_tables();
     s0_time_to_z(); if (upto <= 0) return 0;
@@ -419,7 +482,8 @@ struct Oracle : OracleBase {
     s3_clean(); if (upto <= 3) return 0;
     s4_start_hits(); if (upto <= 4) return 0;
     s5_tracklets((brute & 2) != 0); if (upto <= 5) return 0;
-    s6_select();
+    s6_select(); if (upto <= 6) return 0;
+    s7_refit();
     return 0;
   }
 
@@ -486,6 +550,14 @@ struct Oracle : OracleBase {
     if (s == "trk_par") RET(trk_par, 2)
     if (s == "trk_cov") RET(trk_cov, 2)
     if (s == "trk_chi2") RET(trk_chi2, 2)
+    if (s == "rf_n") RET(rf_n, 0)
+    if (s == "rf_ndf") RET(rf_ndf, 0)
+    if (s == "rf_x") RET(rf_x, 2)
+    if (s == "rf_par") RET(rf_par, 2)
+    if (s == "rf_cov") RET(rf_cov, 2)
+    if (s == "rf_chi2") RET(rf_chi2, 2)
+    if (s == "rf_z0") RET(rf_z0, 2)
+    if (s == "rf_t0") RET(rf_t0, 2)
 #undef RET
     return -1;
   }
