@@ -178,6 +178,8 @@ def run_gpu(args, rank, world, local_rank):
     value = total_clusters / (ms * 1e-3)
     kern = {k: acc[k] / args.steps for k in keys}
     n_tracks, n_refs = res.n_tracks, res.n_cluster_refs
+    # S7 (NEXT-1, not part of the timed S0..S6 step): refit over the owned clusters + collision time, device-resident result
+    refit_ms = float(np.mean([trk.refit_tracks(device_result=True)["ms_refit"] for _ in range(4)][1:]))
 
     # ---- end-to-end arm: host buffers in, host tracks out, every step.  Serial (one frame at a time: latency) and pipelined
     #      (two contexts on two streams, one host thread each: the copies of one frame overlap the kernels of the other).
@@ -275,6 +277,7 @@ def run_gpu(args, rank, world, local_rank):
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
+           "refit": {"ms": refit_ms, "tracks_per_s": n_tracks / (refit_ms * 1e-3), "note": "S7 refit + collision time (SURVEY 8(f).1), outside the timed step"},
            "clocks": clocks}
     print(json.dumps(out))
     if world > 1:

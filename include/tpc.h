@@ -69,6 +69,22 @@ typedef struct {
   const int32_t* cl_index;  /* [n_cluster_refs] index into the caller's arrays of that (sector,row) as passed to tpc_load_clusters */
 } tpc_tracks;
 
+/* Result of tpc_refit_tracks: S7 of DESIGN.md section 4 ("first preliminary fit ... improve the
+ * z-estimation"; readings A37, A38).  One entry per track of the last tpc_find_tracks* call, same order.  Arrays are library-owned,
+ * host memory (device_result = 0) or device memory (device_result = 1), valid until the next call on the context. */
+typedef struct {
+  int64_t n_tracks;
+  const int32_t* n;         /* [n_tracks] clusters used by the inward pass (= owned clusters unless a transport failed) */
+  const int32_t* ndf;       /* [n_tracks] 2*n - 5 */
+  const float*   x;         /* [n_tracks] local x of the refitted state (row of the innermost cluster used) */
+  const float*   par;       /* [n_tracks][5]  y, z, sin(phi), dz/ds, q/pT after the refit over the owned clusters */
+  const float*   cov;       /* [n_tracks][15] lower triangle, row-major */
+  const float*   chi2;      /* [n_tracks] chi2 of the inward pass */
+  const float*   z0;        /* [n_tracks] scaled z of the track at the beam line (x = y = 0), cm */
+  const float*   t0;        /* [n_tracks] collision time estimate -z0 / vdrift, us (about 0 for a triggered primary) */
+  float ms_refit;           /* device time of K7 (CUDA events on the context's stream), ms */
+} tpc_refit;
+
 /* Per-step device times of the last tpc_find_tracks* call (CUDA events on the context's stream), ms. */
 typedef struct {
   float ms_upload;          /* host staging -> device (0 if the clusters were already device-resident) */
@@ -129,6 +145,10 @@ int tpc_load_clusters_batch(tpc_ctx*, const int64_t* unit_off, const float* pad_
 int tpc_find_tracks(tpc_ctx*, tpc_tracks* out);
 /* Same, but the result arrays stay in device memory (only the two counts are read back). */
 int tpc_find_tracks_device(tpc_ctx*, tpc_tracks* out);
+
+/* S7: refit every track of the last tpc_find_tracks* call over the clusters it owns and estimate its collision time.
+ * Errors: TPC_E_ARG (null), TPC_E_STATE (no completed tpc_find_tracks* call on this context), TPC_E_NOMEM, TPC_E_CUDA. */
+int tpc_refit_tracks(tpc_ctx*, int device_result, tpc_refit* out);
 
 /* Forget the clusters and results, keep geometry, parameters and buffers (one call per event / time frame). */
 int tpc_clear(tpc_ctx*);

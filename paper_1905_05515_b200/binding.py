@@ -17,7 +17,7 @@ _SO = os.path.join(_HERE, "libtpc_b200.so")
 
 ABI_SYMBOLS = [
     "tpc_abi_version", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
-    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
+    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
     "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
 
@@ -39,6 +39,11 @@ class _Tracks(C.Structure):
     _fields_ = [("n_tracks", C.c_int64), ("n_cluster_refs", C.c_int64), ("sector", C.c_void_p), ("x", C.c_void_p),
                 ("par", C.c_void_p), ("cov", C.c_void_p), ("chi2", C.c_void_p), ("ndf", C.c_void_p), ("tracklet", C.c_void_p),
                 ("cl_begin", C.c_void_p), ("cl_row", C.c_void_p), ("cl_index", C.c_void_p)]
+
+
+class _Refit(C.Structure):
+    _fields_ = [("n_tracks", C.c_int64)] + [(k, C.c_void_p) for k in ("n", "ndf", "x", "par", "cov", "chi2", "z0", "t0")] + \
+               [("ms_refit", C.c_float)]
 
 
 class _Timings(C.Structure):
@@ -86,6 +91,7 @@ def load_library():
     lib.tpc_load_clusters_batch.argtypes = [vp, _PL, vp, vp, vp]
     lib.tpc_find_tracks.argtypes = [vp, C.POINTER(_Tracks)]
     lib.tpc_find_tracks_device.argtypes = [vp, C.POINTER(_Tracks)]
+    lib.tpc_refit_tracks.argtypes = [vp, C.c_int, C.POINTER(_Refit)]
     lib.tpc_clear.argtypes = [vp]
     lib.tpc_destroy.argtypes = [vp]
     lib.tpc_destroy.restype = None
@@ -248,6 +254,23 @@ def tpc_find_tracks_device(h) -> Tracks:
     return _wrap(t, _dev_tensor)
 
 
+_REFIT_FIELDS = [("n", np.int32, 1), ("ndf", np.int32, 1), ("x", np.float32, 1), ("par", np.float32, 5), ("cov", np.float32, 15),
+                 ("chi2", np.float32, 1), ("z0", np.float32, 1), ("t0", np.float32, 1)]
+
+
+def tpc_refit_tracks(h, device_result=False) -> dict:
+    """S7: refit over the owned clusters + collision time of every track of the last tpc_find_tracks* call (zero-copy views)."""
+    t = _Refit()
+    _check(h, load_library().tpc_refit_tracks(h, 1 if device_result else 0, C.byref(t)))
+    make = _dev_tensor if device_result else _host_array
+    nt = int(t.n_tracks)
+    d = {"n_tracks": nt, "ms_refit": float(t.ms_refit)}
+    for name, dt, w in _REFIT_FIELDS:
+        a = make(getattr(t, name), nt * w, dt)
+        d[name] = a.reshape(nt, w) if w > 1 else a
+    return d
+
+
 class Tracker:
     """Context manager around one tpc_ctx, for the tests and bench.py."""
 
@@ -302,6 +325,9 @@ class Tracker:
 
     def find_tracks_device(self) -> Tracks:
         return tpc_find_tracks_device(self.h)
+
+    def refit_tracks(self, device_result=False) -> dict:
+        return tpc_refit_tracks(self.h, device_result)
 
     def clear(self):
         self._keep = []

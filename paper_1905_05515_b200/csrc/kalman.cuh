@@ -1,0 +1,156 @@
+// kalman.cuh -- fp32 track state, helix transport and Kalman update shared by K5 (tracklet constructor) and K7 (refit).
+// Definition: DESIGN.md section 4, S5.  Written term by term in the documented order; the library is compiled
+// with -fmad=false, so every product is rounded before it is added.
+#pragma once
+#include "tpc_internal.cuh"
+
+namespace tpc {
+
+// lower-triangle indices of the symmetric 5x5 covariance, row-major: (0,0)(1,0)(1,1)(2,0)(2,1)(2,2)(3,0)...(4,4)
+struct State {
+  float y, z, s, t, q;
+  float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+};
+
+__device__ __forceinline__ void reset_cov(State& st, const Params& P) {
+  st.c00 = P.c0[0]; st.c11 = P.c0[1]; st.c22 = P.c0[2]; st.c33 = P.c0[3]; st.c44 = P.c0[4];
+  st.c10 = st.c20 = st.c21 = st.c30 = st.c31 = st.c32 = st.c40 = st.c41 = st.c42 = st.c43 = 0.0f;
+}
+
+// Helix transport x -> x+dx in uniform Bz, covariance C' = F C F^T (F written out: only F02 F04 F12 F13 F14 F24 are non-trivial).
+// false: |sin phi| would leave [-s_max, s_max].
+__device__ __forceinline__ bool propagate(State& st, const float dx, const Params& P) {
+  const float cB = P.cB;
+  const float s = st.s, t = st.t;
+  const float k = cB * st.q;
+  const float kdx = k * dx;
+  const float s1 = s + kdx;
+  if (!(fabsf(s) <= P.smax) || !(fabsf(s1) <= P.smax)) return false;
+  const float c = sqrtf(1.0f - s * s), c1 = sqrtf(1.0f - s1 * s1);
+  const float cc = c + c1, ss = s + s1, tq = ss / cc;
+  const float g = 1.0f + tq * tq;
+  const float L = dx * sqrtf(g);
+  const float h = (0.5f * k) * L, h2 = h * h;
+  float S;
+  if (fabsf(h) < 0.25f) {   // asin(h)/h = 1 + h^2/6 + 3h^4/40 + 15h^6/336 + 105h^8/3456
+    float poly = (float)(105.0 / 3456.0);
+    poly = (float)(15.0 / 336.0) + h2 * poly;
+    poly = (float)(3.0 / 40.0) + h2 * poly;
+    poly = (float)(1.0 / 6.0) + h2 * poly;
+    poly = 1.0f + h2 * poly;
+    S = L * poly;
+  } else {
+    S = (2.0f / k) * asinf(h);
+  }
+  float dSdk;
+  if (fabsf(kdx) >= 1e-2f) {
+    dSdk = (dx / c1 - S) / k;
+  } else {
+    const float sm = (s + 2.0f * s1) / 3.0f;
+    const float cm2 = 1.0f - sm * sm;
+    const float cm = sqrtf(cm2);
+    dSdk = ((dx * dx) * sm) / (2.0f * (cm2 * cm));
+  }
+  const float cc1 = c * c1;
+  const float f02 = ((dx * g) * cc) / (2.0f * cc1);
+  const float f04 = (((dx * dx) * cB) * g) / (2.0f * c1);
+  const float f12 = ((t * dx) * tq) / cc1;
+  const float f13 = S;
+  const float f14 = (t * cB) * dSdk;
+  const float f24 = cB * dx;
+  st.y = st.y + dx * tq;
+  st.z = st.z + t * S;
+  st.s = s1;
+  // T = F C   (row i of T = sum_m F[i][m] C[m][:], accumulated in the order m = 0..4; zero terms add exactly nothing)
+  const float t00 = (st.c00 + f02 * st.c20) + f04 * st.c40;
+  const float t01 = (st.c10 + f02 * st.c21) + f04 * st.c41;
+  const float t02 = (st.c20 + f02 * st.c22) + f04 * st.c42;
+  const float t03 = (st.c30 + f02 * st.c32) + f04 * st.c43;
+  const float t04 = (st.c40 + f02 * st.c42) + f04 * st.c44;
+  const float t10 = ((st.c10 + f12 * st.c20) + f13 * st.c30) + f14 * st.c40;
+  const float t11 = ((st.c11 + f12 * st.c21) + f13 * st.c31) + f14 * st.c41;
+  const float t12 = ((st.c21 + f12 * st.c22) + f13 * st.c32) + f14 * st.c42;
+  const float t13 = ((st.c31 + f12 * st.c32) + f13 * st.c33) + f14 * st.c43;
+  const float t14 = ((st.c41 + f12 * st.c42) + f13 * st.c43) + f14 * st.c44;
+  const float t20 = st.c20 + f24 * st.c40;
+  const float t21 = st.c21 + f24 * st.c41;
+  const float t22 = st.c22 + f24 * st.c42;
+  const float t23 = st.c32 + f24 * st.c43;
+  const float t24 = st.c42 + f24 * st.c44;
+  const float t30 = st.c30, t31 = st.c31, t32 = st.c32, t33 = st.c33, t34 = st.c43;
+  const float t40 = st.c40, t41 = st.c41, t42 = st.c42, t43 = st.c43, t44 = st.c44;
+  // C' = T F^T, lower triangle: C'[i][j] = sum_m T[i][m] F[j][m]
+  st.c00 = (t00 + t02 * f02) + t04 * f04;
+  st.c10 = (t10 + t12 * f02) + t14 * f04;
+  st.c11 = ((t11 + t12 * f12) + t13 * f13) + t14 * f14;
+  st.c20 = (t20 + t22 * f02) + t24 * f04;
+  st.c21 = ((t21 + t22 * f12) + t23 * f13) + t24 * f14;
+  st.c22 = t22 + t24 * f24;
+  st.c30 = (t30 + t32 * f02) + t34 * f04;
+  st.c31 = ((t31 + t32 * f12) + t33 * f13) + t34 * f14;
+  st.c32 = t32 + t34 * f24;
+  st.c33 = t33;
+  st.c40 = (t40 + t42 * f02) + t44 * f04;
+  st.c41 = ((t41 + t42 * f12) + t43 * f13) + t44 * f14;
+  st.c42 = t42 + t44 * f24;
+  st.c43 = t43;
+  st.c44 = t44;
+  (void)t01; (void)t03;
+  return true;
+}
+
+// Kalman update with the joint 2-D measurement (ym, zm), R = diag(sigma_y^2, sigma_z^2); returns the chi2 increment.
+__device__ __forceinline__ float update(State& st, const float ym, const float zm, const Params& P) {
+  const float s00 = st.c00 + P.ry, s10 = st.c10, s11 = st.c11 + P.rz;
+  const float det = s00 * s11 - s10 * s10;
+  const float i00 = s11 / det, i11 = s00 / det, i10 = -s10 / det;
+  const float r0 = ym - st.y, r1 = zm - st.z;
+  // K = C[:,0:2] S^-1
+  const float k00 = st.c00 * i00 + st.c10 * i10, k01 = st.c00 * i10 + st.c10 * i11;
+  const float k10 = st.c10 * i00 + st.c11 * i10, k11 = st.c10 * i10 + st.c11 * i11;
+  const float k20 = st.c20 * i00 + st.c21 * i10, k21 = st.c20 * i10 + st.c21 * i11;
+  const float k30 = st.c30 * i00 + st.c31 * i10, k31 = st.c30 * i10 + st.c31 * i11;
+  const float k40 = st.c40 * i00 + st.c41 * i10, k41 = st.c40 * i10 + st.c41 * i11;
+  // C' = C - K C[0:2,:], lower triangle; C[0][j] = c_j0, C[1][j] = c_j1 (symmetric storage)
+  const float o00 = st.c00, o10 = st.c10, o11 = st.c11, o20 = st.c20, o21 = st.c21, o30 = st.c30, o31 = st.c31, o40 = st.c40, o41 = st.c41;
+  st.c00 = o00 - (k00 * o00 + k01 * o10);
+  st.c10 = o10 - (k10 * o00 + k11 * o10);
+  st.c11 = o11 - (k10 * o10 + k11 * o11);
+  st.c20 = o20 - (k20 * o00 + k21 * o10);
+  st.c21 = o21 - (k20 * o10 + k21 * o11);
+  st.c22 = st.c22 - (k20 * o20 + k21 * o21);
+  st.c30 = o30 - (k30 * o00 + k31 * o10);
+  st.c31 = o31 - (k30 * o10 + k31 * o11);
+  st.c32 = st.c32 - (k30 * o20 + k31 * o21);
+  st.c33 = st.c33 - (k30 * o30 + k31 * o31);
+  st.c40 = o40 - (k40 * o00 + k41 * o10);
+  st.c41 = o41 - (k40 * o10 + k41 * o11);
+  st.c42 = st.c42 - (k40 * o20 + k41 * o21);
+  st.c43 = st.c43 - (k40 * o30 + k41 * o31);
+  st.c44 = st.c44 - (k40 * o40 + k41 * o41);
+  st.y = st.y + (k00 * r0 + k01 * r1);
+  st.z = st.z + (k10 * r0 + k11 * r1);
+  st.s = st.s + (k20 * r0 + k21 * r1);
+  st.t = st.t + (k30 * r0 + k31 * r1);
+  st.q = st.q + (k40 * r0 + k41 * r1);
+  return r0 * (i00 * r0 + i10 * r1) + r1 * (i10 * r0 + i11 * r1);
+}
+
+// arc length over a chord of length L on a circle of curvature k: L * asin(h)/h, h = k L / 2 (series below 0.25, reading A32)
+__device__ __forceinline__ float arc_of_chord(const float L, const float k) {
+  float h = (0.5f * k) * L;
+  const float h2 = h * h;
+  if (fabsf(h) < 0.25f) {
+    float poly = (float)(105.0 / 3456.0);
+    poly = (float)(15.0 / 336.0) + h2 * poly;
+    poly = (float)(3.0 / 40.0) + h2 * poly;
+    poly = (float)(1.0 / 6.0) + h2 * poly;
+    poly = 1.0f + h2 * poly;
+    return L * poly;
+  }
+  if (h > 1.0f) h = 1.0f;
+  if (h < -1.0f) h = -1.0f;
+  return (2.0f / k) * asinf(h);
+}
+
+}  // namespace tpc

@@ -134,6 +134,9 @@ struct tpc_ctx {
   // outputs / debug copies (host)
   PinVec<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; PinVec<float> ho_x, ho_par, ho_cov, ho_chi2;
   PinVec<int64_t> ho_cl_begin;
+  // S7 refit (device + host)
+  DevBuf r_n, r_ndf, r_x, r_par, r_cov, r_chi2, r_z0, r_t0;
+  PinVec<int32_t> hr_n, hr_ndf; PinVec<float> hr_x, hr_par, hr_cov, hr_chi2, hr_z0, hr_t0;
   std::vector<float> dbg_yz; std::vector<int32_t> dbg_perm, dbg_bins, dbg_up, dbg_dn, dbg_su, dbg_sp;
   std::vector<int32_t> dbg_tl_sector, dbg_tl_row, dbg_tl_n, dbg_tl_first, dbg_tl_last, dbg_rowhit; std::vector<float> dbg_tl_chi2, dbg_tl_x, dbg_tl_par, dbg_tl_cov;
 
@@ -225,11 +228,14 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->d_link_up, &c->d_link_dn, &c->d_raw_up, &c->d_raw_dn, &c->d_mask, &c->d_item_count, &c->d_item_base, &c->d_scan_tmp,
                     &c->d_start_unit, &c->d_start_pos, &c->d_counters, &c->d_rowhit, &c->d_tl_n, &c->d_tl_first, &c->d_tl_last, &c->d_tl_chi2,
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
-                    &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index};
+                    &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
+                    &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
   c->ho_sector.release(); c->ho_ndf.release(); c->ho_tracklet.release(); c->ho_cl_row.release(); c->ho_cl_index.release();
   c->ho_x.release(); c->ho_par.release(); c->ho_cov.release(); c->ho_chi2.release(); c->ho_cl_begin.release();
+  c->hr_n.release(); c->hr_ndf.release(); c->hr_x.release(); c->hr_par.release(); c->hr_cov.release(); c->hr_chi2.release();
+  c->hr_z0.release(); c->hr_t0.release();
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
   delete c;
 }
@@ -583,6 +589,48 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
 extern "C" {
 int tpc_find_tracks(tpc_ctx* c, tpc_tracks* out) { return find_tracks_impl(c, out, true); }
 int tpc_find_tracks_device(tpc_ctx* c, tpc_tracks* out) { return find_tracks_impl(c, out, false); }
+// S7 (NEXT-1): K7 over the tracks of the last call; the S5/S6 buffers it reads (rowhit, sorted clusters, track lists) are still live.
+int tpc_refit_tracks(tpc_ctx* c, int device_result, tpc_refit* out) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_refit_tracks: null argument");
+  memset(out, 0, sizeof(*out));
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_refit_tracks: call tpc_find_tracks first");
+  cudaStream_t st = c->stream;
+  Launch L{st, c->sm_count, c->T.k2_threads};
+  const long long nt = c->n_tracks; const size_t ntz = (size_t)std::max(nt, 1LL);
+  CUDA_TRY(c, c->r_n.ensure(ntz * 4)); CUDA_TRY(c, c->r_ndf.ensure(ntz * 4)); CUDA_TRY(c, c->r_x.ensure(ntz * 4));
+  CUDA_TRY(c, c->r_par.ensure(ntz * 20)); CUDA_TRY(c, c->r_cov.ensure(ntz * 60)); CUDA_TRY(c, c->r_chi2.ensure(ntz * 4));
+  CUDA_TRY(c, c->r_z0.ensure(ntz * 4)); CUDA_TRY(c, c->r_t0.ensure(ntz * 4));
+  long long launches = 0;
+  CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
+  LAUNCH_TRY(c, launch_k7_refit(L, nt, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_cl_begin.as<long long>(), c->o_cl_row.as<int>(),
+                                c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_rowhit.as<int>(),
+                                c->r_n.as<int>(), c->r_ndf.as<int>(), c->r_x.as<float>(), c->r_par.as<float>(), c->r_cov.as<float>(),
+                                c->r_chi2.as<float>(), c->r_z0.as<float>(), c->r_t0.as<float>(), c->P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
+  out->n_tracks = nt;
+  if (!device_result) {
+    CUDA_TRY(c, c->hr_n.resize(ntz)); CUDA_TRY(c, c->hr_ndf.resize(ntz)); CUDA_TRY(c, c->hr_x.resize(ntz)); CUDA_TRY(c, c->hr_par.resize(ntz * 5));
+    CUDA_TRY(c, c->hr_cov.resize(ntz * 15)); CUDA_TRY(c, c->hr_chi2.resize(ntz)); CUDA_TRY(c, c->hr_z0.resize(ntz)); CUDA_TRY(c, c->hr_t0.resize(ntz));
+    if (nt > 0) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_n.data(), c->r_n.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_ndf.data(), c->r_ndf.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_x.data(), c->r_x.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_par.data(), c->r_par.p, nt * 20, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_cov.data(), c->r_cov.p, nt * 60, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_chi2.data(), c->r_chi2.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_z0.data(), c->r_z0.p, nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hr_t0.data(), c->r_t0.p, nt * 4, cudaMemcpyDeviceToHost, st));
+    }
+    out->n = c->hr_n.data(); out->ndf = c->hr_ndf.data(); out->x = c->hr_x.data(); out->par = c->hr_par.data(); out->cov = c->hr_cov.data();
+    out->chi2 = c->hr_chi2.data(); out->z0 = c->hr_z0.data(); out->t0 = c->hr_t0.data();
+  } else {
+    out->n = c->r_n.as<int32_t>(); out->ndf = c->r_ndf.as<int32_t>(); out->x = c->r_x.as<float>(); out->par = c->r_par.as<float>();
+    out->cov = c->r_cov.as<float>(); out->chi2 = c->r_chi2.as<float>(); out->z0 = c->r_z0.as<float>(); out->t0 = c->r_t0.as<float>();
+  }
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  CUDA_TRY(c, cudaEventElapsedTime(&out->ms_refit, c->ev[8], c->ev[9]));
+  return TPC_OK;
+}
 int tpc_get_timings(tpc_ctx* c, tpc_timings* out) {
   if (!c || !out) return fail(c, TPC_E_ARG, "tpc_get_timings: null argument");
   if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_get_timings: no tpc_find_tracks call has completed");

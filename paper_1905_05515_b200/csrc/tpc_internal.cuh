@@ -115,6 +115,11 @@ int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_un
                    int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,
                    long long* o_cl_begin, int* o_cl_row, int* o_cl_index, long long n_tracks, long long n_refs, const Params& P);
 
+int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, const int* o_tracklet, const long long* o_cl_begin,
+                    const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_rowhit,
+                    int* rf_n, int* rf_ndf, float* rf_x, float* rf_par, float* rf_cov, float* rf_chi2, float* rf_z0, float* rf_t0,
+                    const Params& P);
+
 // device-wide exclusive scans (own kernels; three launches each)
 int launch_scan_i32(const Launch& L, const int* d_in, int* d_out, int n, int* d_tmp, int* d_total);
 int launch_scan_u64(const Launch& L, const unsigned long long* d_in, unsigned long long* d_out, int n, unsigned long long* d_tmp,

@@ -102,3 +102,25 @@ def compare_tracks(otr, gtr, rel=1e-4, sig=1e-3) -> dict:
             n_bad += 1
     return dict(n_oracle=len(so), n_gpu=len(sg), identical_sets=len(common), frac_identical=len(common) / max(1, len(so)),
                 param_mismatch=n_bad, worst_ratio=worst)
+
+
+def compare_refit(otr, orf, gtr, grf, rel=1e-4, sig=1e-3) -> dict:
+    """S7 (readings A37/A38): refit results of tracks paired by (sector, exact cluster set).  n, ndf, x equal; parameters as in
+    compare_tracks; chi2 within 1e-3 relative; z0 / t0 within rel*|oracle| or sig * the z error (t0 = -z0 / vdrift)."""
+    so, sg = track_sets(otr), track_sets(gtr)
+    common = [k for k in so if k in sg]
+    n_bad = 0
+    dcov = np.array([0, 2, 5, 9, 14])
+    for k in common:
+        i, j = so[k], sg[k]
+        po, pg = orf["par"][i].astype(np.float64), np.asarray(grf["par"][j], dtype=np.float64)
+        so_ = np.sqrt(np.abs(orf["cov"][i][dcov].astype(np.float64)))
+        d = np.abs(po - pg)
+        ok = bool(((d <= rel * np.abs(po)) | (d <= sig * so_)).all())
+        ok &= int(orf["n"][i]) == int(grf["n"][j]) and int(orf["ndf"][i]) == int(grf["ndf"][j]) and float(orf["x"][i]) == float(grf["x"][j])
+        ok &= abs(float(orf["chi2"][i]) - float(grf["chi2"][j])) <= 1e-3 * max(1.0, abs(float(orf["chi2"][i])))
+        for name in ("z0", "t0"):
+            a, b = float(orf[name][i]), float(grf[name][j])
+            ok &= abs(a - b) <= max(rel * abs(a), sig * so_[1] * 10.0)   # z0 adds (dz/ds error) x (arc ~ 1 m) to the z error
+        n_bad += not ok
+    return dict(n_common=len(common), mismatch=n_bad)

@@ -72,6 +72,54 @@ def test_c4_loopers_parity():
     _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, 200, replace=False))
 
 
+def _refit_parity(w):
+    o = P.make_oracle(w).run("s7")
+    otr, orf = o.tracks(), o.refit()
+    with _tracker(w) as trk:
+        trk.load_workload(w)
+        gtr = trk.find_tracks().copy().as_dict()
+        grf = {k: (np.array(v) if isinstance(v, np.ndarray) else v) for k, v in trk.refit_tracks().items()}
+        dev = trk.refit_tracks(device_result=True)
+        for k in ("n", "ndf", "x", "par", "cov", "chi2", "z0", "t0"):
+            assert np.array_equal(dev[k].cpu().numpy(), grf[k], equal_nan=True), k
+    assert grf["n_tracks"] == len(gtr["sector"]) and grf["ms_refit"] > 0
+    res = P.compare_refit(otr, orf, gtr, grf)
+    assert res["n_common"] > 50 and res["n_common"] >= 0.999 * len(otr["sector"]) and res["mismatch"] <= 0.001 * res["n_common"], res
+    return w, gtr, grf
+
+
+def test_refit_parity_triggered_c1():
+    """S7 (NEXT-1): refit + collision time against the oracle; triggered primaries extrapolate to t0 = 0."""
+    w, gtr, grf = _refit_parity(W.config(1))
+    assert abs(float(np.median(grf["t0"]))) < 0.2
+
+
+def test_refit_parity_continuous_c3_scaled():
+    """Continuous frame: the refitted tracks' collision times reproduce the generator's (pure primary tracks)."""
+    w, gtr, grf = _refit_parity(W.config(3, scale=0.1))
+    labs = H.track_labels(w, gtr)
+    R = w.n_rows
+    dt = []
+    for i, (lab, frac) in enumerate(labs):
+        if not (lab >= 0 and frac == 1.0 and w.particles["kind"][lab] == 0 and grf["n"][i] >= 40):
+            continue
+        a, b = gtr["cl_begin"][i], gtr["cl_begin"][i + 1]
+        g = w.unit_off[gtr["sector"][i] * R + gtr["cl_row"][a:b]] + gtr["cl_index"][a:b]
+        if w.leg0[g].all():        # outgoing leg only: a returning leg does not come from the beam line (NEXT-3 identifies those)
+            dt.append(grf["t0"][i] - w.particles["t0"][lab])
+    dt = np.array(dt)
+    assert len(dt) > 500 and abs(np.median(dt)) < 0.05 and np.percentile(np.abs(dt), 99) < 1.0, (len(dt), np.median(dt))
+
+
+def test_refit_before_find_tracks_is_a_state_error():
+    import paper_1905_05515_b200 as T
+    w = W.config(1, scale=0.1)
+    with _tracker(w) as trk:
+        with pytest.raises(T.TpcError) as e:
+            trk.refit_tracks()
+        assert e.value.code == -2
+
+
 def test_empty_and_tiny_inputs():
     w = W.config(1, scale=0.05)
     with _tracker(w) as trk:
