@@ -14,7 +14,6 @@ namespace tpc {
 namespace {
 
 constexpr int K6_THREADS = 128;
-constexpr int K6_ROWS = 5;     // rows per lane and round in k6_owner / k6_count (5 x 32 covers the 152 pad rows in one round)
 constexpr unsigned long long REF_MASK = (1ull << 40) - 1ull;
 
 __device__ __forceinline__ unsigned long long make_key(int n, float chi2, int idx) {
@@ -43,13 +42,9 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const int R,
   const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
   const int* __restrict__ rh = rowhit + (long long)i * R;
   const int r1 = tl_last[i];
-  // K6_ROWS rows per lane and round: all rowhit / unit-offset loads of a round are issued before the first atomic
-  for (int rb = tl_first[i] + lane; rb <= r1; rb += 32 * K6_ROWS) {
-    int p[K6_ROWS]; long long o[K6_ROWS];
-#pragma unroll
-    for (int j = 0; j < K6_ROWS; j++) { const int r = rb + 32 * j; p[j] = r <= r1 ? rh[r] : -1; o[j] = r <= r1 ? su[r].off : 0; }
-#pragma unroll
-    for (int j = 0; j < K6_ROWS; j++) if (p[j] >= 0) atomicMax(&owner[o[j] + p[j]], key);
+  for (int r = tl_first[i] + lane; r <= r1; r += 32) {
+    const int p = rh[r];
+    if (p >= 0) atomicMax(&owner[su[r].off + p], key);
   }
 }
 
@@ -67,14 +62,9 @@ __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const int R,
     const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
     const int* __restrict__ rh = rowhit + (long long)i * R;
     const int r1 = tl_last[i];
-    for (int rb = tl_first[i] + lane; rb <= r1; rb += 32 * K6_ROWS) {
-      int p[K6_ROWS]; long long o[K6_ROWS]; unsigned long long w[K6_ROWS];
-#pragma unroll
-      for (int j = 0; j < K6_ROWS; j++) { const int r = rb + 32 * j; p[j] = r <= r1 ? rh[r] : -1; o[j] = r <= r1 ? su[r].off : 0; }
-#pragma unroll
-      for (int j = 0; j < K6_ROWS; j++) w[j] = p[j] >= 0 ? owner[o[j] + p[j]] : 0ull;
-#pragma unroll
-      for (int j = 0; j < K6_ROWS; j++) owned += p[j] >= 0 && w[j] == key;
+    for (int r = tl_first[i] + lane; r <= r1; r += 32) {
+      const int p = rh[r];
+      if (p >= 0 && owner[su[r].off + p] == key) owned++;
     }
   }
   owned = __reduce_add_sync(0xffffffffu, owned);
@@ -112,21 +102,14 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const int R, 
   }
   if (lane < 5) o_par[t * 5 + lane] = tl_par[(long long)i * 5 + lane];
   if (lane < 15) o_cov[t * 15 + lane] = tl_cov[(long long)i * 15 + lane];
-  for (int rb = r0; rb <= r1; rb += 32 * K6_ROWS) {   // K6_ROWS x 32 rows per round, loads of a round issued together
-    int p[K6_ROWS]; long long g[K6_ROWS]; unsigned long long w[K6_ROWS]; int pi[K6_ROWS];
-#pragma unroll
-    for (int j = 0; j < K6_ROWS; j++) { const int r = rb + 32 * j + lane; p[j] = r <= r1 ? rh[r] : -1; g[j] = r <= r1 ? su[r].off : 0; }
-#pragma unroll
-    for (int j = 0; j < K6_ROWS; j++) { g[j] += p[j]; w[j] = p[j] >= 0 ? owner[g[j]] : 0ull; }
-#pragma unroll
-    for (int j = 0; j < K6_ROWS; j++) pi[j] = p[j] >= 0 && w[j] == key ? perm[g[j]] : 0;
-#pragma unroll
-    for (int j = 0; j < K6_ROWS; j++) {               // ascending rows: ballot + prefix popcount keeps the list ordered
-      const bool own = p[j] >= 0 && w[j] == key;
-      const unsigned m = __ballot_sync(0xffffffffu, own);
-      if (own) { const long long o = k + __popc(m & ((1u << lane) - 1u)); o_cl_row[o] = rb + 32 * j + lane; o_cl_index[o] = pi[j]; }
-      k += __popc(m);
-    }
+  for (int rb = r0; rb <= r1; rb += 32) {       // ascending rows: ballot + prefix popcount keeps the list ordered
+    const int r = rb + lane;
+    long long g = 0;
+    bool own = false;
+    if (r <= r1) { const int p = rh[r]; if (p >= 0) { g = su[r].off + p; own = owner[g] == key; } }
+    const unsigned m = __ballot_sync(0xffffffffu, own);
+    if (own) { const long long o = k + __popc(m & ((1u << lane) - 1u)); o_cl_row[o] = r; o_cl_index[o] = perm[g]; }
+    k += __popc(m);
   }
 }
 
