@@ -3,11 +3,13 @@
 // One CTA per (sector,row) unit.  The bin counters / cursors of the unit live in shared memory (global scratch for units
 // whose grid does not fit).  Passes over the unit's clusters:
 //   B  count      : float4-vectorised, coalesced loads of pad-y and time; z = z_max - vdrift*t; bin; shared-memory atomicAdd
-//   C  scan       : block exclusive scan of the counters -> bin_start (global) and cursors (shared)
-//   D  scatter    : same loads again (L2 hits: a unit is <= a few hundred KB), pos = atomicAdd(cursor[bin]); perm[pos] = i
-//   E1 canonical  : one thread per bin sorts the (about one) entries of its bin by original index -> the order inside a bin is
-//                   ascending original index, i.e. the counting sort is stable and independent of the atomic order
-//   E2 gather     : one thread per sorted position writes float2 (y, z), coalesced
+//   C  scan       : exclusive scan of the counters in place (serial runs per thread + one block scan) -> cursors
+//   D  scatter    : pos = atomicAdd(cursor[bin]); perm[pos] = i (from the shared (y,z) copy, or the same loads again: L2 hits);
+//                   the advanced cursors are the bin_start table shifted by one bin
+//   E  place      : units held in shared memory: one thread per scattered position ranks its index inside its bin and writes
+//                   index and (y, z) to the final position -> ascending original index inside a bin, i.e. the counting sort is
+//                   stable and independent of the atomic order.  Larger units: E1 one thread per bin insertion-sorts its
+//                   (about one) entries, E2 one thread per sorted position gathers float2 (y, z), coalesced
 // Algorithmic HBM bytes per cluster: 8 read (y,t) + 8 (yz) + 4 (perm) + ~4 (bin_start) written = 24.
 #include "tpc_internal.cuh"
 
@@ -36,7 +38,7 @@ __device__ __forceinline__ void for_each_cluster(const float* __restrict__ in_y,
   if (i < n) f(i, py[i], pt[i]);
 }
 
-__global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict__ units, const float* __restrict__ in_y,
+__global__ void __launch_bounds__(1024, 2) k1_grid_build(const UnitDesc* __restrict__ units, const float* __restrict__ in_y,
                                                        const float* __restrict__ in_t, float2* __restrict__ yz,
                                                        int* __restrict__ perm, int* __restrict__ bin_start, int* __restrict__ cursor_g,
                                                        const float zmax, const float vdrift, const int smem_ints) {
@@ -72,17 +74,19 @@ __global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict
   });
   __syncthreads();
 
-  // C: exclusive scan of the counters; bin_start[b] (global) and cursor[b] (cnt) both get the start of bin b.
-  int carry = 0;
-  for (int base = 0; base < nb; base += blockDim.x) {
-    int b = base + threadIdx.x;
-    int v = b < nb ? cnt[b] : 0;
+  // C: exclusive scan of the counters in place (cnt[b] = start of bin b): every thread scans a run of consecutive bins
+  //    serially, one block scan joins the runs.  bin_start is written after pass D from the advanced cursors.
+  {
+    const int K = (nb + (int)blockDim.x - 1) / (int)blockDim.x;
+    const int b0 = min((int)threadIdx.x * K, nb), b1 = min(b0 + K, nb);
+    int sum = 0;
+#pragma unroll 2
+    for (int b = b0; b < b1; b++) sum += cnt[b];
     int total;
-    int ex = block_excl_scan(v, s_warp, &total) + carry;
-    if (b < nb) { cnt[b] = ex; bs[b] = ex; }
-    carry += total;
+    int ex = block_excl_scan(sum, s_warp, &total);
+#pragma unroll 2
+    for (int b = b0; b < b1; b++) { const int v = cnt[b]; cnt[b] = ex; ex += v; }
   }
-  if (threadIdx.x == 0) bs[nb] = n;
   __syncthreads();
 
   // D: scatter original indices to their bins (order inside a bin arbitrary here).
@@ -101,6 +105,28 @@ __global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict
   }
   __syncthreads();
 
+  // after D the cursor of bin b stands at the end of bin b = the start of bin b+1: bin_start, coalesced
+  for (int b = threadIdx.x; b < nb; b += blockDim.x) bs[b + 1] = cnt[b];
+  if (threadIdx.x == 0) bs[0] = 0;
+  float2* __restrict__ out = yz + d.off;
+  if (yz_s) {
+    // E (shared-memory units): stable placement and payload in one pass, one thread per scattered position.  Position p
+    // holds original index i of bin b; its final position is start(b) + #{q in bin b : index at q < i}, so the order inside
+    // a bin is ascending original index whatever order the atomics of pass D produced.  Writes stay inside the bin's range.
+    for (int p = threadIdx.x; p < n; p += blockDim.x) {
+      const int i = pm[p];
+      const float2 c = syz[i];
+      const int b = bin_of(c.y, d.zlo, d.invs, nz) * ny + bin_of(c.x, d.ylo, d.invs, ny);
+      const int lo = b ? cnt[b - 1] : 0, hi = cnt[b];   // after D, cursor[b] = end of bin b
+      int rank = 0;
+#pragma unroll 2
+      for (int q = lo; q < hi; q++) rank += pm[q] < i;
+      pg[lo + rank] = i;
+      out[lo + rank] = c;
+    }
+    return;
+  }
+
   // E1: canonical order inside each bin = ascending original index (insertion sort; bins hold about one cluster).
   for (int b = threadIdx.x; b < nb; b += blockDim.x) {
     const int lo = b ? cnt[b - 1] : 0, hi = cnt[b];   // after D, cursor[b] = end of bin b
@@ -113,17 +139,12 @@ __global__ void __launch_bounds__(1024) k1_grid_build(const UnitDesc* __restrict
   __syncthreads();
 
   // E2: sorted payload, coalesced writes.
-  float2* __restrict__ out = yz + d.off;
-  if (yz_s) {
-    for (int p = threadIdx.x; p < n; p += blockDim.x) { const int i = pm[p]; pg[p] = i; out[p] = syz[i]; }
-  } else {
-    const float* py = in_y + d.src;
-    const float* pt = in_t + d.src;
-    for (int p = threadIdx.x; p < n; p += blockDim.x) {
-      const int i = pm[p];
-      if (perm_s) pg[p] = i;
-      out[p] = make_float2(py[i], __fsub_rn(zmax, __fmul_rn(vdrift, pt[i])));
-    }
+  const float* py = in_y + d.src;
+  const float* pt = in_t + d.src;
+  for (int p = threadIdx.x; p < n; p += blockDim.x) {
+    const int i = pm[p];
+    if (perm_s) pg[p] = i;
+    out[p] = make_float2(py[i], __fsub_rn(zmax, __fmul_rn(vdrift, pt[i])));
   }
 }
 
