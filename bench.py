@@ -178,6 +178,27 @@ def run_gpu(args, rank, world, local_rank):
     value = total_clusters / (ms * 1e-3)
     kern = {k: acc[k] / args.steps for k in keys}
     n_tracks, n_refs = res.n_tracks, res.n_cluster_refs
+    # NEXT-2 variant (seed bridging, reading A39), measured beside the default path, never mixed into `value`
+    variant = None
+    if args.variant and rank == 0:
+        vp = dict(bridge_rows=4.0, bridge_min=8.0)
+        with T.Tracker(**w.geometry(), **vp) as tv:
+            tv.set_stream(stream.cuda_stream)
+            tv.load_batch(w.unit_off, y_d, t_d)
+            for _ in range(args.warmup):
+                rv = tv.find_tracks_device()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(args.steps):
+                rv = tv.find_tracks_device()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            vms = e0.elapsed_time(e1) / args.steps
+            vt = tv.timings()
+            variant = {"params": vp, "ms_per_step": vms, "value": N / (vms * 1e-3), "unit": UNIT, "n_start_hits": int(vt["n_start_hits"]),
+                       "tracks_per_step": int(rv.n_tracks), "cluster_refs_per_step": int(rv.n_cluster_refs),
+                       "kernel_ms": {k: vt[k] for k in keys},
+                       "note": "seed bridging (SURVEY 8(f).2): start hits that continue a lower chain are dropped; efficiency delta in DESIGN.md"}
     # S7 (NEXT-1, not part of the timed S0..S6 step): refit over the owned clusters + collision time, device-resident result
     refit_ms = float(np.mean([trk.refit_tracks(device_result=True)["ms_refit"] for _ in range(4)][1:]))
 
@@ -277,6 +298,7 @@ def run_gpu(args, rank, world, local_rank):
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
+           "variant_seed_bridging": variant,
            "refit": {"ms": refit_ms, "tracks_per_s": n_tracks / (refit_ms * 1e-3), "note": "S7 refit + collision time (SURVEY 8(f).1), outside the timed step"},
            "clocks": clocks}
     print(json.dumps(out))
@@ -293,6 +315,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-sectors", type=int, default=4, help="sectors of the workload the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", action="store_true", help="also time the NEXT-2 seed-bridging variant (extra field, not `value`)")
     ap.add_argument("--param", action="append", default=[], help="library tunable name=value (tpc_set_param), e.g. chunk=1024")
     args = ap.parse_args()
     rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))

@@ -20,6 +20,7 @@
  * permutation invariance + straight lines; S3/S4 invariants; S5 propagate vs closed-form circle,
  * composition, round trip, Jacobian vs finite differences; S5 fit: noise-free helix recovery 1e-5,
  * Bz=0 exact, chi2/ndf = 1 and pulls on smeared tracks; S6 hand-built sharing cases, order invariance.
+ * S4' (NEXT-2) seed bridging: hand-made single dropouts (one start hit per track), subset of the S4 list, brute-force probe.
  * S7 (NEXT-1) refit + collision time: noise-free recovery, chi2/ndf = 1, t0 against the generator's collision times.
  * Absolute efficiency / resolution versus the paper: parity unpinned (PAPER.md:49 gives no number).
  */
@@ -42,6 +43,9 @@ struct Tunables {            // DESIGN.md table T (all are readings; the paper i
   double edge_margin = 1.0;
   int min_hits = 10;
   double grid_min = 1.0, grid_max = 64.0, grid_scale = 1.0;   // S1 bin size clamp; scale is a test knob
+  int bridge_rows = 0;          // NEXT-2 (reading A39): 0 = off; else the deepest row gap a start hit may bridge to a lower chain
+  double bridge_wy = 1.0, bridge_wz = 1.5;
+  int bridge_min = 3;           // clusters the lower chain must have
 };
 
 struct OracleBase {
@@ -225,7 +229,7 @@ struct Oracle : OracleBase {
   }
 
   // ---- S4: start hits = chain beginnings with >= min_seed hits, ascending (sector,row,sorted pos) ----
-  void s4_start_hits() {
+  void s4_start_hits(bool brute = false) {
     start_unit.clear(); start_pos.clear();
     for (int u = 0; u < NS * R; u++) {
       int64_t o = off[u], n = off[u + 1] - o;
@@ -233,9 +237,54 @@ struct Oracle : OracleBase {
         if (!(clean_dn[o + h] < 0 && clean_up[o + h] >= 0)) continue;
         int len = 1; int uu = u; int32_t p = (int32_t)h;
         while (len < T.min_seed) { int32_t nx = clean_up[off[uu] + p]; if (nx < 0) break; p = nx; uu++; len++; }
-        if (len >= T.min_seed) { start_unit.push_back(u); start_pos.push_back((int32_t)h); }
+        if (len < T.min_seed) continue;
+        if (T.bridge_rows > 0 && bridged(u, (int32_t)h, brute)) continue;
+        start_unit.push_back(u); start_pos.push_back((int32_t)h);
       }
     }
+  }
+
+  // ---- S4' (NEXT-2; reading A39): seed bridging.  A missing cluster breaks a chain of mutual links over
+  //      three rows, and every piece longer than min_seed seeds its own tracklet of the SAME track (about 6 per track at 5 %
+  //      dropout, all but one discarded by S6).  A start hit h (row r) is dropped when it continues a lower chain: the straight
+  //      line through h and its second chain cluster w (row r+2), extended down to a row r-g (2 <= g <= bridge_rows), meets the
+  //      TOP c of a chain (no up link, a down link, at least min_seed clusters below), and the line through c and its second
+  //      cluster below, extended up to row r, meets h -- both within (bridge_wy, bridge_wz).  The lower chain's tracklet then
+  //      collects h's clusters in its outward pass (max_gap >= the bridged rows).
+  bool bridged(int u, int32_t h, bool brute) const {
+    const int sec = u / R, r = u % R;
+    if (r + 2 >= R) return false;
+    const int32_t u1 = clean_up[off[u] + h]; if (u1 < 0) return false;
+    const int32_t u2 = clean_up[off[u + 1] + u1]; if (u2 < 0) return false;
+    const Real wy = (Real)T.bridge_wy, wz = (Real)T.bridge_wz;
+    const Real yh = ys[off[u] + h], zh = zs[off[u] + h];
+    const Real dxu = X[r + 2] - X[r];
+    const Real sy = (ys[off[u + 2] + u2] - yh) / dxu, sz = (zs[off[u + 2] + u2] - zh) / dxu;
+    for (int g = 2; g <= T.bridge_rows && r - g >= 2; g++) {
+      const int ud = sec * R + (r - g);
+      const Real dx = X[r] - X[r - g];
+      const Real yp = yh - sy * dx, zp = zh - sz * dx;
+      const Real ylo = yp - wy, yhi = yp + wy, zlo = zp - wz, zhi = zp + wz;
+      bool found = false;
+      for_bins(ud, ylo, yhi, zlo, zhi, brute, [&](int32_t c) {
+        if (found) return;
+        const int64_t gc = off[ud] + c;
+        const Real yc = ys[gc], zc = zs[gc];
+        if (!(yc >= ylo && yc <= yhi && zc >= zlo && zc <= zhi)) return;
+        if (clean_up[gc] >= 0) return;                       // c must be the top of its chain
+        int32_t d1 = clean_dn[gc]; if (d1 < 0) return;
+        int32_t d2 = clean_dn[off[ud - 1] + d1]; if (d2 < 0) return;
+        { int len = 3; int uu = ud - 2; int32_t p = d2;      // at least min_seed clusters: the lower chain has its own start hit
+          while (len < T.bridge_min) { if (uu <= sec * R) break; int32_t nx = clean_dn[off[uu] + p]; if (nx < 0) break; p = nx; uu--; len++; }
+          if (len < T.bridge_min) return; }
+        const Real dxd = X[r - g] - X[r - g - 2];
+        const Real ty = (yc - ys[off[ud - 2] + d2]) / dxd, tz = (zc - zs[off[ud - 2] + d2]) / dxd;
+        const Real yq = yc + ty * dx, zq = zc + tz * dx;     // lower chain extended up to row r
+        if (yh >= yq - wy && yh <= yq + wy && zh >= zq - wz && zh <= zq + wz) found = true;
+      });
+      if (found) return true;
+    }
+    return false;
   }
 
   // ---- S5 building blocks ----
@@ -480,7 +529,7 @@ struct Oracle : OracleBase {
     s1_grid(); if (upto <= 1) return 0;
     s2_neighbours(brute & 1); if (upto <= 2) return 0;
     s3_clean(); if (upto <= 3) return 0;
-    s4_start_hits(); if (upto <= 4) return 0;
+    s4_start_hits((brute & 1) != 0); if (upto <= 4) return 0;
     s5_tracklets((brute & 2) != 0); if (upto <= 5) return 0;
     s6_select(); if (upto <= 6) return 0;
     s7_refit();
@@ -581,6 +630,7 @@ int orc_set_param(void* h, const char* name, double v) {
   else if (s == "c0_y") T.c0[0] = v; else if (s == "c0_z") T.c0[1] = v; else if (s == "c0_sinphi") T.c0[2] = v;
   else if (s == "c0_dzds") T.c0[3] = v; else if (s == "c0_qpt") T.c0[4] = v;
   else if (s == "grid_scale") T.grid_scale = v;
+  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v;
   else return -1;
   return 0;
 }

@@ -24,10 +24,77 @@ __device__ __forceinline__ int clean_up_of(const UnitDesc* __restrict__ units, c
   return link_dn[units[uu + 1].off + up] == p ? up : -1;
 }
 
+// cleaned down-link of sorted position p of unit uu (row rr >= 1): the raw link if mutual, else -1
+__device__ __forceinline__ int clean_dn_of(const UnitDesc* __restrict__ units, const int* link_up, const int* link_dn, int uu, int rr,
+                                           long long off_uu, int p) {
+  const int dn = link_dn[off_uu + p];
+  if (dn < 0 || rr < 1) return -1;
+  return link_up[units[uu - 1].off + dn] == p ? dn : -1;
+}
+
+// S4' seed bridging (NEXT-2 of SURVEY.md section 8(f); reading A39 of DESIGN.md; off unless bridge_rows > 0).  The start hit h
+// of unit u (row r) continues a lower chain -- and is dropped (k3_bridge_flag / k3_bridge_filter below) -- when the straight line through h and its second chain cluster
+// (row r+2), extended down to a row r-g (2 <= g <= bridge_rows), meets the TOP c of a chain of at least bridge_min clusters, and
+// the line through c and its second cluster below, extended up to row r, meets h; both within (bridge_wy, bridge_wz).
+// Every fp32 operation is spelled in the order of the definition (library built with -fmad=false); links are tested for
+// mutuality on the fly, which gives the same answer on raw and on already cleaned tables.
+__device__ bool seed_bridged(const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows, const float2* __restrict__ yz,
+                             const int* __restrict__ bin_start, const int* link_up, const int* link_dn, const int u, const int r,
+                             const int R, const int h, const int u1, const Params& P) {
+  if (r + 2 >= R) return false;
+  const long long off0 = units[u].off, off1 = units[u + 1].off, off2 = units[u + 2].off;
+  const int u2 = clean_up_of(units, link_up, link_dn, u + 1, r + 1, R, off1, u1);
+  if (u2 < 0) return false;
+  const float2 ch = yz[off0 + h], c2 = yz[off2 + u2];
+  const float x_r = rows[r].x;
+  const float dxu = rows[r + 2].x - x_r;
+  const float sy = (c2.x - ch.x) / dxu, sz = (c2.y - ch.y) / dxu;
+  for (int g = 2; g <= P.bridge_rows && r - g >= 2; g++) {
+    const int ud = u - g;
+    const UnitDesc d = units[ud];
+    if (d.n == 0) continue;
+    const float dx = x_r - rows[r - g].x;
+    const float yp = ch.x - sy * dx, zp = ch.y - sz * dx;
+    const float ylo = yp - P.bridge_wy, yhi = yp + P.bridge_wy, zlo = zp - P.bridge_wz, zhi = zp + P.bridge_wz;
+    const int by0 = bin_of(ylo, d.ylo, d.invs, d.ny), by1 = bin_of(yhi, d.ylo, d.invs, d.ny);
+    const int bz0 = bin_of(zlo, d.zlo, d.invs, d.nz), bz1 = bin_of(zhi, d.zlo, d.invs, d.nz);
+    const int* __restrict__ bs = bin_start + d.bin_off;
+    const long long offm1 = units[ud - 1].off, offm2 = units[ud - 2].off;
+    for (int bz = bz0; bz <= bz1; bz++) {
+      const int pe = bs[bz * d.ny + by1 + 1];
+      for (int c = bs[bz * d.ny + by0]; c < pe; c++) {
+        const float2 cc = yz[d.off + c];
+        if (!(cc.x >= ylo && cc.x <= yhi && cc.y >= zlo && cc.y <= zhi)) continue;
+        if (clean_up_of(units, link_up, link_dn, ud, r - g, R, d.off, c) >= 0) continue;      // c must be the top of its chain
+        const int d1 = clean_dn_of(units, link_up, link_dn, ud, r - g, d.off, c);
+        if (d1 < 0) continue;
+        const int d2 = clean_dn_of(units, link_up, link_dn, ud - 1, r - g - 1, offm1, d1);
+        if (d2 < 0) continue;
+        int len = 3, uu = ud - 2, p = d2;
+        while (len < P.bridge_min) {
+          const int rr = uu % R;
+          if (rr == 0) break;
+          const int nx = clean_dn_of(units, link_up, link_dn, uu, rr, units[uu].off, p);
+          if (nx < 0) break;
+          p = nx; uu--; len++;
+        }
+        if (len < P.bridge_min) continue;
+        const float2 cb = yz[offm2 + d2];
+        const float dxd = rows[r - g].x - rows[r - g - 2].x;
+        const float ty = (cc.x - cb.x) / dxd, tz = (cc.y - cb.y) / dxd;
+        const float yq = cc.x + ty * dx, zq = cc.y + tz * dx;
+        if (ch.x >= yq - P.bridge_wy && ch.x <= yq + P.bridge_wy && ch.y >= zq - P.bridge_wz && ch.y <= zq + P.bridge_wz) return true;
+      }
+    }
+  }
+  return false;
+}
+
 __global__ void __launch_bounds__(K3_THREADS) k3_clean_flag(const Item* __restrict__ items, const int chunk,
                                                             const UnitDesc* __restrict__ units, int* link_up, int* link_dn,
-                                                            unsigned* __restrict__ mask, int* __restrict__ item_count, const int R,
-                                                            const int min_seed) {
+                                                            unsigned* __restrict__ mask, int* __restrict__ item_count,
+                                                            const Params P) {
+  const int R = P.R, min_seed = P.min_seed;
   __shared__ int s_count;
   const Item it = items[blockIdx.x];
   const int u = it.unit, r = u % R;
@@ -96,7 +163,48 @@ __global__ void __launch_bounds__(K3_THREADS) k3_compact(const Item* __restrict_
   }
 }
 
+// S4' pass (only when bridge_rows > 0), on the finished S4 list and the fully cleaned link tables: one thread per start hit.
+__global__ void __launch_bounds__(K3_THREADS) k3_bridge_flag(const int M, const int* __restrict__ start_unit,
+                                                             const int* __restrict__ start_pos, const UnitDesc* __restrict__ units,
+                                                             const RowConst* __restrict__ rows, const float2* __restrict__ yz,
+                                                             const int* __restrict__ bin_start, const int* __restrict__ link_up,
+                                                             const int* __restrict__ link_dn, int* __restrict__ keep, const Params P) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M) return;
+  const int u = start_unit[i], h = start_pos[i];
+  const int cu = link_up[units[u].off + h];   // cleaned: a start hit has an up link
+  keep[i] = seed_bridged(units, rows, yz, bin_start, link_up, link_dn, u, u % P.R, P.R, h, cu, P) ? 0 : 1;
+}
+
+// order-preserving filter of the start list: entry i moves to position pos[i] (exclusive scan of keep) when kept
+__global__ void __launch_bounds__(K3_THREADS) k3_bridge_filter(const int M, const int* __restrict__ start_unit,
+                                                               const int* __restrict__ start_pos, const int* __restrict__ keep,
+                                                               const int* __restrict__ pos, int* __restrict__ out_unit,
+                                                               int* __restrict__ out_pos) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= M || !keep[i]) return;
+  out_unit[pos[i]] = start_unit[i];
+  out_pos[pos[i]] = start_pos[i];
+}
+
 }  // namespace
+
+int launch_k3_bridge(const Launch& L, int M, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
+                     const RowConst* d_rows, const float2* d_yz, const int* d_bin_start, const int* d_link_up, const int* d_link_dn,
+                     int* d_keep, int* d_keep_pos, int* d_scan_tmp, int* d_out_unit, int* d_out_pos, int* d_total, const Params& P) {
+  if (M <= 0) {
+    cudaError_t e = cudaMemsetAsync(d_total, 0, sizeof(int), L.stream);
+    return e == cudaSuccess ? 0 : -(int)e;
+  }
+  const int blocks = (M + K3_THREADS - 1) / K3_THREADS;
+  k3_bridge_flag<<<blocks, K3_THREADS, 0, L.stream>>>(M, d_start_unit, d_start_pos, d_units, d_rows, d_yz, d_bin_start, d_link_up,
+                                                      d_link_dn, d_keep, P);
+  int rc = launch_scan_i32(L, d_keep, d_keep_pos, M, d_scan_tmp, d_total);
+  if (rc < 0) return rc;
+  k3_bridge_filter<<<blocks, K3_THREADS, 0, L.stream>>>(M, d_start_unit, d_start_pos, d_keep, d_keep_pos, d_out_unit, d_out_pos);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? 2 + rc : -(int)e;
+}
 
 int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, int* d_link_up,
                           int* d_link_dn, unsigned* d_mask, int* d_item_count, int* d_item_base, int* d_scan_tmp,
@@ -105,8 +213,7 @@ int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int
     cudaError_t e = cudaMemsetAsync(d_total, 0, sizeof(int), L.stream);
     return e == cudaSuccess ? 0 : -(int)e;
   }
-  k3_clean_flag<<<n_items, K3_THREADS, 0, L.stream>>>(d_items, chunk, d_units, d_link_up, d_link_dn, d_mask, d_item_count, P.R,
-                                                       P.min_seed);
+  k3_clean_flag<<<n_items, K3_THREADS, 0, L.stream>>>(d_items, chunk, d_units, d_link_up, d_link_dn, d_mask, d_item_count, P);
   int rc = launch_scan_i32(L, d_item_count, d_item_base, n_items, d_scan_tmp, d_total);
   if (rc < 0) return rc;
   const int warps = K3_THREADS / 32;

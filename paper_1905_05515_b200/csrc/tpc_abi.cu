@@ -87,6 +87,8 @@ struct Tunables {   // DESIGN.md table T
   int debug_keep = 0;
   int chunk = 1024;           // clusters per K2/K3 work item (multiple of 32)
   int k2_threads = 0;         // K2 block size (0 = default 256); tuning knob
+  int bridge_rows = 0, bridge_min = 3;       // NEXT-2 seed bridging (reading A39): 0 = off
+  double bridge_wy = 1.0, bridge_wz = 1.5;
 };
 
 struct UnitSrc { long long src = 0; int n = 0; };
@@ -124,7 +126,7 @@ struct tpc_ctx {
   // S1..S4
   long long N = 0, n_bins = 0; int n_items = 0;
   DevBuf d_yz, d_perm, d_bin_start, d_cursor, d_link_up, d_link_dn, d_raw_up, d_raw_dn, d_mask, d_item_count, d_item_base, d_scan_tmp;
-  DevBuf d_start_unit, d_start_pos, d_counters;
+  DevBuf d_start_unit, d_start_pos, d_counters, d_keep, d_keep_pos, d_start_unit2, d_start_pos2;
   // S5/S6
   int M = 0; long long Mpad = 0;
   DevBuf d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out, d_scan_tmp64;
@@ -229,7 +231,8 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->d_start_unit, &c->d_start_pos, &c->d_counters, &c->d_rowhit, &c->d_tl_n, &c->d_tl_first, &c->d_tl_last, &c->d_tl_chi2,
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
-                    &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0};
+                    &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
+                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
   c->ho_sector.release(); c->ho_ndf.release(); c->ho_tracklet.release(); c->ho_cl_row.release(); c->ho_cl_index.release();
@@ -268,6 +271,9 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "debug_keep") T.debug_keep = v != 0;
   else if (s == "k2_threads") { int k = (int)v; if (k < 32 || k > 256 || (k & 31)) return fail(c, TPC_E_ARG, "k2_threads must be a multiple of 32 in 32..256"); T.k2_threads = k; }
   else if (s == "chunk") { int k = (int)v; if (k < 32 || k > 4096 || (k & 31)) return fail(c, TPC_E_ARG, "chunk must be a multiple of 32 in 32..4096"); T.chunk = k; }
+  else if (s == "bridge_rows") { if (v < 0 || v > 16) return fail(c, TPC_E_ARG, "bridge_rows must be in 0..16"); T.bridge_rows = (int)v; }
+  else if (s == "bridge_min") { if (v < 3 || v > 255) return fail(c, TPC_E_ARG, "bridge_min must be in 3..255"); T.bridge_min = (int)v; }
+  else if (s == "bridge_wy") rc = pos(T.bridge_wy); else if (s == "bridge_wz") rc = pos(T.bridge_wz);
   else return fail(c, TPC_E_ARG, "tpc_set_param: unknown parameter '%s'", name);
   if (rc == TPC_OK) c->rows_valid = false;
   return rc;
@@ -373,6 +379,7 @@ void make_params_and_rows(tpc_ctx* c, std::vector<RowConst>& rows) {
   P.ry = c->sigma_y * c->sigma_y; P.rz = c->sigma_z * c->sigma_z;
   P.smax = (float)T.s_max; P.nsigma = (float)T.n_sigma; P.wmax = (float)T.w_max; P.edge_margin = (float)T.edge_margin;
   P.max_gap = T.max_gap; P.min_hits = T.min_hits;
+  P.bridge_rows = T.bridge_rows; P.bridge_min = T.bridge_min; P.bridge_wy = (float)T.bridge_wy; P.bridge_wz = (float)T.bridge_wz;
 }
 
 // S1 grid descriptor of every unit + CSR offsets + K2/K3 work items.  Returns a tpc_status.
@@ -495,8 +502,27 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, cudaEventRecord(c->ev[4], st));
   CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(c, cudaStreamSynchronize(st));
-  const int M = *c->p_small.as<int>();
+  int M = *c->p_small.as<int>();
   if (M < 0 || M > start_cap) return fail(c, TPC_E_CUDA, "start-hit count %d out of range", M);
+  if (c->T.bridge_rows > 0 && M > 0) {   // S4' (NEXT-2 variant): drop the start hits that continue a lower chain, order kept
+    const size_t Mb = (size_t)M * 4;
+    CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
+    CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
+    LAUNCH_TRY(c, launch_k3_bridge(L, M, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
+                                   c->d_yz.as<float2>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(), c->d_link_dn.as<int>(),
+                                   c->d_keep.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), c->d_start_unit2.as<int>(),
+                                   c->d_start_pos2.as<int>(), d_nstart, P), launches);
+    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    const int M2 = *c->p_small.as<int>();
+    if (M2 < 0 || M2 > M) return fail(c, TPC_E_CUDA, "bridged start-hit count %d out of range", M2);
+    if (M2 > 0) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->d_start_unit.p, c->d_start_unit2.p, (size_t)M2 * 4, cudaMemcpyDeviceToDevice, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->d_start_pos.p, c->d_start_pos2.p, (size_t)M2 * 4, cudaMemcpyDeviceToDevice, st));
+    }
+    CUDA_TRY(c, cudaEventRecord(c->ev[4], st));   // the S4' pass counts as part of K3's time
+    M = M2;
+  }
   if (M > (1 << 24)) return fail(c, TPC_E_CAPACITY, "%d tracklets exceed the 2^24 capacity of the selector key", M);
   const long long Mpad = ((long long)M + 31) & ~31LL;
   c->M = M; c->Mpad = Mpad;

@@ -39,6 +39,8 @@ struct Params {
   float ry, rz;                   // sigma_y^2, sigma_z^2
   float smax, nsigma, wmax, edge_margin;
   int max_gap, min_hits;
+  int bridge_rows, bridge_min;    // NEXT-2 seed bridging (reading A39); bridge_rows = 0: off
+  float bridge_wy, bridge_wz;
 };
 
 // Work item of K2/K3: a chunk of consecutive sorted hits of one unit.
@@ -92,6 +94,10 @@ int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float*
 int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units,
                          const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up,
                          int* d_link_dn, const Params& P);
+
+int launch_k3_bridge(const Launch& L, int M, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
+                     const RowConst* d_rows, const float2* d_yz, const int* d_bin_start, const int* d_link_up, const int* d_link_dn,
+                     int* d_keep, int* d_keep_pos, int* d_scan_tmp, int* d_out_unit, int* d_out_pos, int* d_total, const Params& P);
 
 int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, int* d_link_up,
                           int* d_link_dn, unsigned* d_mask, int* d_item_count, int* d_item_base, int* d_scan_tmp,

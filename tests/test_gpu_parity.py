@@ -120,6 +120,18 @@ def test_refit_before_find_tracks_is_a_state_error():
         assert e.value.code == -2
 
 
+def test_seed_bridging_variant_parity():
+    """NEXT-2 (reading A39): with bridge_rows / bridge_min set on both sides the start-hit list stays bit-exact and the tracks
+    keep the parity bars; fewer tracklets than S4, efficiency within 0.3 % of it."""
+    for w in (W.config(1), W.config(3, scale=0.1)):
+        rng = np.random.default_rng(5)
+        o, otr, gtr, res = _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, 60, replace=False), bridge_rows=4, bridge_min=8)
+        base = P.make_oracle(w).run("s6")
+        assert len(o.get("start_unit")) <= 0.75 * len(base.get("start_unit"))
+        m0, m1 = H.truth_metrics(w, base.tracks()), H.truth_metrics(w, gtr)
+        assert m1["eff"] >= m0["eff"] - 0.003, (m0["eff"], m1["eff"])
+
+
 def test_empty_and_tiny_inputs():
     w = W.config(1, scale=0.05)
     with _tracker(w) as trk:
