@@ -132,6 +132,22 @@ def test_seed_bridging_variant_parity():
         assert m1["eff"] >= m0["eff"] - 0.003, (m0["eff"], m1["eff"])
 
 
+def test_large_units_take_the_partly_shared_k1_path():
+    """Units of about 5 k clusters: K1 keeps cursors + sorted indices in shared memory but gathers (y, z) from global memory
+    (the plan between the all-shared one of C3-sized units and the global-cursor one).  S0-S4 tables bit-exact."""
+    import math
+    w = W.generate(W.Params(seed=9, single_sector=1, mult_fixed=7000, phi_lo=0.0, phi_hi=2 * math.pi / 18, noise_per_sector=20000), "dense")
+    n_unit = np.diff(w.unit_off)
+    assert 4000 < n_unit.max() < 9000
+    o = P.make_oracle(w).run("s4")
+    with _tracker(w, debug_keep=1) as trk:
+        trk.load_workload(w)
+        trk.find_tracks()
+        assert P.compare_grid(w, o, trk, range(0, w.n_rows, 3)) > 40
+        lk = P.compare_links(w, o, trk)
+    assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
+
+
 def test_empty_and_tiny_inputs():
     w = W.config(1, scale=0.05)
     with _tracker(w) as trk:
