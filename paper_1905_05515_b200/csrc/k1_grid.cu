@@ -109,15 +109,32 @@ __global__ void __launch_bounds__(1024, 2) k1_grid_build(const UnitDesc* __restr
   for (int b = threadIdx.x; b < nb; b += blockDim.x) bs[b + 1] = cnt[b];
   if (threadIdx.x == 0) bs[0] = 0;
   float2* __restrict__ out = yz + d.off;
+  // E (units whose scattered indices are in shared memory): stable placement and payload in one pass, one thread per
+  // scattered position.  Position p holds original index i of bin b; its final position is start(b) + #{q in bin b : index at
+  // q < i}, so the order inside a bin is ascending original index whatever order the atomics of pass D produced.  Writes
+  // stay inside the bin's range.  (y, z) from the shared copy, or re-read from the input (L2) for the larger units.
   if (yz_s) {
-    // E (shared-memory units): stable placement and payload in one pass, one thread per scattered position.  Position p
-    // holds original index i of bin b; its final position is start(b) + #{q in bin b : index at q < i}, so the order inside
-    // a bin is ascending original index whatever order the atomics of pass D produced.  Writes stay inside the bin's range.
     for (int p = threadIdx.x; p < n; p += blockDim.x) {
       const int i = pm[p];
       const float2 c = syz[i];
       const int b = bin_of(c.y, d.zlo, d.invs, nz) * ny + bin_of(c.x, d.ylo, d.invs, ny);
       const int lo = b ? cnt[b - 1] : 0, hi = cnt[b];   // after D, cursor[b] = end of bin b
+      int rank = 0;
+#pragma unroll 2
+      for (int q = lo; q < hi; q++) rank += pm[q] < i;
+      pg[lo + rank] = i;
+      out[lo + rank] = c;
+    }
+    return;
+  }
+  if (perm_s) {
+    const float* py = in_y + d.src;
+    const float* pt = in_t + d.src;
+    for (int p = threadIdx.x; p < n; p += blockDim.x) {
+      const int i = pm[p];
+      const float2 c = make_float2(py[i], __fsub_rn(zmax, __fmul_rn(vdrift, pt[i])));
+      const int b = bin_of(c.y, d.zlo, d.invs, nz) * ny + bin_of(c.x, d.ylo, d.invs, ny);
+      const int lo = b ? cnt[b - 1] : 0, hi = cnt[b];
       int rank = 0;
 #pragma unroll 2
       for (int q = lo; q < hi; q++) rank += pm[q] < i;
@@ -143,7 +160,6 @@ __global__ void __launch_bounds__(1024, 2) k1_grid_build(const UnitDesc* __restr
   const float* pt = in_t + d.src;
   for (int p = threadIdx.x; p < n; p += blockDim.x) {
     const int i = pm[p];
-    if (perm_s) pg[p] = i;
     out[p] = make_float2(py[i], __fsub_rn(zmax, __fmul_rn(vdrift, pt[i])));
   }
 }
@@ -157,10 +173,10 @@ int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float*
   int threads = 128;
   while (threads < 1024 && threads * 16 < max_n) threads <<= 1;   // about 8-16 clusters per thread and pass: small CTAs, more of them per SM
   // Shared memory per CTA: the cursors always; the sorted indices and the (y, z) pairs too while that keeps >= 4 CTAs per SM
-  // (56 KB); the sorted indices alone up to 2 CTAs per SM (112 KB).
+  // (56 KB); the sorted indices alone up to 192 KB (one 1024-thread CTA per SM for 20 k-cluster units).
   int ints = max_cursor_ints_smem;
   if (max_yz_ints <= 14 * 1024) ints = ints > max_yz_ints ? ints : max_yz_ints;
-  else if (max_perm_ints <= 28 * 1024) ints = ints > max_perm_ints ? ints : max_perm_ints;
+  else if (max_perm_ints <= 48 * 1024) ints = ints > max_perm_ints ? ints : max_perm_ints;
   size_t smem = (size_t)ints * sizeof(int);
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(k1_grid_build, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
