@@ -21,6 +21,7 @@
  * composition, round trip, Jacobian vs finite differences; S5 fit: noise-free helix recovery 1e-5,
  * Bz=0 exact, chi2/ndf = 1 and pulls on smeared tracks; S6 hand-built sharing cases, order invariance.
  * S4' (NEXT-2) seed bridging: hand-made single dropouts (one start hit per track), subset of the S4 list, brute-force probe.
+ * S8 (NEXT-4) tube adjacency: independent numpy restatement with the closed-form helix, brute force over the rows, truth labels.
  * S7 (NEXT-1) refit + collision time: noise-free recovery, chi2/ndf = 1, t0 against the generator's collision times.
  * Absolute efficiency / resolution versus the paper: parity unpinned (PAPER.md:49 gives no number).
  */
@@ -46,6 +47,7 @@ struct Tunables {            // DESIGN.md table T (all are readings; the paper i
   int bridge_rows = 0;          // NEXT-2 (reading A39): 0 = off; else the deepest row gap a start hit may bridge to a lower chain
   double bridge_wy = 1.0, bridge_wz = 1.5;
   int bridge_min = 3;           // clusters the lower chain must have
+  double tube = 1.5;            // NEXT-4: radius of the tube around a track, cm
 };
 
 struct OracleBase {
@@ -87,6 +89,8 @@ struct Oracle : OracleBase {
   std::vector<double> trk_x, trk_par, trk_cov, trk_chi2;
   // S7 (NEXT-1): refit of the owned clusters + collision-time estimate
   std::vector<int32_t> rf_n, rf_ndf; std::vector<double> rf_x, rf_par, rf_cov, rf_chi2, rf_z0, rf_t0;
+  // S8 (NEXT-4): attachment status of every cluster, caller's order (CSR offset of the unit + index inside the unit)
+  std::vector<int32_t> cl_status, cl_track;
   std::vector<double> z_d, ys_d, zs_d;   // export copies
 
   Oracle(int ns, int nr, const float* rx, double dphi_, double zmax, double tframe, double sy, double sz, double bz_, double vd)
@@ -523,6 +527,49 @@ struct Oracle : OracleBase {
     }
   }
 
+  // ---- S8 (NEXT-4; "The tracker forms tubes of 1.5 cm around each track, and marks
+  //      unattached clusters as adjacent to the tube of the track with the highest transverse momentum it lies in"; reading A40).
+  //      status 1 = attached (in the cluster list of a track), 2 = adjacent, 0 = neither; cl_track = that track, or -1.
+  //      The tube follows the S6 state of the track, transported row by row (helix, parameters only) from the row of the state
+  //      to the row of the track's last cluster; distance in the (y, z) plane of the pad row.
+  void s8_adjacent(bool brute) {
+    const int64_t NT = (int64_t)trk_sector.size();
+    std::vector<int32_t> att(N, -1), adj_t(N, -1); std::vector<Real> adj_q(N, (Real)0);
+    for (int64_t i = 0; i < NT; i++) {
+      const int sec = trk_sector[i]; const int32_t T_ = trk_tracklet[i];
+      for (int64_t k = trk_cl_begin[i]; k < trk_cl_begin[i + 1]; k++) { int r = trk_cl_row[k]; att[off[sec * R + r] + tl_rowhit[(int64_t)T_ * R + r]] = (int32_t)i; }
+    }
+    const Real tube = (Real)T.tube, tube2 = tube * tube, margin = (Real)0.05;
+    for (int64_t i = 0; i < NT; i++) {
+      const int sec = trk_sector[i]; const int32_t T_ = trk_tracklet[i];
+      const int r_first = tl_first[T_], r_last = trk_cl_row[trk_cl_begin[i + 1] - 1];
+      State st; for (int a = 0; a < 5; a++) for (int b = 0; b < 5; b++) st.C[a][b] = 0;
+      const Real zref = (Real)trk_par[i * 5 + 1];
+      st.p[0] = (Real)trk_par[i * 5 + 0]; st.p[1] = 0; st.p[2] = (Real)trk_par[i * 5 + 2]; st.p[3] = (Real)trk_par[i * 5 + 3]; st.p[4] = (Real)trk_par[i * 5 + 4];
+      if (!std::isfinite(st.p[4])) continue;
+      const Real aq = std::fabs(st.p[4]);
+      for (int r = r_first; r <= r_last; r++) {
+        if (r > r_first && !propagate_state(st, X[r] - X[r - 1])) break;
+        const int u = sec * R + r; const int64_t o = off[u];
+        const Real y = st.p[0], zr = st.p[1];
+        const Real ylo = y - tube, yhi = y + tube, zlo = zr - tube, zhi = zr + tube;
+        for_bins(u, ylo, yhi, (zlo + zref) - margin, (zhi + zref) + margin, brute, [&](int32_t p) {
+          const Real dy = ys[o + p] - y, dz = (zs[o + p] - zref) - zr;
+          const Real d2 = dy * dy + dz * dz;
+          if (!(d2 <= tube2) || att[o + p] >= 0) return;
+          if (adj_t[o + p] < 0 || aq < adj_q[o + p] || (aq == adj_q[o + p] && (int32_t)i < adj_t[o + p])) { adj_q[o + p] = aq; adj_t[o + p] = (int32_t)i; }
+        });
+      }
+    }
+    cl_status.assign(N, 0); cl_track.assign(N, -1);
+    for (int u = 0; u < NS * R; u++)
+      for (int64_t g = off[u]; g < off[u + 1]; g++) {
+        const int64_t c = off[u] + perm[g];
+        if (att[g] >= 0) { cl_status[c] = 1; cl_track[c] = att[g]; }
+        else if (adj_t[g] >= 0) { cl_status[c] = 2; cl_track[c] = adj_t[g]; }
+      }
+  }
+
   int run(int upto, int brute) override {
     make_tables();
     s0_time_to_z(); if (upto <= 0) return 0;
@@ -532,7 +579,8 @@ struct Oracle : OracleBase {
     s4_start_hits((brute & 1) != 0); if (upto <= 4) return 0;
     s5_tracklets((brute & 2) != 0); if (upto <= 5) return 0;
     s6_select(); if (upto <= 6) return 0;
-    s7_refit();
+    s7_refit(); if (upto <= 7) return 0;
+    s8_adjacent((brute & 2) != 0);
     return 0;
   }
 
@@ -599,6 +647,8 @@ struct Oracle : OracleBase {
     if (s == "trk_par") RET(trk_par, 2)
     if (s == "trk_cov") RET(trk_cov, 2)
     if (s == "trk_chi2") RET(trk_chi2, 2)
+    if (s == "cl_status") RET(cl_status, 0)
+    if (s == "cl_track") RET(cl_track, 0)
     if (s == "rf_n") RET(rf_n, 0)
     if (s == "rf_ndf") RET(rf_ndf, 0)
     if (s == "rf_x") RET(rf_x, 2)
@@ -630,7 +680,7 @@ int orc_set_param(void* h, const char* name, double v) {
   else if (s == "c0_y") T.c0[0] = v; else if (s == "c0_z") T.c0[1] = v; else if (s == "c0_sinphi") T.c0[2] = v;
   else if (s == "c0_dzds") T.c0[3] = v; else if (s == "c0_qpt") T.c0[4] = v;
   else if (s == "grid_scale") T.grid_scale = v;
-  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v;
+  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "tube") T.tube = v;
   else return -1;
   return 0;
 }
