@@ -178,6 +178,12 @@ def run_gpu(args, rank, world, local_rank):
     value = total_clusters / (ms * 1e-3)
     kern = {k: acc[k] / args.steps for k in keys}
     n_tracks, n_refs = res.n_tracks, res.n_cluster_refs
+    # S8 (NEXT-4, not part of the timed step): attachment status of every cluster (Fig. 7's attached / adjacent)
+    mk = [trk.mark_clusters(1.5, device_result=True) for _ in range(3)]
+    mark_ms = float(np.mean([m["ms_mark"] for m in mk[1:]]))
+    mst = mk[-1]["status"]
+    marks = {"ms": mark_ms, "clusters_per_s": N / (mark_ms * 1e-3), "tube_cm": 1.5, "attached_frac": float((mst == 1).sum().item()) / N,
+             "adjacent_frac": float((mst == 2).sum().item()) / N, "note": "S8 cluster attachment status (SURVEY 8(f).4), outside the timed step"}
     # NEXT-2 variant (seed bridging, reading A39), measured beside the default path, never mixed into `value`
     variant = None
     if args.variant and rank == 0:
@@ -298,7 +304,7 @@ def run_gpu(args, rank, world, local_rank):
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
-           "variant_seed_bridging": variant,
+           "variant_seed_bridging": variant, "cluster_marks": marks,
            "refit": {"ms": refit_ms, "tracks_per_s": n_tracks / (refit_ms * 1e-3), "note": "S7 refit + collision time (SURVEY 8(f).1), outside the timed step"},
            "clocks": clocks}
     print(json.dumps(out))

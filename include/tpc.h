@@ -85,6 +85,17 @@ typedef struct {
   float ms_refit;           /* device time of K7 (CUDA events on the context's stream), ms */
 } tpc_refit;
 
+/* Result of tpc_mark_clusters: S8 of DESIGN.md section 4 ("The tracker forms tubes of 1.5 cm
+ * around each track, and marks unattached clusters as adjacent to the tube of the track with the highest transverse momentum it lies
+ * in"; reading A40).  One entry per loaded cluster, in the caller's order: units (sector*n_rows+row) ascending, inside a unit the index
+ * in the arrays passed to tpc_load_clusters*.  Library-owned, host (device_result = 0) or device memory, valid until the next call. */
+typedef struct {
+  int64_t n_clusters;
+  const int32_t* status;    /* [n_clusters] 0 = in no tube, 1 = attached (in the cluster list of a track), 2 = adjacent */
+  const int32_t* track;     /* [n_clusters] track of the last tpc_find_tracks* call it is attached / adjacent to, -1 for status 0 */
+  float ms_mark;            /* device time of K8 (CUDA events on the context's stream), ms */
+} tpc_cluster_marks;
+
 /* Per-step device times of the last tpc_find_tracks* call (CUDA events on the context's stream), ms. */
 typedef struct {
   float ms_upload;          /* host staging -> device (0 if the clusters were already device-resident) */
@@ -149,6 +160,10 @@ int tpc_find_tracks_device(tpc_ctx*, tpc_tracks* out);
 /* S7: refit every track of the last tpc_find_tracks* call over the clusters it owns and estimate its collision time.
  * Errors: TPC_E_ARG (null), TPC_E_STATE (no completed tpc_find_tracks* call on this context), TPC_E_NOMEM, TPC_E_CUDA. */
 int tpc_refit_tracks(tpc_ctx*, int device_result, tpc_refit* out);
+
+/* S8: attachment status of every cluster with respect to the tracks of the last tpc_find_tracks* call; tube_cm > 0 (the paper: 1.5).
+ * Errors: TPC_E_ARG (null, tube_cm not > 0 or not finite), TPC_E_STATE (no completed tpc_find_tracks* call), TPC_E_NOMEM, TPC_E_CUDA. */
+int tpc_mark_clusters(tpc_ctx*, float tube_cm, int device_result, tpc_cluster_marks* out);
 
 /* Forget the clusters and results, keep geometry, parameters and buffers (one call per event / time frame). */
 int tpc_clear(tpc_ctx*);

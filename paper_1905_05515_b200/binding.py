@@ -17,7 +17,7 @@ _SO = os.path.join(_HERE, "libtpc_b200.so")
 
 ABI_SYMBOLS = [
     "tpc_abi_version", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
-    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
+    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
     "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
 
@@ -44,6 +44,10 @@ class _Tracks(C.Structure):
 class _Refit(C.Structure):
     _fields_ = [("n_tracks", C.c_int64)] + [(k, C.c_void_p) for k in ("n", "ndf", "x", "par", "cov", "chi2", "z0", "t0")] + \
                [("ms_refit", C.c_float)]
+
+
+class _Marks(C.Structure):
+    _fields_ = [("n_clusters", C.c_int64), ("status", C.c_void_p), ("track", C.c_void_p), ("ms_mark", C.c_float)]
 
 
 class _Timings(C.Structure):
@@ -92,6 +96,7 @@ def load_library():
     lib.tpc_find_tracks.argtypes = [vp, C.POINTER(_Tracks)]
     lib.tpc_find_tracks_device.argtypes = [vp, C.POINTER(_Tracks)]
     lib.tpc_refit_tracks.argtypes = [vp, C.c_int, C.POINTER(_Refit)]
+    lib.tpc_mark_clusters.argtypes = [vp, C.c_float, C.c_int, C.POINTER(_Marks)]
     lib.tpc_clear.argtypes = [vp]
     lib.tpc_destroy.argtypes = [vp]
     lib.tpc_destroy.restype = None
@@ -271,6 +276,15 @@ def tpc_refit_tracks(h, device_result=False) -> dict:
     return d
 
 
+def tpc_mark_clusters(h, tube_cm=1.5, device_result=False) -> dict:
+    """S8: attachment status (0 none / 1 attached / 2 adjacent) and track of every cluster, caller's order (zero-copy views)."""
+    t = _Marks()
+    _check(h, load_library().tpc_mark_clusters(h, float(tube_cm), 1 if device_result else 0, C.byref(t)))
+    make = _dev_tensor if device_result else _host_array
+    n = int(t.n_clusters)
+    return {"n_clusters": n, "ms_mark": float(t.ms_mark), "status": make(t.status, n, np.int32), "track": make(t.track, n, np.int32)}
+
+
 class Tracker:
     """Context manager around one tpc_ctx, for the tests and bench.py."""
 
@@ -328,6 +342,9 @@ class Tracker:
 
     def refit_tracks(self, device_result=False) -> dict:
         return tpc_refit_tracks(self.h, device_result)
+
+    def mark_clusters(self, tube_cm=1.5, device_result=False) -> dict:
+        return tpc_mark_clusters(self.h, tube_cm, device_result)
 
     def clear(self):
         self._keep = []

@@ -136,6 +136,8 @@ struct tpc_ctx {
   // outputs / debug copies (host)
   PinVec<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; PinVec<float> ho_x, ho_par, ho_cov, ho_chi2;
   PinVec<int64_t> ho_cl_begin;
+  // S8 cluster marks (device + host)
+  DevBuf m_att, m_adj, m_status, m_track; PinVec<int32_t> hm_status, hm_track;
   // S7 refit (device + host)
   DevBuf r_n, r_ndf, r_x, r_par, r_cov, r_chi2, r_z0, r_t0;
   PinVec<int32_t> hr_n, hr_ndf; PinVec<float> hr_x, hr_par, hr_cov, hr_chi2, hr_z0, hr_t0;
@@ -232,13 +234,13 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
                     &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
-                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2};
+                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->m_att, &c->m_adj, &c->m_status, &c->m_track};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
   c->ho_sector.release(); c->ho_ndf.release(); c->ho_tracklet.release(); c->ho_cl_row.release(); c->ho_cl_index.release();
   c->ho_x.release(); c->ho_par.release(); c->ho_cov.release(); c->ho_chi2.release(); c->ho_cl_begin.release();
   c->hr_n.release(); c->hr_ndf.release(); c->hr_x.release(); c->hr_par.release(); c->hr_cov.release(); c->hr_chi2.release();
-  c->hr_z0.release(); c->hr_t0.release();
+  c->hr_z0.release(); c->hr_t0.release(); c->hm_status.release(); c->hm_track.release();
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
   delete c;
 }
@@ -655,6 +657,40 @@ int tpc_refit_tracks(tpc_ctx* c, int device_result, tpc_refit* out) {
   }
   CUDA_TRY(c, cudaStreamSynchronize(st));
   CUDA_TRY(c, cudaEventElapsedTime(&out->ms_refit, c->ev[8], c->ev[9]));
+  return TPC_OK;
+}
+// S8 (NEXT-4): K8 over the tracks and the grid of the last call.
+int tpc_mark_clusters(tpc_ctx* c, float tube_cm, int device_result, tpc_cluster_marks* out) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_mark_clusters: null argument");
+  memset(out, 0, sizeof(*out));
+  if (!(tube_cm > 0) || !std::isfinite(tube_cm)) return fail(c, TPC_E_ARG, "tpc_mark_clusters: tube_cm must be finite and > 0");
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_mark_clusters: call tpc_find_tracks first");
+  cudaStream_t st = c->stream;
+  Launch L{st, c->sm_count, c->T.k2_threads};
+  const long long N = c->N; const size_t Nz = (size_t)std::max(N, 1LL);
+  CUDA_TRY(c, c->m_att.ensure(Nz * 4)); CUDA_TRY(c, c->m_adj.ensure(Nz * 8)); CUDA_TRY(c, c->m_status.ensure(Nz * 4));
+  CUDA_TRY(c, c->m_track.ensure(Nz * 4));
+  long long launches = 0;
+  CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
+  LAUNCH_TRY(c, launch_k8_status(L, c->n_tracks, N, c->NS * c->R, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_par.as<float>(),
+                                 c->o_cl_begin.as<long long>(), c->o_cl_row.as<int>(), c->d_tl_first.as<int>(), c->d_units.as<UnitDesc>(),
+                                 c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
+                                 c->d_rowhit.as<int>(), c->m_att.as<int>(), (unsigned long long*)c->m_adj.p, c->m_status.as<int>(),
+                                 c->m_track.as<int>(), tube_cm, c->P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
+  out->n_clusters = N;
+  if (!device_result) {
+    CUDA_TRY(c, c->hm_status.resize(Nz)); CUDA_TRY(c, c->hm_track.resize(Nz));
+    if (N > 0) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->hm_status.data(), c->m_status.p, (size_t)N * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hm_track.data(), c->m_track.p, (size_t)N * 4, cudaMemcpyDeviceToHost, st));
+    }
+    out->status = c->hm_status.data(); out->track = c->hm_track.data();
+  } else {
+    out->status = c->m_status.as<int32_t>(); out->track = c->m_track.as<int32_t>();
+  }
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  CUDA_TRY(c, cudaEventElapsedTime(&out->ms_mark, c->ev[8], c->ev[9]));
   return TPC_OK;
 }
 int tpc_get_timings(tpc_ctx* c, tpc_timings* out) {

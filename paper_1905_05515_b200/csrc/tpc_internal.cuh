@@ -126,6 +126,12 @@ int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, co
                     int* rf_n, int* rf_ndf, float* rf_x, float* rf_par, float* rf_cov, float* rf_chi2, float* rf_z0, float* rf_t0,
                     const Params& P);
 
+int launch_k8_status(const Launch& L, long long n_tracks, long long N, int U, const int* o_sector, const int* o_tracklet,
+                     const float* o_par, const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first,
+                     const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
+                     const int* d_rowhit, int* d_att, unsigned long long* d_adj, int* cl_status, int* cl_track, float tube,
+                     const Params& P);
+
 // device-wide exclusive scans (own kernels; three launches each)
 int launch_scan_i32(const Launch& L, const int* d_in, int* d_out, int n, int* d_tmp, int* d_total);
 int launch_scan_u64(const Launch& L, const unsigned long long* d_in, unsigned long long* d_out, int n, unsigned long long* d_tmp,

@@ -111,6 +111,47 @@ def test_refit_parity_continuous_c3_scaled():
     assert len(dt) > 500 and abs(np.median(dt)) < 0.05 and np.percentile(np.abs(dt), 99) < 1.0, (len(dt), np.median(dt))
 
 
+def _marks_parity(w):
+    """S8 (NEXT-4): cluster status bit-exact against the oracle when the track lists are identical (track numbering included)."""
+    o = P.make_oracle(w).run("s8")
+    otr = o.tracks(); ost, otk = o.cluster_status()
+    with _tracker(w) as trk:
+        trk.load_workload(w)
+        gtr = trk.find_tracks().copy().as_dict()
+        m = trk.mark_clusters(1.5)
+        st, tk = np.array(m["status"]), np.array(m["track"])
+        dev = trk.mark_clusters(1.5, device_result=True)
+        assert np.array_equal(dev["status"].cpu().numpy(), st) and np.array_equal(dev["track"].cpu().numpy(), tk)
+        assert m["n_clusters"] == w.n_clusters and m["ms_mark"] > 0
+    same_lists = len(otr["sector"]) == len(gtr["sector"]) and np.array_equal(otr["cl_begin"], gtr["cl_begin"]) and \
+        np.array_equal(otr["cl_index"], gtr["cl_index"]) and np.array_equal(otr["cl_row"], gtr["cl_row"])
+    assert same_lists
+    diff = int(((st != ost) | (tk != otk)).sum())
+    assert diff <= 1e-4 * w.n_clusters, diff         # a tube boundary decided in the last fp32 bit of a transported state
+    return st, tk, ost
+
+
+def test_cluster_marks_parity_c1_and_c3_scaled():
+    for w in (W.config(1), W.config(3, scale=0.1)):
+        st, tk, ost = _marks_parity(w)
+        assert (st == 1).sum() > 0.8 * w.n_clusters and (st == 2).sum() > 0 and (st == 0).sum() > 0
+        assert np.all((tk >= 0) == (st != 0))
+
+
+def test_cluster_marks_argument_and_state_errors():
+    import paper_1905_05515_b200 as T
+    w = W.config(1, scale=0.1)
+    with _tracker(w) as trk:
+        with pytest.raises(T.TpcError) as e:
+            trk.mark_clusters()
+        assert e.value.code == -2
+        trk.load_workload(w); trk.find_tracks()
+        for bad in (0.0, -1.0, float("nan")):
+            with pytest.raises(T.TpcError) as e:
+                trk.mark_clusters(bad)
+            assert e.value.code == -1
+
+
 def test_refit_before_find_tracks_is_a_state_error():
     import paper_1905_05515_b200 as T
     w = W.config(1, scale=0.1)
