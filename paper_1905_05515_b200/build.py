@@ -49,7 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(out)
         if p.returncode:
             raise RuntimeError(f"nvcc failed on {s}")
-    cmd = [_nvcc(), "-shared", "-cudart", "shared", "-o", SO] + [os.path.join(objdir, s[:-3] + ".o") for s in SOURCES] + \
+    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "shared", "-o", SO] + [os.path.join(objdir, s[:-3] + ".o") for s in SOURCES] + \
           ["-Xlinker", "-rpath=/usr/local/cuda/lib64"]
     subprocess.check_call(cmd)
     return SO
