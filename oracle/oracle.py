@@ -16,7 +16,7 @@ _SO = os.path.join(_HERE, "libtpc_oracle.so")
 _SRC = os.path.join(_HERE, "tpc_oracle.cpp")
 _KINDS = {0: (C.c_int32, np.int32), 1: (C.c_int64, np.int64), 2: (C.c_double, np.float64), 3: (C.c_float, np.float32)}
 
-STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6, "s7": 7, "s8": 8}
+STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6, "s7": 7, "s8": 8, "s9": 9}
 
 
 def build(force: bool = False) -> str:
@@ -141,6 +141,11 @@ class Oracle:
     def cluster_status(self):
         """S8 (NEXT-4): (status, track) per cluster in the caller's order; status 0 none / 1 attached / 2 adjacent (run("s8") first)."""
         return self.get("cl_status"), self.get("cl_track")
+
+    def merges(self):
+        """S9 (NEXT-3): next / prev segment of every track across a sector boundary (-1 none), leaver flag, outer state (run("s9") first)."""
+        return {"next": self.get("mg_next"), "prev": self.get("mg_prev"), "leaver": self.get("mg_leaver"),
+                "outer": self.get("mg_outer").reshape(-1, 4)}
 
     def tracklets(self):
         d = {k: self.get("tl_" + k) for k in ("n", "first", "last", "rowhit", "sector", "chi2", "x", "par", "cov", "zref")}

@@ -21,6 +21,8 @@
  * composition, round trip, Jacobian vs finite differences; S5 fit: noise-free helix recovery 1e-5,
  * Bz=0 exact, chi2/ndf = 1 and pulls on smeared tracks; S6 hand-built sharing cases, order invariance.
  * S4' (NEXT-2) seed bridging: hand-made single dropouts (one start hit per track), subset of the S4 list, brute-force probe.
+ * S9 (NEXT-3) cross-sector matching: rotated + transported outer state against the closed-form helix in the neighbour's frame,
+ *   generator labels of the matched pairs, structural invariants.  Looper-leg identification: not built.
  * S8 (NEXT-4) tube adjacency: independent numpy restatement with the closed-form helix, brute force over the rows, truth labels.
  * S7 (NEXT-1) refit + collision time: noise-free recovery, chi2/ndf = 1, t0 against the generator's collision times.
  * Absolute efficiency / resolution versus the paper: parity unpinned (PAPER.md:49 gives no number).
@@ -48,6 +50,8 @@ struct Tunables {            // DESIGN.md table T (all are readings; the paper i
   double bridge_wy = 1.0, bridge_wz = 1.5;
   int bridge_min = 3;           // clusters the lower chain must have
   double tube = 1.5;            // NEXT-4: radius of the tube around a track, cm
+  // NEXT-3 (reading A41): cross-sector segment matching
+  double merge_edge = 3.0; int merge_rows = 8; double merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05;
 };
 
 struct OracleBase {
@@ -91,6 +95,8 @@ struct Oracle : OracleBase {
   std::vector<int32_t> rf_n, rf_ndf; std::vector<double> rf_x, rf_par, rf_cov, rf_chi2, rf_z0, rf_t0;
   // S8 (NEXT-4): attachment status of every cluster, caller's order (CSR offset of the unit + index inside the unit)
   std::vector<int32_t> cl_status, cl_track;
+  // S9 (NEXT-3): cross-sector segment matching
+  std::vector<int32_t> mg_next, mg_prev, mg_leaver; std::vector<double> mg_outer;   // outer: x, y, z, sinphi per track
   std::vector<double> z_d, ys_d, zs_d;   // export copies
 
   Oracle(int ns, int nr, const float* rx, double dphi_, double zmax, double tframe, double sy, double sz, double bz_, double vd)
@@ -570,6 +576,68 @@ struct Oracle : OracleBase {
       }
   }
 
+  // ---- S9 (NEXT-3; "merging of track segments between sectors" in the list of later
+  //      additions; reading A41): a track that leaves its sector through the side edge continues in the neighbouring sector of
+  //      the same side as a separate S6 track.  Outer state of A = its S6 state transported (parameters only) to the row of its
+  //      last cluster.  A is a leaver iff |y_out| >= yedge - merge_edge; the neighbour is the next sector in phi for y_out > 0,
+  //      the previous one for y_out < 0.  The outer state is rotated into the neighbour's frame (x' = x c + y s, y' = -x s + y c,
+  //      sinphi' = sinphi c - cosphi s with (c, s) = (cos, sin)(+-dphi)) and transported to the x of every candidate B of that
+  //      sector with |row_in(B) - row_out(A)| <= merge_rows; B matches iff |dy| <= merge_dy, |dz| <= merge_dz, |dsinphi| <=
+  //      merge_ds, |d(dz/ds)| <= merge_dt.  score = sum of the squared normalised differences; A proposes its best B (score, then
+  //      index), B accepts its best proposer: next[A] = B, prev[B] = A (-1 elsewhere).
+  void s9_merge() {
+    const int64_t NT = (int64_t)trk_sector.size();
+    mg_next.assign(NT, -1); mg_prev.assign(NT, -1); mg_leaver.assign(NT, 0); mg_outer.assign(NT * 4, 0);
+    std::vector<int> r_in(NT), r_out(NT); std::vector<State> outer(NT);
+    for (int64_t i = 0; i < NT; i++) {
+      const int32_t T_ = trk_tracklet[i];
+      r_in[i] = tl_first[T_]; r_out[i] = trk_cl_row[trk_cl_begin[i + 1] - 1];
+      State st; for (int a = 0; a < 5; a++) for (int b = 0; b < 5; b++) st.C[a][b] = 0;
+      for (int k = 0; k < 5; k++) st.p[k] = (Real)trk_par[i * 5 + k];
+      bool ok = std::isfinite(st.p[4]);
+      for (int r = r_in[i] + 1; ok && r <= r_out[i]; r++) ok = propagate_state(st, X[r] - X[r - 1]);
+      outer[i] = st;
+      if (!ok) continue;
+      mg_outer[i * 4 + 0] = (double)X[r_out[i]]; mg_outer[i * 4 + 1] = (double)st.p[0]; mg_outer[i * 4 + 2] = (double)st.p[1]; mg_outer[i * 4 + 3] = (double)st.p[2];
+      if (NS < 36) continue;
+      const Real ya = std::fabs(st.p[0]);
+      if (ya >= yedge[r_out[i]] - (Real)T.merge_edge) mg_leaver[i] = st.p[0] > 0 ? 1 : -1;
+    }
+    const Real cd = (Real)std::cos(dphi), sd = (Real)std::sin(dphi);
+    const Real my = (Real)T.merge_dy, mz = (Real)T.merge_dz, ms = (Real)T.merge_ds, mt = (Real)T.merge_dt;
+    std::vector<int32_t> bestB(NT, -1); std::vector<Real> bestS(NT, (Real)0);
+    for (int64_t a = 0; a < NT; a++) {
+      if (!mg_leaver[a]) continue;
+      const int sec = trk_sector[a], side = sec / 18, k = sec % 18;
+      const int nb = side * 18 + (k + (mg_leaver[a] > 0 ? 1 : 17)) % 18;
+      const Real sgn = mg_leaver[a] > 0 ? (Real)1 : (Real)-1;
+      const State& o = outer[a];
+      const Real x = X[r_out[a]], y = o.p[0], s = o.p[2], c = std::sqrt((Real)1 - s * s);
+      const Real ss = sgn * sd;                          // sin of the signed rotation angle
+      State rot = o;
+      const Real xr = x * cd + y * ss;
+      rot.p[0] = y * cd - x * ss;
+      rot.p[2] = s * cd - c * ss;
+      for (int64_t b = 0; b < NT; b++) {
+        if (trk_sector[b] != nb) continue;
+        int dr = r_in[b] - r_out[a]; if (dr < 0) dr = -dr;
+        if (dr > T.merge_rows) continue;
+        State st = rot;
+        if (!propagate_state(st, X[r_in[b]] - xr)) continue;
+        const Real dy = (Real)trk_par[b * 5 + 0] - st.p[0], dz = (Real)trk_par[b * 5 + 1] - st.p[1];
+        const Real ds = (Real)trk_par[b * 5 + 2] - st.p[2], dt = (Real)trk_par[b * 5 + 3] - st.p[3];
+        if (!(std::fabs(dy) <= my && std::fabs(dz) <= mz && std::fabs(ds) <= ms && std::fabs(dt) <= mt)) continue;
+        const Real ey = dy / my, ez = dz / mz, es = ds / ms, et = dt / mt;
+        const Real score = ((ey * ey + ez * ez) + es * es) + et * et;
+        if (bestB[a] < 0 || score < bestS[a]) { bestB[a] = (int32_t)b; bestS[a] = score; }
+      }
+    }
+    std::vector<int32_t> bestA(NT, -1); std::vector<Real> bestAS(NT, (Real)0);
+    for (int64_t a = 0; a < NT; a++) { const int32_t b = bestB[a]; if (b < 0) continue;
+      if (bestA[b] < 0 || bestS[a] < bestAS[b]) { bestA[b] = (int32_t)a; bestAS[b] = bestS[a]; } }
+    for (int64_t b = 0; b < NT; b++) if (bestA[b] >= 0) { mg_next[bestA[b]] = (int32_t)b; mg_prev[b] = bestA[b]; }
+  }
+
   int run(int upto, int brute) override {
     make_tables();
     s0_time_to_z(); if (upto <= 0) return 0;
@@ -580,7 +648,8 @@ struct Oracle : OracleBase {
     s5_tracklets((brute & 2) != 0); if (upto <= 5) return 0;
     s6_select(); if (upto <= 6) return 0;
     s7_refit(); if (upto <= 7) return 0;
-    s8_adjacent((brute & 2) != 0);
+    s8_adjacent((brute & 2) != 0); if (upto <= 8) return 0;
+    s9_merge();
     return 0;
   }
 
@@ -647,6 +716,10 @@ struct Oracle : OracleBase {
     if (s == "trk_par") RET(trk_par, 2)
     if (s == "trk_cov") RET(trk_cov, 2)
     if (s == "trk_chi2") RET(trk_chi2, 2)
+    if (s == "mg_next") RET(mg_next, 0)
+    if (s == "mg_prev") RET(mg_prev, 0)
+    if (s == "mg_leaver") RET(mg_leaver, 0)
+    if (s == "mg_outer") RET(mg_outer, 2)
     if (s == "cl_status") RET(cl_status, 0)
     if (s == "cl_track") RET(cl_track, 0)
     if (s == "rf_n") RET(rf_n, 0)
@@ -681,6 +754,8 @@ int orc_set_param(void* h, const char* name, double v) {
   else if (s == "c0_dzds") T.c0[3] = v; else if (s == "c0_qpt") T.c0[4] = v;
   else if (s == "grid_scale") T.grid_scale = v;
   else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "tube") T.tube = v;
+  else if (s == "merge_edge") T.merge_edge = v; else if (s == "merge_rows") T.merge_rows = (int)v; else if (s == "merge_dy") T.merge_dy = v;
+  else if (s == "merge_dz") T.merge_dz = v; else if (s == "merge_ds") T.merge_ds = v; else if (s == "merge_dt") T.merge_dt = v;
   else return -1;
   return 0;
 }
