@@ -184,6 +184,10 @@ def run_gpu(args, rank, world, local_rank):
     mst = mk[-1]["status"]
     marks = {"ms": mark_ms, "clusters_per_s": N / (mark_ms * 1e-3), "tube_cm": 1.5, "attached_frac": float((mst == 1).sum().item()) / N,
              "adjacent_frac": float((mst == 2).sum().item()) / N, "note": "S8 cluster attachment status (SURVEY 8(f).4), outside the timed step"}
+    # S9 (NEXT-3, not part of the timed step): cross-sector segment matching
+    mg = [trk.merge_tracks(device_result=True) for _ in range(3)]
+    merges = {"ms": float(np.mean([m["ms_merge"] for m in mg[1:]])), "matched_pairs": int((mg[-1]["next"] >= 0).sum().item()),
+              "note": "S9 cross-sector segment matching (SURVEY 8(f).3), outside the timed step"}
     # NEXT-2 variant (seed bridging, reading A39), measured beside the default path, never mixed into `value`
     variant = None
     if args.variant and rank == 0:
@@ -304,7 +308,7 @@ def run_gpu(args, rank, world, local_rank):
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
-           "variant_seed_bridging": variant, "cluster_marks": marks,
+           "variant_seed_bridging": variant, "cluster_marks": marks, "sector_merges": merges,
            "refit": {"ms": refit_ms, "tracks_per_s": n_tracks / (refit_ms * 1e-3), "note": "S7 refit + collision time (SURVEY 8(f).1), outside the timed step"},
            "clocks": clocks}
     print(json.dumps(out))

@@ -96,6 +96,16 @@ typedef struct {
   float ms_mark;            /* device time of K8 (CUDA events on the context's stream), ms */
 } tpc_cluster_marks;
 
+/* Result of tpc_merge_tracks: S9 of DESIGN.md section 4 ("merging of track segments between
+ * sectors"; reading A41): for every track of the last tpc_find_tracks* call the track that continues it in the neighbouring sector and
+ * the track it continues.  Library-owned, host (device_result = 0) or device memory, valid until the next call on the context. */
+typedef struct {
+  int64_t n_tracks;
+  const int32_t* next;      /* [n_tracks] index of the continuing segment in the neighbouring sector, -1 = none */
+  const int32_t* prev;      /* [n_tracks] index of the segment this track continues, -1 = none */
+  float ms_merge;           /* device time of K9 (CUDA events on the context's stream), ms */
+} tpc_merges;
+
 /* Per-step device times of the last tpc_find_tracks* call (CUDA events on the context's stream), ms. */
 typedef struct {
   float ms_upload;          /* host staging -> device (0 if the clusters were already device-resident) */
@@ -164,6 +174,10 @@ int tpc_refit_tracks(tpc_ctx*, int device_result, tpc_refit* out);
 /* S8: attachment status of every cluster with respect to the tracks of the last tpc_find_tracks* call; tube_cm > 0 (the paper: 1.5).
  * Errors: TPC_E_ARG (null, tube_cm not > 0 or not finite), TPC_E_STATE (no completed tpc_find_tracks* call), TPC_E_NOMEM, TPC_E_CUDA. */
 int tpc_mark_clusters(tpc_ctx*, float tube_cm, int device_result, tpc_cluster_marks* out);
+
+/* S9: match track segments across sector boundaries (tunables merge_edge, merge_rows, merge_dy, merge_dz, merge_ds, merge_dt).
+ * Errors: TPC_E_ARG (null), TPC_E_STATE (no completed tpc_find_tracks* call), TPC_E_NOMEM, TPC_E_CUDA. */
+int tpc_merge_tracks(tpc_ctx*, int device_result, tpc_merges* out);
 
 /* Forget the clusters and results, keep geometry, parameters and buffers (one call per event / time frame). */
 int tpc_clear(tpc_ctx*);

@@ -17,7 +17,7 @@ _SO = os.path.join(_HERE, "libtpc_b200.so")
 
 ABI_SYMBOLS = [
     "tpc_abi_version", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
-    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
+    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
     "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
 
@@ -48,6 +48,10 @@ class _Refit(C.Structure):
 
 class _Marks(C.Structure):
     _fields_ = [("n_clusters", C.c_int64), ("status", C.c_void_p), ("track", C.c_void_p), ("ms_mark", C.c_float)]
+
+
+class _Merges(C.Structure):
+    _fields_ = [("n_tracks", C.c_int64), ("next", C.c_void_p), ("prev", C.c_void_p), ("ms_merge", C.c_float)]
 
 
 class _Timings(C.Structure):
@@ -97,6 +101,7 @@ def load_library():
     lib.tpc_find_tracks_device.argtypes = [vp, C.POINTER(_Tracks)]
     lib.tpc_refit_tracks.argtypes = [vp, C.c_int, C.POINTER(_Refit)]
     lib.tpc_mark_clusters.argtypes = [vp, C.c_float, C.c_int, C.POINTER(_Marks)]
+    lib.tpc_merge_tracks.argtypes = [vp, C.c_int, C.POINTER(_Merges)]
     lib.tpc_clear.argtypes = [vp]
     lib.tpc_destroy.argtypes = [vp]
     lib.tpc_destroy.restype = None
@@ -285,6 +290,15 @@ def tpc_mark_clusters(h, tube_cm=1.5, device_result=False) -> dict:
     return {"n_clusters": n, "ms_mark": float(t.ms_mark), "status": make(t.status, n, np.int32), "track": make(t.track, n, np.int32)}
 
 
+def tpc_merge_tracks(h, device_result=False) -> dict:
+    """S9: next / prev segment of every track across a sector boundary, -1 = none (zero-copy views)."""
+    t = _Merges()
+    _check(h, load_library().tpc_merge_tracks(h, 1 if device_result else 0, C.byref(t)))
+    make = _dev_tensor if device_result else _host_array
+    n = int(t.n_tracks)
+    return {"n_tracks": n, "ms_merge": float(t.ms_merge), "next": make(t.next, n, np.int32), "prev": make(t.prev, n, np.int32)}
+
+
 class Tracker:
     """Context manager around one tpc_ctx, for the tests and bench.py."""
 
@@ -345,6 +359,9 @@ class Tracker:
 
     def mark_clusters(self, tube_cm=1.5, device_result=False) -> dict:
         return tpc_mark_clusters(self.h, tube_cm, device_result)
+
+    def merge_tracks(self, device_result=False) -> dict:
+        return tpc_merge_tracks(self.h, device_result)
 
     def clear(self):
         self._keep = []

@@ -1,0 +1,126 @@
+// k9_merge.cu -- K9: S9 cross-sector segment matching (NEXT-3 of SURVEY.md section 8(f); "merging of track segments
+// between sectors" in the list of additions; reading A41 of DESIGN.md).  Looper-leg identification is not part of it.
+//
+//   k9_ranges  : first track of every sector (the S6 tracks are in ascending sector order) by binary search
+//   k9_outer   : one lane per track: S6 state transported (parameters only) to the row of the track's last cluster; a track
+//                whose outer end lies within merge_edge of the side edge of its sector is a leaver towards the next / previous
+//                sector in phi
+//   k9_propose : one lane per leaver A: outer state rotated into the neighbour's frame, transported to the first row of every
+//                track B of that sector that starts within merge_rows rows of A's end, compared inside the four windows; the
+//                best B (score, then index) receives atomicMin of (score bits, A)
+//   k9_accept  : one thread per track B: its best proposer A -> next[A] = B, prev[B] = A
+// fp32, every operation spelled in the order of the definition (reading A41; library built with -fmad=false).
+#include "kalman.cuh"
+
+namespace tpc {
+namespace {
+
+constexpr int K9_THREADS = 128;
+constexpr unsigned long long K9_NONE = ~0ull;
+
+__global__ void k9_ranges(const long long n_tracks, const int NS, const int* __restrict__ o_sector, int* __restrict__ sec_begin) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s > NS) return;
+  long long lo = 0, hi = n_tracks;   // first track with sector >= s
+  while (lo < hi) { const long long mid = (lo + hi) >> 1; if (o_sector[mid] < s) lo = mid + 1; else hi = mid; }
+  sec_begin[s] = (int)lo;
+}
+
+__global__ void __launch_bounds__(K9_THREADS) k9_outer(const long long n_tracks, const int* __restrict__ o_tracklet,
+                                                       const float* __restrict__ o_par, const long long* __restrict__ cl_begin,
+                                                       const int* __restrict__ cl_row, const int* __restrict__ tl_first,
+                                                       const RowConst* __restrict__ rows, float* __restrict__ outer,
+                                                       int* __restrict__ row_in, int* __restrict__ row_out, int* __restrict__ leaver,
+                                                       const K9Params M, const Params P) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_tracks) return;
+  const float* __restrict__ ip = o_par + i * 5;
+  State st = {};
+  st.y = ip[0]; st.z = ip[1]; st.s = ip[2]; st.t = ip[3]; st.q = ip[4];
+  const int r0 = tl_first[o_tracklet[i]], r1 = cl_row[cl_begin[i + 1] - 1];
+  bool ok = isfinite(st.q);
+  for (int r = r0 + 1; ok && r <= r1; r++) ok = propagate(st, rows[r].x - rows[r - 1].x, P);
+  row_in[i] = r0; row_out[i] = r1;
+  float* __restrict__ o = outer + i * 4;
+  int lv = 0;
+  if (ok) {
+    o[0] = rows[r1].x; o[1] = st.y; o[2] = st.z; o[3] = st.s;
+    if (P.NS >= 36 && fabsf(st.y) >= rows[r1].yedge - M.edge) lv = st.y > 0.0f ? 1 : -1;
+  } else {
+    o[0] = o[1] = o[2] = o[3] = 0.0f;
+  }
+  leaver[i] = lv;
+}
+
+__global__ void __launch_bounds__(K9_THREADS) k9_propose(const long long n_tracks, const int* __restrict__ o_sector,
+                                                         const float* __restrict__ o_par, const RowConst* __restrict__ rows,
+                                                         const float* __restrict__ outer, const int* __restrict__ row_in,
+                                                         const int* __restrict__ row_out, const int* __restrict__ leaver,
+                                                         const int* __restrict__ sec_begin, unsigned long long* __restrict__ cand,
+                                                         const K9Params M, const Params P) {
+  const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= n_tracks) return;
+  const int lv = leaver[a];
+  if (!lv) return;
+  const int sec = o_sector[a], side = sec / 18, k = sec % 18;
+  const int nb = side * 18 + (k + (lv > 0 ? 1 : 17)) % 18;
+  const float sgn = lv > 0 ? 1.0f : -1.0f;
+  const float* __restrict__ o = outer + a * 4;
+  const float x = o[0], y = o[1], s = o[3], c = sqrtf(1.0f - s * s);
+  const float ss = sgn * M.sd;
+  State rot = {};
+  const float xr = x * M.cd + y * ss;
+  rot.y = y * M.cd - x * ss; rot.z = o[2]; rot.s = s * M.cd - c * ss; rot.t = o_par[a * 5 + 3]; rot.q = o_par[a * 5 + 4];
+  const int ra = row_out[a];
+  int best = -1; float bests = 0.0f;
+  const int b1 = sec_begin[nb + 1];
+  for (int b = sec_begin[nb]; b < b1; b++) {
+    const int rb = row_in[b];
+    int dr = rb - ra; if (dr < 0) dr = -dr;
+    if (dr > M.rows) continue;
+    State st = rot;
+    if (!propagate(st, rows[rb].x - xr, P)) continue;
+    const float* __restrict__ pb = o_par + (long long)b * 5;
+    const float dy = pb[0] - st.y, dz = pb[1] - st.z, ds = pb[2] - st.s, dt = pb[3] - st.t;
+    if (!(fabsf(dy) <= M.dy && fabsf(dz) <= M.dz && fabsf(ds) <= M.ds && fabsf(dt) <= M.dt)) continue;
+    const float ey = dy / M.dy, ez = dz / M.dz, es = ds / M.ds, et = dt / M.dt;
+    const float score = ((ey * ey + ez * ez) + es * es) + et * et;
+    if (best < 0 || score < bests) { best = b; bests = score; }
+  }
+  if (best >= 0) atomicMin(&cand[best], ((unsigned long long)__float_as_uint(bests) << 32) | (unsigned long long)(unsigned)a);
+}
+
+__global__ void __launch_bounds__(256) k9_accept(const long long n_tracks, const unsigned long long* __restrict__ cand,
+                                                 int* __restrict__ next, int* __restrict__ prev) {
+  const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= n_tracks) return;
+  const unsigned long long kk = cand[b];
+  if (kk == K9_NONE) return;
+  const int a = (int)(unsigned)(kk & 0xffffffffull);
+  next[a] = (int)b;      // every A proposes to one B only: no two B write the same next[A]
+  prev[b] = a;
+}
+
+}  // namespace
+
+int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_sector, const int* o_tracklet, const float* o_par,
+                    const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first, const RowConst* d_rows, float* d_outer,
+                    int* d_row_in, int* d_row_out, int* d_leaver, int* d_sec_begin, unsigned long long* d_cand, int* d_next,
+                    int* d_prev, const K9Params& M, const Params& P) {
+  if (n_tracks <= 0) return 0;
+  cudaError_t e = cudaMemsetAsync(d_cand, 0xff, (size_t)n_tracks * sizeof(unsigned long long), L.stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_next, 0xff, (size_t)n_tracks * sizeof(int), L.stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_prev, 0xff, (size_t)n_tracks * sizeof(int), L.stream);
+  if (e != cudaSuccess) return -(int)e;
+  const int blocks = (int)((n_tracks + K9_THREADS - 1) / K9_THREADS);
+  k9_ranges<<<(NS + 1 + 63) / 64, 64, 0, L.stream>>>(n_tracks, NS, o_sector, d_sec_begin);
+  k9_outer<<<blocks, K9_THREADS, 0, L.stream>>>(n_tracks, o_tracklet, o_par, o_cl_begin, o_cl_row, d_tl_first, d_rows, d_outer, d_row_in,
+                                               d_row_out, d_leaver, M, P);
+  k9_propose<<<blocks, K9_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_par, d_rows, d_outer, d_row_in, d_row_out, d_leaver, d_sec_begin,
+                                                 d_cand, M, P);
+  k9_accept<<<(int)((n_tracks + 255) / 256), 256, 0, L.stream>>>(n_tracks, d_cand, d_next, d_prev);
+  e = cudaGetLastError();
+  return e == cudaSuccess ? 4 : -(int)e;
+}
+
+}  // namespace tpc

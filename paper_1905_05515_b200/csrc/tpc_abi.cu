@@ -89,6 +89,7 @@ struct Tunables {   // DESIGN.md table T
   int k2_threads = 0;         // K2 block size (0 = default 256); tuning knob
   int bridge_rows = 0, bridge_min = 3;       // NEXT-2 seed bridging (reading A39): 0 = off
   double bridge_wy = 1.0, bridge_wz = 1.5;
+  double merge_edge = 3.0, merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05; int merge_rows = 8;   // NEXT-3 (reading A41)
 };
 
 struct UnitSrc { long long src = 0; int n = 0; };
@@ -136,6 +137,8 @@ struct tpc_ctx {
   // outputs / debug copies (host)
   PinVec<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; PinVec<float> ho_x, ho_par, ho_cov, ho_chi2;
   PinVec<int64_t> ho_cl_begin;
+  // S9 merges (device + host)
+  DevBuf g_outer, g_row_in, g_row_out, g_leaver, g_sec_begin, g_cand, g_next, g_prev; PinVec<int32_t> hg_next, hg_prev;
   // S8 cluster marks (device + host)
   DevBuf m_att, m_adj, m_status, m_track; PinVec<int32_t> hm_status, hm_track;
   // S7 refit (device + host)
@@ -234,13 +237,14 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
                     &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
-                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->m_att, &c->m_adj, &c->m_status, &c->m_track};
+                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->m_att, &c->m_adj, &c->m_status, &c->m_track,
+                    &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_cand, &c->g_next, &c->g_prev};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
   c->ho_sector.release(); c->ho_ndf.release(); c->ho_tracklet.release(); c->ho_cl_row.release(); c->ho_cl_index.release();
   c->ho_x.release(); c->ho_par.release(); c->ho_cov.release(); c->ho_chi2.release(); c->ho_cl_begin.release();
   c->hr_n.release(); c->hr_ndf.release(); c->hr_x.release(); c->hr_par.release(); c->hr_cov.release(); c->hr_chi2.release();
-  c->hr_z0.release(); c->hr_t0.release(); c->hm_status.release(); c->hm_track.release();
+  c->hr_z0.release(); c->hr_t0.release(); c->hm_status.release(); c->hm_track.release(); c->hg_next.release(); c->hg_prev.release();
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
   delete c;
 }
@@ -276,6 +280,9 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "bridge_rows") { if (v < 0 || v > 16) return fail(c, TPC_E_ARG, "bridge_rows must be in 0..16"); T.bridge_rows = (int)v; }
   else if (s == "bridge_min") { if (v < 3 || v > 255) return fail(c, TPC_E_ARG, "bridge_min must be in 3..255"); T.bridge_min = (int)v; }
   else if (s == "bridge_wy") rc = pos(T.bridge_wy); else if (s == "bridge_wz") rc = pos(T.bridge_wz);
+  else if (s == "merge_edge") rc = nonneg(T.merge_edge); else if (s == "merge_dy") rc = pos(T.merge_dy); else if (s == "merge_dz") rc = pos(T.merge_dz);
+  else if (s == "merge_ds") rc = pos(T.merge_ds); else if (s == "merge_dt") rc = pos(T.merge_dt);
+  else if (s == "merge_rows") { if (v < 0 || v > 255) return fail(c, TPC_E_ARG, "merge_rows must be in 0..255"); T.merge_rows = (int)v; }
   else return fail(c, TPC_E_ARG, "tpc_set_param: unknown parameter '%s'", name);
   if (rc == TPC_OK) c->rows_valid = false;
   return rc;
@@ -691,6 +698,42 @@ int tpc_mark_clusters(tpc_ctx* c, float tube_cm, int device_result, tpc_cluster_
   }
   CUDA_TRY(c, cudaStreamSynchronize(st));
   CUDA_TRY(c, cudaEventElapsedTime(&out->ms_mark, c->ev[8], c->ev[9]));
+  return TPC_OK;
+}
+// S9 (NEXT-3): K9 over the tracks of the last call.
+int tpc_merge_tracks(tpc_ctx* c, int device_result, tpc_merges* out) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_merge_tracks: null argument");
+  memset(out, 0, sizeof(*out));
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_merge_tracks: call tpc_find_tracks first");
+  cudaStream_t st = c->stream;
+  Launch L{st, c->sm_count, c->T.k2_threads};
+  const long long nt = c->n_tracks; const size_t ntz = (size_t)std::max(nt, 1LL);
+  CUDA_TRY(c, c->g_outer.ensure(ntz * 16)); CUDA_TRY(c, c->g_row_in.ensure(ntz * 4)); CUDA_TRY(c, c->g_row_out.ensure(ntz * 4));
+  CUDA_TRY(c, c->g_leaver.ensure(ntz * 4)); CUDA_TRY(c, c->g_sec_begin.ensure((size_t)(c->NS + 2) * 4)); CUDA_TRY(c, c->g_cand.ensure(ntz * 8));
+  CUDA_TRY(c, c->g_next.ensure(ntz * 4)); CUDA_TRY(c, c->g_prev.ensure(ntz * 4));
+  const Tunables& T = c->T;
+  K9Params M{(float)T.merge_edge, (float)T.merge_dy, (float)T.merge_dz, (float)T.merge_ds, (float)T.merge_dt,
+             (float)cos((double)c->dphi), (float)sin((double)c->dphi), T.merge_rows};
+  long long launches = 0;
+  CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
+  LAUNCH_TRY(c, launch_k9_merge(L, nt, c->NS, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_par.as<float>(), c->o_cl_begin.as<long long>(),
+                                c->o_cl_row.as<int>(), c->d_tl_first.as<int>(), c->d_rows.as<RowConst>(), c->g_outer.as<float>(),
+                                c->g_row_in.as<int>(), c->g_row_out.as<int>(), c->g_leaver.as<int>(), c->g_sec_begin.as<int>(),
+                                (unsigned long long*)c->g_cand.p, c->g_next.as<int>(), c->g_prev.as<int>(), M, c->P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
+  out->n_tracks = nt;
+  if (!device_result) {
+    CUDA_TRY(c, c->hg_next.resize(ntz)); CUDA_TRY(c, c->hg_prev.resize(ntz));
+    if (nt > 0) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->hg_next.data(), c->g_next.p, (size_t)nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hg_prev.data(), c->g_prev.p, (size_t)nt * 4, cudaMemcpyDeviceToHost, st));
+    }
+    out->next = c->hg_next.data(); out->prev = c->hg_prev.data();
+  } else {
+    out->next = c->g_next.as<int32_t>(); out->prev = c->g_prev.as<int32_t>();
+  }
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  CUDA_TRY(c, cudaEventElapsedTime(&out->ms_merge, c->ev[8], c->ev[9]));
   return TPC_OK;
 }
 int tpc_get_timings(tpc_ctx* c, tpc_timings* out) {

@@ -43,6 +43,9 @@ struct Params {
   float bridge_wy, bridge_wz;
 };
 
+// S9 (NEXT-3) matching parameters (reading A41), rounded to float once on the host
+struct K9Params { float edge, dy, dz, ds, dt, cd, sd; int rows; };
+
 // Work item of K2/K3: a chunk of consecutive sorted hits of one unit.
 struct Item { int unit; int start; };
 
@@ -131,6 +134,11 @@ int launch_k8_status(const Launch& L, long long n_tracks, long long N, int U, co
                      const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
                      const int* d_rowhit, int* d_att, unsigned long long* d_adj, int* cl_status, int* cl_track, float tube,
                      const Params& P);
+
+int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_sector, const int* o_tracklet, const float* o_par,
+                    const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first, const RowConst* d_rows, float* d_outer,
+                    int* d_row_in, int* d_row_out, int* d_leaver, int* d_sec_begin, unsigned long long* d_cand, int* d_next,
+                    int* d_prev, const K9Params& M, const Params& P);
 
 // device-wide exclusive scans (own kernels; three launches each)
 int launch_scan_i32(const Launch& L, const int* d_in, int* d_out, int n, int* d_tmp, int* d_total);

@@ -152,12 +152,42 @@ def test_cluster_marks_argument_and_state_errors():
             assert e.value.code == -1
 
 
+def test_cross_sector_merges_parity_c2_and_c3_scaled():
+    """S9 (NEXT-3): next / prev arrays identical to the oracle's when the track lists are identical; matched pairs carry one label."""
+    for w in (W.config(2), W.config(3, scale=0.1)):
+        o = P.make_oracle(w).run("s9")
+        otr, om = o.tracks(), o.merges()
+        with _tracker(w) as trk:
+            trk.load_workload(w)
+            gtr = trk.find_tracks().copy().as_dict()
+            m = trk.merge_tracks()
+            nx, pv = np.array(m["next"]), np.array(m["prev"])
+            dev = trk.merge_tracks(device_result=True)
+            assert np.array_equal(dev["next"].cpu().numpy(), nx) and np.array_equal(dev["prev"].cpu().numpy(), pv)
+            assert m["ms_merge"] > 0 and m["n_tracks"] == len(gtr["sector"])
+        assert np.array_equal(otr["cl_begin"], gtr["cl_begin"]) and np.array_equal(otr["cl_index"], gtr["cl_index"])
+        n_m = int((om["next"] >= 0).sum())
+        assert n_m > 500
+        diff = int((nx != om["next"]).sum() + (pv != om["prev"]).sum())
+        assert diff <= 2e-3 * n_m, (diff, n_m)          # a window edge decided in the last fp32 bit of a transported state
+        labs = H.track_labels(w, gtr)
+        pairs = [(a, int(b)) for a, b in enumerate(nx) if b >= 0]
+        assert sum(1 for a, b in pairs if labs[a][0] != labs[b][0]) <= 0.005 * len(pairs)
+    w1 = W.config(1)                                      # one sector: nothing to merge
+    with _tracker(w1) as trk:
+        trk.load_workload(w1); trk.find_tracks()
+        assert np.all(np.array(trk.merge_tracks()["next"]) == -1)
+
+
 def test_refit_before_find_tracks_is_a_state_error():
     import paper_1905_05515_b200 as T
     w = W.config(1, scale=0.1)
     with _tracker(w) as trk:
         with pytest.raises(T.TpcError) as e:
             trk.refit_tracks()
+        assert e.value.code == -2
+        with pytest.raises(T.TpcError) as e:
+            trk.merge_tracks()
         assert e.value.code == -2
 
 
