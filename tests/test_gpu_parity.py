@@ -219,6 +219,18 @@ def test_large_units_take_the_partly_shared_k1_path():
     assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
 
 
+def test_next_rows_on_an_empty_result():
+    """S7 / S8 / S9 on a frame without tracks: empty arrays, status 0 everywhere."""
+    w = W.config(1, scale=0.05)
+    with _tracker(w) as trk:
+        y = np.array([1.0, 2.0, -3.0], np.float32); t = np.array([10.0, 20.0, 30.0], np.float32)
+        trk.load(0, 5, y, t)
+        assert trk.find_tracks().n_tracks == 0
+        assert trk.refit_tracks()["n_tracks"] == 0 and trk.merge_tracks()["n_tracks"] == 0
+        m = trk.mark_clusters()
+        assert m["n_clusters"] == 3 and np.all(m["status"] == 0) and np.all(m["track"] == -1)
+
+
 def test_empty_and_tiny_inputs():
     w = W.config(1, scale=0.05)
     with _tracker(w) as trk:
@@ -338,6 +350,11 @@ def test_abi_state_and_argument_errors_on_device():
         with pytest.raises(T.TpcError) as e:
             trk.set_param("no_such_parameter", 1.0)
         assert e.value.code == -1
+        for name, bad in (("bridge_rows", 17), ("bridge_rows", -1), ("bridge_min", 2), ("bridge_wy", 0.0), ("merge_rows", 256),
+                          ("merge_dy", -1.0), ("merge_ds", float("inf"))):
+            with pytest.raises(T.TpcError) as e:
+                trk.set_param(name, bad)
+            assert e.value.code == -1, name
         trk.load_workload(w)
         with pytest.raises(T.TpcError) as e:
             trk.set_param("wy", 2.0)                         # tunables are frozen after the first load
@@ -347,6 +364,10 @@ def test_abi_state_and_argument_errors_on_device():
             trk.links(0, 5, cleaned=False)                   # raw links need debug_keep
         assert e.value.code == -2
         trk.clear()
+        for call in (trk.refit_tracks, trk.mark_clusters, trk.merge_tracks):   # results are gone after tpc_clear
+            with pytest.raises(T.TpcError) as e:
+                call()
+            assert e.value.code == -2
         trk.set_param("wy", 1.5)                             # allowed again after tpc_clear
         # a second load of the same (sector,row) replaces the first
         y = w.y[w.unit_off[7]:w.unit_off[8]]; t = w.t[w.unit_off[7]:w.unit_off[8]]
