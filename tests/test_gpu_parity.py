@@ -297,6 +297,38 @@ def test_c5_scaled_large_frame_invariants():
         assert mg["eff_primary"] > 0.95 and mg["fake_rate"] < 0.02
 
 
+def test_c5_full_size_sampled_sector_parity():
+    """BASELINE.json configs[4] at full size (10 ms frame, ~84 M clusters, 15 k clusters per unit: the largest K1 plan, the longest
+    z range).  Sectors are independent, so the oracle run on ONE sector alone is the oracle's answer for that sector of the
+    whole frame: grid tables, link tables, start list and tracks of sector 11 compared as in the full parity tests."""
+    w = W.config(5)
+    assert w.n_clusters > 70e6
+    sec = 11
+    ws = w.sector_slice([sec])
+    o = P.make_oracle(ws).run("s6")
+    otr = o.tracks()
+    R = w.n_rows
+    with _tracker(w, debug_keep=1) as trk:
+        trk.load_workload(w)
+        r = trk.find_tracks()
+        sel = np.nonzero(r.sector == sec)[0]
+        assert len(sel) > 10000 and np.all(np.diff(sel) == 1)
+        a, b = int(sel[0]), int(sel[-1]) + 1
+        cb = r.cl_begin[a:b + 1]
+        gtr = dict(sector=r.sector[a:b].copy(), x=r.x[a:b].copy(), par=r.par[a:b].copy(), cov=r.cov[a:b].copy(), chi2=r.chi2[a:b].copy(),
+                   ndf=r.ndf[a:b].copy(), cl_begin=(cb - cb[0]).copy(), cl_row=r.cl_row[cb[0]:cb[-1]].copy(),
+                   cl_index=r.cl_index[cb[0]:cb[-1]].copy())
+        units = range(sec * R, (sec + 1) * R, 9)
+        assert P.compare_grid(ws, o, trk, units) > 10
+        for u in units:
+            lo, hi = int(ws.unit_off[u]), int(ws.unit_off[u + 1])
+            for cleaned, (nu, nd) in ((False, ("link_up", "link_dn")), (True, ("clean_up", "clean_dn"))):
+                up, dn = trk.links(u // R, u % R, cleaned)
+                assert np.array_equal(up, o.get(nu)[lo:hi]) and np.array_equal(dn, o.get(nd)[lo:hi]), (u, cleaned)
+    res = P.compare_tracks(otr, gtr)
+    assert res["n_oracle"] > 10000 and res["frac_identical"] >= 0.999 and res["param_mismatch"] <= 0.001 * res["n_oracle"], res
+
+
 def _inject(w, unit, y_extra, t_extra):
     """Copy of workload w with extra clusters appended to one (sector,row) unit (labels -1)."""
     import copy
