@@ -171,15 +171,19 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
                                                             const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
                                                             const float2* __restrict__ yz, const int* __restrict__ perm,
                                                             const int* __restrict__ bin_start, int* __restrict__ link_up,
-                                                            int* __restrict__ link_dn, const Params P, const int stage_bytes) {
+                                                            int* __restrict__ link_dn, const Params P, const int stage_bytes, const int split) {
   extern __shared__ __align__(128) unsigned char s_stage[];
   __shared__ __align__(8) uint64_t s_bar;
   __shared__ Stage s_st;
 
-  const Item it = items[blockIdx.x];
+  // a K2 CTA covers 1/split of a work item (the items are shared with K3, which wants larger chunks): smaller slabs, more CTAs
+  // per SM to overlap the staging latency of one with the search of the others
+  Item it = items[blockIdx.x / split];
+  it.start += (int)(blockIdx.x % split) * chunk;
   const int u = it.unit, r = u % P.R;
   const UnitDesc d = units[u];
   const int cnt = min(chunk, d.n - it.start);
+  if (cnt <= 0) return;
   int* __restrict__ lup = link_up + d.off + it.start;
   int* __restrict__ ldn = link_dn + d.off + it.start;
   const float2* __restrict__ own = yz + d.off + it.start;
@@ -253,12 +257,15 @@ int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int 
                          const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up,
                          int* d_link_dn, const Params& P) {
   if (n_items <= 0) return 0;
+  // default: half items of 512 clusters, 128 threads (8 CTAs / SM); the k2_threads knob keeps whole items
+  const int split = L.k2_threads > 0 || chunk < 512 || (chunk & 63) ? 1 : 2;
+  chunk /= split;
   const int stage_bytes = ((chunk * K2_STAGE_PER_CLUSTER + 4096) + 127) & ~127;
-  const int threads = L.k2_threads > 0 ? L.k2_threads : K2_THREADS;
+  const int threads = L.k2_threads > 0 ? L.k2_threads : (split == 2 ? 128 : K2_THREADS);
   cudaError_t e = cudaFuncSetAttribute(k2_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, stage_bytes);
   if (e != cudaSuccess) return -(int)e;
-  k2_neighbours<<<n_items, threads, stage_bytes, L.stream>>>(d_items, chunk, d_units, d_rows, d_yz, d_perm, d_bin_start, d_link_up,
-                                                           d_link_dn, P, stage_bytes);
+  k2_neighbours<<<n_items * split, threads, stage_bytes, L.stream>>>(d_items, chunk, d_units, d_rows, d_yz, d_perm, d_bin_start,
+                                                                   d_link_up, d_link_dn, P, stage_bytes, split);
   e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }
