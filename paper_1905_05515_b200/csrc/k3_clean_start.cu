@@ -49,7 +49,11 @@ __device__ bool seed_bridged(const UnitDesc* __restrict__ units, const RowConst*
   const float x_r = rows[r].x;
   const float dxu = rows[r + 2].x - x_r;
   const float sy = (c2.x - ch.x) / dxu, sz = (c2.y - ch.y) / dxu;
-  for (int g = 2; g <= P.bridge_rows && r - g >= 2; g++) {
+  // probed rows in the order 4, 2, 3, 5, 6, ...: one missing cluster leaves exactly four rows between the chains, so most bridged
+  // start hits are decided by the first probe ("some row matches" does not depend on the order)
+  for (int k = 2; k <= P.bridge_rows; k++) {
+    const int g = P.bridge_rows < 4 ? k : (k == 2 ? 4 : (k <= 4 ? k - 1 : k));
+    if (r - g < 2) continue;
     const int ud = u - g;
     const UnitDesc d = units[ud];
     if (d.n == 0) continue;
