@@ -16,6 +16,7 @@ namespace tpc {
 namespace {
 
 constexpr int K5_THREADS = 128;
+constexpr int K5_MAX_ROWS = 256;   // rows held in the shared-memory copy of the row table (the launcher checks R)
 
 // Cluster pick-up on one row: nearest cluster (dy^2+dz^2, then original index) inside the window
 // min(w_max, n_sigma*sqrt(C + sigma^2)) around the extrapolated position; -1 = none.  Returns the cluster in *hit.
@@ -96,6 +97,10 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
   int i = -1, r0 = 0, r = 0, nxt = -1, a_next = -1, a_next2 = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
   float zref = 0.0f, chi2 = 0.0f;
   State st = {};
+  // per-row x and sector half-width in shared memory (2 x 1 KB): read by every lane at every step
+  __shared__ float s_rx[K5_MAX_ROWS], s_re[K5_MAX_ROWS];
+  for (int k = threadIdx.x; k < R && k < K5_MAX_ROWS; k += blockDim.x) { s_rx[k] = rows[k].x; s_re[k] = rows[k].yedge; }
+  __syncthreads();
   __shared__ float s_snap[20][K5_THREADS];   // state after the last Phase-C update, per lane (written often, read once)
   const int tx = threadIdx.x;
   __shared__ float s_sv[7][K5_THREADS];       // state after the outermost update (5 parameters) + that cluster (y, z)
@@ -140,7 +145,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     float2 c_pref = make_float2(0.f, 0.f);
     if (hit_pref >= 0) c_pref = yz[su[rn].off + hit_pref];
     __syncwarp();
-    if (moving) { n_prop++; prop_ok = propagate(st, rows[rn].x - rows[r].x, P); }
+    if (moving) { n_prop++; prop_ok = propagate(st, s_rx[rn] - s_rx[r], P); }
 
     // ---- 2a. per-phase decision: which measurement this step uses (a linked / assigned hit, a pick-up, or none)
     bool have = false, finish = false, do_pick = false;
@@ -150,7 +155,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
       hit = start_pos[i];
       c = yz[su[r0].off + hit];
       const float2 c0 = c;          // Phase A start: direction from the origin, first update with the start hit
-      const float x = rows[r0].x, y = c0.x;
+      const float x = s_rx[r0], y = c0.x;
       const float rr = sqrtf(x * x + y * y);
       st.y = y; st.z = 0.0f; st.s = y / rr; st.t = P.continuous ? 0.0f : zref / rr; st.q = 0.0f;
       reset_cov(st, P);
@@ -159,7 +164,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
       if (!prop_ok) mode = MD_TRANS;
       else { hit = nxt; c = c_pref; have = true; }
     } else if (mode == MD_B) {      // outward extrapolation with pick-up
-      if (!prop_ok || fabsf(st.y) > rows[rn].yedge + P.edge_margin) mode = MD_TRANS;
+      if (!prop_ok || fabsf(st.y) > s_re[rn] + P.edge_margin) mode = MD_TRANS;
       else { do_pick = true; r = rn; }
     } else if (mode == MD_TRANS) {  // Phase C start: state after the outermost update, fresh covariance, refit inward
       st.y = s_sv[0][tx]; st.z = s_sv[1][tx]; st.s = s_sv[2][tx]; st.t = s_sv[3][tx]; st.q = s_sv[4][tx];
@@ -172,7 +177,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
         const int a = a_next;                   // rowhit of this row, read one step ahead (-1 below r0: never visited before)
         r = rn;
         if (a >= 0) { hit = a; c = c_pref; have = true; }
-        else if (fabsf(st.y) > rows[rn].yedge + P.edge_margin) {
+        else if (fabsf(st.y) > s_re[rn] + P.edge_margin) {
           if (rn < first_assigned) finish = true;
           else if (rn < r0) rh[rn] = -1;       // skipped row inside the tracklet's range: reads as "no cluster"
         } else do_pick = true;
@@ -261,6 +266,7 @@ int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_sta
                         float* d_tl_cov, unsigned long long* d_counters, const Params& P) {
   (void)Mpad;
   if (M <= 0) return 0;
+  if (P.R > K5_MAX_ROWS) return -(int)cudaErrorInvalidValue;   // tpc_create limits n_rows to 255 (selector key)
   int* d_queue = reinterpret_cast<int*>(d_counters + 3);   // work-queue head, zeroed with the counters by the caller
   int per_sm = 0;
   cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k5_tracklets, K5_THREADS, 0);
