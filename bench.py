@@ -95,6 +95,21 @@ def oracle_run(w, sectors):
     return time.perf_counter() - t0, ws.n_clusters, 1
 
 
+def oracle_run_parallel(w, n_threads):
+    """The same oracle, one independent instance per sector on n_threads host threads (sectors are independent; the paper's CPU
+    tracking scales linearly with cores).  Returns (seconds, clusters, threads)."""
+    import threading
+    from tests import parity as P
+    n_threads = max(1, min(n_threads, w.n_sectors))
+    orcs = [P.make_oracle(w.sector_slice([s])) for s in range(n_threads)]      # ctypes calls release the GIL
+    n = sum(int(w.unit_off[(s + 1) * w.n_rows] - w.unit_off[s * w.n_rows]) for s in range(n_threads))
+    th = [threading.Thread(target=o.run, args=("s6",)) for o in orcs]
+    t0 = time.perf_counter()
+    [t.start() for t in th]
+    [t.join() for t in th]
+    return time.perf_counter() - t0, n, n_threads
+
+
 def run_reference(args, rank, world):
     if rank != 0:
         return
@@ -297,6 +312,16 @@ def run_gpu(args, rank, world, local_rank):
         dt, n, cores = oracle_run(w, list(range(args.ref_sectors)))
         cpu = {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
                "sample": f"sectors 0..{args.ref_sectors - 1} of C{args.config} ({n} clusters), full S0..S6, fp32 oracle instance, 1 thread"}
+    cpu_par = None
+    if cpu is not None:
+        try:
+            cores = len(os.sched_getaffinity(0))
+        except AttributeError:
+            cores = os.cpu_count() or 1
+        dt, n, nth = oracle_run_parallel(w, min(36, cores))
+        cpu_par = {"value": n / dt, "unit": UNIT, "cores": nth, "kind": "oracle, one instance per sector", "seconds": dt,
+                   "sample": f"sectors 0..{nth - 1} of C{args.config} ({n} clusters), one thread each, full S0..S6",
+                   "host_cores": cores}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": f"C{args.config}: {w.params.t_frame:g} us frame, {N} clusters, {w.n_collisions} collisions per GPU",
@@ -308,7 +333,7 @@ def run_gpu(args, rank, world, local_rank):
                    "d2h_bytes_per_step": d2h, "mode": f"{NF} frames in flight ({NF} contexts, {NF} streams, one host thread each): copies overlap kernels",
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
-           "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu,
+           "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu, "cpu_baseline_parallel": cpu_par,
            "variant_seed_bridging": variant, "cluster_marks": marks, "sector_merges": merges,
            "refit": {"ms": refit_ms, "tracks_per_s": n_tracks / (refit_ms * 1e-3), "note": "S7 refit + collision time (SURVEY 8(f).1), outside the timed step"},
            "clocks": clocks}
