@@ -206,24 +206,29 @@ def run_gpu(args, rank, world, local_rank):
     # NEXT-2 variant (seed bridging, reading A39), measured beside the default path, never mixed into `value`
     variant = None
     if args.variant and rank == 0:
-        vp = dict(bridge_rows=4.0, bridge_min=8.0)
-        with T.Tracker(**w.geometry(), **vp) as tv:
-            tv.set_stream(stream.cuda_stream)
-            tv.load_batch(w.unit_off, y_d, t_d)
-            for _ in range(args.warmup):
-                rv = tv.find_tracks_device()
-            torch.cuda.synchronize()
-            e0.record(stream)
-            for _ in range(args.steps):
-                rv = tv.find_tracks_device()
-            e1.record(stream)
-            torch.cuda.synchronize()
-            vms = e0.elapsed_time(e1) / args.steps
-            vt = tv.timings()
-            variant = {"params": vp, "ms_per_step": vms, "value": N / (vms * 1e-3), "unit": UNIT, "n_start_hits": int(vt["n_start_hits"]),
-                       "tracks_per_step": int(rv.n_tracks), "cluster_refs_per_step": int(rv.n_cluster_refs),
-                       "kernel_ms": {k: vt[k] for k in keys},
-                       "note": "seed bridging (SURVEY 8(f).2): start hits that continue a lower chain are dropped; efficiency delta in DESIGN.md"}
+        variant = {}
+        for vname, vp in (("drop_bridged", dict(bridge_rows=4.0, bridge_min=8.0)),
+                          ("rescue_wave", dict(bridge_rows=4.0, bridge_min=3.0, bridge_rescue=1.0))):
+            with T.Tracker(**w.geometry(), **vp) as tv:
+                tv.set_stream(stream.cuda_stream)
+                tv.load_batch(w.unit_off, y_d, t_d)
+                for _ in range(args.warmup):
+                    rv = tv.find_tracks_device()
+                torch.cuda.synchronize()
+                e0.record(stream)
+                for _ in range(args.steps):
+                    rv = tv.find_tracks_device()
+                e1.record(stream)
+                torch.cuda.synchronize()
+                vms = e0.elapsed_time(e1) / args.steps
+                vt = tv.timings()
+                variant[vname] = {"params": vp, "ms_per_step": vms, "value": N / (vms * 1e-3), "unit": UNIT,
+                                  "n_start_hits": int(vt["n_start_hits"]), "n_tracklets_fitted": int(vt["n_tracklets_kept"]),
+                                  "tracks_per_step": int(rv.n_tracks), "cluster_refs_per_step": int(rv.n_cluster_refs),
+                                  "kernel_ms": {k: vt[k] for k in keys}}
+        variant["note"] = ("seed bridging (SURVEY 8(f).2, readings A39 / A39c): drop_bridged drops the start hits that continue a lower "
+                           "chain; rescue_wave fits them in a second K5 wave when the first left their chain unused; efficiency in "
+                           "DESIGN.md section 11")
     # S7 (NEXT-1, not part of the timed S0..S6 step): refit over the owned clusters + collision time, device-resident result
     refit_ms = float(np.mean([trk.refit_tracks(device_result=True)["ms_refit"] for _ in range(4)][1:]))
 

@@ -49,6 +49,7 @@ struct Tunables {            // DESIGN.md table T (all are readings; the paper i
   int bridge_rows = 0;          // NEXT-2 (reading A39): 0 = off; else the deepest row gap a start hit may bridge to a lower chain
   double bridge_wy = 1.0, bridge_wz = 1.5;
   int bridge_min = 3;           // clusters the lower chain must have
+  int bridge_rescue = 0;        // 1: dropped start hits get their tracklet after all when the first wave left their chain unused
   double tube = 1.5;            // NEXT-4: radius of the tube around a track, cm
   // NEXT-3 (reading A41): cross-sector segment matching
   double merge_edge = 3.0; int merge_rows = 8; double merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05;
@@ -95,6 +96,7 @@ struct Oracle : OracleBase {
   std::vector<int32_t> rf_n, rf_ndf; std::vector<double> rf_x, rf_par, rf_cov, rf_chi2, rf_z0, rf_t0;
   // S8 (NEXT-4): attachment status of every cluster, caller's order (CSR offset of the unit + index inside the unit)
   std::vector<int32_t> cl_status, cl_track;
+  std::vector<int32_t> start_wave;   // 1 = first wave, 2 = bridged start hit kept for the rescue wave (bridge_rescue)
   // S9 (NEXT-3): cross-sector segment matching
   std::vector<int32_t> mg_next, mg_prev, mg_leaver; std::vector<double> mg_outer;   // outer: x, y, z, sinphi per track
   std::vector<double> z_d, ys_d, zs_d;   // export copies
@@ -240,7 +242,7 @@ struct Oracle : OracleBase {
 
   // ---- S4: start hits = chain beginnings with >= min_seed hits, ascending (sector,row,sorted pos) ----
   void s4_start_hits(bool brute = false) {
-    start_unit.clear(); start_pos.clear();
+    start_unit.clear(); start_pos.clear(); start_wave.clear();
     for (int u = 0; u < NS * R; u++) {
       int64_t o = off[u], n = off[u + 1] - o;
       for (int64_t h = 0; h < n; h++) {
@@ -248,8 +250,9 @@ struct Oracle : OracleBase {
         int len = 1; int uu = u; int32_t p = (int32_t)h;
         while (len < T.min_seed) { int32_t nx = clean_up[off[uu] + p]; if (nx < 0) break; p = nx; uu++; len++; }
         if (len < T.min_seed) continue;
-        if (T.bridge_rows > 0 && bridged(u, (int32_t)h, brute)) continue;
-        start_unit.push_back(u); start_pos.push_back((int32_t)h);
+        int wave = 1;
+        if (T.bridge_rows > 0 && bridged(u, (int32_t)h, brute)) { if (!T.bridge_rescue) continue; wave = 2; }
+        start_unit.push_back(u); start_pos.push_back((int32_t)h); start_wave.push_back(wave);
       }
     }
   }
@@ -385,7 +388,7 @@ struct Oracle : OracleBase {
     int64_t M = (int64_t)start_unit.size();
     tl_n.assign(M, 0); tl_first.assign(M, -1); tl_last.assign(M, -1); tl_rowhit.assign(M * R, -1); tl_sector.assign(M, 0);
     tl_chi2.assign(M, 0); tl_x.assign(M, 0); tl_par.assign(M * 5, 0); tl_cov.assign(M * 15, 0); tl_zref.assign(M, 0);
-    for (int64_t i = 0; i < M; i++) {
+    auto fit = [&](int64_t i) {
       int u0 = start_unit[i], sec = u0 / R, r0 = u0 % R; int32_t h0 = start_pos[i];
       int32_t* rowhit = &tl_rowhit[i * R];
       auto Y = [&](int r, int32_t p) { return ys[off[sec * R + r] + p]; };
@@ -433,6 +436,22 @@ struct Oracle : OracleBase {
       for (int k = 0; k < 5; k++) tl_par[i * 5 + k] = (double)snap.p[k];
       tl_par[i * 5 + 1] = (double)(snap.p[1] + zref);
       int c = 0; for (int a = 0; a < 5; a++) for (int b = 0; b <= a; b++) tl_cov[i * 15 + c++] = (double)snap.C[a][b];
+    };
+    const bool two = T.bridge_rows > 0 && T.bridge_rescue;
+    for (int64_t i = 0; i < M; i++) { tl_sector[i] = start_unit[i] / R; if (!two || start_wave[i] == 1) fit(i); }
+    // S4' with rescue (reading A39c): the first wave fits the start hits that are not bridged; a bridged start hit is fitted in the
+    // second wave unless every cluster of its chain is used by a kept first-wave tracklet (then that tracklet covers its track)
+    if (two) {
+      std::vector<char> used(N, 0);
+      for (int64_t i = 0; i < M; i++) if (start_wave[i] == 1 && tracklet_kept(i)) {
+        const int sec = tl_sector[i];
+        for (int r = tl_first[i]; r <= tl_last[i]; r++) { int32_t p = tl_rowhit[i * R + r]; if (p >= 0) used[off[sec * R + r] + p] = 1; }
+      }
+      for (int64_t i = 0; i < M; i++) if (start_wave[i] == 2) {
+        int uu = start_unit[i]; int32_t p = start_pos[i]; bool all = true;
+        for (;;) { if (!used[off[uu] + p]) { all = false; break; } int32_t nx = clean_up[off[uu] + p]; if (nx < 0) break; p = nx; uu++; }
+        if (!all) fit(i);
+      }
     }
   }
 
@@ -716,6 +735,7 @@ struct Oracle : OracleBase {
     if (s == "trk_par") RET(trk_par, 2)
     if (s == "trk_cov") RET(trk_cov, 2)
     if (s == "trk_chi2") RET(trk_chi2, 2)
+    if (s == "start_wave") RET(start_wave, 0)
     if (s == "mg_next") RET(mg_next, 0)
     if (s == "mg_prev") RET(mg_prev, 0)
     if (s == "mg_leaver") RET(mg_leaver, 0)
@@ -753,7 +773,7 @@ int orc_set_param(void* h, const char* name, double v) {
   else if (s == "c0_y") T.c0[0] = v; else if (s == "c0_z") T.c0[1] = v; else if (s == "c0_sinphi") T.c0[2] = v;
   else if (s == "c0_dzds") T.c0[3] = v; else if (s == "c0_qpt") T.c0[4] = v;
   else if (s == "grid_scale") T.grid_scale = v;
-  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "tube") T.tube = v;
+  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "bridge_rescue") T.bridge_rescue = (int)v; else if (s == "tube") T.tube = v;
   else if (s == "merge_edge") T.merge_edge = v; else if (s == "merge_rows") T.merge_rows = (int)v; else if (s == "merge_dy") T.merge_dy = v;
   else if (s == "merge_dz") T.merge_dz = v; else if (s == "merge_ds") T.merge_ds = v; else if (s == "merge_dt") T.merge_dt = v;
   else return -1;

@@ -81,7 +81,8 @@ __device__ __forceinline__ int pickup(const UnitDesc& d, const float2* __restric
 // one from a global work queue (persistent CTAs), so short and long tracklets balance out.
 enum : int { MD_FETCH = 0, MD_INIT, MD_A, MD_B, MD_TRANS, MD_C, MD_EXIT };
 
-__global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const int* __restrict__ start_unit,
+__global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const int* __restrict__ run_list,
+                                                              const int* __restrict__ start_unit,
                                                               const int* __restrict__ start_pos, const UnitDesc* __restrict__ units,
                                                               const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                               const int* __restrict__ perm, const int* __restrict__ bin_start,
@@ -117,8 +118,9 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
       if (lane == leader) base = atomicAdd(queue, __popc(need));
       base = __shfl_sync(FULL, base, leader);
       if (mode == MD_FETCH) {
-        i = base + __popc(need & ((1u << lane) - 1u));
+        i = base + __popc(need & ((1u << lane) - 1u));   // queue position; M = entries to run
         if (i < M) {
+          if (run_list) i = run_list[i];                 // a sub-list of the start hits (rescue variant): tracklet index = list entry
           const int u0 = start_unit[i];
           const int h0 = start_pos[i];
           const int sec = u0 / R;
@@ -260,7 +262,8 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
 
 }  // namespace
 
-int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
+int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
+                        const UnitDesc* d_units,
                         const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, const int* d_link_up,
                         int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2, float* d_tl_par,
                         float* d_tl_cov, unsigned long long* d_counters, const Params& P) {
@@ -275,7 +278,7 @@ int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_sta
   int blocks = L.sm_count * per_sm;                         // persistent CTAs: one resident wave
   const int need = (M + K5_THREADS - 1) / K5_THREADS;
   if (blocks > need) blocks = need;
-  k5_tracklets<<<blocks, K5_THREADS, 0, L.stream>>>(M, d_start_unit, d_start_pos, d_units, d_rows, d_yz, d_perm, d_bin_start, d_link_up,
+  k5_tracklets<<<blocks, K5_THREADS, 0, L.stream>>>(M, d_run_list, d_start_unit, d_start_pos, d_units, d_rows, d_yz, d_perm, d_bin_start, d_link_up,
                                                     d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_counters,
                                                     d_queue, P);
   e = cudaGetLastError();

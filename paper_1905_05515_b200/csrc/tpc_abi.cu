@@ -88,6 +88,7 @@ struct Tunables {   // DESIGN.md table T
   int chunk = 1024;           // clusters per K2/K3 work item (multiple of 32)
   int k2_threads = 0;         // K2 block size (0 = default 256); tuning knob
   int bridge_rows = 0, bridge_min = 3;       // NEXT-2 seed bridging (reading A39): 0 = off
+  int bridge_rescue = 0;                     // 1: dropped start hits are fitted in a second wave when the first left their chain unused (A39c)
   double bridge_wy = 1.0, bridge_wz = 1.5;
   double merge_edge = 3.0, merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05; int merge_rows = 8;   // NEXT-3 (reading A41)
 };
@@ -127,7 +128,7 @@ struct tpc_ctx {
   // S1..S4
   long long N = 0, n_bins = 0; int n_items = 0;
   DevBuf d_yz, d_perm, d_bin_start, d_cursor, d_link_up, d_link_dn, d_raw_up, d_raw_dn, d_mask, d_item_count, d_item_base, d_scan_tmp;
-  DevBuf d_start_unit, d_start_pos, d_counters, d_keep, d_keep_pos, d_start_unit2, d_start_pos2;
+  DevBuf d_start_unit, d_start_pos, d_counters, d_keep, d_keep_pos, d_start_unit2, d_start_pos2, d_flag2, d_used;
   // S5/S6
   int M = 0; long long Mpad = 0;
   DevBuf d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out, d_scan_tmp64;
@@ -237,7 +238,7 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
                     &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
-                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->m_att, &c->m_adj, &c->m_status, &c->m_track,
+                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->d_flag2, &c->d_used, &c->m_att, &c->m_adj, &c->m_status, &c->m_track,
                     &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_cand, &c->g_next, &c->g_prev};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
@@ -280,6 +281,7 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "bridge_rows") { if (v < 0 || v > 16) return fail(c, TPC_E_ARG, "bridge_rows must be in 0..16"); T.bridge_rows = (int)v; }
   else if (s == "bridge_min") { if (v < 3 || v > 255) return fail(c, TPC_E_ARG, "bridge_min must be in 3..255"); T.bridge_min = (int)v; }
   else if (s == "bridge_wy") rc = pos(T.bridge_wy); else if (s == "bridge_wz") rc = pos(T.bridge_wz);
+  else if (s == "bridge_rescue") T.bridge_rescue = v != 0;
   else if (s == "merge_edge") rc = nonneg(T.merge_edge); else if (s == "merge_dy") rc = pos(T.merge_dy); else if (s == "merge_dz") rc = pos(T.merge_dz);
   else if (s == "merge_ds") rc = pos(T.merge_ds); else if (s == "merge_dt") rc = pos(T.merge_dt);
   else if (s == "merge_rows") { if (v < 0 || v > 255) return fail(c, TPC_E_ARG, "merge_rows must be in 0..255"); T.merge_rows = (int)v; }
@@ -513,7 +515,8 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, cudaStreamSynchronize(st));
   int M = *c->p_small.as<int>();
   if (M < 0 || M > start_cap) return fail(c, TPC_E_CUDA, "start-hit count %d out of range", M);
-  if (c->T.bridge_rows > 0 && M > 0) {   // S4' (NEXT-2 variant): drop the start hits that continue a lower chain, order kept
+  const bool rescue = c->T.bridge_rows > 0 && c->T.bridge_rescue && M > 0;
+  if (c->T.bridge_rows > 0 && !rescue && M > 0) {   // S4' (NEXT-2 variant): drop the start hits that continue a lower chain, order kept
     const size_t Mb = (size_t)M * 4;
     CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
     CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
@@ -546,10 +549,52 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, c->d_scan_tmp64.ensure((size_t)(M / SCAN_TILE + 4) * 8));
   unsigned long long* d_k5cnt = (unsigned long long*)(c->d_counters.as<char>() + 128);
   CUDA_TRY(c, cudaMemsetAsync(d_k5cnt, 0, 32, st));
-  LAUNCH_TRY(c, launch_k5_tracklets(L, M, Mpad, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
-                                    c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
-                                    c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
-                                    c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt, P), launches);
+  auto run_k5 = [&](int n_run, const int* list) -> int {
+    LAUNCH_TRY(c, launch_k5_tracklets(L, n_run, Mpad, list, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
+                                      c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
+                                      c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
+                                      c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt, P), launches);
+    return TPC_OK;
+  };
+  long long n_fitted = M;
+  if (!rescue) {
+    rc = run_k5(M, nullptr);
+    if (rc != TPC_OK) return rc;
+  } else {
+    // S4' with rescue (reading A39c): first wave = the start hits that are not bridged; second wave = the bridged ones whose chain
+    // the first wave did not use completely.  Tracklet index = position in the full S4 list in both waves; the others keep n = 0.
+    const size_t Mb = (size_t)M * 4;
+    CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
+    CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_flag2.ensure(Mb)); CUDA_TRY(c, c->d_used.ensure((size_t)std::max(N, 1LL)));
+    CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
+    CUDA_TRY(c, cudaMemsetAsync(c->d_tl_n.p, 0, Mb, st));
+    CUDA_TRY(c, cudaMemsetAsync(c->d_tl_first.p, 0xff, Mb, st)); CUDA_TRY(c, cudaMemsetAsync(c->d_tl_last.p, 0xff, Mb, st));
+    int* list1 = c->d_start_unit2.as<int>(); int* list2 = c->d_start_pos2.as<int>();
+    LAUNCH_TRY(c, launch_k3_bridge_lists(L, M, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
+                                         c->d_yz.as<float2>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(), c->d_link_dn.as<int>(),
+                                         c->d_keep.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), list1, d_nstart, P), launches);
+    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    const int M1 = *c->p_small.as<int>();
+    if (M1 < 0 || M1 > M) return fail(c, TPC_E_CUDA, "first-wave start-hit count %d out of range", M1);
+    rc = run_k5(M1, list1);
+    if (rc != TPC_OK) return rc;
+    LAUNCH_TRY(c, launch_k3_rescue_list(L, M, M1, list1, c->d_keep.as<int>(), c->d_start_unit.as<int>(), c->d_start_pos.as<int>(),
+                                        c->d_units.as<UnitDesc>(), c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
+                                        c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned char*)c->d_used.p, N,
+                                        c->d_flag2.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), list2, d_nstart, P), launches);
+    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    const int M2 = *c->p_small.as<int>();
+    if (M2 < 0 || M2 > M - M1) return fail(c, TPC_E_CUDA, "rescue-wave start-hit count %d out of range", M2);
+    if (M2 > 0) {
+      int* d_queue = reinterpret_cast<int*>(d_k5cnt + 3);
+      CUDA_TRY(c, cudaMemsetAsync(d_queue, 0, sizeof(int), st));
+      rc = run_k5(M2, list2);
+      if (rc != TPC_OK) return rc;
+    }
+    n_fitted = (long long)M1 + M2;
+  }
   CUDA_TRY(c, cudaEventRecord(c->ev[5], st));
 
   // ---- K6: S6
@@ -612,7 +657,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   for (int i = 0; i < 7; i++) CUDA_TRY(c, cudaEventElapsedTime(ms[i], c->ev[i], c->ev[i + 1]));
   CUDA_TRY(c, cudaEventElapsedTime(&tm.ms_total, c->ev[0], c->ev[7]));
   tm.n_clusters = N; tm.n_bins = c->n_bins; tm.n_start_hits = M; tm.n_tracks = nt; tm.n_cluster_refs = nr; tm.launches = launches;
-  tm.n_tracklets_kept = -1;
+  tm.n_tracklets_kept = n_fitted;   // tracklets actually fitted (= start hits unless the rescue variant skipped duplicates)
   { const unsigned long long* k5 = (const unsigned long long*)(c->p_small.as<char>() + 128);
     tm.n_propagations = (int64_t)k5[0]; tm.n_updates = (int64_t)k5[1]; tm.n_pickups = (int64_t)k5[2]; }
   c->have_result = true;
@@ -814,8 +859,9 @@ int tpc_debug_get_tracklets(tpc_ctx* c, tpc_tracklet_view* out) {
     CUDA_TRY(c, cudaMemcpy(c->dbg_tl_cov.data(), c->d_tl_cov.p, (size_t)M * 60, cudaMemcpyDeviceToHost));
     CUDA_TRY(c, cudaMemcpy(raw.data(), c->d_rowhit.p, raw.size() * 4, cudaMemcpyDeviceToHost));
     for (int i = 0; i < M; i++) {
-      c->dbg_tl_sector[i] = su[i] / R; c->dbg_tl_row[i] = su[i] % R; c->dbg_tl_x[i] = c->row_x[c->dbg_tl_first[i]];
-      for (int r = c->dbg_tl_first[i]; r <= c->dbg_tl_last[i]; r++) c->dbg_rowhit[(size_t)r * M + i] = raw[(size_t)i * R + r];
+      c->dbg_tl_sector[i] = su[i] / R; c->dbg_tl_row[i] = su[i] % R; const int f = c->dbg_tl_first[i];
+      c->dbg_tl_x[i] = f >= 0 && f < R ? c->row_x[f] : 0.0f;   // tracklets the rescue variant did not fit carry first = last = -1
+      for (int r = std::max(f, 0); f >= 0 && r <= c->dbg_tl_last[i] && r < R; r++) c->dbg_rowhit[(size_t)r * M + i] = raw[(size_t)i * R + r];
     }
   }
   out->n_tracklets = M; out->sector = c->dbg_tl_sector.data(); out->start_row = c->dbg_tl_row.data(); out->n_hits = c->dbg_tl_n.data();

@@ -102,11 +102,20 @@ int launch_k3_bridge(const Launch& L, int M, const int* d_start_unit, const int*
                      const RowConst* d_rows, const float2* d_yz, const int* d_bin_start, const int* d_link_up, const int* d_link_dn,
                      int* d_keep, int* d_keep_pos, int* d_scan_tmp, int* d_out_unit, int* d_out_pos, int* d_total, const Params& P);
 
+int launch_k3_bridge_lists(const Launch& L, int M, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
+                           const RowConst* d_rows, const float2* d_yz, const int* d_bin_start, const int* d_link_up, const int* d_link_dn,
+                           int* d_keep, int* d_pos, int* d_scan_tmp, int* d_list1, int* d_total, const Params& P);
+int launch_k3_rescue_list(const Launch& L, int M, int M1, const int* d_list1, const int* d_keep, const int* d_start_unit,
+                          const int* d_start_pos, const UnitDesc* d_units, const int* d_link_up, const int* d_rowhit, const int* d_tl_n,
+                          const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned char* d_used, long long N,
+                          int* d_flag2, int* d_pos, int* d_scan_tmp, int* d_list2, int* d_total, const Params& P);
+
 int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, int* d_link_up,
                           int* d_link_dn, unsigned* d_mask, int* d_item_count, int* d_item_base, int* d_scan_tmp,
                           int* d_start_unit, int* d_start_pos, int* d_total, const Params& P);
 
-int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
+int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
+                        const UnitDesc* d_units,
                         const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, const int* d_link_up,
                         int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2, float* d_tl_par,
                         float* d_tl_cov, unsigned long long* d_counters, const Params& P);

@@ -231,6 +231,31 @@ def test_next_rows_on_an_empty_result():
         assert m["n_clusters"] == 3 and np.all(m["status"] == 0) and np.all(m["track"] == -1)
 
 
+def test_seed_bridging_rescue_variant_parity():
+    """NEXT-2, reading A39c (bridge_rescue = 1 on both sides): full S4 start list, bridged start hits fitted only when the first wave
+    left their chain unused.  Same parity bars; the set of fitted tracklets is identical; at most 60 % of the tracklets are fitted;
+    efficiency within 0.1 % of the default path."""
+    kw = dict(bridge_rows=4, bridge_min=3, bridge_rescue=1)
+    for w in (W.config(1), W.config(2), W.config(3, scale=0.1)):
+        rng = np.random.default_rng(6)
+        o = P.make_oracle(w, **kw).run("s6")
+        with _tracker(w, debug_keep=1, **kw) as trk:
+            trk.load_workload(w)
+            gtr = trk.find_tracks().copy().as_dict()
+            lk = P.compare_links(w, o, trk)
+            tm = trk.timings()
+            tl = trk.tracklets()
+        assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
+        ofit = o.get("tl_first") >= 0
+        assert np.array_equal(tl["first"] >= 0, ofit)                     # the same tracklets were fitted
+        assert tm["n_start_hits"] == len(ofit) and tm["n_tracklets_kept"] == int(ofit.sum()) <= 0.6 * len(ofit)
+        res = P.compare_tracks(o.tracks(), gtr)
+        assert res["frac_identical"] >= 0.999 and res["param_mismatch"] <= 0.001 * res["n_oracle"], res
+        base = P.make_oracle(w).run("s6")
+        m0, m1 = H.truth_metrics(w, base.tracks()), H.truth_metrics(w, gtr)
+        assert m1["eff"] >= m0["eff"] - 0.001, (m0["eff"], m1["eff"])
+
+
 def test_empty_and_tiny_inputs():
     w = W.config(1, scale=0.05)
     with _tracker(w) as trk:

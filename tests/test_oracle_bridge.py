@@ -105,3 +105,61 @@ def test_bridging_trades_few_tracks_for_fewer_tracklets():
         m0, m1 = H.truth_metrics(w, o0.tracks()), H.truth_metrics(w, o1.tracks())
         assert len(o1.get("start_unit")) <= 0.72 * len(o0.get("start_unit"))
         assert m1["eff"] >= m0["eff"] - 0.003 and m1["fake_rate"] <= m0["fake_rate"] + 0.002, (m0["eff"], m1["eff"])
+
+
+# ------------------------------------------------------------------ S4' with rescue wave (reading A39c)
+def _fitted(o):
+    return o.get("tl_first") >= 0
+
+
+def test_rescue_variant_skips_only_seeds_whose_chain_is_used():
+    """bridge_rescue = 1: the start list is S4's; the first wave is exactly the non-bridged start hits; a bridged start hit is
+    left unfitted iff every cluster of its chain of links lies on a kept first-wave tracklet (recomputed here from the tracklets)."""
+    w = W.config(1)
+    base = Oracle.for_workload(w).run("s6")
+    o = Oracle.for_workload(w, bridge_rows=4, bridge_min=3, bridge_rescue=1).run("s6")
+    plain = Oracle.for_workload(w, bridge_rows=4, bridge_min=3).run("s4")
+    assert _starts(o) == _starts(base)
+    wave = o.get("start_wave"); fit = _fitted(o)
+    assert [s for s, wv in zip(_starts(o), wave) if wv == 1] == _starts(plain)
+    assert np.all(fit[wave == 1]) and 0 < fit[wave == 2].sum() < (wave == 2).sum()
+    tl = o.tracklets(); R = w.n_rows; off = w.unit_off
+    used = np.zeros(w.n_clusters, bool)
+    for i in np.nonzero((wave == 1) & (tl["n"] >= 10))[0]:
+        rows = np.nonzero(tl["rowhit"][i] >= 0)[0]
+        rows = rows[(rows >= tl["first"][i]) & (rows <= tl["last"][i])]
+        used[off[tl["sector"][i] * R + rows] + tl["rowhit"][i][rows]] = True
+    up = o.get("clean_up")
+    for i in np.nonzero(wave == 2)[0]:
+        u, p = int(o.get("start_unit")[i]), int(o.get("start_pos")[i]); all_used = True
+        while True:
+            g = off[u] + p
+            if not used[g]:
+                all_used = False; break
+            if up[g] < 0:
+                break
+            p = int(up[g]); u += 1
+        assert fit[i] == (not all_used), i
+
+
+def test_rescue_variant_on_hand_made_dropouts_and_truth():
+    """Noise-free tracks with two removed clusters: one fitted tracklet per track instead of three, same tracks.  C1 and a
+    C2-shaped event: at most 60 % of the tracklets fitted, efficiency within 0.1 % of S4's, no extra fakes."""
+    w0 = _tracks()
+    row = _row_of(w0)
+    full = [p for p in range(len(w0.particles["pt"])) if (w0.label == p).sum() == w0.n_rows]
+    sel = np.isin(w0.label, full)
+    w = _remove(w0, ~sel | (sel & ((row == 50) | (row == 100))))
+    a = Oracle.for_workload(w, sigma_y=0.1, sigma_z=0.15).run("s6")
+    b = Oracle.for_workload(w, sigma_y=0.1, sigma_z=0.15, bridge_rows=4, bridge_min=3, bridge_rescue=1).run("s6")
+    assert _fitted(a).sum() == 3 * len(full) and _fitted(b).sum() == len(full)
+    ta, tb = a.tracks(), b.tracks()
+    sets = lambda t: sorted(tuple(zip(t["cl_row"][t["cl_begin"][i]:t["cl_begin"][i + 1]].tolist(),
+                                      t["cl_index"][t["cl_begin"][i]:t["cl_begin"][i + 1]].tolist())) for i in range(len(t["sector"])))
+    assert len(ta["sector"]) == len(tb["sector"]) == len(full) and sets(ta) == sets(tb)     # same tracks (another duplicate may win)
+    for w in (W.config(1), W.config(2, scale=0.2)):
+        o0 = Oracle.for_workload(w).run("s6")
+        o1 = Oracle.for_workload(w, bridge_rows=4, bridge_min=3, bridge_rescue=1).run("s6")
+        m0, m1 = H.truth_metrics(w, o0.tracks()), H.truth_metrics(w, o1.tracks())
+        assert _fitted(o1).sum() <= 0.6 * _fitted(o0).sum()
+        assert m1["eff"] >= m0["eff"] - 0.001 and m1["fake_rate"] <= m0["fake_rate"] + 0.001, (m0["eff"], m1["eff"])
