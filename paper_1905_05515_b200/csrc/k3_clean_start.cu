@@ -198,29 +198,11 @@ __global__ void __launch_bounds__(K3_THREADS) k3_index_list(const int M, const i
   if (i < M && flag[i]) list[pos[i]] = i;
 }
 
-// rescue variant, after the first wave of K5: one warp per first-wave tracklet marks the clusters of every kept tracklet as used
-__global__ void __launch_bounds__(K3_THREADS) k3_mark_used(const int M1, const int* __restrict__ list1, const int R, const int min_hits,
-                                                           const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
-                                                           const int* __restrict__ rowhit, const int* __restrict__ tl_n,
-                                                           const int* __restrict__ tl_first, const int* __restrict__ tl_last,
-                                                           const float* __restrict__ tl_chi2, unsigned char* __restrict__ used) {
-  const int q = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
-  if (q >= M1) return;
-  const int i = list1[q];
-  if (!(tl_n[i] >= min_hits && isfinite(tl_chi2[i]))) return;
-  const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
-  const int* __restrict__ rh = rowhit + (long long)i * R;
-  const int r1 = tl_last[i];
-  for (int r = tl_first[i] + lane; r <= r1; r += 32) {
-    const int p = rh[r];
-    if (p >= 0) used[su[r].off + p] = 1;
-  }
-}
-
-// a dropped start hit is rescued (fitted in the second wave) unless every cluster of its chain was used by the first wave
+// a dropped start hit is rescued (fitted in the second wave) unless every cluster of its chain lies on a kept first-wave tracklet,
+// i.e. carries an owner key (the first half of the selector, k6_owner, has run over the first wave)
 __global__ void __launch_bounds__(K3_THREADS) k3_rescue_flag(const int M, const int* __restrict__ keep, const int* __restrict__ start_unit,
                                                              const int* __restrict__ start_pos, const UnitDesc* __restrict__ units,
-                                                             const int* __restrict__ link_up, const unsigned char* __restrict__ used,
+                                                             const int* __restrict__ link_up, const unsigned long long* __restrict__ owner,
                                                              int* __restrict__ flag2) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= M) return;
@@ -229,7 +211,7 @@ __global__ void __launch_bounds__(K3_THREADS) k3_rescue_flag(const int M, const 
     int u = start_unit[i], p = start_pos[i];
     for (;;) {
       const long long g = units[u].off + p;
-      if (!used[g]) { f = 1; break; }
+      if (owner[g] == 0ull) { f = 1; break; }
       const int nx = link_up[g];          // cleaned table
       if (nx < 0) break;
       p = nx; u++;
@@ -261,23 +243,16 @@ int launch_k3_bridge_lists(const Launch& L, int M, const int* d_start_unit, cons
 // part 2, after the first wave: list2 = dropped start hits whose chain the first wave left (partly) unused; *d_total = their number
 int launch_k3_rescue_list(const Launch& L, int M, int M1, const int* d_list1, const int* d_keep, const int* d_start_unit,
                           const int* d_start_pos, const UnitDesc* d_units, const int* d_link_up, const int* d_rowhit, const int* d_tl_n,
-                          const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned char* d_used, long long N,
+                          const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, const unsigned long long* d_owner, long long N,
                           int* d_flag2, int* d_pos, int* d_scan_tmp, int* d_list2, int* d_total, const Params& P) {
-  cudaError_t e = cudaMemsetAsync(d_used, 0, (size_t)(N > 0 ? N : 1), L.stream);
-  if (e != cudaSuccess) return -(int)e;
-  int launches = 0;
-  if (M1 > 0) {
-    k3_mark_used<<<(int)(((long long)M1 * 32 + K3_THREADS - 1) / K3_THREADS), K3_THREADS, 0, L.stream>>>(
-        M1, d_list1, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_used);
-    launches++;
-  }
+  (void)M1; (void)d_list1; (void)d_rowhit; (void)d_tl_n; (void)d_tl_first; (void)d_tl_last; (void)d_tl_chi2; (void)N; (void)P;
   const int blocks = (M + K3_THREADS - 1) / K3_THREADS;
-  k3_rescue_flag<<<blocks, K3_THREADS, 0, L.stream>>>(M, d_keep, d_start_unit, d_start_pos, d_units, d_link_up, d_used, d_flag2);
+  k3_rescue_flag<<<blocks, K3_THREADS, 0, L.stream>>>(M, d_keep, d_start_unit, d_start_pos, d_units, d_link_up, d_owner, d_flag2);
   int rc = launch_scan_i32(L, d_flag2, d_pos, M, d_scan_tmp, d_total);
   if (rc < 0) return rc;
   k3_index_list<<<blocks, K3_THREADS, 0, L.stream>>>(M, d_flag2, d_pos, d_list2);
-  e = cudaGetLastError();
-  return e == cudaSuccess ? launches + 2 + rc : -(int)e;
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? 2 + rc : -(int)e;
 }
 
 int launch_k3_bridge(const Launch& L, int M, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,

@@ -25,14 +25,15 @@ __device__ __forceinline__ unsigned long long make_key(int n, float chi2, int id
 
 // All three kernels map ONE WARP to one tracklet: the lanes read 32 consecutive rows of its rowhit line (coalesced) and issue
 // their owner-key atomics / owner reads in parallel.
-__global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const int R, const int min_hits,
+__global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const int* __restrict__ run_list, const int R, const int min_hits,
                                                        const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
                                                        const int* __restrict__ rowhit, const int* __restrict__ tl_n,
                                                        const int* __restrict__ tl_first, const int* __restrict__ tl_last,
                                                        const float* __restrict__ tl_chi2, unsigned long long* __restrict__ owner,
                                                        unsigned long long* __restrict__ tl_key) {
-  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
-  if (i >= M) return;
+  const int q = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+  if (q >= M) return;
+  const int i = run_list ? run_list[q] : q;   // M entries of a run list (rescue variant), or all tracklets
   const int n = tl_n[i];
   const float chi2 = tl_chi2[i];
   const bool kept = n >= min_hits && isfinite(chi2);
@@ -119,24 +120,39 @@ int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const 
                      const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
                      const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
                      unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
-                     unsigned long long* d_total, const Params& P) {
+                     unsigned long long* d_total, const Params& P, bool owner_done) {
   (void)d_rows; (void)d_perm;
   if (M <= 0) {
     cudaError_t e = cudaMemsetAsync(d_total, 0, sizeof(unsigned long long), L.stream);
     return e == cudaSuccess ? 0 : -(int)e;
   }
-  cudaError_t e = cudaMemsetAsync(d_owner, 0, (size_t)N * sizeof(unsigned long long), L.stream);
-  if (e != cudaSuccess) return -(int)e;
+  cudaError_t e = cudaSuccess;
   (void)Mpad;
   const int blocks = (int)(((long long)M * 32 + K6_THREADS - 1) / K6_THREADS);
-  k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first, d_tl_last,
-                                                 d_tl_chi2, d_owner, d_tl_key);
+  if (!owner_done) {   // (the rescue variant raised the owner keys wave by wave: launch_k6_owner)
+    e = cudaMemsetAsync(d_owner, 0, (size_t)N * sizeof(unsigned long long), L.stream);
+    if (e != cudaSuccess) return -(int)e;
+    k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M, nullptr, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first,
+                                                   d_tl_last, d_tl_chi2, d_owner, d_tl_key);
+  }
   k6_count<<<blocks, K6_THREADS, 0, L.stream>>>(M, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_first, d_tl_last, d_owner,
                                                  d_tl_key, d_scan_in);
   int rc = launch_scan_u64(L, d_scan_in, d_scan_out, M, d_scan_tmp, d_total);
   if (rc < 0) return rc;
   e = cudaGetLastError();
-  return e == cudaSuccess ? 2 + rc : -(int)e;
+  return e == cudaSuccess ? (owner_done ? 1 : 2) + rc : -(int)e;
+}
+
+// owner keys of the n_run tracklets of a run list (rescue variant: one call per K5 wave; the caller zeroes d_owner and d_tl_key first)
+int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int* d_start_unit, const UnitDesc* d_units, const int* d_rowhit,
+                    const int* d_tl_n, const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner,
+                    unsigned long long* d_tl_key, const Params& P) {
+  if (n_run <= 0) return 0;
+  const int blocks = (int)(((long long)n_run * 32 + K6_THREADS - 1) / K6_THREADS);
+  k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(n_run, d_run_list, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first,
+                                                 d_tl_last, d_tl_chi2, d_owner, d_tl_key);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? 1 : -(int)e;
 }
 
 int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,

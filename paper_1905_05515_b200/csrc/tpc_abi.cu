@@ -565,7 +565,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
     // the first wave did not use completely.  Tracklet index = position in the full S4 list in both waves; the others keep n = 0.
     const size_t Mb = (size_t)M * 4;
     CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
-    CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_flag2.ensure(Mb)); CUDA_TRY(c, c->d_used.ensure((size_t)std::max(N, 1LL)));
+    CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_flag2.ensure(Mb));
     CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
     CUDA_TRY(c, cudaMemsetAsync(c->d_tl_n.p, 0, Mb, st));
     CUDA_TRY(c, cudaMemsetAsync(c->d_tl_first.p, 0xff, Mb, st)); CUDA_TRY(c, cudaMemsetAsync(c->d_tl_last.p, 0xff, Mb, st));
@@ -579,9 +579,15 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
     if (M1 < 0 || M1 > M) return fail(c, TPC_E_CUDA, "first-wave start-hit count %d out of range", M1);
     rc = run_k5(M1, list1);
     if (rc != TPC_OK) return rc;
+    // first half of the selector over the first wave: its owner keys are the "used" marks of the rescue test
+    CUDA_TRY(c, cudaMemsetAsync(c->d_owner.p, 0, (size_t)std::max(N, 1LL) * 8, st));
+    CUDA_TRY(c, cudaMemsetAsync(c->d_tl_key.p, 0, Mz * 8, st));
+    LAUNCH_TRY(c, launch_k6_owner(L, M1, list1, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
+                                  c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned long long*)c->d_owner.p,
+                                  (unsigned long long*)c->d_tl_key.p, P), launches);
     LAUNCH_TRY(c, launch_k3_rescue_list(L, M, M1, list1, c->d_keep.as<int>(), c->d_start_unit.as<int>(), c->d_start_pos.as<int>(),
                                         c->d_units.as<UnitDesc>(), c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
-                                        c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned char*)c->d_used.p, N,
+                                        c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (const unsigned long long*)c->d_owner.p, N,
                                         c->d_flag2.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), list2, d_nstart, P), launches);
     CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaStreamSynchronize(st));
@@ -592,6 +598,9 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
       CUDA_TRY(c, cudaMemsetAsync(d_queue, 0, sizeof(int), st));
       rc = run_k5(M2, list2);
       if (rc != TPC_OK) return rc;
+      LAUNCH_TRY(c, launch_k6_owner(L, M2, list2, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
+                                    c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned long long*)c->d_owner.p,
+                                    (unsigned long long*)c->d_tl_key.p, P), launches);
     }
     n_fitted = (long long)M1 + M2;
   }
@@ -602,7 +611,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   LAUNCH_TRY(c, launch_k6_select(L, M, Mpad, N, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
                                  c->d_perm.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(),
                                  c->d_tl_chi2.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
-                                 c->d_scan_out.as<u64>(), c->d_scan_tmp64.as<u64>(), d_total64, P), launches);
+                                 c->d_scan_out.as<u64>(), c->d_scan_tmp64.as<u64>(), d_total64, P, rescue), launches);
   CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 64, d_total64, 8, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 128, d_k5cnt, 24, cudaMemcpyDeviceToHost, st));
   CUDA_TRY(c, cudaStreamSynchronize(st));

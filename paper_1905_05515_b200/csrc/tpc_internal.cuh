@@ -107,7 +107,7 @@ int launch_k3_bridge_lists(const Launch& L, int M, const int* d_start_unit, cons
                            int* d_keep, int* d_pos, int* d_scan_tmp, int* d_list1, int* d_total, const Params& P);
 int launch_k3_rescue_list(const Launch& L, int M, int M1, const int* d_list1, const int* d_keep, const int* d_start_unit,
                           const int* d_start_pos, const UnitDesc* d_units, const int* d_link_up, const int* d_rowhit, const int* d_tl_n,
-                          const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned char* d_used, long long N,
+                          const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, const unsigned long long* d_owner, long long N,
                           int* d_flag2, int* d_pos, int* d_scan_tmp, int* d_list2, int* d_total, const Params& P);
 
 int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, int* d_link_up,
@@ -124,7 +124,10 @@ int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const 
                      const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
                      const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
                      unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
-                     unsigned long long* d_total, const Params& P);
+                     unsigned long long* d_total, const Params& P, bool owner_done);
+int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int* d_start_unit, const UnitDesc* d_units, const int* d_rowhit,
+                    const int* d_tl_n, const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner,
+                    unsigned long long* d_tl_key, const Params& P);
 
 int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
                    const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
