@@ -31,7 +31,7 @@ UNIT = "clusters/s"
 # algorithmic HBM bytes per cluster
 BYTES_PER_CLUSTER = {"grid": 24.0, "neighbours": 20.0, "clean_start": 24.0}
 # fp32 operations (no FMA: one flop per instruction) per S5 primitive, counted from k5_tracklets.cu
-FLOP_PROPAGATE, FLOP_UPDATE, FLOP_PICKUP = 170.0, 132.0, 28.0
+FLOP_PROPAGATE, FLOP_UPDATE, FLOP_PICKUP = 173.0, 133.0, 28.0   # after reading A42 (reciprocals: 3 fewer divisions, more products)
 
 
 def _peaks():

@@ -312,7 +312,8 @@ struct Oracle : OracleBase {
     Real s1 = s + kdx;
     if (!(std::fabs(s) <= smax) || !(std::fabs(s1) <= smax)) return false;
     Real c = std::sqrt((Real)1 - s * s), c1 = std::sqrt((Real)1 - s1 * s1);
-    Real cc = c + c1, ss = s + s1, tq = ss / cc;
+    // reading A42: one reciprocal per distinct denominator (1/(c+c1), 1/(c c1), 1/c1 = c * 1/(c c1)), products rounded one by one
+    Real cc = c + c1, ss = s + s1, icc = (Real)1 / cc, tq = ss * icc;
     Real g = (Real)1 + tq * tq;
     Real L = dx * std::sqrt(g);
     Real h = ((Real)0.5 * k) * L, h2 = h * h;
@@ -328,14 +329,14 @@ struct Oracle : OracleBase {
     } else S = ((Real)2 / k) * std::asin(h);
     Real dSdk;
     const Real kthr = sizeof(Real) == 4 ? (Real)1e-2 : (Real)1e-3;
-    if (std::fabs(kdx) >= kthr) dSdk = (dx / c1 - S) / k;
-    else { Real sm = (s + (Real)2 * s1) / (Real)3; Real cm2 = (Real)1 - sm * sm; Real cm = std::sqrt(cm2);
+    Real cc1 = c * c1, icc1 = (Real)1 / cc1, ic1 = c * icc1;
+    if (std::fabs(kdx) >= kthr) dSdk = (dx * ic1 - S) / k;
+    else { Real sm = (s + (Real)2 * s1) * (Real)(1.0 / 3.0); Real cm2 = (Real)1 - sm * sm; Real cm = std::sqrt(cm2);
       dSdk = ((dx * dx) * sm) / ((Real)2 * (cm2 * cm)); }
-    Real cc1 = c * c1;
     Real F[5][5]; for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) F[i][j] = i == j ? (Real)1 : (Real)0;
-    F[0][2] = ((dx * g) * cc) / ((Real)2 * cc1);
-    F[0][4] = (((dx * dx) * cB) * g) / ((Real)2 * c1);
-    F[1][2] = ((t * dx) * tq) / cc1;
+    F[0][2] = ((dx * g) * cc) * ((Real)0.5 * icc1);
+    F[0][4] = (((dx * dx) * cB) * g) * ((Real)0.5 * ic1);
+    F[1][2] = ((t * dx) * tq) * icc1;
     F[1][3] = S;
     F[1][4] = (t * cB) * dSdk;
     F[2][4] = cB * dx;
@@ -352,7 +353,8 @@ struct Oracle : OracleBase {
     const Real ry = (Real)sigma_y * (Real)sigma_y, rz = (Real)sigma_z * (Real)sigma_z;
     Real s00 = st.C[0][0] + ry, s10 = st.C[1][0], s11 = st.C[1][1] + rz;
     Real det = s00 * s11 - s10 * s10;
-    Real i00 = s11 / det, i11 = s00 / det, i10 = -s10 / det;
+    Real idet = (Real)1 / det;   // reading A42: S^-1 through one reciprocal
+    Real i00 = s11 * idet, i11 = s00 * idet, i10 = -s10 * idet;
     Real r0 = ym - st.p[0], r1 = zm - st.p[1];
     Real K0[5], K1[5];
     for (int i = 0; i < 5; i++) { K0[i] = st.C[i][0] * i00 + st.C[i][1] * i10; K1[i] = st.C[i][0] * i10 + st.C[i][1] * i11; }

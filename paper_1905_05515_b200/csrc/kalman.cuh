@@ -27,7 +27,8 @@ __device__ __forceinline__ bool propagate(State& st, const float dx, const Param
   const float s1 = s + kdx;
   if (!(fabsf(s) <= P.smax) || !(fabsf(s1) <= P.smax)) return false;
   const float c = sqrtf(1.0f - s * s), c1 = sqrtf(1.0f - s1 * s1);
-  const float cc = c + c1, ss = s + s1, tq = ss / cc;
+  // reading A42: one reciprocal per distinct denominator
+  const float cc = c + c1, ss = s + s1, icc = 1.0f / cc, tq = ss * icc;
   const float g = 1.0f + tq * tq;
   const float L = dx * sqrtf(g);
   const float h = (0.5f * k) * L, h2 = h * h;
@@ -42,19 +43,19 @@ __device__ __forceinline__ bool propagate(State& st, const float dx, const Param
   } else {
     S = (2.0f / k) * asinf(h);
   }
+  const float cc1 = c * c1, icc1 = 1.0f / cc1, ic1 = c * icc1;
   float dSdk;
   if (fabsf(kdx) >= 1e-2f) {
-    dSdk = (dx / c1 - S) / k;
+    dSdk = (dx * ic1 - S) / k;
   } else {
-    const float sm = (s + 2.0f * s1) / 3.0f;
+    const float sm = (s + 2.0f * s1) * (float)(1.0 / 3.0);
     const float cm2 = 1.0f - sm * sm;
     const float cm = sqrtf(cm2);
     dSdk = ((dx * dx) * sm) / (2.0f * (cm2 * cm));
   }
-  const float cc1 = c * c1;
-  const float f02 = ((dx * g) * cc) / (2.0f * cc1);
-  const float f04 = (((dx * dx) * cB) * g) / (2.0f * c1);
-  const float f12 = ((t * dx) * tq) / cc1;
+  const float f02 = ((dx * g) * cc) * (0.5f * icc1);
+  const float f04 = (((dx * dx) * cB) * g) * (0.5f * ic1);
+  const float f12 = ((t * dx) * tq) * icc1;
   const float f13 = S;
   const float f14 = (t * cB) * dSdk;
   const float f24 = cB * dx;
@@ -103,7 +104,8 @@ __device__ __forceinline__ bool propagate(State& st, const float dx, const Param
 __device__ __forceinline__ float update(State& st, const float ym, const float zm, const Params& P) {
   const float s00 = st.c00 + P.ry, s10 = st.c10, s11 = st.c11 + P.rz;
   const float det = s00 * s11 - s10 * s10;
-  const float i00 = s11 / det, i11 = s00 / det, i10 = -s10 / det;
+  const float idet = 1.0f / det;
+  const float i00 = s11 * idet, i11 = s00 * idet, i10 = -s10 * idet;
   const float r0 = ym - st.y, r1 = zm - st.z;
   // K = C[:,0:2] S^-1
   const float k00 = st.c00 * i00 + st.c10 * i10, k01 = st.c00 * i10 + st.c10 * i11;
