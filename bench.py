@@ -30,8 +30,10 @@ METRIC = "tpc_clusters_per_s"
 UNIT = "clusters/s"
 # algorithmic HBM bytes per cluster
 BYTES_PER_CLUSTER = {"grid": 24.0, "neighbours": 20.0, "clean_start": 24.0}
-# fp32 operations (no FMA: one flop per instruction) per S5 primitive, counted from k5_tracklets.cu
-FLOP_PROPAGATE, FLOP_UPDATE, FLOP_PICKUP = 173.0, 133.0, 28.0   # after reading A42 (reciprocals: 3 fewer divisions, more products)
+# fp32 flops per S5 primitive, counted from csrc/kalman.cuh / k5_tracklets.cu: a fused multiply-add (reading A43)
+# counts two flops, everything else one; INST_* are the fp32 instructions that carry them (an FMA is one instruction)
+FLOP_PROPAGATE, FLOP_UPDATE, FLOP_PICKUP = 173.0, 133.0, 28.0
+INST_PROPAGATE, INST_UPDATE, INST_PICKUP = 112.0, 79.0, 28.0
 
 
 def _peaks():
@@ -289,7 +291,8 @@ def run_gpu(args, rank, world, local_rank):
 
     # ---- roofline of every kernel; the dominant one goes into "roofline"
     hbm_peak, peak_src, sm_max = _peaks()
-    alu_peak = 148 * 128 * sm_max * 1e6 / 1e12      # TFLOP/s, one fp32 op per lane per clock (FMA contraction is off)
+    issue_peak = 148 * 128 * sm_max * 1e6 / 1e12    # T fp32 instructions/s: one per lane per clock
+    alu_peak = 2.0 * issue_peak                     # TFLOP/s: the FMA peak (two flops per lane per clock)
     traffic = {}
     tp = os.path.join(ROOT, "profiles", f"traffic_c{args.config}.csv")   # DRAM bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
@@ -304,8 +307,10 @@ def run_gpu(args, rank, world, local_rank):
                        "ms": kern[key], "traffic": traffic.get(name)}
     flops = FLOP_PROPAGATE * tm["n_propagations"] + FLOP_UPDATE * tm["n_updates"] + FLOP_PICKUP * tm["n_pickups"]
     a = flops / (kern["ms_tracklets"] * 1e-3) / 1e12
+    insts = INST_PROPAGATE * tm["n_propagations"] + INST_UPDATE * tm["n_updates"] + INST_PICKUP * tm["n_pickups"]
     roofs["tracklets"] = {"bound": "alu", "achieved": a, "peak": alu_peak, "unit": "TFLOP/s", "frac": a / alu_peak,
-                          "peak_source": "148 SM x 128 fp32 lanes x sm_max_mhz, no FMA (DESIGN.md section 8)", "ms": kern["ms_tracklets"],
+                          "peak_source": "148 SM x 128 fp32 lanes x 2 flop (FMA) x sm_max_mhz (DESIGN.md section 8)", "ms": kern["ms_tracklets"],
+                          "fp32_inst_frac": insts / (kern["ms_tracklets"] * 1e-3) / 1e12 / issue_peak,
                           "traffic": traffic.get("tracklets")}
     roofs["selector"] = {"bound": "hbm", "achieved": None, "peak": hbm_peak, "unit": "GB/s", "frac": None, "ms": kern["ms_selector"],
                          "traffic": traffic.get("selector")}

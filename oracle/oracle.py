@@ -20,9 +20,18 @@ STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6, "s7": 7
 
 
 def build(force: bool = False) -> str:
-    """g++ -O2 -ffp-contract=off: every fp32 product is rounded before it is added (no FMA)."""
+    """g++ -O2 -ffp-contract=off: a product is rounded before it is added unless the source says std::fma (reading A43 of DESIGN.md:
+    the S5 transport / update).  -mfma, when the host has the instruction, only makes std::fma the hardware instruction instead of a
+    libm call; the result is the correctly rounded one either way."""
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC", _SRC, "-o", _SO])
+        hw = []
+        try:
+            with open("/proc/cpuinfo") as f:
+                if " fma " in f.read():
+                    hw = ["-mfma"]
+        except OSError:
+            pass
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off"] + hw + ["-std=c++17", "-shared", "-fPIC", _SRC, "-o", _SO])
     return _SO
 
 

@@ -13,7 +13,8 @@
  * notation; each function names the step it implements.
  *
  * Two instances: Real=float (the parity reference: decisions are taken in fp32, the kernel's
- * precision, with contraction off) and Real=double (closed-form pins).
+ * precision, with contraction off; the only fused multiply-adds are the std::fma calls of the S5 transport / update, reading A43)
+ * and Real=double (closed-form pins).
  * Build: g++ -O2 -ffp-contract=off -shared -fPIC oracle/tpc_oracle.cpp -o oracle/libtpc_oracle.so
  *
  * Pins (tests/test_oracle_*.py): S0 closed form; S1 invariants; S2 brute force O(N^2) + bin-size and
@@ -311,27 +312,28 @@ struct Oracle : OracleBase {
     Real kdx = k * dx;
     Real s1 = s + kdx;
     if (!(std::fabs(s) <= smax) || !(std::fabs(s1) <= smax)) return false;
-    Real c = std::sqrt((Real)1 - s * s), c1 = std::sqrt((Real)1 - s1 * s1);
+    // reading A43: every a + p*q of the transport and of the update below is ONE fused multiply-add, std::fma(p, q, a)
+    Real c = std::sqrt(std::fma(-s, s, (Real)1)), c1 = std::sqrt(std::fma(-s1, s1, (Real)1));
     // reading A42: one reciprocal per distinct denominator (1/(c+c1), 1/(c c1), 1/c1 = c * 1/(c c1)), products rounded one by one
     Real cc = c + c1, ss = s + s1, icc = (Real)1 / cc, tq = ss * icc;
-    Real g = (Real)1 + tq * tq;
+    Real g = std::fma(tq, tq, (Real)1);
     Real L = dx * std::sqrt(g);
     Real h = ((Real)0.5 * k) * L, h2 = h * h;
     const Real hthr = sizeof(Real) == 4 ? (Real)0.25 : (Real)1e-3;
     Real S;
     if (std::fabs(h) < hthr) {   // asin(h)/h = 1 + h^2/6 + 3h^4/40 + 15h^6/336 + 105h^8/3456 + ...
       Real poly = (Real)(105.0 / 3456.0);
-      poly = (Real)(15.0 / 336.0) + h2 * poly;
-      poly = (Real)(3.0 / 40.0) + h2 * poly;
-      poly = (Real)(1.0 / 6.0) + h2 * poly;
-      poly = (Real)1 + h2 * poly;
+      poly = std::fma(h2, poly, (Real)(15.0 / 336.0));
+      poly = std::fma(h2, poly, (Real)(3.0 / 40.0));
+      poly = std::fma(h2, poly, (Real)(1.0 / 6.0));
+      poly = std::fma(h2, poly, (Real)1);
       S = L * poly;
     } else S = ((Real)2 / k) * std::asin(h);
     Real dSdk;
     const Real kthr = sizeof(Real) == 4 ? (Real)1e-2 : (Real)1e-3;
     Real cc1 = c * c1, icc1 = (Real)1 / cc1, ic1 = c * icc1;
-    if (std::fabs(kdx) >= kthr) dSdk = (dx * ic1 - S) / k;
-    else { Real sm = (s + (Real)2 * s1) * (Real)(1.0 / 3.0); Real cm2 = (Real)1 - sm * sm; Real cm = std::sqrt(cm2);
+    if (std::fabs(kdx) >= kthr) dSdk = std::fma(dx, ic1, -S) / k;
+    else { Real sm = (s + (Real)2 * s1) * (Real)(1.0 / 3.0); Real cm2 = std::fma(-sm, sm, (Real)1); Real cm = std::sqrt(cm2);
       dSdk = ((dx * dx) * sm) / ((Real)2 * (cm2 * cm)); }
     Real F[5][5]; for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) F[i][j] = i == j ? (Real)1 : (Real)0;
     F[0][2] = ((dx * g) * cc) * ((Real)0.5 * icc1);
@@ -340,10 +342,10 @@ struct Oracle : OracleBase {
     F[1][3] = S;
     F[1][4] = (t * cB) * dSdk;
     F[2][4] = cB * dx;
-    st.p[0] = y + dx * tq; st.p[1] = zz + t * S; st.p[2] = s1;
+    st.p[0] = std::fma(dx, tq, y); st.p[1] = std::fma(t, S, zz); st.p[2] = s1;
     Real Tm[5][5], Cn[5][5];
-    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = a + F[i][m] * st.C[m][j]; Tm[i][j] = a; }
-    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = a + Tm[i][m] * F[j][m]; Cn[i][j] = a; }
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = std::fma(F[i][m], st.C[m][j], a); Tm[i][j] = a; }
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = std::fma(Tm[i][m], F[j][m], a); Cn[i][j] = a; }
     for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = Cn[i][j]; st.C[j][i] = Cn[i][j]; }   // symmetrise: lower triangle mirrored
     return true;
   }
@@ -352,17 +354,18 @@ struct Oracle : OracleBase {
   Real update_state(State& st, Real ym, Real zm) const {
     const Real ry = (Real)sigma_y * (Real)sigma_y, rz = (Real)sigma_z * (Real)sigma_z;
     Real s00 = st.C[0][0] + ry, s10 = st.C[1][0], s11 = st.C[1][1] + rz;
-    Real det = s00 * s11 - s10 * s10;
+    Real det = std::fma(-s10, s10, s00 * s11);   // reading A43: fused multiply-adds, as in the transport
     Real idet = (Real)1 / det;   // reading A42: S^-1 through one reciprocal
     Real i00 = s11 * idet, i11 = s00 * idet, i10 = -s10 * idet;
     Real r0 = ym - st.p[0], r1 = zm - st.p[1];
     Real K0[5], K1[5];
-    for (int i = 0; i < 5; i++) { K0[i] = st.C[i][0] * i00 + st.C[i][1] * i10; K1[i] = st.C[i][0] * i10 + st.C[i][1] * i11; }
+    for (int i = 0; i < 5; i++) { K0[i] = std::fma(st.C[i][1], i10, st.C[i][0] * i00); K1[i] = std::fma(st.C[i][1], i11, st.C[i][0] * i10); }
     Real Cn[5][5];
-    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) Cn[i][j] = st.C[i][j] - (K0[i] * st.C[0][j] + K1[i] * st.C[1][j]);
-    for (int i = 0; i < 5; i++) st.p[i] = st.p[i] + (K0[i] * r0 + K1[i] * r1);
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) Cn[i][j] = std::fma(-K1[i], st.C[1][j], std::fma(-K0[i], st.C[0][j], st.C[i][j]));
+    for (int i = 0; i < 5; i++) st.p[i] = std::fma(K1[i], r1, std::fma(K0[i], r0, st.p[i]));
     for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = Cn[i][j]; st.C[j][i] = Cn[i][j]; }
-    return r0 * (i00 * r0 + i10 * r1) + r1 * (i10 * r0 + i11 * r1);
+    Real u0 = std::fma(i10, r1, i00 * r0), u1 = std::fma(i11, r1, i10 * r0);
+    return std::fma(r1, u1, r0 * u0);
   }
 
   void reset_cov(State& st) const { for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) st.C[i][j] = i == j ? (Real)T.c0[i] : (Real)0; }

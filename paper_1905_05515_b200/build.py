@@ -2,7 +2,8 @@
 
 Run as `python -m paper_1905_05515_b200.build [--force]`; `__graft_entry__.build()` calls `build()`.
 nvcc cross-compiles without a GPU.  -fmad=false: no FMA contraction anywhere in the library, so every fp32 product is rounded
-before it is added, as the fp32 definition of the decision predicates requires (D-list).
+before it is added, as the fp32 definition of the decision predicates requires (D-list); the fused
+multiply-adds that reading A43 defines for the S5 transport / update are explicit __fmaf_rn calls in csrc/kalman.cuh.
 """
 from __future__ import annotations
 

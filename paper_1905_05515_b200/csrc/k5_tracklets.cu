@@ -5,7 +5,8 @@
 // entries live in registers, fp32.  Phases: A seed fit along the cleaned up-links, B outward extrapolation row by row in the
 // uniform Bz helix with cluster pick-up from the S1 grid, C inward refit + inward extrapolation.  z is carried relative to the
 // start hit (z_rel = z - z_ref, formed in fp32 before use) so that long continuous time frames (|z| up to 2.6e4 cm) keep
-// full fp32 resolution.  Arithmetic is written term by term in the documented order and compiled without FMA contraction,
+// full fp32 resolution.  Arithmetic is written term by term in the documented order and compiled without FMA contraction (the fused multiply-adds of
+// the transport / update are explicit, reading A43),
 // so pick-up decisions agree with the fp32 definition.
 // rowhit layout: [tracklet][row]: a lane writes and re-reads consecutive rows of its own tracklet (L2-resident while the tracklet
 // is alive).  Only rows between the first and the last row a tracklet visits are written; tl_first / tl_last delimit the valid
