@@ -108,7 +108,12 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
   __shared__ float s_sv[7][K5_THREADS];       // state after the outermost update (5 parameters) + that cluster (y, z)
   const UnitDesc* __restrict__ su = units;
   int* __restrict__ rh = rowhit;
-  unsigned n_prop = 0, n_upd = 0, n_pick = 0;
+  // work counters of the current tracklet packed into one register (transports: bits 0-10, updates: 11-21, pick-ups: 22-31; a tracklet
+  // has at most 2 R < 2^9 of each), added to the CTA's shared counters when the tracklet finishes
+  unsigned work = 0;
+  __shared__ unsigned s_work[3];
+  if (threadIdx.x < 3) s_work[threadIdx.x] = 0;
+  __syncthreads();
 
   for (;;) {
     // ---- work queue: lanes without a tracklet take the next start hits (one atomic per warp)
@@ -148,7 +153,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     float2 c_pref = make_float2(0.f, 0.f);
     if (hit_pref >= 0) c_pref = yz[su[rn].off + hit_pref];
     __syncwarp();
-    if (moving) { n_prop++; prop_ok = propagate(st, s_rx[rn] - s_rx[r], P); }
+    if (moving) { work += 1u; prop_ok = propagate(st, s_rx[rn] - s_rx[r], P); }
 
     // ---- 2a. per-phase decision: which measurement this step uses (a linked / assigned hit, a pick-up, or none)
     bool have = false, finish = false, do_pick = false;
@@ -188,7 +193,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     }
     // ---- 2b. cluster pick-up from the grid (phase B and phase C lanes together)
     __syncwarp();
-    if (do_pick) { n_pick++; hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c); }
+    if (do_pick) { work += 1u << 22; hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c); }
     __syncwarp();
     if (do_pick) {
       have = hit >= 0;
@@ -205,7 +210,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     // ---- 3. Kalman update (all lanes that have a measurement, whatever their phase)
     float dchi = 0.0f;
     __syncwarp();
-    if (have) { n_upd++; dchi = update(st, c.x, c.y - zref, P); }
+    if (have) { work += 1u << 11; dchi = update(st, c.x, c.y - zref, P); }
     __syncwarp();
 
     // ---- 4. bookkeeping and phase transitions
@@ -248,17 +253,14 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
       float* __restrict__ oc = tl_cov + (long long)i * 15;
 #pragma unroll
       for (int k = 0; k < 15; k++) oc[k] = s_snap[5 + k][tx];
+      atomicAdd(&s_work[0], work & 0x7ffu); atomicAdd(&s_work[1], (work >> 11) & 0x7ffu); atomicAdd(&s_work[2], work >> 22);
+      work = 0;
       mode = MD_FETCH;
     }
   }
-  // work counters: one atomic per warp
-  for (int d = 16; d > 0; d >>= 1) {
-    n_prop += __shfl_down_sync(FULL, n_prop, d); n_upd += __shfl_down_sync(FULL, n_upd, d); n_pick += __shfl_down_sync(FULL, n_pick, d);
-  }
-  if (lane == 0) {
-    atomicAdd(&counters[0], (unsigned long long)n_prop); atomicAdd(&counters[1], (unsigned long long)n_upd);
-    atomicAdd(&counters[2], (unsigned long long)n_pick);
-  }
+  // work counters: one atomic per CTA and counter (every tracklet has flushed its counts when its lane left the loop)
+  __syncthreads();
+  if (threadIdx.x < 3) atomicAdd(&counters[threadIdx.x], (unsigned long long)s_work[threadIdx.x]);
 }
 
 }  // namespace
