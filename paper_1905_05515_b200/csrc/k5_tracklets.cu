@@ -133,7 +133,8 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
           r0 = u0 - sec * R;
           su = units + (long long)sec * R;
           rh = rowhit + (long long)i * R;
-          zref = yz[su[r0].off + h0].y;
+          const float2 c0 = yz[su[r0].off + h0];   // the start hit: read once, here; INIT takes it from (st.y, zref) and its position from nxt
+          st.y = c0.x; zref = c0.y; nxt = h0;
           mode = MD_INIT;
         } else {
           mode = MD_EXIT;
@@ -160,10 +161,9 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     float2 c = make_float2(0.f, 0.f);
     int hit = -1;
     if (mode == MD_INIT) {
-      hit = start_pos[i];
-      c = yz[su[r0].off + hit];
-      const float2 c0 = c;          // Phase A start: direction from the origin, first update with the start hit
-      const float x = s_rx[r0], y = c0.x;
+      hit = nxt;
+      c = make_float2(st.y, zref);  // Phase A start: direction from the origin, first update with the start hit
+      const float x = s_rx[r0], y = c.x;
       const float rr = sqrtf(x * x + y * y);
       st.y = y; st.z = 0.0f; st.s = y / rr; st.t = P.continuous ? 0.0f : zref / rr; st.q = 0.0f;
       reset_cov(st, P);
