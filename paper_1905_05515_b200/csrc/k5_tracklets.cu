@@ -152,7 +152,8 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     // transport, so its load is issued here and its latency hides behind the transport arithmetic
     const int hit_pref = mode == MD_A ? nxt : (mode == MD_C ? a_next : -1);
     float2 c_pref = make_float2(0.f, 0.f);
-    if (hit_pref >= 0) c_pref = yz[su[rn].off + hit_pref];
+    int nxt_up = -1;   // phase A: the up-link of the linked cluster is read here as well, a whole transport + update ahead of its use
+    if (hit_pref >= 0) { const long long o = su[rn].off + hit_pref; c_pref = yz[o]; if (mode == MD_A) nxt_up = link_up[o]; }
     __syncwarp();
     if (moving) { work += 1u; prop_ok = propagate(st, s_rx[rn] - s_rx[r], P); }
 
@@ -224,7 +225,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     } else if (mode == MD_A) {      // (a failed transport already switched the lane to MD_TRANS)
       r = rn; rh[rn] = hit;
       s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = rn; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y;
-      nxt = link_up[su[rn].off + hit];
+      nxt = nxt_up;
       if (nxt < 0) { gap = 0; mode = rn + 1 < R ? MD_B : MD_TRANS; }
     } else if (mode == MD_B) {
       if (have) { gap = 0; s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = rn; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y; }
