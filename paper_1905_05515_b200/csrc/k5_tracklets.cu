@@ -133,8 +133,10 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
           r0 = u0 - sec * R;
           su = units + (long long)sec * R;
           rh = rowhit + (long long)i * R;
-          const float2 c0 = yz[su[r0].off + h0];   // the start hit: read once, here; INIT takes it from (st.y, zref) and its position from nxt
+          const long long o0 = su[r0].off + h0;
+          const float2 c0 = yz[o0];   // the start hit: read once, here; INIT takes it from (st.y, zref), its position from nxt
           st.y = c0.x; zref = c0.y; nxt = h0;
+          a_next = link_up[o0];       // and its up-link (a_next is free until phase C)
           mode = MD_INIT;
         } else {
           mode = MD_EXIT;
@@ -219,7 +221,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     if (mode == MD_INIT) {
       rh[r0] = hit; r = r0;
       s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = r0; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y;
-      nxt = link_up[su[r0].off + hit];
+      nxt = a_next;
       gap = 0;
       mode = nxt >= 0 ? MD_A : (r0 + 1 < R ? MD_B : MD_TRANS);
     } else if (mode == MD_A) {      // (a failed transport already switched the lane to MD_TRANS)
