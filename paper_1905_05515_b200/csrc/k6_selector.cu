@@ -36,14 +36,14 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const int* _
   const int i = run_list ? run_list[q] : q;   // M entries of a run list (rescue variant), or all tracklets
   const int n = tl_n[i];
   const float chi2 = tl_chi2[i];
+  const int u0 = start_unit[i], r_lo = tl_first[i], r1 = tl_last[i];   // read with n and chi2, not after the decision they feed
   const bool kept = n >= min_hits && isfinite(chi2);
   const unsigned long long key = kept ? make_key(n, chi2, i) : 0ull;
   if (lane == 0) tl_key[i] = key;
   if (!kept) return;
-  const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
+  const UnitDesc* __restrict__ su = units + (long long)(u0 / R) * R;
   const int* __restrict__ rh = rowhit + (long long)i * R;
-  const int r1 = tl_last[i];
-  for (int r = tl_first[i] + lane; r <= r1; r += 32) {
+  for (int r = r_lo + lane; r <= r1; r += 32) {
     const int p = rh[r];
     if (p >= 0) atomicMax(&owner[su[r].off + p], key);
   }
@@ -58,12 +58,12 @@ __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const int R,
   const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
   if (i >= M) return;
   const unsigned long long key = tl_key[i];
+  const int u0 = start_unit[i], r_lo = tl_first[i], r1 = tl_last[i];     // read with the key, not after the decision it feeds
   int owned = 0;
   if (key) {
-    const UnitDesc* __restrict__ su = units + (long long)(start_unit[i] / R) * R;
+    const UnitDesc* __restrict__ su = units + (long long)(u0 / R) * R;
     const int* __restrict__ rh = rowhit + (long long)i * R;
-    const int r1 = tl_last[i];
-    for (int r = tl_first[i] + lane; r <= r1; r += 32) {
+    for (int r = r_lo + lane; r <= r1; r += 32) {
       const int p = rh[r];
       if (p >= 0 && owner[su[r].off + p] == key) owned++;
     }
