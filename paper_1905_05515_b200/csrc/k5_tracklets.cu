@@ -96,7 +96,10 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
   const unsigned FULL = 0xffffffffu;
   const int R = P.R, lane = threadIdx.x & 31;
   int mode = MD_FETCH;
-  int i = -1, r0 = 0, r = 0, nxt = -1, a_next = -1, a_next2 = -1, r_out = 0, gap = 0, n = 0, r_snap = 0, first_assigned = 0;
+  int i = -1, r0 = 0, r = 0, nxt = -1, a_next = -1, a_next2 = -1, r_out = 0;
+  // four small per-tracklet integers (each below 256: tpc_create limits n_rows to 255) in ONE register, so that the row step stays inside
+  // 80 registers: byte 0 = n (updates of phase C), 1 = gap (consecutive rows without a cluster), 2 = first_assigned, 3 = r_snap
+  unsigned pk = 0;
   float zref = 0.0f, chi2 = 0.0f;
   State st = {};
   // per-row x and sector half-width in shared memory (2 x 1 KB): read by every lane at every step
@@ -180,7 +183,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
     } else if (mode == MD_TRANS) {  // Phase C start: state after the outermost update, fresh covariance, refit inward
       st.y = s_sv[0][tx]; st.z = s_sv[1][tx]; st.s = s_sv[2][tx]; st.t = s_sv[3][tx]; st.q = s_sv[4][tx];
       reset_cov(st, P);
-      chi2 = 0.0f; n = 0; first_assigned = r0; gap = 0;
+      chi2 = 0.0f; pk = (pk & 0xff000000u) | ((unsigned)r0 << 16);   // n = 0, gap = 0, first_assigned = r0
       c = make_float2(s_sv[5][tx], s_sv[6][tx]); have = true; r = r_out;
     } else if (mode == MD_C) {
       if (!prop_ok) finish = true;
@@ -189,7 +192,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
         r = rn;
         if (a >= 0) { hit = a; c = c_pref; have = true; }
         else if (fabsf(st.y) > s_re[rn] + P.edge_margin) {
-          if (rn < first_assigned) finish = true;
+          if (rn < (int)((pk >> 16) & 0xffu)) finish = true;
           else if (rn < r0) rh[rn] = -1;       // skipped row inside the tracklet's range: reads as "no cluster"
         } else do_pick = true;
       }
@@ -202,11 +205,12 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
       have = hit >= 0;
       if (mode == MD_B) {
         rh[rn] = hit;
-        if (!have && ++gap > P.max_gap) mode = MD_TRANS;
+        if (!have) { pk += 0x100u; if ((int)((pk >> 8) & 0xffu) > P.max_gap) mode = MD_TRANS; }
       } else {
         if (rn < r0 || have) rh[rn] = hit;
-        if (have) { if (rn < first_assigned) { first_assigned = rn; gap = 0; } }
-        else if (rn < first_assigned && ++gap > P.max_gap) finish = true;
+        const int fa = (int)((pk >> 16) & 0xffu);
+        if (have) { if (rn < fa) pk = (pk & 0xff0000ffu) | ((unsigned)rn << 16); }   // first_assigned = rn, gap = 0
+        else if (rn < fa) { pk += 0x100u; if ((int)((pk >> 8) & 0xffu) > P.max_gap) finish = true; }
       }
     }
 
@@ -222,24 +226,24 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
       rh[r0] = hit; r = r0;
       s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = r0; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y;
       nxt = a_next;
-      gap = 0;
+      pk &= 0xffff00ffu;   // gap = 0
       mode = nxt >= 0 ? MD_A : (r0 + 1 < R ? MD_B : MD_TRANS);
     } else if (mode == MD_A) {      // (a failed transport already switched the lane to MD_TRANS)
       r = rn; rh[rn] = hit;
       s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = rn; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y;
       nxt = nxt_up;
-      if (nxt < 0) { gap = 0; mode = rn + 1 < R ? MD_B : MD_TRANS; }
+      if (nxt < 0) { pk &= 0xffff00ffu; mode = rn + 1 < R ? MD_B : MD_TRANS; }
     } else if (mode == MD_B) {
-      if (have) { gap = 0; s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = rn; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y; }
+      if (have) { pk &= 0xffff00ffu; s_sv[0][tx] = st.y; s_sv[1][tx] = st.z; s_sv[2][tx] = st.s; s_sv[3][tx] = st.t; s_sv[4][tx] = st.q; r_out = rn; s_sv[5][tx] = c.x; s_sv[6][tx] = c.y; }
       if (rn + 1 >= R) mode = MD_TRANS;
     } else if (mode == MD_TRANS) {
       if (have) {                   // (have is false only for lanes that switched to MD_TRANS in step 2 of this iteration)
-        chi2 = chi2 + dchi; n = 1; r_snap = r_out; save_snap = true;
+        chi2 = chi2 + dchi; pk = (pk & 0x00ffff00u) | 1u | ((unsigned)r_out << 24); save_snap = true;   // n = 1, r_snap = r_out
         if (r_out - 1 >= 0) { mode = MD_C; a_next = r_out - 1 >= r0 ? rh[r_out - 1] : -1; a_next2 = r_out - 2 >= r0 ? rh[r_out - 2] : -1; }
         else finish = true;
       }
     } else if (mode == MD_C) {
-      if (have) { chi2 = chi2 + dchi; n++; r_snap = rn; save_snap = true; }
+      if (have) { chi2 = chi2 + dchi; pk = ((pk + 1u) & 0x00ffffffu) | ((unsigned)rn << 24); save_snap = true; }   // n++, r_snap = rn
       if (!finish && rn == 0) finish = true;
       if (!finish) { a_next = a_next2; a_next2 = rn - 2 >= r0 ? rh[rn - 2] : -1; }   // rowhit is read two rows ahead
     }
@@ -250,7 +254,7 @@ __global__ void __launch_bounds__(K5_THREADS, 6) k5_tracklets(const int M, const
           s_snap[15][tx] = st.c40; s_snap[16][tx] = st.c41; s_snap[17][tx] = st.c42; s_snap[18][tx] = st.c43; s_snap[19][tx] = st.c44; }
 
     if (finish) {   // tracklet complete: hits exist exactly on the rows [r_snap, r_out] that carry a non-negative rowhit
-      tl_n[i] = n; tl_first[i] = r_snap; tl_last[i] = r_out; tl_chi2[i] = chi2;
+      tl_n[i] = (int)(pk & 0xffu); tl_first[i] = (int)(pk >> 24); tl_last[i] = r_out; tl_chi2[i] = chi2;
       float* __restrict__ op = tl_par + (long long)i * 5;
       op[0] = s_snap[0][tx]; op[1] = s_snap[1][tx] + zref; op[2] = s_snap[2][tx]; op[3] = s_snap[3][tx]; op[4] = s_snap[4][tx];
       float* __restrict__ oc = tl_cov + (long long)i * 15;
