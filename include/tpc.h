@@ -13,8 +13,8 @@
  *  - All functions return 0 (TPC_OK) or a negative tpc_status; no exception or abort crosses this boundary.
  *    tpc_last_error gives a human-readable message for the last failure on that context.
  *  - "host or device" pointers are classified with cudaPointerGetAttributes.  Input arrays are COPIED (the
- *    caller keeps ownership; host memory may be freed on return, device memory once the context's stream has
- *    reached the copy).  Output arrays are LIBRARY-OWNED and stay valid until the next tpc_find_tracks*,
+ *    caller keeps ownership; host memory -- pageable or pinned -- may be freed or overwritten as soon as the load call
+ *    returns, device memory once the context's stream has reached the copy).  Output arrays are LIBRARY-OWNED and stay valid until the next tpc_find_tracks*,
  *    tpc_clear or tpc_destroy on the same context.
  *  - A context is not thread-safe; different contexts are independent.  All device work of a context is issued
  *    on one CUDA stream (tpc_set_stream; default: the legacy default stream).
@@ -96,8 +96,8 @@ typedef struct {
   float ms_mark;            /* device time of K8 (CUDA events on the context's stream), ms */
 } tpc_cluster_marks;
 
-/* Result of tpc_merge_tracks: S9 of DESIGN.md section 4 ("merging of track segments between
- * sectors"; reading A41): for every track of the last tpc_find_tracks* call the track that continues it in the neighbouring sector and
+/* Result of tpc_merge_tracks: S9 of DESIGN.md section 4 ("Locally, e. g. at the TPC sector
+ * boundaries, there are still some improvements to be done"; the matching rule is this build's reading A41, the paper prints none): for every track of the last tpc_find_tracks* call the track that continues it in the neighbouring sector and
  * the track it continues.  Library-owned, host (device_result = 0) or device memory, valid until the next call on the context. */
 typedef struct {
   int64_t n_tracks;

@@ -19,43 +19,67 @@ _KINDS = {0: (C.c_int32, np.int32), 1: (C.c_int64, np.int64), 2: (C.c_double, np
 STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6, "s7": 7, "s8": 8, "s9": 9}
 
 
+_SO_PLAIN = os.path.join(_HERE, "libtpc_oracle_plain.so")
+
+
+def _flags():
+    hw = []
+    try:
+        with open("/proc/cpuinfo") as f:
+            if " fma " in f.read():
+                hw = ["-mfma"]
+    except OSError:
+        pass
+    return ["g++", "-O2", "-ffp-contract=off"] + hw + ["-std=c++17", "-shared", "-fPIC"]
+
+
 def build(force: bool = False) -> str:
     """g++ -O2 -ffp-contract=off: a product is rounded before it is added unless the source says std::fma (reading A43 of DESIGN.md:
     the S5 transport / update).  -mfma, when the host has the instruction, only makes std::fma the hardware instruction instead of a
-    libm call; the result is the correctly rounded one either way."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        hw = []
-        try:
-            with open("/proc/cpuinfo") as f:
-                if " fma " in f.read():
-                    hw = ["-mfma"]
-        except OSError:
-            pass
-        subprocess.check_call(["g++", "-O2", "-ffp-contract=off"] + hw + ["-std=c++17", "-shared", "-fPIC", _SRC, "-o", _SO])
+    libm call; the result is the correctly rounded one either way.
+    Also builds the test-only second instance (-DS5_PLAIN_ORDER -> libtpc_oracle_plain.so): the S5 transport / update in the
+    operation order of SURVEY.md section 8(c) as first written (own division per entry, no fused multiply-add)."""
+    for so, extra in ((_SO, []), (_SO_PLAIN, ["-DS5_PLAIN_ORDER"])):
+        if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+            subprocess.check_call(_flags() + extra + [_SRC, "-o", so])
     return _SO
 
 
-_lib = None
+def build_sanitized() -> str:
+    """The oracle with -fsanitize=address,undefined as a stand-alone check of its own memory safety (tests/test_oracle_sanitize.py
+    runs it in a subprocess with libasan preloaded)."""
+    so = os.path.join(_HERE, "libtpc_oracle_asan.so")
+    if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+        subprocess.check_call(_flags() + ["-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer", _SRC, "-o", so])
+    return so
 
 
-def _load():
-    global _lib
-    if _lib is None:
-        lib = C.CDLL(build())
+_libs = {}
+
+
+def _load(which: str = "default"):
+    if which not in _libs:
+        build()
+        path = {"default": _SO, "plain": _SO_PLAIN}.get(which, which)     # or an explicit path (sanitized build)
+        lib = C.CDLL(path)
         lib.orc_create.restype = C.c_void_p
         lib.orc_create.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float)] + [C.c_double] * 7
         lib.orc_destroy.argtypes = [C.c_void_p]
         lib.orc_set_param.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
         lib.orc_load.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_float), C.POINTER(C.c_float)]
         lib.orc_run.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        lib.orc_run_range.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         lib.orc_get.argtypes = [C.c_void_p, C.c_char_p, C.POINTER(C.c_void_p), C.POINTER(C.c_int64), C.POINTER(C.c_int)]
         lib.orc_propagate.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
         lib.orc_update.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, C.c_double,
                                    C.POINTER(C.c_double)]
+        lib.orc_pickup.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_int, C.c_int, C.c_double, C.c_int]
+        lib.orc_set_links.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         lib.orc_set_tracklets.argtypes = [C.c_void_p, C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                                           C.POINTER(C.c_double), C.POINTER(C.c_int32)]
-        _lib = lib
-    return _lib
+        assert lib.orc_plain_order() == (1 if which == "plain" else 0) or which not in ("default", "plain")
+        _libs[which] = lib
+    return _libs[which]
 
 
 def _fp(a, ct):
@@ -66,8 +90,9 @@ class Oracle:
     """One oracle context.  `double=False` is the fp32 parity reference, `double=True` the fp64 pin instance."""
 
     def __init__(self, n_sectors, n_rows, row_x, sector_dphi, z_max, t_frame, sigma_y, sigma_z, bz, vdrift,
-                 double=False, **params):
-        self.lib = _load()
+                 double=False, plain_order=False, lib=None, **params):
+        # plain_order: the test-only build with the S5 arithmetic in SURVEY section 8(c)'s first operation order (no fma, own divisions)
+        self.lib = _load(lib if lib else ("plain" if plain_order else "default"))
         self.n_sectors, self.n_rows = int(n_sectors), int(n_rows)
         self.row_x = np.ascontiguousarray(row_x, dtype=np.float32)
         self.h = self.lib.orc_create(int(double), self.n_sectors, self.n_rows, _fp(self.row_x, C.c_float),
@@ -105,6 +130,22 @@ class Oracle:
     def run(self, upto="s6", brute_links=False, brute_pickup=False):
         self.lib.orc_run(self.h, STAGES[upto], int(brute_links) | (int(brute_pickup) << 1))
         return self
+
+    def run_range(self, first, upto, brute_links=False, brute_pickup=False):
+        """Stages first..upto only (earlier ones have run or were set by hand: set_links)."""
+        self.lib.orc_run_range(self.h, STAGES[first], STAGES[upto], int(brute_links) | (int(brute_pickup) << 1))
+        return self
+
+    def set_links(self, up, dn):
+        """Hand-set cleaned link tables (sorted positions in rows r+1 / r-1, -1 none), for hand-built S4 / S5 cases."""
+        up = np.ascontiguousarray(up, dtype=np.int32); dn = np.ascontiguousarray(dn, dtype=np.int32)
+        assert up.shape[0] == dn.shape[0] == self.unit_off[-1]
+        self.lib.orc_set_links(self.h, _fp(up, C.c_int32), _fp(dn, C.c_int32))
+
+    def pickup(self, par, cov, sector, row, zref=0.0, brute=False):
+        """S5 pick-up alone: sorted position of the cluster picked on (sector,row) for the state (par, cov), -1 none (S1 must have run)."""
+        par = np.array(par, dtype=np.float64); cov = np.array(cov, dtype=np.float64)
+        return int(self.lib.orc_pickup(self.h, _fp(par, C.c_double), _fp(cov, C.c_double), int(sector), int(row), float(zref), int(brute)))
 
     def get(self, name):
         p, n, k = C.c_void_p(), C.c_int64(), C.c_int()

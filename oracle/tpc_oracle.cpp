@@ -26,6 +26,13 @@
  *   generator labels of the matched pairs, structural invariants.  Looper-leg identification: not built.
  * S8 (NEXT-4) tube adjacency: independent numpy restatement with the closed-form helix, brute force over the rows, truth labels.
  * S7 (NEXT-1) refit + collision time: noise-free recovery, chi2/ndf = 1, t0 against the generator's collision times.
+ * S5 pick-up (window n_sigma*sqrt(C+sigma^2) capped at w_max, plain squared distance, original-index tie-break) and the Phase B / C
+ *   control flow (max_gap, sector edge + margin, first_assigned, reading A33, ungated Phase A / assigned rows): hand-built cases in
+ *   tests/test_oracle_s5_control.py, each listing the one-line mutations it fails under.  S2 in continuous mode (the benchmarked
+ *   mode): numpy restatement with unequal row pitch, tests/test_oracle_ca.py.
+ * Second, TEST-ONLY fp32 build -DS5_PLAIN_ORDER (reading A44): the S5 arithmetic in SURVEY 8(c)'s first operation order; the margin
+ *   of the parity claim against an independently ordered reference (tests/test_oracle_plain_order.py, tests/test_gpu_parity.py).
+ * The file is also built with -fsanitize=address,undefined and run in tests/test_oracle_sanitize.py.
  * Absolute efficiency / resolution versus the paper: parity unpinned (PAPER.md:49 gives no number).
  */
 #include <cmath>
@@ -64,6 +71,9 @@ struct OracleBase {
   virtual int propagate(double* par, double* cov, double dx) = 0;
   virtual int update(double* par, double* cov, double ym, double zm, double* chi2) = 0;
   virtual int set_tracklets(int64_t n, const int32_t* sector, const int32_t* nh, const double* chi2, const int32_t* rowhit) = 0;
+  virtual int pickup_hook(const double* par, const double* cov, int sector, int row, double zref, int brute) = 0;
+  virtual int set_links(const int32_t* up, const int32_t* dn) = 0;
+  virtual int run_range(int from, int upto, int brute) = 0;
   Tunables T;
   std::string err;
 };
@@ -304,6 +314,69 @@ struct Oracle : OracleBase {
   // ---- S5 building blocks ----
   struct State { Real p[5]; Real C[5][5]; };
 
+#ifdef S5_PLAIN_ORDER
+  // ---- TEST-ONLY second fp32 build (-DS5_PLAIN_ORDER, liboracle "plain"): the S5 transport / update in the operation order of
+  //      SURVEY.md section 8(c) as first written -- every Jacobian entry and every entry of S^-1 with its own division, every
+  //      a + p*q as a rounded product followed by a rounded sum (no std::fma, no shared reciprocal).  Mathematically identical to
+  //      the default build below (readings A42 / A43 only regroup roundings); tests/test_gpu_parity.py::test_parity_against_plain_order_oracle
+  //      checks that the CUDA path also meets the north_star bars against THIS independently ordered reference.
+  bool propagate_state(State& st, Real dx) const {
+    const Real smax = (Real)T.s_max;
+    Real y = st.p[0], zz = st.p[1], s = st.p[2], t = st.p[3], q = st.p[4];
+    Real k = cB * q;
+    Real kdx = k * dx;
+    Real s1 = s + kdx;
+    if (!(std::fabs(s) <= smax) || !(std::fabs(s1) <= smax)) return false;
+    Real c = std::sqrt((Real)1 - s * s), c1 = std::sqrt((Real)1 - s1 * s1);
+    Real cc = c + c1, ss = s + s1, tq = ss / cc;
+    Real g = (Real)1 + tq * tq;
+    Real L = dx * std::sqrt(g);
+    Real h = ((Real)0.5 * k) * L, h2 = h * h;
+    const Real hthr = sizeof(Real) == 4 ? (Real)0.25 : (Real)1e-3;
+    Real S;
+    if (std::fabs(h) < hthr) {   // asin(h)/h = 1 + h^2/6 + 3h^4/40 + 15h^6/336 + 105h^8/3456 + ...
+      Real poly = (Real)(105.0 / 3456.0);
+      poly = (Real)(15.0 / 336.0) + h2 * poly;
+      poly = (Real)(3.0 / 40.0) + h2 * poly;
+      poly = (Real)(1.0 / 6.0) + h2 * poly;
+      poly = (Real)1 + h2 * poly;
+      S = L * poly;
+    } else S = ((Real)2 / k) * std::asin(h);
+    Real dSdk;
+    const Real kthr = sizeof(Real) == 4 ? (Real)1e-2 : (Real)1e-3;
+    if (std::fabs(kdx) >= kthr) dSdk = (dx / c1 - S) / k;
+    else { Real sm = (s + (Real)2 * s1) / (Real)3; Real cm2 = (Real)1 - sm * sm; Real cm = std::sqrt(cm2);
+      dSdk = ((dx * dx) * sm) / ((Real)2 * (cm2 * cm)); }
+    Real cc1 = c * c1;
+    Real F[5][5]; for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) F[i][j] = i == j ? (Real)1 : (Real)0;
+    F[0][2] = ((dx * g) * cc) / ((Real)2 * cc1);
+    F[0][4] = (((dx * dx) * cB) * g) / ((Real)2 * c1);
+    F[1][2] = ((t * dx) * tq) / cc1;
+    F[1][3] = S;
+    F[1][4] = (t * cB) * dSdk;
+    F[2][4] = cB * dx;
+    st.p[0] = y + dx * tq; st.p[1] = zz + t * S; st.p[2] = s1;
+    Real Tm[5][5], Cn[5][5];
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = a + F[i][m] * st.C[m][j]; Tm[i][j] = a; }
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { Real a = 0; for (int m = 0; m < 5; m++) a = a + Tm[i][m] * F[j][m]; Cn[i][j] = a; }
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = Cn[i][j]; st.C[j][i] = Cn[i][j]; }
+    return true;
+  }
+  Real update_state(State& st, Real ym, Real zm) const {
+    const Real ry = (Real)sigma_y * (Real)sigma_y, rz = (Real)sigma_z * (Real)sigma_z;
+    Real s00 = st.C[0][0] + ry, s10 = st.C[1][0], s11 = st.C[1][1] + rz;
+    Real det = s00 * s11 - s10 * s10;
+    Real i00 = s11 / det, i11 = s00 / det, i10 = -s10 / det;
+    Real r0 = ym - st.p[0], r1 = zm - st.p[1];
+    Real K0[5], K1[5];
+    for (int i = 0; i < 5; i++) { K0[i] = st.C[i][0] * i00 + st.C[i][1] * i10; K1[i] = st.C[i][0] * i10 + st.C[i][1] * i11; }
+    Real Cn[5][5];
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) Cn[i][j] = st.C[i][j] - (K0[i] * st.C[0][j] + K1[i] * st.C[1][j]);
+    for (int i = 0; i < 5; i++) st.p[i] = st.p[i] + (K0[i] * r0 + K1[i] * r1);
+    for (int i = 0; i < 5; i++) for (int j = 0; j <= i; j++) { st.C[i][j] = Cn[i][j]; st.C[j][i] = Cn[i][j]; }
+    return r0 * (i00 * r0 + i10 * r1) + r1 * (i10 * r0 + i11 * r1);
+  }
+#else
   // propagate the state from its x to x+dx on the helix in uniform Bz; false = |sin(phi)| leaves [-s_max, s_max]
   bool propagate_state(State& st, Real dx) const {
     const Real smax = (Real)T.s_max;
@@ -367,6 +440,8 @@ struct Oracle : OracleBase {
     Real u0 = std::fma(i10, r1, i00 * r0), u1 = std::fma(i11, r1, i10 * r0);
     return std::fma(r1, u1, r0 * u0);
   }
+
+#endif   // S5_PLAIN_ORDER
 
   void reset_cov(State& st) const { for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) st.C[i][j] = i == j ? (Real)T.c0[i] : (Real)0; }
 
@@ -600,8 +675,8 @@ struct Oracle : OracleBase {
       }
   }
 
-  // ---- S9 (NEXT-3; "merging of track segments between sectors" in the list of later
-  //      additions; reading A41): a track that leaves its sector through the side edge continues in the neighbouring sector of
+  // ---- S9 (NEXT-3; PAPER.md:49 says only "Locally, e. g. at the TPC sector boundaries, there are still some improvements to be done"; matching segments across the boundary is this build's reading A41 of that sentence, not a rule the paper prints;
+  //      reading A41): a track that leaves its sector through the side edge continues in the neighbouring sector of
   //      the same side as a separate S6 track.  Outer state of A = its S6 state transported (parameters only) to the row of its
   //      last cluster.  A is a leaver iff |y_out| >= yedge - merge_edge; the neighbour is the next sector in phi for y_out > 0,
   //      the previous one for y_out < 0.  The outer state is rotated into the neighbour's frame (x' = x c + y s, y' = -x s + y c,
@@ -611,6 +686,9 @@ struct Oracle : OracleBase {
   //      index), B accepts its best proposer: next[A] = B, prev[B] = A (-1 elsewhere).
   void s9_merge() {
     const int64_t NT = (int64_t)trk_sector.size();
+    // sectors per closed ring in phi (18 for 20 degree sectors), one ring per side; 0 when the sectors do not close a ring
+    int ring = (int)std::lround(2.0 * M_PI / dphi);
+    if (ring < 2 || std::fabs(ring * dphi - 2.0 * M_PI) > 1e-3 || NS % ring != 0) ring = 0;
     mg_next.assign(NT, -1); mg_prev.assign(NT, -1); mg_leaver.assign(NT, 0); mg_outer.assign(NT * 4, 0);
     std::vector<int> r_in(NT), r_out(NT); std::vector<State> outer(NT);
     for (int64_t i = 0; i < NT; i++) {
@@ -623,7 +701,7 @@ struct Oracle : OracleBase {
       outer[i] = st;
       if (!ok) continue;
       mg_outer[i * 4 + 0] = (double)X[r_out[i]]; mg_outer[i * 4 + 1] = (double)st.p[0]; mg_outer[i * 4 + 2] = (double)st.p[1]; mg_outer[i * 4 + 3] = (double)st.p[2];
-      if (NS < 36) continue;
+      if (ring == 0) continue;
       const Real ya = std::fabs(st.p[0]);
       if (ya >= yedge[r_out[i]] - (Real)T.merge_edge) mg_leaver[i] = st.p[0] > 0 ? 1 : -1;
     }
@@ -632,8 +710,8 @@ struct Oracle : OracleBase {
     std::vector<int32_t> bestB(NT, -1); std::vector<Real> bestS(NT, (Real)0);
     for (int64_t a = 0; a < NT; a++) {
       if (!mg_leaver[a]) continue;
-      const int sec = trk_sector[a], side = sec / 18, k = sec % 18;
-      const int nb = side * 18 + (k + (mg_leaver[a] > 0 ? 1 : 17)) % 18;
+      const int sec = trk_sector[a], side = sec / ring, k = sec % ring;
+      const int nb = side * ring + (k + (mg_leaver[a] > 0 ? 1 : ring - 1)) % ring;
       const Real sgn = mg_leaver[a] > 0 ? (Real)1 : (Real)-1;
       const State& o = outer[a];
       const Real x = X[r_out[a]], y = o.p[0], s = o.p[2], c = std::sqrt((Real)1 - s * s);
@@ -662,19 +740,34 @@ struct Oracle : OracleBase {
     for (int64_t b = 0; b < NT; b++) if (bestA[b] >= 0) { mg_next[bestA[b]] = (int32_t)b; mg_prev[b] = bestA[b]; }
   }
 
-  int run(int upto, int brute) override {
+  int run(int upto, int brute) override { return run_range(0, upto, brute); }
+  // stages from..upto (the earlier ones must have run, or been set by hand: set_links); test hook for hand-built cases
+  int run_range(int from, int upto, int brute) override {
     make_tables();
-    s0_time_to_z(); if (upto <= 0) return 0;
-    s1_grid(); if (upto <= 1) return 0;
-    s2_neighbours(brute & 1); if (upto <= 2) return 0;
-    s3_clean(); if (upto <= 3) return 0;
-    s4_start_hits((brute & 1) != 0); if (upto <= 4) return 0;
-    s5_tracklets((brute & 2) != 0); if (upto <= 5) return 0;
-    s6_select(); if (upto <= 6) return 0;
-    s7_refit(); if (upto <= 7) return 0;
-    s8_adjacent((brute & 2) != 0); if (upto <= 8) return 0;
-    s9_merge();
+    for (int st = from; st <= upto; st++) {
+      switch (st) {
+        case 0: s0_time_to_z(); break;
+        case 1: s1_grid(); break;
+        case 2: s2_neighbours(brute & 1); break;
+        case 3: s3_clean(); break;
+        case 4: s4_start_hits((brute & 1) != 0); break;
+        case 5: s5_tracklets((brute & 2) != 0); break;
+        case 6: s6_select(); break;
+        case 7: s7_refit(); break;
+        case 8: s8_adjacent((brute & 2) != 0); break;
+        case 9: s9_merge(); break;
+        default: break;
+      }
+    }
     return 0;
+  }
+
+  // test hooks: the S5 pick-up alone on a hand-given state (S1 must have run), and hand-set cleaned link tables (sorted positions)
+  int pickup_hook(const double* par, const double* cov, int sector, int row, double zref, int brute) override {
+    make_tables(); State st; to_state(st, par, cov); return pickup(sector, row, st, (Real)zref, brute != 0);
+  }
+  int set_links(const int32_t* up, const int32_t* dn) override {
+    clean_up.assign(up, up + N); clean_dn.assign(dn, dn + N); link_up = clean_up; link_dn = clean_dn; return 0;
   }
 
   // hand-built tracklets for S6 pins (requires S1 to have run so that perm/off exist)
@@ -789,6 +882,17 @@ int orc_run(void* h, int upto, int brute) { return ((OracleBase*)h)->run(upto, b
 int orc_get(void* h, const char* name, const void** p, int64_t* n, int* kind) { return ((OracleBase*)h)->get(name, p, n, kind); }
 int orc_propagate(void* h, double* par, double* cov, double dx) { return ((OracleBase*)h)->propagate(par, cov, dx); }
 int orc_update(void* h, double* par, double* cov, double ym, double zm, double* chi2) { return ((OracleBase*)h)->update(par, cov, ym, zm, chi2); }
+int orc_pickup(void* h, const double* par, const double* cov, int sector, int row, double zref, int brute) {
+  return ((OracleBase*)h)->pickup_hook(par, cov, sector, row, zref, brute); }
+int orc_set_links(void* h, const int32_t* up, const int32_t* dn) { return ((OracleBase*)h)->set_links(up, dn); }
+int orc_run_range(void* h, int from, int upto, int brute) { return ((OracleBase*)h)->run_range(from, upto, brute); }
+int orc_plain_order(void) {
+#ifdef S5_PLAIN_ORDER
+  return 1;
+#else
+  return 0;
+#endif
+}
 int orc_set_tracklets(void* h, int64_t n, const int32_t* sector, const int32_t* nh, const double* chi2, const int32_t* rowhit) {
   return ((OracleBase*)h)->set_tracklets(n, sector, nh, chi2, rowhit); }
 }

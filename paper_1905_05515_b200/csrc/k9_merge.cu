@@ -1,5 +1,6 @@
-// k9_merge.cu -- K9: S9 cross-sector segment matching (NEXT-3 of SURVEY.md section 8(f); "merging of track segments
-// between sectors" in the list of additions; reading A41 of DESIGN.md).  Looper-leg identification is not part of it.
+// k9_merge.cu -- K9: S9 cross-sector segment matching (NEXT-3 of SURVEY.md section 8(f); PAPER.md:49 says only "Locally, e. g. at the
+// TPC sector boundaries, there are still some improvements to be done"; matching segments across the boundary is this build's
+// reading A41 of DESIGN.md).  Looper-leg identification is not part of it.
 //
 //   k9_ranges  : first track of every sector (the S6 tracks are in ascending sector order) by binary search
 //   k9_outer   : one lane per track: S6 state transported (parameters only) to the row of the track's last cluster; a track
@@ -45,7 +46,7 @@ __global__ void __launch_bounds__(K9_THREADS) k9_outer(const long long n_tracks,
   int lv = 0;
   if (ok) {
     o[0] = rows[r1].x; o[1] = st.y; o[2] = st.z; o[3] = st.s;
-    if (P.NS >= 36 && fabsf(st.y) >= rows[r1].yedge - M.edge) lv = st.y > 0.0f ? 1 : -1;
+    if (M.per_side > 0 && fabsf(st.y) >= rows[r1].yedge - M.edge) lv = st.y > 0.0f ? 1 : -1;
   } else {
     o[0] = o[1] = o[2] = o[3] = 0.0f;
   }
@@ -62,8 +63,9 @@ __global__ void __launch_bounds__(K9_THREADS) k9_propose(const long long n_track
   if (a >= n_tracks) return;
   const int lv = leaver[a];
   if (!lv) return;
-  const int sec = o_sector[a], side = sec / 18, k = sec % 18;
-  const int nb = side * 18 + (k + (lv > 0 ? 1 : 17)) % 18;
+  // sectors form closed rings of per_side sectors (one ring per side); the neighbour stays on the ring, hence below NS
+  const int sec = o_sector[a], side = sec / M.per_side, k = sec % M.per_side;
+  const int nb = side * M.per_side + (k + (lv > 0 ? 1 : M.per_side - 1)) % M.per_side;
   const float sgn = lv > 0 ? 1.0f : -1.0f;
   const float* __restrict__ o = outer + a * 4;
   const float x = o[0], y = o[1], s = o[3], c = sqrtf(1.0f - s * s);

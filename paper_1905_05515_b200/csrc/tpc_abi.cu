@@ -149,6 +149,7 @@ struct tpc_ctx {
   std::vector<int32_t> dbg_tl_sector, dbg_tl_row, dbg_tl_n, dbg_tl_first, dbg_tl_last, dbg_rowhit; std::vector<float> dbg_tl_chi2, dbg_tl_x, dbg_tl_par, dbg_tl_cov;
 
   cudaEvent_t ev[10] = {};
+  cudaEvent_t ev_load = nullptr;   // end of a direct H2D copy from the caller's pinned memory (stage_append)
   tpc_timings timings = {};
 };
 
@@ -225,6 +226,9 @@ int tpc_create(const tpc_geometry* g, float bz, float vdrift, tpc_ctx** out) {
   for (auto& ev : c->ev) {
     if (cudaEventCreate(&ev) != cudaSuccess) { int rc = fail(nullptr, TPC_E_CUDA, "tpc_create: cudaEventCreate failed"); delete c; return rc; }
   }
+  if (cudaEventCreateWithFlags(&c->ev_load, cudaEventDisableTiming) != cudaSuccess) {
+    int rc = fail(nullptr, TPC_E_CUDA, "tpc_create: cudaEventCreate failed"); tpc_destroy(c); return rc;
+  }
   *out = c;
   return TPC_OK;
 }
@@ -247,6 +251,7 @@ void tpc_destroy(tpc_ctx* c) {
   c->hr_n.release(); c->hr_ndf.release(); c->hr_x.release(); c->hr_par.release(); c->hr_cov.release(); c->hr_chi2.release();
   c->hr_z0.release(); c->hr_t0.release(); c->hm_status.release(); c->hm_track.release(); c->hg_next.release(); c->hg_prev.release();
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
+  if (c->ev_load) cudaEventDestroy(c->ev_load);
   delete c;
 }
 
@@ -314,6 +319,11 @@ static int stage_append(tpc_ctx* c, const float* y, const float* t, long long n,
     CUDA_TRY(c, c->d_in_t.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_in_y.as<float>() + pos, y, bytes, kind, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_in_t.as<float>() + pos, t, bytes, kind, c->stream));
+    if (ky != 2) {   // the DMA reads the caller's pinned host memory: it must have finished when the call returns (tpc.h: host
+                     // inputs may be freed or overwritten on return); a device source follows stream order instead
+      CUDA_TRY(c, cudaEventRecord(c->ev_load, c->stream));
+      CUDA_TRY(c, cudaEventSynchronize(c->ev_load));
+    }
   } else {        // pageable (or small) host source: copy into the pinned arena now, upload at tpc_find_tracks
     CUDA_TRY(c, c->h_y.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4));
     CUDA_TRY(c, c->h_t.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4));
@@ -766,8 +776,13 @@ int tpc_merge_tracks(tpc_ctx* c, int device_result, tpc_merges* out) {
   CUDA_TRY(c, c->g_leaver.ensure(ntz * 4)); CUDA_TRY(c, c->g_sec_begin.ensure((size_t)(c->NS + 2) * 4)); CUDA_TRY(c, c->g_cand.ensure(ntz * 8));
   CUDA_TRY(c, c->g_next.ensure(ntz * 4)); CUDA_TRY(c, c->g_prev.ensure(ntz * 4));
   const Tunables& T = c->T;
+  // sectors per ring: 2 pi / dphi when that is an integer (to 1e-3 rad over the ring) and n_sectors is a whole number of rings
+  // (one per side); otherwise the geometry has no neighbouring sectors and nothing is merged
+  const double ring = 2.0 * M_PI / (double)c->dphi;
+  int per_side = (int)lround(ring);
+  if (per_side < 2 || fabs((double)per_side * (double)c->dphi - 2.0 * M_PI) > 1e-3 || c->NS % per_side != 0) per_side = 0;
   K9Params M{(float)T.merge_edge, (float)T.merge_dy, (float)T.merge_dz, (float)T.merge_ds, (float)T.merge_dt,
-             (float)cos((double)c->dphi), (float)sin((double)c->dphi), T.merge_rows};
+             (float)cos((double)c->dphi), (float)sin((double)c->dphi), T.merge_rows, per_side};
   long long launches = 0;
   CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
   LAUNCH_TRY(c, launch_k9_merge(L, nt, c->NS, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_par.as<float>(), c->o_cl_begin.as<long long>(),

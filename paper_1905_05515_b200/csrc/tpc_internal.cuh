@@ -44,7 +44,8 @@ struct Params {
 };
 
 // S9 (NEXT-3) matching parameters (reading A41), rounded to float once on the host
-struct K9Params { float edge, dy, dz, ds, dt, cd, sd; int rows; };
+struct K9Params { float edge, dy, dz, ds, dt, cd, sd; int rows;
+                  int per_side; };   // sectors per closed ring in phi (18 for 20 degree sectors); 0 = the sectors do not close a ring: nothing to merge
 
 // Work item of K2/K3: a chunk of consecutive sorted hits of one unit.
 struct Item { int unit; int start; };

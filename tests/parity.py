@@ -82,17 +82,30 @@ def track_sets(tr) -> dict:
     return d
 
 
+_DCOV = np.array([0, 2, 5, 9, 14])
+_TRI = [(a, b) for a in range(5) for b in range(a + 1)]
+
+
+def _cov_ratio(co, cg, rel=1e-4) -> float:
+    """Largest |dC_ab| / (rel * sqrt(C_aa C_bb)) over the 15 lower-triangle entries (scale-aware: off-diagonals pass through 0)."""
+    co = np.asarray(co, dtype=np.float64); cg = np.asarray(cg, dtype=np.float64)
+    dg = np.sqrt(np.abs(co[_DCOV]))
+    scale = np.array([dg[a] * dg[b] for a, b in _TRI])
+    return float(np.max(np.abs(co - cg) / (rel * scale + 1e-300)))
+
+
 def compare_tracks(otr, gtr, rel=1e-4, sig=1e-3) -> dict:
-    """Reading A31/A19: pair tracks by (sector, exact cluster set); parameters within rel*|oracle| or sig*sqrt(C_ii)."""
+    """Reading A31/A19: pair tracks by (sector, exact cluster set); parameters within rel*|oracle| or sig*sqrt(C_ii); the 15
+    covariance entries within rel * sqrt(C_aa C_bb); chi2 within 1e-3 relative; ndf and x equal.
+    Also reports how many pairs are bit-identical in every number (parameters, covariance, chi2)."""
     so, sg = track_sets(otr), track_sets(gtr)
     common = [k for k in so if k in sg]
-    n_bad = 0
-    worst = 0.0
-    dcov = np.array([0, 2, 5, 9, 14])
+    n_bad = n_cov_bad = n_exact = 0
+    worst = worst_cov = 0.0
     for k in common:
         i, j = so[k], sg[k]
         po, pg = otr["par"][i].astype(np.float64), np.asarray(gtr["par"][j], dtype=np.float64)
-        so_ = np.sqrt(np.abs(otr["cov"][i][dcov].astype(np.float64)))
+        so_ = np.sqrt(np.abs(otr["cov"][i][_DCOV].astype(np.float64)))
         d = np.abs(po - pg)
         ok = (d <= rel * np.abs(po)) | (d <= sig * so_)
         worst = max(worst, float(np.max(d / np.maximum(rel * np.abs(po), sig * so_ + 1e-300))))
@@ -100,8 +113,33 @@ def compare_tracks(otr, gtr, rel=1e-4, sig=1e-3) -> dict:
         if not ok.all() or abs(c2o - c2g) > 1e-3 * max(1.0, abs(c2o)) or int(otr["ndf"][i]) != int(gtr["ndf"][j]) or \
                 float(otr["x"][i]) != float(gtr["x"][j]):
             n_bad += 1
+        rc = _cov_ratio(otr["cov"][i], gtr["cov"][j], rel)
+        worst_cov = max(worst_cov, rc)
+        n_cov_bad += rc > 1.0
+        n_exact += bool(np.array_equal(otr["par"][i].astype(np.float32), np.asarray(gtr["par"][j], dtype=np.float32)) and
+                        np.array_equal(otr["cov"][i].astype(np.float32), np.asarray(gtr["cov"][j], dtype=np.float32)) and
+                        np.float32(c2o) == np.float32(c2g))
     return dict(n_oracle=len(so), n_gpu=len(sg), identical_sets=len(common), frac_identical=len(common) / max(1, len(so)),
-                param_mismatch=n_bad, worst_ratio=worst)
+                param_mismatch=n_bad, worst_ratio=worst, cov_mismatch=int(n_cov_bad), worst_cov_ratio=worst_cov, bit_identical=n_exact)
+
+
+def compare_tracklets(o, tl) -> dict:
+    """S5 output before selection, tracklet by tracklet (same index = same start hit): n, first, last and the rowhit table must be
+    equal; chi2, the 5 parameters and the 15 covariance entries of tracklets with n >= 1 are compared bit for bit (both sides
+    spell the same fp32 operation order)."""
+    ot = o.tracklets()
+    M = len(ot["n"])
+    assert len(tl["n"]) == M, (len(tl["n"]), M)
+    fitted = ot["first"] >= 0
+    out = dict(n_tracklets=M)
+    out["n_diff"] = int((ot["n"] != tl["n"]).sum())
+    out["range_diff"] = int(((ot["first"] != tl["first"]) | (ot["last"] != tl["last"]))[fitted].sum())
+    out["rowhit_diff"] = int((ot["rowhit"] != tl["rowhit"]).any(axis=1).sum())
+    f32 = np.float32
+    out["chi2_diff"] = int((ot["chi2"].astype(f32) != tl["chi2"].astype(f32))[fitted & np.isfinite(ot["chi2"])].sum())
+    out["par_diff"] = int((ot["par"].astype(f32) != tl["par"].astype(f32)).any(axis=1)[fitted].sum())
+    out["cov_diff"] = int((ot["cov"].astype(f32) != tl["cov"].astype(f32)).any(axis=1)[fitted].sum())
+    return out
 
 
 def compare_refit(otr, orf, gtr, grf, rel=1e-4, sig=1e-3) -> dict:
@@ -110,7 +148,7 @@ def compare_refit(otr, orf, gtr, grf, rel=1e-4, sig=1e-3) -> dict:
     so, sg = track_sets(otr), track_sets(gtr)
     common = [k for k in so if k in sg]
     n_bad = 0
-    dcov = np.array([0, 2, 5, 9, 14])
+    dcov = _DCOV
     for k in common:
         i, j = so[k], sg[k]
         po, pg = orf["par"][i].astype(np.float64), np.asarray(grf["par"][j], dtype=np.float64)
@@ -119,6 +157,7 @@ def compare_refit(otr, orf, gtr, grf, rel=1e-4, sig=1e-3) -> dict:
         ok = bool(((d <= rel * np.abs(po)) | (d <= sig * so_)).all())
         ok &= int(orf["n"][i]) == int(grf["n"][j]) and int(orf["ndf"][i]) == int(grf["ndf"][j]) and float(orf["x"][i]) == float(grf["x"][j])
         ok &= abs(float(orf["chi2"][i]) - float(grf["chi2"][j])) <= 1e-3 * max(1.0, abs(float(orf["chi2"][i])))
+        ok &= _cov_ratio(orf["cov"][i], grf["cov"][j], rel) <= 1.0
         for name in ("z0", "t0"):
             a, b = float(orf[name][i]), float(grf[name][j])
             ok &= abs(a - b) <= max(rel * abs(a), sig * so_[1] * 10.0)   # z0 adds (dz/ds error) x (arc ~ 1 m) to the z error

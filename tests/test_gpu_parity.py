@@ -19,7 +19,25 @@ def _tracker(w, **params):
     return T.Tracker(**P.abi_geometry(w), **params)
 
 
-def _full_parity(w, grid_units=None, per_unit=False, **params):
+def _assert_track_bars(res):
+    """north_star bars (>= 99.9 % identical cluster sets, parameters within 1e-4 / 1e-3 sigma) AND what is measured on B200
+    against the default oracle build, which spells the same fp32 operation order as csrc/kalman.cuh: every
+    oracle track has a GPU partner with the identical cluster set, no extra GPU track, and parameters, covariance and chi2 of every
+    pair are bit-identical.  No flip is legitimate here (no libm call is reached, sqrt / div / fma are IEEE on both sides), so the
+    bar is 0, not a fraction."""
+    assert res["frac_identical"] >= 0.999, res
+    assert res["identical_sets"] == res["n_oracle"] == res["n_gpu"], res
+    assert res["param_mismatch"] == 0 and res["cov_mismatch"] == 0, res
+    assert res["bit_identical"] == res["identical_sets"], res
+
+
+def _assert_tracklets_equal(o, trk):
+    d = P.compare_tracklets(o, trk.tracklets())
+    assert d["n_tracklets"] > 0 and all(v == 0 for k, v in d.items() if k != "n_tracklets"), d
+    return d
+
+
+def _full_parity(w, grid_units=None, per_unit=False, tracklets=False, **params):
     o = P.make_oracle(w, **params).run("s6")
     with _tracker(w, debug_keep=1, **params) as trk:
         trk.load_workload(w, per_unit=per_unit)
@@ -27,20 +45,20 @@ def _full_parity(w, grid_units=None, per_unit=False, **params):
         ng = P.compare_grid(w, o, trk, grid_units)
         lk = P.compare_links(w, o, trk)
         tm = trk.timings()
+        if tracklets:                   # S5 output before the selector, tracklet by tracklet
+            _assert_tracklets_equal(o, trk)
     assert ng > 0
     assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
     otr = o.tracks()
     res = P.compare_tracks(otr, gtr)
-    assert res["frac_identical"] >= 0.999, res
-    assert res["n_gpu"] - res["identical_sets"] <= max(1, 0.001 * res["n_oracle"]), res
-    assert res["param_mismatch"] <= 0.001 * res["n_oracle"], res
-    assert tm["n_clusters"] == w.n_clusters and tm["n_start_hits"] == lk["n_start"] and tm["launches"] >= 10
+    _assert_track_bars(res)
+    assert tm["n_clusters"] == w.n_clusters and tm["n_start_hits"] == lk["n_start"] and tm["launches"] >= 8
     return o, otr, gtr, res
 
 
 def test_c1_full_parity_and_truth():
     w = W.config(1)
-    o, otr, gtr, res = _full_parity(w)
+    o, otr, gtr, res = _full_parity(w, tracklets=True)
     mo, mg = H.truth_metrics(w, otr), H.truth_metrics(w, gtr)
     assert abs(mo["eff"] - mg["eff"]) <= 1e-3 and abs(mo["fake_rate"] - mg["fake_rate"]) <= 1e-3
     assert mg["eff"] > 0.95
@@ -55,7 +73,7 @@ def test_c2_full_parity():
     w = W.config(2)
     rng = np.random.default_rng(0)
     units = rng.choice(w.n_sectors * w.n_rows, 300, replace=False)
-    o, otr, gtr, res = _full_parity(w, grid_units=units)
+    o, otr, gtr, res = _full_parity(w, grid_units=units, tracklets=True)
     mo, mg = H.truth_metrics(w, otr), H.truth_metrics(w, gtr)
     assert abs(mo["eff"] - mg["eff"]) <= 1e-3 and abs(mo["fake_rate"] - mg["fake_rate"]) <= 1e-3
 
@@ -63,7 +81,31 @@ def test_c2_full_parity():
 def test_c3_scaled_continuous_parity():
     w = W.config(3, scale=0.1)     # 200 us frame, ~1.2 M clusters, z down to -516 cm
     rng = np.random.default_rng(1)
-    _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, 200, replace=False))
+    _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, 200, replace=False), tracklets=True)
+
+
+def test_parity_against_plain_order_oracle():
+    """The CUDA path against the SECOND, test-only fp32 build of the oracle (-DS5_PLAIN_ORDER: the S5 transport / update in the
+    operation order SURVEY.md section 8(c) first wrote -- own division per Jacobian entry, no fused multiply-add, i.e. before
+    readings A42 / A43 regrouped the roundings).  This is the margin of the parity claim against an independently ordered
+    reference (reading A44).  Bars: S0-S4 tables do not depend on the S5 order (bit-exact as always); >= 99.9 % of the
+    oracle's tracks have a GPU partner with the identical cluster set (north_star); parameters of pairs: fp32 roundings of a
+    150-step filter with a prior variance of 100 on q/pT move q/pT by up to a few 0.1 sigma, for ANY two fp32 orders (both
+    builds differ from the fp64 instance by the same amount, tests/test_oracle_plain_order.py), so the bar that arithmetic
+    supports is: >= 95 % of the pairs within north_star's 1e-4 relative / 1e-3 sigma, every pair within 1 sigma (1000 x).  The
+    measured worst ratio and fractions are printed."""
+    for name, w in (("C1", W.config(1)), ("C2", W.config(2)), ("C3@0.1", W.config(3, scale=0.1))):
+        o = P.make_oracle(w, plain_order=True).run("s6")
+        with _tracker(w, debug_keep=1) as trk:
+            trk.load_workload(w)
+            gtr = trk.find_tracks().copy().as_dict()
+            lk = P.compare_links(w, o, trk)
+        assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
+        res = P.compare_tracks(o.tracks(), gtr)
+        print(f"plain-order oracle vs CUDA, {name}: {res}")
+        assert res["frac_identical"] >= 0.999, res
+        assert res["n_gpu"] - res["identical_sets"] <= max(1, 0.001 * res["n_oracle"]), res
+        assert res["param_mismatch"] <= 0.05 * res["identical_sets"] and res["worst_ratio"] <= 1000.0, res
 
 
 def test_c4_loopers_parity():
@@ -84,7 +126,7 @@ def _refit_parity(w):
             assert np.array_equal(dev[k].cpu().numpy(), grf[k], equal_nan=True), k
     assert grf["n_tracks"] == len(gtr["sector"]) and grf["ms_refit"] > 0
     res = P.compare_refit(otr, orf, gtr, grf)
-    assert res["n_common"] > 50 and res["n_common"] >= 0.999 * len(otr["sector"]) and res["mismatch"] <= 0.001 * res["n_common"], res
+    assert res["n_common"] > 50 and res["n_common"] == len(otr["sector"]) and res["mismatch"] == 0, res    # measured: 0 (same fp32 order)
     return w, gtr, grf
 
 
@@ -127,7 +169,7 @@ def _marks_parity(w):
         np.array_equal(otr["cl_index"], gtr["cl_index"]) and np.array_equal(otr["cl_row"], gtr["cl_row"])
     assert same_lists
     diff = int(((st != ost) | (tk != otk)).sum())
-    assert diff <= 1e-4 * w.n_clusters, diff         # a tube boundary decided in the last fp32 bit of a transported state
+    assert diff == 0, diff         # identical tracks + the same fp32 transport on both sides: no tube boundary can flip
     return st, tk, ost
 
 
@@ -169,7 +211,7 @@ def test_cross_sector_merges_parity_c2_and_c3_scaled():
         n_m = int((om["next"] >= 0).sum())
         assert n_m > 500
         diff = int((nx != om["next"]).sum() + (pv != om["prev"]).sum())
-        assert diff <= 2e-3 * n_m, (diff, n_m)          # a window edge decided in the last fp32 bit of a transported state
+        assert diff == 0, (diff, n_m)          # identical tracks + the same fp32 transport on both sides: no window edge can flip
         labs = H.track_labels(w, gtr)
         pairs = [(a, int(b)) for a, b in enumerate(nx) if b >= 0]
         assert sum(1 for a, b in pairs if labs[a][0] != labs[b][0]) <= 0.005 * len(pairs)
@@ -250,7 +292,7 @@ def test_seed_bridging_rescue_variant_parity():
         assert np.array_equal(tl["first"] >= 0, ofit)                     # the same tracklets were fitted
         assert tm["n_start_hits"] == len(ofit) and tm["n_tracklets_kept"] == int(ofit.sum()) <= 0.6 * len(ofit)
         res = P.compare_tracks(o.tracks(), gtr)
-        assert res["frac_identical"] >= 0.999 and res["param_mismatch"] <= 0.001 * res["n_oracle"], res
+        _assert_track_bars(res)
         base = P.make_oracle(w).run("s6")
         m0, m1 = H.truth_metrics(w, base.tracks()), H.truth_metrics(w, gtr)
         assert m1["eff"] >= m0["eff"] - 0.001, (m0["eff"], m1["eff"])
@@ -284,6 +326,24 @@ def test_device_inputs_and_device_outputs_match_host_path():
         dev = trk.find_tracks_device()
         for k, v in dev.as_dict().items():
             assert np.array_equal(v.cpu().numpy(), host[k]), k
+
+
+def test_pinned_host_source_may_be_overwritten_on_return():
+    """include/tpc.h: input arrays are copied; host memory may be freed or overwritten as soon as the load call returns.  A large
+    pinned source takes the direct-DMA path of the loader (no staging copy): the call must not return before the DMA has read it."""
+    import torch
+    w = W.config(2)
+    assert w.n_clusters >= (1 << 16)
+    with _tracker(w) as trk:
+        trk.load_workload(w)
+        ref = trk.find_tracks().copy().as_dict()
+    y_h, t_h = torch.from_numpy(w.y.copy()).pin_memory(), torch.from_numpy(w.t.copy()).pin_memory()
+    with _tracker(w) as trk:
+        trk.load_batch(w.unit_off, y_h, t_h)
+        y_h.fill_(float("nan")); t_h.fill_(-1.0)          # the caller reuses its ring buffer right away
+        got = trk.find_tracks().as_dict()
+        for k in ref:
+            assert np.array_equal(ref[k], got[k]), k
 
 
 def test_c3_full_size_parity():
@@ -325,33 +385,36 @@ def test_c5_scaled_large_frame_invariants():
 def test_c5_full_size_sampled_sector_parity():
     """BASELINE.json configs[4] at full size (10 ms frame, ~84 M clusters, 15 k clusters per unit: the largest K1 plan, the longest
     z range).  Sectors are independent, so the oracle run on ONE sector alone is the oracle's answer for that sector of the
-    whole frame: grid tables, link tables, start list and tracks of sector 11 compared as in the full parity tests."""
+    whole frame: grid tables, link tables and tracks of four sectors spread over both sides (2, 11 on side A; 20, 31 on side C)
+    compared as in the full parity tests."""
     w = W.config(5)
     assert w.n_clusters > 70e6
-    sec = 11
-    ws = w.sector_slice([sec])
-    o = P.make_oracle(ws).run("s6")
-    otr = o.tracks()
     R = w.n_rows
     with _tracker(w, debug_keep=1) as trk:
         trk.load_workload(w)
         r = trk.find_tracks()
-        sel = np.nonzero(r.sector == sec)[0]
-        assert len(sel) > 10000 and np.all(np.diff(sel) == 1)
-        a, b = int(sel[0]), int(sel[-1]) + 1
-        cb = r.cl_begin[a:b + 1]
-        gtr = dict(sector=r.sector[a:b].copy(), x=r.x[a:b].copy(), par=r.par[a:b].copy(), cov=r.cov[a:b].copy(), chi2=r.chi2[a:b].copy(),
-                   ndf=r.ndf[a:b].copy(), cl_begin=(cb - cb[0]).copy(), cl_row=r.cl_row[cb[0]:cb[-1]].copy(),
-                   cl_index=r.cl_index[cb[0]:cb[-1]].copy())
-        units = range(sec * R, (sec + 1) * R, 9)
-        assert P.compare_grid(ws, o, trk, units) > 10
-        for u in units:
-            lo, hi = int(ws.unit_off[u]), int(ws.unit_off[u + 1])
-            for cleaned, (nu, nd) in ((False, ("link_up", "link_dn")), (True, ("clean_up", "clean_dn"))):
-                up, dn = trk.links(u // R, u % R, cleaned)
-                assert np.array_equal(up, o.get(nu)[lo:hi]) and np.array_equal(dn, o.get(nd)[lo:hi]), (u, cleaned)
-    res = P.compare_tracks(otr, gtr)
-    assert res["n_oracle"] > 10000 and res["frac_identical"] >= 0.999 and res["param_mismatch"] <= 0.001 * res["n_oracle"], res
+        for sec in (2, 11, 20, 31):
+            ws = w.sector_slice([sec])
+            o = P.make_oracle(ws).run("s6")
+            otr = o.tracks()
+            sel = np.nonzero(r.sector == sec)[0]
+            assert len(sel) > 10000 and np.all(np.diff(sel) == 1)
+            a, b = int(sel[0]), int(sel[-1]) + 1
+            cb = r.cl_begin[a:b + 1]
+            gtr = dict(sector=r.sector[a:b].copy(), x=r.x[a:b].copy(), par=r.par[a:b].copy(), cov=r.cov[a:b].copy(), chi2=r.chi2[a:b].copy(),
+                       ndf=r.ndf[a:b].copy(), cl_begin=(cb - cb[0]).copy(), cl_row=r.cl_row[cb[0]:cb[-1]].copy(),
+                       cl_index=r.cl_index[cb[0]:cb[-1]].copy())
+            units = range(sec * R + (sec % 9), (sec + 1) * R, 9)
+            assert P.compare_grid(ws, o, trk, units) > 10
+            for u in units:
+                lo, hi = int(ws.unit_off[u]), int(ws.unit_off[u + 1])
+                for cleaned, (nu, nd) in ((False, ("link_up", "link_dn")), (True, ("clean_up", "clean_dn"))):
+                    up, dn = trk.links(u // R, u % R, cleaned)
+                    assert np.array_equal(up, o.get(nu)[lo:hi]) and np.array_equal(dn, o.get(nd)[lo:hi]), (u, cleaned)
+            res = P.compare_tracks(otr, gtr)
+            assert res["n_oracle"] > 10000, res
+            _assert_track_bars(res)
+            del o, otr, ws
 
 
 def _inject(w, unit, y_extra, t_extra):
@@ -388,7 +451,7 @@ def test_degenerate_units_dense_overflow_and_nonfinite():
         lk = P.compare_links(w, o, trk)
     assert lk["raw"] == 0 and lk["cleaned"] == 0 and lk["start_equal"], lk
     res = P.compare_tracks(o.tracks(), gtr)
-    assert res["frac_identical"] >= 0.999 and res["param_mismatch"] == 0, res
+    _assert_track_bars(res)
 
 
 def test_abi_state_and_argument_errors_on_device():

@@ -180,6 +180,75 @@ def test_s2_python_brute_force_restatement(c1_small):
     assert n_links > 500
 
 
+def test_s2_continuous_mode_restatement_with_unequal_row_pitch():
+    """O(N^2) numpy-fp32 restatement of S2 for t_frame > 0, the mode the benchmark runs (reading A6: window centre z, half-width
+    wzu_r = dzdx_max * (x_{r+1} - x_r) + wz0 upwards and wzd_r = dzdx_max * (x_r - x_{r-1}) + wz0 downwards), written from DESIGN.md
+    section 4 and not from the oracle's code.  The row pitch alternates 0.75 / 1.5 cm so that wzu != wzd on every row, the weights
+    a_r != b_r enter the residual, and the tracks carry collision-time shifts (z down to -900 cm) and slopes dz/dx up to 1.9, so
+    that true neighbours lie between the smaller and the larger half-width.
+    Fails under: wzu / wzd swapped; window centre z * x'/x as in triggered mode; a and b swapped in ey / ez; thr from the wrong pitch."""
+    f = np.float32
+    rng = np.random.default_rng(77)
+    R = 40
+    pitch = np.where(np.arange(R - 1) % 2 == 0, 0.75, 1.5)
+    X = (90.0 + np.concatenate([[0.0], np.cumsum(pitch)])).astype(np.float32)
+    t_frame, vd, zmax = 400.0, 2.5, 250.0
+    rows_y = [[] for _ in range(R)]; rows_z = [[] for _ in range(R)]
+    n_tracks = 40
+    for k in range(n_tracks):                       # straight lines from the beam line (Bz plays no role in S2), shifted in z
+        tphi = rng.uniform(-0.15, 0.15); dzdx = rng.uniform(1.3, 1.9) * rng.choice([-1, 1]) if k % 2 else rng.uniform(-0.8, 0.8)
+        zshift = -rng.uniform(0.0, 900.0)
+        for r in range(R):
+            if rng.uniform() < 0.05:
+                continue
+            rows_y[r].append(X[r] * tphi + rng.normal(0, 0.1)); rows_z[r].append(X[r] * dzdx * 0.1 + 60.0 + zshift + dzdx * (X[r] - X[0]) + rng.normal(0, 0.15))
+    for r in range(R):                              # noise
+        for _ in range(15):
+            rows_y[r].append(rng.uniform(-15, 15)); rows_z[r].append(rng.uniform(-990.0, 240.0))
+    off = np.zeros(R + 1, np.int64); off[1:] = np.cumsum([len(v) for v in rows_y])
+    y = np.concatenate([np.array(v, np.float32) for v in rows_y]); zz = np.concatenate([np.array(v, np.float64) for v in rows_z])
+    t = ((zmax - zz) / vd).astype(np.float32)
+    geo = dict(n_sectors=1, n_rows=R, row_x=X, sector_dphi=2 * math.pi / 18, z_max=zmax, t_frame=t_frame, sigma_y=0.1, sigma_z=0.15, bz=0.5, vdrift=vd)
+    o = Oracle(**geo); o.load(off, y, t); o.run("s2")
+
+    class _W:                                        # the slice of the Workload interface _links_in_original_index reads
+        n_sectors, n_rows, unit_off, n_clusters = 1, R, off, len(y)
+    up_o, dn_o = _links_in_original_index(_W, o)
+    z = (f(zmax) - f(vd) * t).astype(f)              # S0, fp32: product rounded, then subtracted
+    wy, dzdx_max, wz0, cut2 = f(1.5), 1.5, 0.75, 1.75
+    Xd = X.astype(np.float64)
+    n_links = n_between = 0
+    for r in range(1, R - 1):
+        a, b = off[r], off[r + 1]; au, bu = off[r + 1], off[r + 2]; ad, bd = off[r - 1], off[r]
+        A64, B64 = Xd[r + 1] - Xd[r], Xd[r] - Xd[r - 1]
+        tu, td, A, B = f(Xd[r + 1] / Xd[r]), f(Xd[r - 1] / Xd[r]), f(A64), f(B64)
+        thr = f(cut2 * 0.5 * (A64 * A64 + B64 * B64))
+        wzu, wzd = f(dzdx_max * A64 + wz0), f(dzdx_max * B64 + wz0)
+        assert wzu != wzd
+        for h in range(a, b):
+            yh, zh = y[h], z[h]
+            ycu, ycd = f(yh * tu), f(yh * td)
+            cu = [i for i in range(au, bu) if f(ycu - wy) <= y[i] <= f(ycu + wy) and f(zh - wzu) <= z[i] <= f(zh + wzu)]
+            cd = [i for i in range(ad, bd) if f(ycd - wy) <= y[i] <= f(ycd + wy) and f(zh - wzd) <= z[i] <= f(zh + wzd)]
+            best = None
+            for i in cu:
+                for j in cd:
+                    ey = f(f(B * f(y[i] - yh)) - f(A * f(yh - y[j])))
+                    ez = f(f(B * f(z[i] - zh)) - f(A * f(zh - z[j])))
+                    D = f(f(ey * ey) + f(ez * ez))
+                    key = (float(D), i - au, j - ad)
+                    if best is None or key < best:
+                        best = key
+            if best is not None and f(best[0]) < thr:
+                assert (up_o[h], dn_o[h]) == (best[1], best[2]), (r, h)
+                n_links += 1
+                lo, hi = min(wzu, wzd), max(wzu, wzd)
+                n_between += lo < abs(z[au + best[1]] - zh) <= hi or lo < abs(z[ad + best[2]] - zh) <= hi
+            else:
+                assert (up_o[h], dn_o[h]) == (-1, -1), (r, h)
+    assert n_links > 800 and n_between > 100          # the unequal half-widths decide links here
+
+
 def test_s2_invariant_under_bin_size(c1):
     ref = Oracle.for_workload(c1).run("s4")
     r_up, r_dn = _links_in_original_index(c1, ref)

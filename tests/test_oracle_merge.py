@@ -1,5 +1,6 @@
-"""Pins of the oracle's S9 (NEXT-3 of SURVEY.md section 8(f); PAPER.md:49 lists the merging of track segments between
-sectors among the later additions; reading A41 of DESIGN.md): a track that leaves its sector through the side edge is
+"""Pins of the oracle's S9 (NEXT-3 of SURVEY.md section 8(f); PAPER.md:49 says only "Locally, e. g. at the TPC sector
+boundaries, there are still some improvements to be done" -- matching segments across the boundary is this build's reading A41
+of DESIGN.md, not a rule the paper prints): a track that leaves its sector through the side edge is
 matched with its continuation in the neighbouring sector.
 
 No formula is re-typed: the rotation + transport chain is pinned by running it with windows a thousand times tighter on
