@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libtpc_b200.so")
 SOURCES = ["tpc_abi.cu", "scan.cu", "k1_grid.cu", "k2_neighbours.cu", "k3_clean_start.cu", "k5_tracklets.cu", "k6_selector.cu", "k7_refit.cu", "k8_tube.cu", "k9_merge.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-cudart", "shared"]
+              "-Xcompiler", "-fPIC", "-cudart", "shared"] + os.environ.get("TPC_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

@@ -131,7 +131,7 @@ struct tpc_ctx {
   DevBuf d_start_unit, d_start_pos, d_counters, d_keep, d_keep_pos, d_start_unit2, d_start_pos2, d_flag2, d_used;
   // S5/S6
   int M = 0; long long Mpad = 0;
-  DevBuf d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out, d_scan_tmp64;
+  DevBuf d_k5scratch, d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out, d_scan_tmp64;
   // outputs (device)
   long long n_tracks = 0, n_refs = 0;
   DevBuf o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row, o_cl_index;
@@ -238,7 +238,7 @@ void tpc_destroy(tpc_ctx* c) {
   cudaStreamSynchronize(c->stream);
   DevBuf* bufs[] = {&c->d_in_y, &c->d_in_t, &c->d_rows, &c->d_units, &c->d_items, &c->d_yz, &c->d_perm, &c->d_bin_start, &c->d_cursor,
                     &c->d_link_up, &c->d_link_dn, &c->d_raw_up, &c->d_raw_dn, &c->d_mask, &c->d_item_count, &c->d_item_base, &c->d_scan_tmp,
-                    &c->d_start_unit, &c->d_start_pos, &c->d_counters, &c->d_rowhit, &c->d_tl_n, &c->d_tl_first, &c->d_tl_last, &c->d_tl_chi2,
+                    &c->d_start_unit, &c->d_start_pos, &c->d_counters, &c->d_k5scratch, &c->d_rowhit, &c->d_tl_n, &c->d_tl_first, &c->d_tl_last, &c->d_tl_chi2,
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
                     &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
@@ -552,6 +552,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   // ---- K5: S5
   const size_t Mz = (size_t)std::max(M, 1);
   CUDA_TRY(c, c->d_rowhit.ensure((size_t)std::max(Mpad, 32LL) * R * 4));
+  CUDA_TRY(c, c->d_k5scratch.ensure(k5_scratch_bytes(M)));
   CUDA_TRY(c, c->d_tl_n.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_first.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_last.ensure(Mz * 4));
   CUDA_TRY(c, c->d_tl_chi2.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_par.ensure(Mz * 20)); CUDA_TRY(c, c->d_tl_cov.ensure(Mz * 60));
   CUDA_TRY(c, c->d_owner.ensure((size_t)(N + 4) * 8)); CUDA_TRY(c, c->d_tl_key.ensure(Mz * 8));
@@ -560,10 +561,11 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   unsigned long long* d_k5cnt = (unsigned long long*)(c->d_counters.as<char>() + 128);
   CUDA_TRY(c, cudaMemsetAsync(d_k5cnt, 0, 32, st));
   auto run_k5 = [&](int n_run, const int* list) -> int {
-    LAUNCH_TRY(c, launch_k5_tracklets(L, n_run, Mpad, list, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
+    LAUNCH_TRY(c, launch_k5_tracklets(L, n_run, M, list, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
                                       c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
                                       c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
-                                      c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt, P), launches);
+                                      c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt,
+                                      c->d_k5scratch.p, P), launches);
     return TPC_OK;
   };
   long long n_fitted = M;
@@ -604,8 +606,6 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
     const int M2 = *c->p_small.as<int>();
     if (M2 < 0 || M2 > M - M1) return fail(c, TPC_E_CUDA, "rescue-wave start-hit count %d out of range", M2);
     if (M2 > 0) {
-      int* d_queue = reinterpret_cast<int*>(d_k5cnt + 3);
-      CUDA_TRY(c, cudaMemsetAsync(d_queue, 0, sizeof(int), st));
       rc = run_k5(M2, list2);
       if (rc != TPC_OK) return rc;
       LAUNCH_TRY(c, launch_k6_owner(L, M2, list2, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),

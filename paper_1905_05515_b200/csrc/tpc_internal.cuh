@@ -115,11 +115,11 @@ int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int
                           int* d_link_dn, unsigned* d_mask, int* d_item_count, int* d_item_base, int* d_scan_tmp,
                           int* d_start_unit, int* d_start_pos, int* d_total, const Params& P);
 
-int launch_k5_tracklets(const Launch& L, int M, long long Mpad, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
-                        const UnitDesc* d_units,
-                        const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, const int* d_link_up,
-                        int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2, float* d_tl_par,
-                        float* d_tl_cov, unsigned long long* d_counters, const Params& P);
+size_t k5_scratch_bytes(long long M);   // handoff records + task lists + control block of the K5 phase kernels
+int launch_k5_tracklets(const Launch& L, int n_run, int M, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
+                        const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
+                        const int* d_link_up, int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2,
+                        float* d_tl_par, float* d_tl_cov, unsigned long long* d_counters, void* d_scratch, const Params& P);
 
 int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const int* d_start_unit, const UnitDesc* d_units,
                      const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
