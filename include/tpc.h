@@ -144,7 +144,10 @@ typedef struct {
 int tpc_create(const tpc_geometry* geometry, float bz_tesla, float vdrift_cm_per_us, tpc_ctx** out);
 
 /* Tunables of DESIGN.md table T by name: wy wz dzdx_max wz0 cut2 min_seed c0_y c0_z c0_sinphi c0_dzds c0_qpt s_max n_sigma
- * w_max max_gap edge_margin min_hits grid_scale, plus debug_keep (1 = keep pre-cleaning link tables for tpc_debug_get_links).
+ * w_max max_gap edge_margin min_hits grid_scale, plus debug_keep (1 = keep pre-cleaning link tables for tpc_debug_get_links) and
+ * pinned_async (default 0; 1 = a PINNED host source of tpc_load_clusters* is read by DMA on the context's stream AFTER the load call
+ * has returned: the caller then keeps those buffers untouched until the next tpc_find_tracks* on the context returns.  With 0 the
+ * load call returns only when the library has read its inputs, as the conventions above state).
  * Only before the first load after tpc_create / tpc_clear. */
 int tpc_set_param(tpc_ctx*, const char* name, double value);
 

@@ -241,11 +241,9 @@ int launch_k3_bridge_lists(const Launch& L, int M, const int* d_start_unit, cons
 }
 
 // part 2, after the first wave: list2 = dropped start hits whose chain the first wave left (partly) unused; *d_total = their number
-int launch_k3_rescue_list(const Launch& L, int M, int M1, const int* d_list1, const int* d_keep, const int* d_start_unit,
-                          const int* d_start_pos, const UnitDesc* d_units, const int* d_link_up, const int* d_rowhit, const int* d_tl_n,
-                          const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, const unsigned long long* d_owner, long long N,
-                          int* d_flag2, int* d_pos, int* d_scan_tmp, int* d_list2, int* d_total, const Params& P) {
-  (void)M1; (void)d_list1; (void)d_rowhit; (void)d_tl_n; (void)d_tl_first; (void)d_tl_last; (void)d_tl_chi2; (void)N; (void)P;
+int launch_k3_rescue_list(const Launch& L, int M, const int* d_keep, const int* d_start_unit, const int* d_start_pos,
+                          const UnitDesc* d_units, const int* d_link_up, const unsigned long long* d_owner,
+                          int* d_flag2, int* d_pos, int* d_scan_tmp, int* d_list2, int* d_total) {
   const int blocks = (M + K3_THREADS - 1) / K3_THREADS;
   k3_rescue_flag<<<blocks, K3_THREADS, 0, L.stream>>>(M, d_keep, d_start_unit, d_start_pos, d_units, d_link_up, d_owner, d_flag2);
   int rc = launch_scan_i32(L, d_flag2, d_pos, M, d_scan_tmp, d_total);

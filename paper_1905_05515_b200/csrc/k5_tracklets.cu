@@ -180,7 +180,7 @@ __device__ __forceinline__ bool flush_now(const int mode, const bool drained) {
 
 // ---------------------------------------------------------------------------------------------------------------------------
 // Phase A: seed fit along the chain of cleaned up-links (no gate).  Task = start hit (or an entry of run_list).
-__global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M, const int* __restrict__ run_list,
+__global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, const int* __restrict__ M_dev, const int* __restrict__ run_list,
                                                               const int* __restrict__ start_unit, const int* __restrict__ start_pos,
                                                               const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
                                                               const float2* __restrict__ yz, const int* __restrict__ link_up,
@@ -188,6 +188,7 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M, const
                                                               int* __restrict__ list_c, int* __restrict__ ctl,
                                                               unsigned long long* __restrict__ counters, const Params P) {
   K5_PROLOGUE();
+  const int M = M_dev ? min(*M_dev, M_host) : M_host;   // task count: in device memory (default path: no read-back after K3) or given
   int i = -1, u0 = 0, r = 0, nxt = -1, hit0 = -1;
   bool ok = true;
   float zref = 0.0f;
@@ -558,7 +559,9 @@ size_t k5_scratch_bytes(long long M) {   // TlRec array + three task lists + con
 }
 
 // d_scratch: k5_scratch_bytes(M) bytes, 128-byte aligned.  d_counters: three 64-bit work counters (accumulated).
-int launch_k5_tracklets(const Launch& L, int n_run, int M, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
+// n_run tasks (entries of d_run_list, or the first n_run start hits); with d_n_run the count is read from device memory and n_run is
+// its upper bound.  M: capacity of the per-tracklet arrays / scratch.
+int launch_k5_tracklets(const Launch& L, int n_run, const int* d_n_run, int M, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
                         const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
                         const int* d_link_up, int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2,
                         float* d_tl_par, float* d_tl_cov, unsigned long long* d_counters, void* d_scratch, const Params& P) {
@@ -579,7 +582,7 @@ int launch_k5_tracklets(const Launch& L, int n_run, int M, const int* d_run_list
     nb_c = persistent_blocks(k5c_refit_in, L.sm_count); nb_d = persistent_blocks(k5d_extend_in, L.sm_count);
   }
   const int need = (n_run + K5_THREADS - 1) / K5_THREADS;
-  k5a_seed_fit<<<nb_a < need ? nb_a : need, K5_THREADS, 0, L.stream>>>(n_run, d_run_list, d_start_unit, d_start_pos, d_units, d_rows, d_yz,
+  k5a_seed_fit<<<nb_a < need ? nb_a : need, K5_THREADS, 0, L.stream>>>(n_run, d_n_run, d_run_list, d_start_unit, d_start_pos, d_units, d_rows, d_yz,
                                                                       d_link_up, d_rowhit, rec, list_b, list_c, ctl, d_counters, P);
   k5b_extend_out<<<nb_b < need ? nb_b : need, K5_THREADS, 0, L.stream>>>(list_b, d_units, d_rows, d_yz, d_perm, d_bin_start, d_rowhit, rec,
                                                                         list_c, ctl, d_counters, P);

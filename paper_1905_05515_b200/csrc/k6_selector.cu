@@ -5,7 +5,8 @@
 //   bits 63..56  n (<= 255 rows)
 //   bits 55..24  bitwise NOT of the order-preserving image of the fp32 quality chi2/ndf (lower quality wins)
 //   bits 23..0   0xFFFFFF - tracklet index (lower index wins)                       -> at most 2^24 tracklets per call
-// One warp per tracklet in all three kernels.
+// One warp per tracklet in all three kernels (grid-stride over the tracklets: the tracklet count may live in device memory, so
+// that the host does not have to read it back between K3 and K6).
 // k6_owner : atomicMax of the key on owner[cluster]          k6_count : owned clusters per tracklet, track flag
 // scan     : exclusive prefix sum of (flag << 40 | owned)     k6_emit  : compacted tracks + CSR cluster lists, in tracklet order
 #include "tpc_internal.cuh"
@@ -25,14 +26,15 @@ __device__ __forceinline__ unsigned long long make_key(int n, float chi2, int id
 
 // All three kernels map ONE WARP to one tracklet: the lanes read 32 consecutive rows of its rowhit line (coalesced) and issue
 // their owner-key atomics / owner reads in parallel.
-__global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const int* __restrict__ run_list, const int R, const int min_hits,
+__global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M_cap, const int* __restrict__ M_dev, const int* __restrict__ run_list, const int R, const int min_hits,
                                                        const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
                                                        const int* __restrict__ rowhit, const int* __restrict__ tl_n,
                                                        const int* __restrict__ tl_first, const int* __restrict__ tl_last,
                                                        const float* __restrict__ tl_chi2, unsigned long long* __restrict__ owner,
                                                        unsigned long long* __restrict__ tl_key) {
-  const int q = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
-  if (q >= M) return;
+  const int lane = threadIdx.x & 31, n_warps = (int)(((long long)gridDim.x * blockDim.x) >> 5);
+  const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
+  for (int q = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); q < M; q += n_warps) {
   const int i = run_list ? run_list[q] : q;   // M entries of a run list (rescue variant), or all tracklets
   const int n = tl_n[i];
   const float chi2 = tl_chi2[i];
@@ -40,23 +42,26 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M, const int* _
   const bool kept = n >= min_hits && isfinite(chi2);
   const unsigned long long key = kept ? make_key(n, chi2, i) : 0ull;
   if (lane == 0) tl_key[i] = key;
-  if (!kept) return;
+  if (!kept) continue;
   const UnitDesc* __restrict__ su = units + (long long)(u0 / R) * R;
   const int* __restrict__ rh = rowhit + (long long)i * R;
   for (int r = r_lo + lane; r <= r1; r += 32) {
     const int p = rh[r];
     if (p >= 0) atomicMax(&owner[su[r].off + p], key);
   }
+  }
 }
 
-__global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const int R, const int min_hits,
+__global__ void __launch_bounds__(K6_THREADS) k6_count(const int M_cap, const int* __restrict__ M_dev, const int R, const int min_hits,
                                                        const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
                                                        const int* __restrict__ rowhit, const int* __restrict__ tl_first,
                                                        const int* __restrict__ tl_last, const unsigned long long* __restrict__ owner,
                                                        const unsigned long long* __restrict__ tl_key,
                                                        unsigned long long* __restrict__ scan_in) {
-  const int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
-  if (i >= M) return;
+  const int lane = threadIdx.x & 31, n_warps = (int)(((long long)gridDim.x * blockDim.x) >> 5);
+  const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
+  for (int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); i < M_cap; i += n_warps) {
+  if (i >= M) { if (lane == 0) scan_in[i] = 0ull; continue; }   // the scan runs over the capacity: entries beyond the count are 0
   const unsigned long long key = tl_key[i];
   const int u0 = start_unit[i], r_lo = tl_first[i], r1 = tl_last[i];     // read with the key, not after the decision it feeds
   int owned = 0;
@@ -70,9 +75,10 @@ __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M, const int R,
   }
   owned = __reduce_add_sync(0xffffffffu, owned);
   if (lane == 0) scan_in[i] = owned >= min_hits && key ? ((1ull << 40) | (unsigned long long)owned) : 0ull;
+  }
 }
 
-__global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const int R, const int* __restrict__ start_unit,
+__global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M_cap, const int* __restrict__ M_dev, const int R, const int* __restrict__ start_unit,
                                                       const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
                                                       const int* __restrict__ perm, const int* __restrict__ rowhit,
                                                       const int* __restrict__ tl_n, const int* __restrict__ tl_first,
@@ -85,11 +91,17 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const int R, 
                                                       float* __restrict__ o_x, float* __restrict__ o_par, float* __restrict__ o_cov,
                                                       float* __restrict__ o_chi2, int* __restrict__ o_ndf, int* __restrict__ o_tracklet,
                                                       long long* __restrict__ o_cl_begin, int* __restrict__ o_cl_row,
-                                                      int* __restrict__ o_cl_index, const long long n_tracks, const long long n_refs) {
+                                                      int* __restrict__ o_cl_index, const unsigned long long* __restrict__ total,
+                                                      const long long cap_tracks, const long long cap_refs) {
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const int i = (int)(gt >> 5), lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, n_warps = (int)(((long long)gridDim.x * blockDim.x) >> 5);
+  const unsigned long long tot = *total;                       // (tracks << 40 | cluster references) of the scan
+  const long long n_tracks = (long long)(tot >> 40), n_refs = (long long)(tot & REF_MASK);
+  if (n_tracks > cap_tracks || n_refs > cap_refs) return;      // the caller sees the totals and repeats the call with larger buffers
   if (gt == 0) o_cl_begin[n_tracks] = n_refs;
-  if (i >= M || scan_in[i] == 0ull) return;
+  const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
+  for (int i = (int)(gt >> 5); i < M; i += n_warps) {
+  if (scan_in[i] == 0ull) continue;
   const unsigned long long so = scan_out[i];
   const long long t = (long long)(so >> 40);
   long long k = (long long)(so & REF_MASK);
@@ -112,32 +124,38 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M, const int R, 
     if (own) { const long long o = k + __popc(m & ((1u << lane) - 1u)); o_cl_row[o] = r; o_cl_index[o] = perm[g]; }
     k += __popc(m);
   }
+  }
 }
 
 }  // namespace
 
-int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const int* d_start_unit, const UnitDesc* d_units,
-                     const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
+// grid of the warp-per-tracklet kernels: enough warps to fill the GPU several times over, never more than one warp per tracklet
+static int k6_blocks(const Launch& L, long long M) {
+  const long long want = (M * 32 + K6_THREADS - 1) / K6_THREADS, cap = (long long)L.sm_count * 16 * 8;
+  return (int)(want < 1 ? 1 : (want < cap ? want : cap));
+}
+
+// d_M: tracklet count in device memory (or nullptr: M_cap is the count); M_cap: capacity of the per-tracklet arrays
+int launch_k6_select(const Launch& L, int M_cap, const int* d_M, long long N, const int* d_start_unit, const UnitDesc* d_units,
+                     const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
                      const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
                      unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
                      unsigned long long* d_total, const Params& P, bool owner_done) {
-  (void)d_rows; (void)d_perm;
-  if (M <= 0) {
+  if (M_cap <= 0) {
     cudaError_t e = cudaMemsetAsync(d_total, 0, sizeof(unsigned long long), L.stream);
     return e == cudaSuccess ? 0 : -(int)e;
   }
   cudaError_t e = cudaSuccess;
-  (void)Mpad;
-  const int blocks = (int)(((long long)M * 32 + K6_THREADS - 1) / K6_THREADS);
+  const int blocks = k6_blocks(L, M_cap);
   if (!owner_done) {   // (the rescue variant raised the owner keys wave by wave: launch_k6_owner)
     e = cudaMemsetAsync(d_owner, 0, (size_t)N * sizeof(unsigned long long), L.stream);
     if (e != cudaSuccess) return -(int)e;
-    k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M, nullptr, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first,
+    k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M_cap, d_M, nullptr, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first,
                                                    d_tl_last, d_tl_chi2, d_owner, d_tl_key);
   }
-  k6_count<<<blocks, K6_THREADS, 0, L.stream>>>(M, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_first, d_tl_last, d_owner,
+  k6_count<<<blocks, K6_THREADS, 0, L.stream>>>(M_cap, d_M, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_first, d_tl_last, d_owner,
                                                  d_tl_key, d_scan_in);
-  int rc = launch_scan_u64(L, d_scan_in, d_scan_out, M, d_scan_tmp, d_total);
+  int rc = launch_scan_u64(L, d_scan_in, d_scan_out, M_cap, d_scan_tmp, d_total);
   if (rc < 0) return rc;
   e = cudaGetLastError();
   return e == cudaSuccess ? (owner_done ? 1 : 2) + rc : -(int)e;
@@ -148,25 +166,24 @@ int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int
                     const int* d_tl_n, const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner,
                     unsigned long long* d_tl_key, const Params& P) {
   if (n_run <= 0) return 0;
-  const int blocks = (int)(((long long)n_run * 32 + K6_THREADS - 1) / K6_THREADS);
-  k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(n_run, d_run_list, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first,
-                                                 d_tl_last, d_tl_chi2, d_owner, d_tl_key);
+  k6_owner<<<k6_blocks(L, n_run), K6_THREADS, 0, L.stream>>>(n_run, nullptr, d_run_list, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n,
+                                                              d_tl_first, d_tl_last, d_tl_chi2, d_owner, d_tl_key);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }
 
-int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
+// d_total: (tracks << 40 | references) written by the scan; the output arrays hold cap_tracks tracks / cap_refs references
+int launch_k6_emit(const Launch& L, int M_cap, const int* d_M, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
                    const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
                    const float* d_tl_chi2, const float* d_tl_par, const float* d_tl_cov, const unsigned long long* d_owner,
                    const unsigned long long* d_tl_key, const unsigned long long* d_scan_in, const unsigned long long* d_scan_out,
                    int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,
-                   long long* o_cl_begin, int* o_cl_row, int* o_cl_index, long long n_tracks, long long n_refs, const Params& P) {
-  (void)Mpad;
-  const int blocks = M > 0 ? (int)(((long long)M * 32 + K6_THREADS - 1) / K6_THREADS) : 1;
-  k6_emit<<<blocks, K6_THREADS, 0, L.stream>>>(M, P.R, d_start_unit, d_units, d_rows, d_perm, d_rowhit, d_tl_n, d_tl_first,
-                                                d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out,
-                                                o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row, o_cl_index,
-                                                n_tracks, n_refs);
+                   long long* o_cl_begin, int* o_cl_row, int* o_cl_index, const unsigned long long* d_total, long long cap_tracks,
+                   long long cap_refs, const Params& P) {
+  k6_emit<<<k6_blocks(L, M_cap), K6_THREADS, 0, L.stream>>>(M_cap, d_M, P.R, d_start_unit, d_units, d_rows, d_perm, d_rowhit, d_tl_n, d_tl_first,
+                                                             d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out,
+                                                             o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row,
+                                                             o_cl_index, d_total, cap_tracks, cap_refs);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }

@@ -123,6 +123,10 @@ struct tpc_ctx {
   PinBuf p_units, p_items, p_small;
   DevBuf d_rows, d_units, d_items;
   bool rows_valid = false;
+  bool tables_ready = false;     // per-unit grid descriptors / work items computed and uploaded for the clusters loaded now
+  int t_msm = 0, t_max_n = 0, t_max_perm = 0, t_max_yz = 0; long long t_cursor_total = 0;   // K1 launch plan of those tables
+  int pinned_async = 0;          // 1: a pinned host source is read by DMA after the load call returned (caller keeps it untouched until tpc_find_tracks*)
+  cudaEvent_t ev_tables = nullptr;   // end of the last table upload (the pinned staging copy may be rewritten after it)
   Params P;
 
   // S1..S4
@@ -131,6 +135,7 @@ struct tpc_ctx {
   DevBuf d_start_unit, d_start_pos, d_counters, d_keep, d_keep_pos, d_start_unit2, d_start_pos2, d_flag2, d_used;
   // S5/S6
   int M = 0; long long Mpad = 0;
+  long long m_cap_hint = 0;      // capacity guess for the per-tracklet buffers of the next call (1.25 x the last count)
   DevBuf d_k5scratch, d_rowhit, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out, d_scan_tmp64;
   // outputs (device)
   long long n_tracks = 0, n_refs = 0;
@@ -149,6 +154,7 @@ struct tpc_ctx {
   std::vector<int32_t> dbg_tl_sector, dbg_tl_row, dbg_tl_n, dbg_tl_first, dbg_tl_last, dbg_rowhit; std::vector<float> dbg_tl_chi2, dbg_tl_x, dbg_tl_par, dbg_tl_cov;
 
   cudaEvent_t ev[10] = {};
+  bool load_pending = false;     // ev_load recorded, not yet waited for
   cudaEvent_t ev_load = nullptr;   // end of a direct H2D copy from the caller's pinned memory (stage_append)
   tpc_timings timings = {};
 };
@@ -176,6 +182,8 @@ int pointer_kind(const void* p) {
   if (a.type == cudaMemoryTypeHost) return 1;
   return 0;
 }
+
+int prepare_tables(tpc_ctx* c);
 
 void add_dirty(tpc_ctx* c, long long a, long long b) {
   if (!c->dirty.empty() && c->dirty.back().second == a) c->dirty.back().second = b;
@@ -226,7 +234,8 @@ int tpc_create(const tpc_geometry* g, float bz, float vdrift, tpc_ctx** out) {
   for (auto& ev : c->ev) {
     if (cudaEventCreate(&ev) != cudaSuccess) { int rc = fail(nullptr, TPC_E_CUDA, "tpc_create: cudaEventCreate failed"); delete c; return rc; }
   }
-  if (cudaEventCreateWithFlags(&c->ev_load, cudaEventDisableTiming) != cudaSuccess) {
+  if (cudaEventCreateWithFlags(&c->ev_load, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&c->ev_tables, cudaEventDisableTiming) != cudaSuccess) {
     int rc = fail(nullptr, TPC_E_CUDA, "tpc_create: cudaEventCreate failed"); tpc_destroy(c); return rc;
   }
   *out = c;
@@ -252,6 +261,7 @@ void tpc_destroy(tpc_ctx* c) {
   c->hr_z0.release(); c->hr_t0.release(); c->hm_status.release(); c->hm_track.release(); c->hg_next.release(); c->hg_prev.release();
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
   if (c->ev_load) cudaEventDestroy(c->ev_load);
+  if (c->ev_tables) cudaEventDestroy(c->ev_tables);
   delete c;
 }
 
@@ -281,6 +291,7 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "min_hits") { if (v < 3 || v > 255) return fail(c, TPC_E_ARG, "min_hits must be in 3..255 (ndf = 2n-5 > 0)"); T.min_hits = (int)v; }
   else if (s == "grid_scale") rc = pos(T.grid_scale);
   else if (s == "debug_keep") T.debug_keep = v != 0;
+  else if (s == "pinned_async") c->pinned_async = v != 0;
   else if (s == "k2_threads") { int k = (int)v; if (k < 32 || k > 256 || (k & 31)) return fail(c, TPC_E_ARG, "k2_threads must be a multiple of 32 in 32..256"); T.k2_threads = k; }
   else if (s == "chunk") { int k = (int)v; if (k < 32 || k > 4096 || (k & 31)) return fail(c, TPC_E_ARG, "chunk must be a multiple of 32 in 32..4096"); T.chunk = k; }
   else if (s == "bridge_rows") { if (v < 0 || v > 16) return fail(c, TPC_E_ARG, "bridge_rows must be in 0..16"); T.bridge_rows = (int)v; }
@@ -291,7 +302,7 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "merge_ds") rc = pos(T.merge_ds); else if (s == "merge_dt") rc = pos(T.merge_dt);
   else if (s == "merge_rows") { if (v < 0 || v > 255) return fail(c, TPC_E_ARG, "merge_rows must be in 0..255"); T.merge_rows = (int)v; }
   else return fail(c, TPC_E_ARG, "tpc_set_param: unknown parameter '%s'", name);
-  if (rc == TPC_OK) c->rows_valid = false;
+  if (rc == TPC_OK) { c->rows_valid = false; c->tables_ready = false; }
   return rc;
 }
 
@@ -299,7 +310,7 @@ int tpc_clear(tpc_ctx* c) {
   if (!c) return TPC_E_ARG;
   cudaStreamSynchronize(c->stream);   // staged device copies may still read caller memory; outputs are about to be invalidated
   std::fill(c->usrc.begin(), c->usrc.end(), UnitSrc());
-  c->arena_pos = 0; c->dirty.clear(); c->loaded_any = false; c->have_result = false;
+  c->arena_pos = 0; c->dirty.clear(); c->loaded_any = false; c->have_result = false; c->tables_ready = false;
   c->N = 0; c->M = 0; c->n_tracks = 0; c->n_refs = 0;
   return TPC_OK;
 }
@@ -319,10 +330,11 @@ static int stage_append(tpc_ctx* c, const float* y, const float* t, long long n,
     CUDA_TRY(c, c->d_in_t.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_in_y.as<float>() + pos, y, bytes, kind, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_in_t.as<float>() + pos, t, bytes, kind, c->stream));
-    if (ky != 2) {   // the DMA reads the caller's pinned host memory: it must have finished when the call returns (tpc.h: host
-                     // inputs may be freed or overwritten on return); a device source follows stream order instead
+    if (ky != 2 && !c->pinned_async) {   // the DMA reads the caller's pinned host memory: it must have finished when the load call
+      // returns (tpc.h: host inputs may be freed or overwritten on return) unless the caller opted into pinned_async; the caller of
+      // stage_append waits on this event after its own host work.  A device source follows stream order instead.
       CUDA_TRY(c, cudaEventRecord(c->ev_load, c->stream));
-      CUDA_TRY(c, cudaEventSynchronize(c->ev_load));
+      c->load_pending = true;
     }
   } else {        // pageable (or small) host source: copy into the pinned arena now, upload at tpc_find_tracks
     CUDA_TRY(c, c->h_y.ensure_keep(end_bytes + 64, (size_t)c->arena_pos * 4));
@@ -343,9 +355,10 @@ int tpc_load_clusters(tpc_ctx* c, int sector, int row, const float* pad_y, const
   long long pos = 0;
   int rc = stage_append(c, pad_y, time, n, &pos);
   if (rc != TPC_OK) return rc;
+  if (c->load_pending) { c->load_pending = false; CUDA_TRY(c, cudaEventSynchronize(c->ev_load)); }
   UnitSrc& u = c->usrc[(size_t)sector * c->R + row];
   u.src = pos; u.n = n;
-  c->loaded_any = true; c->have_result = false;
+  c->loaded_any = true; c->have_result = false; c->tables_ready = false;
   return TPC_OK;
 }
 
@@ -367,8 +380,10 @@ int tpc_load_clusters_batch(tpc_ctx* c, const int64_t* unit_off, const float* pa
   int rc = stage_append(c, pad_y ? pad_y + unit_off[0] : nullptr, time ? time + unit_off[0] : nullptr, n, &pos);
   if (rc != TPC_OK) return rc;
   for (int u = 0; u < U; u++) { c->usrc[u].src = pos + (unit_off[u] - unit_off[0]); c->usrc[u].n = (int)(unit_off[u + 1] - unit_off[u]); }
-  c->loaded_any = true; c->have_result = false;
-  return TPC_OK;
+  c->loaded_any = true; c->have_result = false; c->tables_ready = false;
+  rc = prepare_tables(c);      // host tables + their upload while the cluster DMA (if any) is running
+  if (c->load_pending) { c->load_pending = false; CUDA_TRY(c, cudaEventSynchronize(c->ev_load)); }
+  return rc;
 }
 
 }  // extern "C"
@@ -440,6 +455,34 @@ int make_units(tpc_ctx* c, int* max_smem_cursor, long long* cursor_total, int* m
   return TPC_OK;
 }
 
+// Per-row constants, per-unit grid descriptors and K2/K3 work items for the clusters loaded now, computed on the host and uploaded
+// (asynchronously, on the context's stream).  Runs once per loaded frame: at the end of tpc_load_clusters_batch, or at the first
+// tpc_find_tracks* after per-unit loads.
+int prepare_tables(tpc_ctx* c) {
+  cudaStream_t st = c->stream;
+  const int U = c->NS * c->R;
+  std::vector<RowConst> rows;
+  make_params_and_rows(c, rows);
+  int rc = make_units(c, &c->t_msm, &c->t_cursor_total, &c->t_max_n, &c->t_max_perm, &c->t_max_yz);
+  if (rc != TPC_OK) return rc;
+  const int n_items = c->n_items;
+  CUDA_TRY(c, cudaEventSynchronize(c->ev_tables));   // an earlier upload may still be reading the pinned staging copy
+  CUDA_TRY(c, c->d_rows.ensure(rows.size() * sizeof(RowConst)));
+  CUDA_TRY(c, c->d_units.ensure((size_t)U * sizeof(UnitDesc)));
+  CUDA_TRY(c, c->d_items.ensure((size_t)std::max(n_items, 1) * sizeof(Item)));
+  CUDA_TRY(c, c->p_units.ensure((size_t)U * sizeof(UnitDesc) + rows.size() * sizeof(RowConst)));
+  CUDA_TRY(c, c->p_items.ensure((size_t)std::max(n_items, 1) * sizeof(Item)));
+  memcpy(c->p_units.p, c->h_units.data(), (size_t)U * sizeof(UnitDesc));
+  memcpy((char*)c->p_units.p + (size_t)U * sizeof(UnitDesc), rows.data(), rows.size() * sizeof(RowConst));
+  if (n_items) memcpy(c->p_items.p, c->h_items.data(), (size_t)n_items * sizeof(Item));
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_units.p, c->p_units.p, (size_t)U * sizeof(UnitDesc), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_rows.p, (char*)c->p_units.p + (size_t)U * sizeof(UnitDesc), rows.size() * sizeof(RowConst), cudaMemcpyHostToDevice, st));
+  if (n_items) CUDA_TRY(c, cudaMemcpyAsync(c->d_items.p, c->p_items.p, (size_t)n_items * sizeof(Item), cudaMemcpyHostToDevice, st));
+  CUDA_TRY(c, cudaEventRecord(c->ev_tables, st));
+  c->tables_ready = true;
+  return TPC_OK;
+}
+
 int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   if (!c || !out) return fail(c, TPC_E_ARG, "tpc_find_tracks: null argument");
   memset(out, 0, sizeof(*out));
@@ -450,17 +493,13 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   c->have_result = false;
   tpc_timings& tm = c->timings; memset(&tm, 0, sizeof(tm));
 
-  // ---- host tables
-  std::vector<RowConst> rows;
-  make_params_and_rows(c, rows);
-  int msm = 0, max_n = 0, max_perm = 0, max_yz = 0; long long cursor_total = 0;
-  int rc = make_units(c, &msm, &cursor_total, &max_n, &max_perm, &max_yz);
+  CUDA_TRY(c, cudaEventRecord(c->ev[0], st));
+  // ---- host tables (already computed and uploaded by tpc_load_clusters_batch; per-unit loads: here) + staged host clusters
+  int rc = c->tables_ready ? (int)TPC_OK : prepare_tables(c);
   if (rc != TPC_OK) return rc;
+  const int msm = c->t_msm, max_n = c->t_max_n, max_perm = c->t_max_perm, max_yz = c->t_max_yz; const long long cursor_total = c->t_cursor_total;
   const long long N = c->N; const int n_items = c->n_items; const int chunk = c->T.chunk;
   const Params& P = c->P;
-
-  CUDA_TRY(c, cudaEventRecord(c->ev[0], st));
-  // ---- upload: staged host clusters + tables
   CUDA_TRY(c, c->d_in_y.ensure_keep((size_t)(c->arena_pos + 16) * 4, (size_t)c->arena_pos * 4, st));
   CUDA_TRY(c, c->d_in_t.ensure_keep((size_t)(c->arena_pos + 16) * 4, (size_t)c->arena_pos * 4, st));
   for (auto& rg : c->dirty) {
@@ -469,18 +508,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
     CUDA_TRY(c, cudaMemcpyAsync(c->d_in_t.as<float>() + rg.first, c->h_t.as<float>() + rg.first, b, cudaMemcpyHostToDevice, st));
   }
   c->dirty.clear();
-  CUDA_TRY(c, c->d_rows.ensure(rows.size() * sizeof(RowConst)));
-  CUDA_TRY(c, c->d_units.ensure((size_t)U * sizeof(UnitDesc)));
-  CUDA_TRY(c, c->d_items.ensure((size_t)std::max(n_items, 1) * sizeof(Item)));
-  CUDA_TRY(c, c->p_units.ensure((size_t)U * sizeof(UnitDesc) + rows.size() * sizeof(RowConst)));
-  CUDA_TRY(c, c->p_items.ensure((size_t)std::max(n_items, 1) * sizeof(Item)));
   CUDA_TRY(c, c->p_small.ensure(256));
-  memcpy(c->p_units.p, c->h_units.data(), (size_t)U * sizeof(UnitDesc));
-  memcpy((char*)c->p_units.p + (size_t)U * sizeof(UnitDesc), rows.data(), rows.size() * sizeof(RowConst));
-  if (n_items) memcpy(c->p_items.p, c->h_items.data(), (size_t)n_items * sizeof(Item));
-  CUDA_TRY(c, cudaMemcpyAsync(c->d_units.p, c->p_units.p, (size_t)U * sizeof(UnitDesc), cudaMemcpyHostToDevice, st));
-  CUDA_TRY(c, cudaMemcpyAsync(c->d_rows.p, (char*)c->p_units.p + (size_t)U * sizeof(UnitDesc), rows.size() * sizeof(RowConst), cudaMemcpyHostToDevice, st));
-  if (n_items) CUDA_TRY(c, cudaMemcpyAsync(c->d_items.p, c->p_items.p, (size_t)n_items * sizeof(Item), cudaMemcpyHostToDevice, st));
   CUDA_TRY(c, cudaEventRecord(c->ev[1], st));
 
   // ---- buffers of S1..S4
@@ -521,125 +549,158 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
                                       c->d_link_dn.as<int>(), c->d_mask.as<unsigned>(), c->d_item_count.as<int>(), c->d_item_base.as<int>(),
                                       c->d_scan_tmp.as<int>(), c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), d_nstart, P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[4], st));
-  CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(c, cudaStreamSynchronize(st));
-  int M = *c->p_small.as<int>();
-  if (M < 0 || M > start_cap) return fail(c, TPC_E_CUDA, "start-hit count %d out of range", M);
-  const bool rescue = c->T.bridge_rows > 0 && c->T.bridge_rescue && M > 0;
-  if (c->T.bridge_rows > 0 && !rescue && M > 0) {   // S4' (NEXT-2 variant): drop the start hits that continue a lower chain, order kept
-    const size_t Mb = (size_t)M * 4;
-    CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
-    CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
-    LAUNCH_TRY(c, launch_k3_bridge(L, M, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
-                                   c->d_yz.as<float2>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(), c->d_link_dn.as<int>(),
-                                   c->d_keep.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), c->d_start_unit2.as<int>(),
-                                   c->d_start_pos2.as<int>(), d_nstart, P), launches);
-    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(c, cudaStreamSynchronize(st));
-    const int M2 = *c->p_small.as<int>();
-    if (M2 < 0 || M2 > M) return fail(c, TPC_E_CUDA, "bridged start-hit count %d out of range", M2);
-    if (M2 > 0) {
-      CUDA_TRY(c, cudaMemcpyAsync(c->d_start_unit.p, c->d_start_unit2.p, (size_t)M2 * 4, cudaMemcpyDeviceToDevice, st));
-      CUDA_TRY(c, cudaMemcpyAsync(c->d_start_pos.p, c->d_start_pos2.p, (size_t)M2 * 4, cudaMemcpyDeviceToDevice, st));
-    }
-    CUDA_TRY(c, cudaEventRecord(c->ev[4], st));   // the S4' pass counts as part of K3's time
-    M = M2;
-  }
-  if (M > (1 << 24)) return fail(c, TPC_E_CAPACITY, "%d tracklets exceed the 2^24 capacity of the selector key", M);
-  const long long Mpad = ((long long)M + 31) & ~31LL;
-  c->M = M; c->Mpad = Mpad;
-
-  // ---- K5: S5
-  const size_t Mz = (size_t)std::max(M, 1);
-  CUDA_TRY(c, c->d_rowhit.ensure((size_t)std::max(Mpad, 32LL) * R * 4));
-  CUDA_TRY(c, c->d_k5scratch.ensure(k5_scratch_bytes(M)));
-  CUDA_TRY(c, c->d_tl_n.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_first.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_last.ensure(Mz * 4));
-  CUDA_TRY(c, c->d_tl_chi2.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_par.ensure(Mz * 20)); CUDA_TRY(c, c->d_tl_cov.ensure(Mz * 60));
-  CUDA_TRY(c, c->d_owner.ensure((size_t)(N + 4) * 8)); CUDA_TRY(c, c->d_tl_key.ensure(Mz * 8));
-  CUDA_TRY(c, c->d_scan_in.ensure(Mz * 8)); CUDA_TRY(c, c->d_scan_out.ensure(Mz * 8));
-  CUDA_TRY(c, c->d_scan_tmp64.ensure((size_t)(M / SCAN_TILE + 4) * 8));
+  typedef unsigned long long u64;
   unsigned long long* d_k5cnt = (unsigned long long*)(c->d_counters.as<char>() + 128);
-  CUDA_TRY(c, cudaMemsetAsync(d_k5cnt, 0, 32, st));
-  auto run_k5 = [&](int n_run, const int* list) -> int {
-    LAUNCH_TRY(c, launch_k5_tracklets(L, n_run, M, list, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
-                                      c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
-                                      c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
-                                      c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt,
-                                      c->d_k5scratch.p, P), launches);
-    return TPC_OK;
-  };
-  long long n_fitted = M;
-  if (!rescue) {
-    rc = run_k5(M, nullptr);
-    if (rc != TPC_OK) return rc;
-  } else {
-    // S4' with rescue (reading A39c): first wave = the start hits that are not bridged; second wave = the bridged ones whose chain
-    // the first wave did not use completely.  Tracklet index = position in the full S4 list in both waves; the others keep n = 0.
-    const size_t Mb = (size_t)M * 4;
-    CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
-    CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_flag2.ensure(Mb));
-    CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
-    CUDA_TRY(c, cudaMemsetAsync(c->d_tl_n.p, 0, Mb, st));
-    CUDA_TRY(c, cudaMemsetAsync(c->d_tl_first.p, 0xff, Mb, st)); CUDA_TRY(c, cudaMemsetAsync(c->d_tl_last.p, 0xff, Mb, st));
-    int* list1 = c->d_start_unit2.as<int>(); int* list2 = c->d_start_pos2.as<int>();
-    LAUNCH_TRY(c, launch_k3_bridge_lists(L, M, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
-                                         c->d_yz.as<float2>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(), c->d_link_dn.as<int>(),
-                                         c->d_keep.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), list1, d_nstart, P), launches);
-    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(c, cudaStreamSynchronize(st));
-    const int M1 = *c->p_small.as<int>();
-    if (M1 < 0 || M1 > M) return fail(c, TPC_E_CUDA, "first-wave start-hit count %d out of range", M1);
-    rc = run_k5(M1, list1);
-    if (rc != TPC_OK) return rc;
-    // first half of the selector over the first wave: its owner keys are the "used" marks of the rescue test
-    CUDA_TRY(c, cudaMemsetAsync(c->d_owner.p, 0, (size_t)std::max(N, 1LL) * 8, st));
-    CUDA_TRY(c, cudaMemsetAsync(c->d_tl_key.p, 0, Mz * 8, st));
-    LAUNCH_TRY(c, launch_k6_owner(L, M1, list1, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
-                                  c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned long long*)c->d_owner.p,
-                                  (unsigned long long*)c->d_tl_key.p, P), launches);
-    LAUNCH_TRY(c, launch_k3_rescue_list(L, M, M1, list1, c->d_keep.as<int>(), c->d_start_unit.as<int>(), c->d_start_pos.as<int>(),
-                                        c->d_units.as<UnitDesc>(), c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
-                                        c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (const unsigned long long*)c->d_owner.p, N,
-                                        c->d_flag2.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), list2, d_nstart, P), launches);
-    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(c, cudaStreamSynchronize(st));
-    const int M2 = *c->p_small.as<int>();
-    if (M2 < 0 || M2 > M - M1) return fail(c, TPC_E_CUDA, "rescue-wave start-hit count %d out of range", M2);
-    if (M2 > 0) {
-      rc = run_k5(M2, list2);
+  const bool variant = c->T.bridge_rows > 0;
+  // Default path: NO device -> host read between K3 and the end of the call.  The number of start hits M stays in device memory
+  // (d_nstart); the per-tracklet buffers are sized for a capacity M_cap guessed from the frame size and from the previous call, the
+  // kernels read M themselves, and the guess is checked when the counters are read at the end (a frame that exceeds it is
+  // processed again from K5 with larger buffers: the S1-S4 tables stay valid).  The seed-bridging variants (off by default) size
+  // their run lists on the host and keep the read-backs.
+  long long M_cap = std::min<long long>(start_cap, std::max<long long>(c->m_cap_hint, N / 12 + 1024));
+  int M = -1;                    // known on the host only in the variants, or at the end
+  long long nt = 0, nr = 0, n_fitted = 0;
+  for (int attempt = 0;; attempt++) {
+    bool rescue = false;
+    if (variant) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaStreamSynchronize(st));
+      M = *c->p_small.as<int>();
+      if (M < 0 || M > start_cap) return fail(c, TPC_E_CUDA, "start-hit count %d out of range", M);
+      rescue = c->T.bridge_rescue && M > 0;
+      if (!rescue && M > 0) {   // S4' (NEXT-2 variant): drop the start hits that continue a lower chain, order kept
+        const size_t Mb = (size_t)M * 4;
+        CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
+        CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
+        LAUNCH_TRY(c, launch_k3_bridge(L, M, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
+                                       c->d_yz.as<float2>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(), c->d_link_dn.as<int>(),
+                                       c->d_keep.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), c->d_start_unit2.as<int>(),
+                                       c->d_start_pos2.as<int>(), d_nstart, P), launches);
+        CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+        const int M2 = *c->p_small.as<int>();
+        if (M2 < 0 || M2 > M) return fail(c, TPC_E_CUDA, "bridged start-hit count %d out of range", M2);
+        if (M2 > 0) {
+          CUDA_TRY(c, cudaMemcpyAsync(c->d_start_unit.p, c->d_start_unit2.p, (size_t)M2 * 4, cudaMemcpyDeviceToDevice, st));
+          CUDA_TRY(c, cudaMemcpyAsync(c->d_start_pos.p, c->d_start_pos2.p, (size_t)M2 * 4, cudaMemcpyDeviceToDevice, st));
+        }
+        CUDA_TRY(c, cudaEventRecord(c->ev[4], st));   // the S4' pass counts as part of K3's time
+        M = M2;
+      }
+      M_cap = M;
+    }
+    if (M_cap > (1 << 24)) M_cap = 1 << 24;      // capacity of the selector key; a larger M is reported below
+    const int Mc = (int)M_cap;
+    const int* d_M = variant ? nullptr : d_nstart;   // where the kernels read the tracklet count
+
+    // ---- K5: S5
+    const size_t Mz = (size_t)std::max(Mc, 1);
+    CUDA_TRY(c, c->d_rowhit.ensure((size_t)(Mz + 32) * R * 4));
+    CUDA_TRY(c, c->d_k5scratch.ensure(k5_scratch_bytes(Mc)));
+    CUDA_TRY(c, c->d_tl_n.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_first.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_last.ensure(Mz * 4));
+    CUDA_TRY(c, c->d_tl_chi2.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_par.ensure(Mz * 20)); CUDA_TRY(c, c->d_tl_cov.ensure(Mz * 60));
+    CUDA_TRY(c, c->d_owner.ensure((size_t)(N + 4) * 8)); CUDA_TRY(c, c->d_tl_key.ensure(Mz * 8));
+    CUDA_TRY(c, c->d_scan_in.ensure(Mz * 8)); CUDA_TRY(c, c->d_scan_out.ensure(Mz * 8));
+    CUDA_TRY(c, c->d_scan_tmp64.ensure((size_t)(Mc / SCAN_TILE + 4) * 8));
+    CUDA_TRY(c, cudaMemsetAsync(d_k5cnt, 0, 32, st));
+    auto run_k5 = [&](int n_run, const int* d_n, const int* list) -> int {
+      LAUNCH_TRY(c, launch_k5_tracklets(L, n_run, d_n, Mc, list, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
+                                        c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
+                                        c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
+                                        c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt,
+                                        c->d_k5scratch.p, P), launches);
+      return TPC_OK;
+    };
+    n_fitted = -1;                 // = M unless the rescue variant skipped duplicates
+    if (!rescue) {
+      rc = run_k5(Mc, d_M, nullptr);
       if (rc != TPC_OK) return rc;
-      LAUNCH_TRY(c, launch_k6_owner(L, M2, list2, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
+    } else {
+      // S4' with rescue (reading A39c): first wave = the start hits that are not bridged; second wave = the bridged ones whose chain
+      // the first wave did not use completely.  Tracklet index = position in the full S4 list in both waves; the others keep n = 0.
+      const size_t Mb = (size_t)M * 4;
+      CUDA_TRY(c, c->d_keep.ensure(Mb)); CUDA_TRY(c, c->d_keep_pos.ensure(Mb)); CUDA_TRY(c, c->d_start_unit2.ensure(Mb));
+      CUDA_TRY(c, c->d_start_pos2.ensure(Mb)); CUDA_TRY(c, c->d_flag2.ensure(Mb));
+      CUDA_TRY(c, c->d_scan_tmp.ensure((size_t)(std::max(M, n_items) / SCAN_TILE + 4) * 4));
+      CUDA_TRY(c, cudaMemsetAsync(c->d_tl_n.p, 0, Mb, st));
+      CUDA_TRY(c, cudaMemsetAsync(c->d_tl_first.p, 0xff, Mb, st)); CUDA_TRY(c, cudaMemsetAsync(c->d_tl_last.p, 0xff, Mb, st));
+      int* list1 = c->d_start_unit2.as<int>(); int* list2 = c->d_start_pos2.as<int>();
+      LAUNCH_TRY(c, launch_k3_bridge_lists(L, M, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
+                                           c->d_yz.as<float2>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(), c->d_link_dn.as<int>(),
+                                           c->d_keep.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), list1, d_nstart, P), launches);
+      CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaStreamSynchronize(st));
+      const int M1 = *c->p_small.as<int>();
+      if (M1 < 0 || M1 > M) return fail(c, TPC_E_CUDA, "first-wave start-hit count %d out of range", M1);
+      rc = run_k5(M1, nullptr, list1);
+      if (rc != TPC_OK) return rc;
+      // first half of the selector over the first wave: its owner keys are the "used" marks of the rescue test
+      CUDA_TRY(c, cudaMemsetAsync(c->d_owner.p, 0, (size_t)std::max(N, 1LL) * 8, st));
+      CUDA_TRY(c, cudaMemsetAsync(c->d_tl_key.p, 0, Mz * 8, st));
+      LAUNCH_TRY(c, launch_k6_owner(L, M1, list1, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
                                     c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned long long*)c->d_owner.p,
                                     (unsigned long long*)c->d_tl_key.p, P), launches);
+      LAUNCH_TRY(c, launch_k3_rescue_list(L, M, c->d_keep.as<int>(), c->d_start_unit.as<int>(), c->d_start_pos.as<int>(),
+                                          c->d_units.as<UnitDesc>(), c->d_link_up.as<int>(), (const unsigned long long*)c->d_owner.p,
+                                          c->d_flag2.as<int>(), c->d_keep_pos.as<int>(), c->d_scan_tmp.as<int>(), list2, d_nstart), launches);
+      CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaStreamSynchronize(st));
+      const int M2 = *c->p_small.as<int>();
+      if (M2 < 0 || M2 > M - M1) return fail(c, TPC_E_CUDA, "rescue-wave start-hit count %d out of range", M2);
+      if (M2 > 0) {
+        rc = run_k5(M2, nullptr, list2);
+        if (rc != TPC_OK) return rc;
+        LAUNCH_TRY(c, launch_k6_owner(L, M2, list2, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
+                                      c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned long long*)c->d_owner.p,
+                                      (unsigned long long*)c->d_tl_key.p, P), launches);
+      }
+      n_fitted = (long long)M1 + M2;
     }
-    n_fitted = (long long)M1 + M2;
-  }
-  CUDA_TRY(c, cudaEventRecord(c->ev[5], st));
+    CUDA_TRY(c, cudaEventRecord(c->ev[5], st));
 
-  // ---- K6: S6
-  typedef unsigned long long u64;
-  LAUNCH_TRY(c, launch_k6_select(L, M, Mpad, N, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
-                                 c->d_perm.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(),
-                                 c->d_tl_chi2.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
-                                 c->d_scan_out.as<u64>(), c->d_scan_tmp64.as<u64>(), d_total64, P, rescue), launches);
-  CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 64, d_total64, 8, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 128, d_k5cnt, 24, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(c, cudaStreamSynchronize(st));
-  const u64 total = *(u64*)(c->p_small.as<char>() + 64);
-  const long long nt = (long long)(total >> 40), nr = (long long)(total & ((1ull << 40) - 1ull));
+    // ---- K6: S6.  Output capacity: every tracklet a track, every cluster referenced once (a cluster has one owner).
+    const long long cap_tracks = std::max<long long>(Mc, 1), cap_refs = std::max<long long>(N, 1);
+    CUDA_TRY(c, c->o_sector.ensure(cap_tracks * 4)); CUDA_TRY(c, c->o_x.ensure(cap_tracks * 4)); CUDA_TRY(c, c->o_par.ensure(cap_tracks * 20));
+    CUDA_TRY(c, c->o_cov.ensure(cap_tracks * 60)); CUDA_TRY(c, c->o_chi2.ensure(cap_tracks * 4)); CUDA_TRY(c, c->o_ndf.ensure(cap_tracks * 4));
+    CUDA_TRY(c, c->o_tracklet.ensure(cap_tracks * 4)); CUDA_TRY(c, c->o_cl_begin.ensure((cap_tracks + 1) * 8));
+    CUDA_TRY(c, c->o_cl_row.ensure(cap_refs * 4)); CUDA_TRY(c, c->o_cl_index.ensure(cap_refs * 4));
+    LAUNCH_TRY(c, launch_k6_select(L, Mc, d_M, N, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(),
+                                   c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(),
+                                   c->d_tl_chi2.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
+                                   c->d_scan_out.as<u64>(), c->d_scan_tmp64.as<u64>(), d_total64, P, rescue), launches);
+    LAUNCH_TRY(c, launch_k6_emit(L, Mc, d_M, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_perm.as<int>(),
+                                 c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(),
+                                 c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
+                                 c->d_scan_out.as<u64>(), c->o_sector.as<int>(), c->o_x.as<float>(), c->o_par.as<float>(), c->o_cov.as<float>(),
+                                 c->o_chi2.as<float>(), c->o_ndf.as<int>(), c->o_tracklet.as<int>(), c->o_cl_begin.as<long long>(),
+                                 c->o_cl_row.as<int>(), c->o_cl_index.as<int>(), d_total64, cap_tracks, cap_refs, P), launches);
+    CUDA_TRY(c, cudaEventRecord(c->ev[6], st));
+
+    // ---- the one read-back of the call: start-hit count, (tracks, references), S5 work counters
+    if (!variant) CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 64, d_total64, 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 128, d_k5cnt, 24, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    if (!variant) {
+      M = *c->p_small.as<int>();
+      if (M < 0 || M > start_cap) return fail(c, TPC_E_CUDA, "start-hit count %d out of range", M);
+      if (M > (1 << 24)) return fail(c, TPC_E_CAPACITY, "%d tracklets exceed the 2^24 capacity of the selector key", M);
+      if (M > M_cap) {             // the capacity guess was too small: repeat S5 / S6 with room for all M start hits
+        if (attempt >= 2) return fail(c, TPC_E_CUDA, "tracklet capacity did not converge (%d start hits)", M);
+        M_cap = std::min<long long>(start_cap, (long long)M + M / 8 + 1024);
+        continue;
+      }
+    } else if (M > (1 << 24)) return fail(c, TPC_E_CAPACITY, "%d tracklets exceed the 2^24 capacity of the selector key", M);
+    const u64 total = *(u64*)(c->p_small.as<char>() + 64);
+    nt = (long long)(total >> 40); nr = (long long)(total & ((1ull << 40) - 1ull));
+    if (nt > cap_tracks || nr > cap_refs) return fail(c, TPC_E_CUDA, "selector totals out of range (%lld tracks, %lld references)", nt, nr);
+    if (n_fitted < 0) n_fitted = M;
+    break;
+  }
+  c->m_cap_hint = (long long)M + M / 4 + 1024;   // next frame: 25 % headroom over this one
+  c->M = M; c->Mpad = ((long long)M + 31) & ~31LL;
   c->n_tracks = nt; c->n_refs = nr;
   const size_t ntz = (size_t)std::max(nt, 1LL), nrz = (size_t)std::max(nr, 1LL);
-  CUDA_TRY(c, c->o_sector.ensure(ntz * 4)); CUDA_TRY(c, c->o_x.ensure(ntz * 4)); CUDA_TRY(c, c->o_par.ensure(ntz * 20));
-  CUDA_TRY(c, c->o_cov.ensure(ntz * 60)); CUDA_TRY(c, c->o_chi2.ensure(ntz * 4)); CUDA_TRY(c, c->o_ndf.ensure(ntz * 4));
-  CUDA_TRY(c, c->o_tracklet.ensure(ntz * 4)); CUDA_TRY(c, c->o_cl_begin.ensure((ntz + 1) * 8));
-  CUDA_TRY(c, c->o_cl_row.ensure(nrz * 4)); CUDA_TRY(c, c->o_cl_index.ensure(nrz * 4));
-  LAUNCH_TRY(c, launch_k6_emit(L, M, Mpad, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_perm.as<int>(),
-                               c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(),
-                               c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
-                               c->d_scan_out.as<u64>(), c->o_sector.as<int>(), c->o_x.as<float>(), c->o_par.as<float>(), c->o_cov.as<float>(),
-                               c->o_chi2.as<float>(), c->o_ndf.as<int>(), c->o_tracklet.as<int>(), c->o_cl_begin.as<long long>(),
-                               c->o_cl_row.as<int>(), c->o_cl_index.as<int>(), nt, nr, P), launches);
-  CUDA_TRY(c, cudaEventRecord(c->ev[6], st));
 
   // ---- result
   out->n_tracks = nt; out->n_cluster_refs = nr;

@@ -106,23 +106,22 @@ int launch_k3_bridge(const Launch& L, int M, const int* d_start_unit, const int*
 int launch_k3_bridge_lists(const Launch& L, int M, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
                            const RowConst* d_rows, const float2* d_yz, const int* d_bin_start, const int* d_link_up, const int* d_link_dn,
                            int* d_keep, int* d_pos, int* d_scan_tmp, int* d_list1, int* d_total, const Params& P);
-int launch_k3_rescue_list(const Launch& L, int M, int M1, const int* d_list1, const int* d_keep, const int* d_start_unit,
-                          const int* d_start_pos, const UnitDesc* d_units, const int* d_link_up, const int* d_rowhit, const int* d_tl_n,
-                          const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, const unsigned long long* d_owner, long long N,
-                          int* d_flag2, int* d_pos, int* d_scan_tmp, int* d_list2, int* d_total, const Params& P);
+int launch_k3_rescue_list(const Launch& L, int M, const int* d_keep, const int* d_start_unit, const int* d_start_pos,
+                          const UnitDesc* d_units, const int* d_link_up, const unsigned long long* d_owner,
+                          int* d_flag2, int* d_pos, int* d_scan_tmp, int* d_list2, int* d_total);
 
 int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, int* d_link_up,
                           int* d_link_dn, unsigned* d_mask, int* d_item_count, int* d_item_base, int* d_scan_tmp,
                           int* d_start_unit, int* d_start_pos, int* d_total, const Params& P);
 
 size_t k5_scratch_bytes(long long M);   // handoff records + task lists + control block of the K5 phase kernels
-int launch_k5_tracklets(const Launch& L, int n_run, int M, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
+int launch_k5_tracklets(const Launch& L, int n_run, const int* d_n_run, int M, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
                         const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
                         const int* d_link_up, int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2,
                         float* d_tl_par, float* d_tl_cov, unsigned long long* d_counters, void* d_scratch, const Params& P);
 
-int launch_k6_select(const Launch& L, int M, long long Mpad, long long N, const int* d_start_unit, const UnitDesc* d_units,
-                     const RowConst* d_rows, const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
+int launch_k6_select(const Launch& L, int M_cap, const int* d_M, long long N, const int* d_start_unit, const UnitDesc* d_units,
+                     const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
                      const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
                      unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
                      unsigned long long* d_total, const Params& P, bool owner_done);
@@ -130,12 +129,13 @@ int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int
                     const int* d_tl_n, const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner,
                     unsigned long long* d_tl_key, const Params& P);
 
-int launch_k6_emit(const Launch& L, int M, long long Mpad, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
+int launch_k6_emit(const Launch& L, int M_cap, const int* d_M, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
                    const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
                    const float* d_tl_chi2, const float* d_tl_par, const float* d_tl_cov, const unsigned long long* d_owner,
                    const unsigned long long* d_tl_key, const unsigned long long* d_scan_in, const unsigned long long* d_scan_out,
                    int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,
-                   long long* o_cl_begin, int* o_cl_row, int* o_cl_index, long long n_tracks, long long n_refs, const Params& P);
+                   long long* o_cl_begin, int* o_cl_row, int* o_cl_index, const unsigned long long* d_total, long long cap_tracks,
+                   long long cap_refs, const Params& P);
 
 int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, const int* o_tracklet, const long long* o_cl_begin,
                     const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_rowhit,
