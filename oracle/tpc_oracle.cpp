@@ -58,6 +58,7 @@ struct Tunables {            // DESIGN.md table T (all are readings; the paper i
   double bridge_wy = 1.0, bridge_wz = 1.5;
   int bridge_min = 3;           // clusters the lower chain must have
   int bridge_rescue = 0;        // 1: dropped start hits get their tracklet after all when the first wave left their chain unused
+  int link_skip = 0;            // NEXT-2 as SURVEY 8(f).2 wrote it (reading A45): 1 = a link may skip one pad row
   double tube = 1.5;            // NEXT-4: radius of the tube around a track, cm
   // NEXT-3 (reading A41): cross-sector segment matching
   double merge_edge = 3.0; int merge_rows = 8; double merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05;
@@ -85,6 +86,7 @@ struct Oracle : OracleBase {
   bool continuous;
   // per-row constants (double -> Real once)
   std::vector<Real> X, tu, td, ar, br, thr, wzu, wzd, yedge;
+  std::vector<Real> tu2, td2, ar2, br2, wzu2, wzd2, thr21, thr12, thr22;   // S2' (link_skip): the same constants for a row distance of 2
   Real cB;
   // clusters
   int64_t N = 0; std::vector<int64_t> off;           // [U+1]
@@ -96,6 +98,7 @@ struct Oracle : OracleBase {
   std::vector<double> g_ylo_d, g_zlo_d, g_invs_d;
   // S2/S3
   std::vector<int32_t> link_up, link_dn, clean_up, clean_dn;
+  std::vector<int32_t> link_up_k, link_dn_k, clean_up_k, clean_dn_k;   // row distance of each link (1, or 2 with link_skip; 0 = no link)
   // S4
   std::vector<int32_t> start_unit, start_pos;
   // S5
@@ -128,6 +131,18 @@ struct Oracle : OracleBase {
       thr[r] = (Real)(T.cut2 * 0.5 * (a * a + b * b));
       wzu[r] = (Real)(T.dzdx_max * a + T.wz0); wzd[r] = (Real)(T.dzdx_max * b + T.wz0);
       yedge[r] = (Real)(x * std::tan(0.5 * dphi));
+    }
+    // S2' (reading A45): row distance 2 upwards (index "2" first) / downwards; thr_{ku kd} = cut2 * 0.5 * (a_ku^2 + b_kd^2)
+    tu2.assign(R, 1); td2.assign(R, 1); ar2.assign(R, 0); br2.assign(R, 0); wzu2.assign(R, 0); wzd2.assign(R, 0);
+    thr21.assign(R, 0); thr12.assign(R, 0); thr22.assign(R, 0);
+    for (int r = 0; r < R; r++) {
+      double x = row_x[r], xu = r + 1 < R ? row_x[r + 1] : x, xd = r > 0 ? row_x[r - 1] : x;
+      double xu2 = r + 2 < R ? row_x[r + 2] : x, xd2 = r > 1 ? row_x[r - 2] : x;
+      double a = xu - x, b = x - xd, a2 = xu2 - x, b2 = x - xd2;
+      tu2[r] = (Real)(xu2 / x); td2[r] = (Real)(xd2 / x); ar2[r] = (Real)a2; br2[r] = (Real)b2;
+      wzu2[r] = (Real)(T.dzdx_max * a2 + T.wz0); wzd2[r] = (Real)(T.dzdx_max * b2 + T.wz0);
+      thr21[r] = (Real)(T.cut2 * 0.5 * (a2 * a2 + b * b)); thr12[r] = (Real)(T.cut2 * 0.5 * (a * a + b2 * b2));
+      thr22[r] = (Real)(T.cut2 * 0.5 * (a2 * a2 + b2 * b2));
     }
     cB = (Real)(-0.00299792458 * bz);
   }
@@ -201,7 +216,7 @@ struct Oracle : OracleBase {
 
   // ---- S2: neighbour finder -- best (up,down) pair by collinearity, window centred on the from-origin projection ----
   void s2_neighbours(bool brute) {
-    link_up.assign(N, -1); link_dn.assign(N, -1);
+    link_up.assign(N, -1); link_dn.assign(N, -1); link_up_k.assign(N, 0); link_dn_k.assign(N, 0);
     const Real wy = (Real)T.wy, wz = (Real)T.wz;
     std::vector<int32_t> cu, cd;
     for (int sec = 0; sec < NS; sec++)
@@ -232,21 +247,85 @@ struct Oracle : OracleBase {
               if (!have || D < bestD || (D == bestD && (iu < bpu || (iu == bpu && id < bpd)))) {
                 have = true; bestD = D; bu = pu; bd = pd; bpu = iu; bpd = id; }
             }
-          if (have && bestD < thr[r]) { link_up[o + h] = bu; link_dn[o + h] = bd; }
+          if (have && bestD < thr[r]) { link_up[o + h] = bu; link_dn[o + h] = bd; link_up_k[o + h] = 1; link_dn_k[o + h] = 1; }
+        }
+      }
+    if (T.link_skip) s2_skip_links(brute);
+  }
+
+  // ---- S2' (NEXT-2 as SURVEY.md section 8(f).2 wrote it: "links that may skip a row"; reading A45; off unless link_skip = 1).
+  //      A hit WITHOUT an accepted pair on the adjacent rows (S2 above is unchanged and final for the others) looks one row
+  //      further: candidates on rows r+1, r+2 / r-1, r-2 in the windows of S2 scaled to the row distance k (centre y * x_{r+-k}/x_r;
+  //      half-width k*wy; z: centre z * x_{r+-k}/x_r with half-width k*wz in triggered mode, centre z with half-width
+  //      dzdx_max*|dx| + wz0 in continuous mode).  Pair residual as in S2 with the actual distances a = x_u - x_r, b = x_r - x_d:
+  //      ey = b (y_u - y) - a (y - y_d), ez likewise, D = ey^2 + ez^2, accepted iff D < cut2 * 0.5 * (a^2 + b^2).
+  //      Level 3: pairs that skip one row on one side, (k_u, k_d) = (2,1) and (1,2); if none is accepted, level 4: (2,2).
+  //      Within a level the accepted pair with the minimum key (D, k_u, original index of up, original index of down) wins.
+  void s2_skip_links(bool brute) {
+    const Real wy = (Real)T.wy, wz = (Real)T.wz;
+    std::vector<int32_t> cu[3], cd[3];   // [k] candidates at row distance k
+    for (int sec = 0; sec < NS; sec++)
+      for (int r = 1; r <= R - 2; r++) {
+        const int u = sec * R + r; const int64_t o = off[u], n = off[u + 1] - o;
+        for (int64_t h = 0; h < n; h++) {
+          if (link_up[o + h] >= 0) continue;
+          const Real y = ys[o + h], zz = zs[o + h];
+          for (int k = 1; k <= 2; k++) {
+            cu[k].clear(); cd[k].clear();
+            const Real kk = (Real)k;
+            if (r + k <= R - 1) {
+              const Real t_ = k == 1 ? tu[r] : tu2[r];
+              const Real yc = y * t_, zc = continuous ? zz : zz * t_, hwy = kk * wy, hw = continuous ? (k == 1 ? wzu[r] : wzu2[r]) : kk * wz;
+              const Real ylo = yc - hwy, yhi = yc + hwy, zlo = zc - hw, zhi = zc + hw;
+              const int64_t ou = off[u + k];
+              for_bins(u + k, ylo, yhi, zlo, zhi, brute, [&](int32_t p) {
+                const Real yu = ys[ou + p], zu = zs[ou + p];
+                if (yu >= ylo && yu <= yhi && zu >= zlo && zu <= zhi) cu[k].push_back(p); });
+            }
+            if (r - k >= 0) {
+              const Real t_ = k == 1 ? td[r] : td2[r];
+              const Real yc = y * t_, zc = continuous ? zz : zz * t_, hwy = kk * wy, hw = continuous ? (k == 1 ? wzd[r] : wzd2[r]) : kk * wz;
+              const Real ylo = yc - hwy, yhi = yc + hwy, zlo = zc - hw, zhi = zc + hw;
+              const int64_t od = off[u - k];
+              for_bins(u - k, ylo, yhi, zlo, zhi, brute, [&](int32_t p) {
+                const Real yd = ys[od + p], zd = zs[od + p];
+                if (yd >= ylo && yd <= yhi && zd >= zlo && zd <= zhi) cd[k].push_back(p); });
+            }
+          }
+          bool have = false; Real bestD = 0; int bku = 0, bkd = 0; int32_t bu = -1, bd = -1, bpu = 0, bpd = 0;
+          auto level = [&](int ku, int kd) {
+            const Real a = ku == 1 ? ar[r] : ar2[r], b = kd == 1 ? br[r] : br2[r];
+            const Real lim = ku == 1 ? thr12[r] : (kd == 1 ? thr21[r] : thr22[r]);
+            const int64_t ou = off[u + ku], od = off[u - kd];
+            for (int32_t pu : cu[ku])
+              for (int32_t pd : cd[kd]) {
+                Real dyu = ys[ou + pu] - y, dyd = y - ys[od + pd]; Real m1 = b * dyu, m2 = a * dyd; Real ey = m1 - m2;
+                Real dzu = zs[ou + pu] - zz, dzd = zz - zs[od + pd]; Real m3 = b * dzu, m4 = a * dzd; Real ez = m3 - m4;
+                Real e1 = ey * ey, e2 = ez * ez; Real D = e1 + e2;
+                if (!(D < lim)) continue;
+                const int32_t iu = perm[ou + pu], id = perm[od + pd];
+                if (!have || D < bestD || (D == bestD && (ku < bku || (ku == bku && (iu < bpu || (iu == bpu && id < bpd)))))) {
+                  have = true; bestD = D; bku = ku; bkd = kd; bu = pu; bd = pd; bpu = iu; bpd = id; }
+              }
+          };
+          level(1, 2); level(2, 1);
+          if (!have) level(2, 2);
+          if (have) { link_up[o + h] = bu; link_dn[o + h] = bd; link_up_k[o + h] = bku; link_dn_k[o + h] = bkd; }
         }
       }
   }
 
   // ---- S3: mutual-link cleaner (double-buffered definition) ----
   void s3_clean() {
-    clean_up.assign(N, -1); clean_dn.assign(N, -1);
+    clean_up.assign(N, -1); clean_dn.assign(N, -1); clean_up_k.assign(N, 0); clean_dn_k.assign(N, 0);
     for (int sec = 0; sec < NS; sec++)
       for (int r = 0; r < R; r++) {
         int u = sec * R + r; int64_t o = off[u], n = off[u + 1] - o;
         for (int64_t h = 0; h < n; h++) {
           int32_t up = link_up[o + h], dn = link_dn[o + h];
-          if (up >= 0 && r + 1 < R && link_dn[off[u + 1] + up] == (int32_t)h) clean_up[o + h] = up;
-          if (dn >= 0 && r > 0 && link_up[off[u - 1] + dn] == (int32_t)h) clean_dn[o + h] = dn;
+          const int ku = link_up_k[o + h], kd = link_dn_k[o + h];   // row distance of the link (1; 2 only with link_skip)
+          if (up >= 0 && r + ku < R && link_dn[off[u + ku] + up] == (int32_t)h && link_dn_k[off[u + ku] + up] == ku) { clean_up[o + h] = up; clean_up_k[o + h] = ku; }
+          if (dn >= 0 && r - kd >= 0 && link_up[off[u - kd] + dn] == (int32_t)h && link_up_k[off[u - kd] + dn] == kd) { clean_dn[o + h] = dn; clean_dn_k[o + h] = kd; }
         }
       }
   }
@@ -259,10 +338,10 @@ struct Oracle : OracleBase {
       for (int64_t h = 0; h < n; h++) {
         if (!(clean_dn[o + h] < 0 && clean_up[o + h] >= 0)) continue;
         int len = 1; int uu = u; int32_t p = (int32_t)h;
-        while (len < T.min_seed) { int32_t nx = clean_up[off[uu] + p]; if (nx < 0) break; p = nx; uu++; len++; }
+        while (len < T.min_seed) { int32_t nx = clean_up[off[uu] + p]; if (nx < 0) break; const int k = clean_up_k[off[uu] + p]; p = nx; uu += k; len++; }
         if (len < T.min_seed) continue;
         int wave = 1;
-        if (T.bridge_rows > 0 && bridged(u, (int32_t)h, brute)) { if (!T.bridge_rescue) continue; wave = 2; }
+        if (T.bridge_rows > 0 && !T.link_skip && bridged(u, (int32_t)h, brute)) { if (!T.bridge_rescue) continue; wave = 2; }
         start_unit.push_back(u); start_pos.push_back((int32_t)h); start_wave.push_back(wave);
       }
     }
@@ -484,8 +563,9 @@ struct Oracle : OracleBase {
       State saved = st; int r_out = r0;
       for (;;) {   // Phase A: follow the cleaned up-links, no gate
         int32_t up = clean_up[off[sec * R + r] + h]; if (up < 0) break;
-        if (!propagate_state(st, X[r + 1] - X[r])) { ok = false; break; }
-        r++; h = up; update_state(st, Y(r, h), Z(r, h) - zref); rowhit[r] = h; saved = st; r_out = r;
+        const int k = clean_up_k[off[sec * R + r] + h];     // 1; 2 = the link skips a row (S2', link_skip): one transport over both rows
+        if (!propagate_state(st, X[r + k] - X[r])) { ok = false; break; }
+        r += k; h = up; update_state(st, Y(r, h), Z(r, h) - zref); rowhit[r] = h; saved = st; r_out = r;
       }
       if (ok) {    // Phase B: extrapolate outward with pick-up
         int gap = 0;
@@ -767,7 +847,10 @@ struct Oracle : OracleBase {
     make_tables(); State st; to_state(st, par, cov); return pickup(sector, row, st, (Real)zref, brute != 0);
   }
   int set_links(const int32_t* up, const int32_t* dn) override {
-    clean_up.assign(up, up + N); clean_dn.assign(dn, dn + N); link_up = clean_up; link_dn = clean_dn; return 0;
+    clean_up.assign(up, up + N); clean_dn.assign(dn, dn + N); link_up = clean_up; link_dn = clean_dn;
+    clean_up_k.assign(N, 0); clean_dn_k.assign(N, 0);
+    for (int64_t g = 0; g < N; g++) { clean_up_k[g] = clean_up[g] >= 0; clean_dn_k[g] = clean_dn[g] >= 0; }
+    link_up_k = clean_up_k; link_dn_k = clean_dn_k; return 0;
   }
 
   // hand-built tracklets for S6 pins (requires S1 to have run so that perm/off exist)
@@ -809,6 +892,10 @@ struct Oracle : OracleBase {
     if (s == "grid_invs") RET(g_invs_d, 2)
     if (s == "link_up") RET(link_up, 0)
     if (s == "link_dn") RET(link_dn, 0)
+    if (s == "link_up_k") RET(link_up_k, 0)
+    if (s == "link_dn_k") RET(link_dn_k, 0)
+    if (s == "clean_up_k") RET(clean_up_k, 0)
+    if (s == "clean_dn_k") RET(clean_dn_k, 0)
     if (s == "clean_up") RET(clean_up, 0)
     if (s == "clean_dn") RET(clean_dn, 0)
     if (s == "start_unit") RET(start_unit, 0)
@@ -871,7 +958,7 @@ int orc_set_param(void* h, const char* name, double v) {
   else if (s == "c0_y") T.c0[0] = v; else if (s == "c0_z") T.c0[1] = v; else if (s == "c0_sinphi") T.c0[2] = v;
   else if (s == "c0_dzds") T.c0[3] = v; else if (s == "c0_qpt") T.c0[4] = v;
   else if (s == "grid_scale") T.grid_scale = v;
-  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "bridge_rescue") T.bridge_rescue = (int)v; else if (s == "tube") T.tube = v;
+  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "bridge_rescue") T.bridge_rescue = (int)v; else if (s == "tube") T.tube = v; else if (s == "link_skip") T.link_skip = (int)v;
   else if (s == "merge_edge") T.merge_edge = v; else if (s == "merge_rows") T.merge_rows = (int)v; else if (s == "merge_dy") T.merge_dy = v;
   else if (s == "merge_dz") T.merge_dz = v; else if (s == "merge_ds") T.merge_ds = v; else if (s == "merge_dt") T.merge_dt = v;
   else return -1;
