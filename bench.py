@@ -209,7 +209,8 @@ def run_gpu(args, rank, world, local_rank):
     variant = None
     if args.variant and rank == 0:
         variant = {}
-        for vname, vp in (("drop_bridged", dict(bridge_rows=4.0, bridge_min=8.0)),
+        for vname, vp in (("skip_links", dict(link_skip=1.0)),
+                          ("drop_bridged", dict(bridge_rows=4.0, bridge_min=8.0)),
                           ("rescue_wave", dict(bridge_rows=4.0, bridge_min=3.0, bridge_rescue=1.0))):
             with T.Tracker(**w.geometry(), **vp) as tv:
                 tv.set_stream(stream.cuda_stream)
@@ -228,9 +229,10 @@ def run_gpu(args, rank, world, local_rank):
                                   "n_start_hits": int(vt["n_start_hits"]), "n_tracklets_fitted": int(vt["n_tracklets_kept"]),
                                   "tracks_per_step": int(rv.n_tracks), "cluster_refs_per_step": int(rv.n_cluster_refs),
                                   "kernel_ms": {k: vt[k] for k in keys}}
-        variant["note"] = ("seed bridging (SURVEY 8(f).2, readings A39 / A39c): drop_bridged drops the start hits that continue a lower "
-                           "chain; rescue_wave fits them in a second K5 wave when the first left their chain unused; efficiency in "
-                           "DESIGN.md section 11")
+        variant["note"] = ("NEXT-2 variants (SURVEY 8(f).2), all off by default because they change the result: skip_links = S2', links "
+                           "that may skip one pad row (reading A45); seed bridging (readings A39 / A39c): drop_bridged drops the start hits "
+                           "that continue a lower chain, rescue_wave fits them in a second K5 wave when the first left their chain unused; "
+                           "efficiency versus generator truth in DESIGN.md section 11")
     # S7 (NEXT-1, not part of the timed S0..S6 step): refit over the owned clusters + collision time, device-resident result
     refit_ms = float(np.mean([trk.refit_tracks(device_result=True)["ms_refit"] for _ in range(4)][1:]))
 

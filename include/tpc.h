@@ -145,6 +145,9 @@ int tpc_create(const tpc_geometry* geometry, float bz_tesla, float vdrift_cm_per
 
 /* Tunables of DESIGN.md table T by name: wy wz dzdx_max wz0 cut2 min_seed c0_y c0_z c0_sinphi c0_dzds c0_qpt s_max n_sigma
  * w_max max_gap edge_margin min_hits grid_scale, plus debug_keep (1 = keep pre-cleaning link tables for tpc_debug_get_links) and
+ * link_skip (default 0; 1 = S2', the gap-tolerant seeding variant of SURVEY.md section 8(f).2: a cluster without an accepted pair on
+ * the adjacent rows may link over one missing row; changes the result), bridge_rows / bridge_min /
+ * bridge_rescue (seed-bridging variants, readings A39 / A39c; ignored with link_skip), and
  * pinned_async (default 0; 1 = a PINNED host source of tpc_load_clusters* is read by DMA on the context's stream AFTER the load call
  * has returned: the caller then keeps those buffers untouched until the next tpc_find_tracks* on the context returns.  With 0 the
  * load call returns only when the library has read its inputs, as the conventions above state).
@@ -193,6 +196,9 @@ int tpc_get_timings(tpc_ctx*, tpc_timings* out);
 int tpc_debug_get_grid(tpc_ctx*, int sector, int row, tpc_grid_view* out);
 /* cleaned = 0: S2 tables (needs debug_keep = 1), 1: after S3.  up/dn: [n] positions in the sorted order of row+1 / row-1, -1 = none. */
 int tpc_debug_get_links(tpc_ctx*, int sector, int row, int cleaned, const int32_t** up, const int32_t** dn, int32_t* n);
+/* Row distance of the links returned by the LAST tpc_debug_get_links call: 1 for a link to the adjacent row, 2 for a link that skips
+ * a row (only with tpc_set_param("link_skip", 1): S2' of DESIGN.md reading A45), 0 where there is no link.  [n] entries each. */
+int tpc_debug_get_link_rows(tpc_ctx*, const int8_t** up_k, const int8_t** dn_k, int32_t* n);
 /* start hits in list order: unit = sector*n_rows+row and sorted position. */
 int tpc_debug_get_start_hits(tpc_ctx*, const int32_t** unit, const int32_t** pos, int64_t* n);
 int tpc_debug_get_tracklets(tpc_ctx*, tpc_tracklet_view* out);

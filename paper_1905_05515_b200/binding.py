@@ -18,7 +18,7 @@ _SO = os.path.join(_HERE, "libtpc_b200.so")
 ABI_SYMBOLS = [
     "tpc_abi_version", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
     "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
-    "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
+    "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_link_rows", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
 
 _PF, _PI, _PL = C.POINTER(C.c_float), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
@@ -110,6 +110,7 @@ def load_library():
     lib.tpc_get_timings.argtypes = [vp, C.POINTER(_Timings)]
     lib.tpc_debug_get_grid.argtypes = [vp, C.c_int, C.c_int, C.POINTER(_GridView)]
     lib.tpc_debug_get_links.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(_PI), C.POINTER(_PI), C.POINTER(C.c_int32)]
+    lib.tpc_debug_get_link_rows.argtypes = [vp, C.POINTER(C.POINTER(C.c_int8)), C.POINTER(C.POINTER(C.c_int8)), C.POINTER(C.c_int32)]
     lib.tpc_debug_get_start_hits.argtypes = [vp, C.POINTER(_PI), C.POINTER(_PI), C.POINTER(C.c_int64)]
     lib.tpc_debug_get_tracklets.argtypes = [vp, C.POINTER(_TrackletView)]
     _lib = lib
@@ -386,6 +387,16 @@ class Tracker:
         if n.value == 0:
             return np.zeros(0, np.int32), np.zeros(0, np.int32)
         return (np.ctypeslib.as_array(up, shape=(n.value,)).copy(), np.ctypeslib.as_array(dn, shape=(n.value,)).copy())
+
+    def link_rows(self, sector, row, cleaned=True):
+        """(up, dn, up_k, dn_k): link positions and their row distances (1; 2 = the link skips a row, link_skip only; 0 = no link)."""
+        up, dn = self.links(sector, row, cleaned)
+        a, b, n = C.POINTER(C.c_int8)(), C.POINTER(C.c_int8)(), C.c_int32()
+        _check(self.h, load_library().tpc_debug_get_link_rows(self.h, C.byref(a), C.byref(b), C.byref(n)))
+        m = len(up)
+        if m == 0:
+            return up, dn, np.zeros(0, np.int8), np.zeros(0, np.int8)
+        return up, dn, np.ctypeslib.as_array(a, shape=(m,)).copy(), np.ctypeslib.as_array(b, shape=(m,)).copy()
 
     def start_hits(self):
         u, p, n = _PI(), _PI(), C.c_int64()

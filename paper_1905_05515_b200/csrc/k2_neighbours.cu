@@ -251,6 +251,173 @@ __global__ void __launch_bounds__(K2_THREADS) k2_neighbours(const Item* __restri
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------------
+// S2' (NEXT-2 as SURVEY.md section 8(f).2 wrote it: "links that may skip a row"; reading A45 of DESIGN.md; link_skip = 1 only).
+// Runs after k2_neighbours, one thread per cluster.  A cluster that S2 linked keeps its pair (the tables are re-encoded as
+// position << 1 | k - 1 with k = 1).  A cluster S2 left unlinked looks one row further: candidates on rows r+-1, r+-2 in the S2
+// windows scaled to the row distance k; pairs (k_u, k_d) = (1,2) and (2,1) first, (2,2) only if none of those is accepted; a pair
+// is accepted iff D < cut2 * 0.5 * (a^2 + b^2) with the actual row distances a, b; the accepted pair with the minimum key
+// (D, k_u, original index up, original index down) wins.  Reads go to global memory (L2): about one cluster in six takes this path.
+struct SkipWin { float ylo, yhi, zlo, zhi; int by0, by1, bz0, bz1; bool any; };
+
+__device__ __forceinline__ SkipWin skip_window(const float y, const float z, const float t, const float hwy, const float hwz,
+                                               const bool continuous, const UnitDesc& g) {
+  SkipWin w;
+  const float yc = __fmul_rn(y, t), zc = continuous ? z : __fmul_rn(z, t);
+  w.ylo = __fsub_rn(yc, hwy); w.yhi = __fadd_rn(yc, hwy); w.zlo = __fsub_rn(zc, hwz); w.zhi = __fadd_rn(zc, hwz);
+  w.any = g.n > 0;
+  w.by0 = bin_of(w.ylo, g.ylo, g.invs, g.ny); w.by1 = bin_of(w.yhi, g.ylo, g.invs, g.ny);
+  w.bz0 = bin_of(w.zlo, g.zlo, g.invs, g.nz); w.bz1 = bin_of(w.zhi, g.zlo, g.invs, g.nz);
+  return w;
+}
+
+struct SkipBest { bool have; float D; int ku, kd, pu, pd; };
+
+// all pairs (candidate of window wu on unit gu) x (candidate of window wd on unit gd) at row distances (ku, kd)
+__device__ __forceinline__ void skip_level(SkipBest& best, const int ku, const int kd, const SkipWin& wu, const SkipWin& wd,
+                                           const UnitDesc& gu, const UnitDesc& gd, const float a, const float b, const float lim,
+                                           const float y, const float z, const float2* __restrict__ yz, const int* __restrict__ perm,
+                                           const int* __restrict__ bin_start) {
+  if (!wu.any || !wd.any) return;
+  const int* __restrict__ bsu = bin_start + gu.bin_off;
+  const int* __restrict__ bsd = bin_start + gd.bin_off;
+  const float2* __restrict__ hu = yz + gu.off;
+  const float2* __restrict__ hd = yz + gd.off;
+  for (int bz = wu.bz0; bz <= wu.bz1; bz++) {
+    const int pe = bsu[bz * gu.ny + wu.by1 + 1];
+    for (int p = bsu[bz * gu.ny + wu.by0]; p < pe; p++) {
+      const float2 cu = hu[p];
+      if (!(cu.x >= wu.ylo && cu.x <= wu.yhi && cu.y >= wu.zlo && cu.y <= wu.zhi)) continue;
+      for (int bzd = wd.bz0; bzd <= wd.bz1; bzd++) {
+        const int qe = bsd[bzd * gd.ny + wd.by1 + 1];
+        for (int q = bsd[bzd * gd.ny + wd.by0]; q < qe; q++) {
+          const float2 cd = hd[q];
+          if (!(cd.x >= wd.ylo && cd.x <= wd.yhi && cd.y >= wd.zlo && cd.y <= wd.zhi)) continue;
+          const float ey = __fsub_rn(__fmul_rn(b, __fsub_rn(cu.x, y)), __fmul_rn(a, __fsub_rn(y, cd.x)));
+          const float ez = __fsub_rn(__fmul_rn(b, __fsub_rn(cu.y, z)), __fmul_rn(a, __fsub_rn(z, cd.y)));
+          const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+          if (!(D < lim)) continue;
+          bool better = !best.have || D < best.D;
+          if (best.have && D == best.D) {   // exact tie: k_u, then the original indices (rare)
+            if (ku != best.ku) better = ku < best.ku;
+            else {
+              const int iu = perm[gu.off + p], ib = perm[gu.off + best.pu];   // same k_u: same up row
+              better = iu < ib || (iu == ib && kd == best.kd && perm[gd.off + q] < perm[gd.off + best.pd]);
+            }
+          }
+          if (better) { best.have = true; best.D = D; best.ku = ku; best.kd = kd; best.pu = p; best.pd = q; }
+        }
+      }
+    }
+  }
+}
+
+// fast path of S2': like k2_neighbours, the candidates of the (at most two) bin rows of a window are scanned once into a bit mask
+struct SkipMask { Win w; unsigned m; bool ok; };   // ok = false: more than two bin rows or more than 32 candidates (generic path)
+
+__device__ __forceinline__ SkipMask skip_scan(const SkipWin& sw, const UnitDesc& g, const float2* __restrict__ yz,
+                                              const int* __restrict__ bin_start) {
+  SkipMask r; r.m = 0u; r.ok = true;
+  r.w.ylo = sw.ylo; r.w.yhi = sw.yhi; r.w.zlo = sw.zlo; r.w.zhi = sw.zhi; r.w.wide = false; r.w.a0 = r.w.n0 = r.w.a1m = r.w.n = 0;
+  if (!sw.any) return r;
+  if (sw.bz1 - sw.bz0 > 1) { r.ok = false; return r; }
+  const int* __restrict__ bs = bin_start + g.bin_off;
+  const int ra = sw.bz0 * g.ny;
+  r.w.a0 = bs[ra + sw.by0]; r.w.n0 = bs[ra + sw.by1 + 1] - r.w.a0; r.w.n = r.w.n0;
+  if (sw.bz1 > sw.bz0) { const int rb = ra + g.ny; const int a1 = bs[rb + sw.by0]; r.w.n += bs[rb + sw.by1 + 1] - a1; r.w.a1m = a1 - r.w.n0; }
+  if (r.w.n > 32) { r.ok = false; return r; }
+  const float2* __restrict__ hits = yz + g.off;
+#pragma unroll 1
+  for (int j = 0; j < r.w.n; j++) { if (in_win(hits[win_pos(r.w, j)], r.w)) r.m |= 1u << j; }
+  return r;
+}
+
+__device__ __forceinline__ void skip_level_masks(SkipBest& best, const int ku, const int kd, const SkipMask& mu, const SkipMask& md,
+                                                 const UnitDesc& gu, const UnitDesc& gd, const float a, const float b, const float lim,
+                                                 const float y, const float z, const float2* __restrict__ yz,
+                                                 const int* __restrict__ perm) {
+  const float2* __restrict__ hu = yz + gu.off;
+  const float2* __restrict__ hd = yz + gd.off;
+  unsigned m1 = md.m ? mu.m : 0u;
+  while (m1) {
+    const int j = __ffs(m1) - 1; m1 &= m1 - 1u;
+    const int p = win_pos(mu.w, j);
+    const float2 cu = hu[p];
+    unsigned m2 = md.m;
+    while (m2) {
+      const int i = __ffs(m2) - 1; m2 &= m2 - 1u;
+      const int q = win_pos(md.w, i);
+      const float2 cd = hd[q];
+      const float ey = __fsub_rn(__fmul_rn(b, __fsub_rn(cu.x, y)), __fmul_rn(a, __fsub_rn(y, cd.x)));
+      const float ez = __fsub_rn(__fmul_rn(b, __fsub_rn(cu.y, z)), __fmul_rn(a, __fsub_rn(z, cd.y)));
+      const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+      if (!(D < lim)) continue;
+      bool better = !best.have || D < best.D;
+      if (best.have && D == best.D) {   // exact tie: k_u, then the original indices (rare)
+        if (ku != best.ku) better = ku < best.ku;
+        else { const int iu = perm[gu.off + p], ib = perm[gu.off + best.pu]; better = iu < ib || (iu == ib && perm[gd.off + q] < perm[gd.off + best.pd]); }
+      }
+      if (better) { best.have = true; best.D = D; best.ku = ku; best.kd = kd; best.pu = p; best.pd = q; }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) k2_skip_links(const Item* __restrict__ items, const int chunk, const UnitDesc* __restrict__ units,
+                                                     const RowConst* __restrict__ rows, const float2* __restrict__ yz,
+                                                     const int* __restrict__ perm, const int* __restrict__ bin_start,
+                                                     int* __restrict__ link_up, int* __restrict__ link_dn, const Params P) {
+  const Item it = items[blockIdx.x];
+  const int u = it.unit, R = P.R, r = u % R;
+  const UnitDesc d = units[u];
+  const int cnt = min(chunk, d.n - it.start);
+  const bool searchable = r >= 1 && r <= R - 2;
+  const RowConst rc = rows[r];
+  // pass 1: re-encode the pairs S2 found; the clusters it left unlinked are collected in shared memory, so that pass 2 runs with
+  // all lanes busy (they are about one cluster in six)
+  __shared__ int s_list[4096];   // chunk <= 4096 (tpc_set_param)
+  __shared__ int s_n;
+  if (threadIdx.x == 0) s_n = 0;
+  __syncthreads();
+  for (int k = threadIdx.x; k < cnt; k += blockDim.x) {
+    const long long g = d.off + it.start + k;
+    const int eu = link_up[g];
+    if (eu >= 0) { link_up[g] = eu << 1; link_dn[g] = link_dn[g] << 1; }   // S2's pair: row distance 1 on both sides
+    else if (searchable) s_list[atomicAdd(&s_n, 1)] = k;
+  }
+  __syncthreads();
+  const int n_open = s_n;
+  if (n_open == 0) return;
+  const bool cont = P.continuous != 0;
+  const bool up2 = r + 2 <= R - 1, dn2 = r - 2 >= 0;
+  const UnitDesc gu1 = units[u + 1], gd1 = units[u - 1];
+  const UnitDesc gu2 = up2 ? units[u + 2] : gu1, gd2 = dn2 ? units[u - 2] : gd1;
+  const float wy1 = __fmul_rn(1.0f, P.wy), wy2 = __fmul_rn(2.0f, P.wy), wz1 = __fmul_rn(1.0f, P.wz), wz2 = __fmul_rn(2.0f, P.wz);
+  for (int j = threadIdx.x; j < n_open; j += blockDim.x) {
+    const int k = s_list[j];
+    const long long g = d.off + it.start + k;
+    const float2 h = yz[g];
+    const float y = h.x, z = h.y;
+    const SkipWin wu1 = skip_window(y, z, rc.tu, wy1, cont ? rc.wzu : wz1, cont, gu1);
+    const SkipWin wd1 = skip_window(y, z, rc.td, wy1, cont ? rc.wzd : wz1, cont, gd1);
+    SkipBest best; best.have = false; best.D = 0.0f; best.ku = best.kd = 0; best.pu = best.pd = -1;
+    SkipWin wu2 = wu1, wd2 = wd1; wu2.any = wd2.any = false;
+    if (dn2) wd2 = skip_window(y, z, rc.td2, wy2, cont ? rc.wzd2 : wz2, cont, gd2);
+    if (up2) wu2 = skip_window(y, z, rc.tu2, wy2, cont ? rc.wzu2 : wz2, cont, gu2);
+    const SkipMask mu1 = skip_scan(wu1, gu1, yz, bin_start), md1 = skip_scan(wd1, gd1, yz, bin_start);
+    const SkipMask mu2 = skip_scan(wu2, gu2, yz, bin_start), md2 = skip_scan(wd2, gd2, yz, bin_start);
+    if (mu1.ok && md1.ok && mu2.ok && md2.ok) {
+      skip_level_masks(best, 1, 2, mu1, md2, gu1, gd2, rc.a, rc.b2, rc.thr12, y, z, yz, perm);
+      skip_level_masks(best, 2, 1, mu2, md1, gu2, gd1, rc.a2, rc.b, rc.thr21, y, z, yz, perm);
+      if (!best.have) skip_level_masks(best, 2, 2, mu2, md2, gu2, gd2, rc.a2, rc.b2, rc.thr22, y, z, yz, perm);
+    } else {   // tiny bins or very dense rows: nested scan over all bin rows of both windows
+      if (dn2) skip_level(best, 1, 2, wu1, wd2, gu1, gd2, rc.a, rc.b2, rc.thr12, y, z, yz, perm, bin_start);
+      if (up2) skip_level(best, 2, 1, wu2, wd1, gu2, gd1, rc.a2, rc.b, rc.thr21, y, z, yz, perm, bin_start);
+      if (!best.have && up2 && dn2) skip_level(best, 2, 2, wu2, wd2, gu2, gd2, rc.a2, rc.b2, rc.thr22, y, z, yz, perm, bin_start);
+    }
+    if (best.have) { link_up[g] = (best.pu << 1) | (best.ku - 1); link_dn[g] = (best.pd << 1) | (best.kd - 1); }
+  }
+}
+
 }  // namespace
 
 int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units,
@@ -267,6 +434,14 @@ int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int 
   k2_neighbours<<<n_items * split, threads, stage_bytes, L.stream>>>(d_items, chunk, d_units, d_rows, d_yz, d_perm, d_bin_start,
                                                                    d_link_up, d_link_dn, P, stage_bytes, split);
   e = cudaGetLastError();
+  return e == cudaSuccess ? 1 : -(int)e;
+}
+
+int launch_k2_skip_links(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, const RowConst* d_rows,
+                         const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up, int* d_link_dn, const Params& P) {
+  if (n_items <= 0) return 0;
+  k2_skip_links<<<n_items, 256, 0, L.stream>>>(d_items, chunk, d_units, d_rows, d_yz, d_perm, d_bin_start, d_link_up, d_link_dn, P);
+  cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }
 

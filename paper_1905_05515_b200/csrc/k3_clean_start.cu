@@ -94,6 +94,17 @@ __device__ bool seed_bridged(const UnitDesc* __restrict__ units, const RowConst*
   return false;
 }
 
+// S2' tables (link_skip = 1): an entry is (position << 1 | k - 1), k = row distance of the link.  Cleaned up-link of sorted position
+// p of unit uu (row rr): the raw entry if the partner k rows up points back with the same entry shape, else -1.
+__device__ __forceinline__ int clean_up_enc(const UnitDesc* __restrict__ units, const int* link_up, const int* link_dn, int uu, int rr,
+                                            int R, long long off_uu, int p) {
+  const int e = link_up[off_uu + p];
+  if (e < 0) return -1;
+  const int k = (e & 1) + 1;
+  if (rr + k >= R) return -1;
+  return link_dn[units[uu + k].off + (e >> 1)] == ((p << 1) | (k - 1)) ? e : -1;
+}
+
 __global__ void __launch_bounds__(K3_THREADS) k3_clean_flag(const Item* __restrict__ items, const int chunk,
                                                             const UnitDesc* __restrict__ units, int* link_up, int* link_dn,
                                                             unsigned* __restrict__ mask, int* __restrict__ item_count,
@@ -116,16 +127,24 @@ __global__ void __launch_bounds__(K3_THREADS) k3_clean_flag(const Item* __restri
       const long long g = d.off + h;
       const int up = link_up[g], dn = link_dn[g];
       int cu = -1, cd = -1;
-      if (up >= 0 && r + 1 < R && link_dn[units[u + 1].off + up] == h) cu = up;
-      if (dn >= 0 && r > 0 && link_up[units[u - 1].off + dn] == h) cd = dn;
+      if (!P.link_skip) {
+        if (up >= 0 && r + 1 < R && link_dn[units[u + 1].off + up] == h) cu = up;
+        if (dn >= 0 && r > 0 && link_up[units[u - 1].off + dn] == h) cd = dn;
+      } else {   // S2' entries carry the row distance: mutual iff the partner k rows away holds (h, k)
+        if (up >= 0) { const int k = (up & 1) + 1; if (r + k < R && link_dn[units[u + k].off + (up >> 1)] == ((h << 1) | (k - 1))) cu = up; }
+        if (dn >= 0) { const int k = (dn & 1) + 1; if (r - k >= 0 && link_up[units[u - k].off + (dn >> 1)] == ((h << 1) | (k - 1))) cd = dn; }
+      }
       if (cu != up) link_up[g] = -1;
       if (cd != dn) link_dn[g] = -1;
       if (cd < 0 && cu >= 0) {   // S4: chain of at least min_seed clusters starting here
         int len = 2, uu = u + 1, p = cu;
+        if (P.link_skip) { uu = u + (cu & 1) + 1; p = cu >> 1; }
         while (len < min_seed) {
-          const int nx = clean_up_of(units, link_up, link_dn, uu, uu % R, R, units[uu].off, p);
+          const int nx = P.link_skip ? clean_up_enc(units, link_up, link_dn, uu, uu % R, R, units[uu].off, p)
+                                     : clean_up_of(units, link_up, link_dn, uu, uu % R, R, units[uu].off, p);
           if (nx < 0) break;
-          p = nx; uu++; len++;
+          if (P.link_skip) { uu += (nx & 1) + 1; p = nx >> 1; } else { p = nx; uu++; }
+          len++;
         }
         start = len >= min_seed;
       }

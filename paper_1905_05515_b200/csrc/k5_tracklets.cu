@@ -240,10 +240,12 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
     const bool run = mode == MD_RUN, init = mode == MD_INIT;
     float2 c = cl;
     int nxt_up = -1;
-    if (run) { const long long o = su[r + 1].off + nxt; c = yz[o]; nxt_up = link_up[o]; }   // linked cluster + its own up-link
+    // link entry: the position in the next row; with S2' (link_skip) position << 1 | k - 1, k = row distance of the link
+    const int kk = P.link_skip ? (nxt & 1) + 1 : 1, pos = P.link_skip ? nxt >> 1 : nxt;
+    if (run) { const long long o = su[r + kk].off + pos; c = yz[o]; nxt_up = link_up[o]; }   // linked cluster + its own up-link
     bool prop_ok = true;
     __syncwarp();
-    if (run) { work += 1u; prop_ok = propagate(st, s_rx[r + 1] - s_rx[r], P); }
+    if (run) { work += 1u; prop_ok = propagate(st, s_rx[r + kk] - s_rx[r], P); }   // one transport over the whole link
     if (init) {   // direction from the origin, first update with the start hit
       const float x = s_rx[r], y = c.x;
       const float rr = sqrtf(x * x + y * y);
@@ -257,7 +259,10 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
     if (init) { rh[r] = hit0; mode = nxt >= 0 ? MD_RUN : MD_DONE; }
     else if (run) {
       if (!prop_ok) { ok = false; mode = MD_DONE; }      // a failed transport ends Phase A and skips Phase B
-      else { r++; rh[r] = nxt; cl = c; nxt = nxt_up; if (nxt < 0) mode = MD_DONE; }
+      else {
+        if (kk == 2) rh[r + 1] = -1;                       // the skipped row holds no cluster of this tracklet (yet)
+        r += kk; rh[r] = pos; cl = c; nxt = nxt_up; if (nxt < 0) mode = MD_DONE;
+      }
     }
   }
   K5_EPILOGUE();

@@ -88,6 +88,7 @@ struct Tunables {   // DESIGN.md table T
   int chunk = 1024;           // clusters per K2/K3 work item (multiple of 32)
   int k2_threads = 0;         // K2 block size (0 = default 256); tuning knob
   int bridge_rows = 0, bridge_min = 3;       // NEXT-2 seed bridging (reading A39): 0 = off
+  int link_skip = 0;                         // NEXT-2 (reading A45): 1 = links may skip one pad row (S2')
   int bridge_rescue = 0;                     // 1: dropped start hits are fitted in a second wave when the first left their chain unused (A39c)
   double bridge_wy = 1.0, bridge_wz = 1.5;
   double merge_edge = 3.0, merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05; int merge_rows = 8;   // NEXT-3 (reading A41)
@@ -150,6 +151,7 @@ struct tpc_ctx {
   // S7 refit (device + host)
   DevBuf r_n, r_ndf, r_x, r_par, r_cov, r_chi2, r_z0, r_t0;
   PinVec<int32_t> hr_n, hr_ndf; PinVec<float> hr_x, hr_par, hr_cov, hr_chi2, hr_z0, hr_t0;
+  std::vector<int8_t> dbg_up_k, dbg_dn_k;
   std::vector<float> dbg_yz; std::vector<int32_t> dbg_perm, dbg_bins, dbg_up, dbg_dn, dbg_su, dbg_sp;
   std::vector<int32_t> dbg_tl_sector, dbg_tl_row, dbg_tl_n, dbg_tl_first, dbg_tl_last, dbg_rowhit; std::vector<float> dbg_tl_chi2, dbg_tl_x, dbg_tl_par, dbg_tl_cov;
 
@@ -298,6 +300,7 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "bridge_min") { if (v < 3 || v > 255) return fail(c, TPC_E_ARG, "bridge_min must be in 3..255"); T.bridge_min = (int)v; }
   else if (s == "bridge_wy") rc = pos(T.bridge_wy); else if (s == "bridge_wz") rc = pos(T.bridge_wz);
   else if (s == "bridge_rescue") T.bridge_rescue = v != 0;
+  else if (s == "link_skip") { if (v != 0 && v != 1) return fail(c, TPC_E_ARG, "link_skip must be 0 or 1"); T.link_skip = (int)v; }
   else if (s == "merge_edge") rc = nonneg(T.merge_edge); else if (s == "merge_dy") rc = pos(T.merge_dy); else if (s == "merge_dz") rc = pos(T.merge_dz);
   else if (s == "merge_ds") rc = pos(T.merge_ds); else if (s == "merge_dt") rc = pos(T.merge_dt);
   else if (s == "merge_rows") { if (v < 0 || v > 255) return fail(c, TPC_E_ARG, "merge_rows must be in 0..255"); T.merge_rows = (int)v; }
@@ -404,7 +407,13 @@ void make_params_and_rows(tpc_ctx* c, std::vector<RowConst>& rows) {
     k.thr = (float)(T.cut2 * 0.5 * (a * a + b * b));
     k.wzu = (float)(T.dzdx_max * a + T.wz0); k.wzd = (float)(T.dzdx_max * b + T.wz0);
     k.yedge = (float)(x * tan(0.5 * dphi));
-    k.pad[0] = k.pad[1] = k.pad[2] = 0.f;
+    const double xu2 = r + 2 < R ? (double)c->row_x[r + 2] : x, xd2 = r > 1 ? (double)c->row_x[r - 2] : x;
+    const double a2 = xu2 - x, b2 = x - xd2;
+    k.tu2 = (float)(xu2 / x); k.td2 = (float)(xd2 / x); k.a2 = (float)a2; k.b2 = (float)b2;
+    k.wzu2 = (float)(T.dzdx_max * a2 + T.wz0); k.wzd2 = (float)(T.dzdx_max * b2 + T.wz0);
+    k.thr21 = (float)(T.cut2 * 0.5 * (a2 * a2 + b * b)); k.thr12 = (float)(T.cut2 * 0.5 * (a * a + b2 * b2));
+    k.thr22 = (float)(T.cut2 * 0.5 * (a2 * a2 + b2 * b2));
+    for (float& f : k.pad) f = 0.f;
   }
   Params& P = c->P;
   P.NS = c->NS; P.R = R; P.continuous = c->t_frame > 0 ? 1 : 0;
@@ -415,7 +424,8 @@ void make_params_and_rows(tpc_ctx* c, std::vector<RowConst>& rows) {
   P.ry = c->sigma_y * c->sigma_y; P.rz = c->sigma_z * c->sigma_z;
   P.smax = (float)T.s_max; P.nsigma = (float)T.n_sigma; P.wmax = (float)T.w_max; P.edge_margin = (float)T.edge_margin;
   P.max_gap = T.max_gap; P.min_hits = T.min_hits;
-  P.bridge_rows = T.bridge_rows; P.bridge_min = T.bridge_min; P.bridge_wy = (float)T.bridge_wy; P.bridge_wz = (float)T.bridge_wz;
+  P.bridge_rows = T.link_skip ? 0 : T.bridge_rows; P.bridge_min = T.bridge_min; P.bridge_wy = (float)T.bridge_wy; P.bridge_wz = (float)T.bridge_wz;
+  P.link_skip = T.link_skip;
 }
 
 // S1 grid descriptor of every unit + CSR offsets + K2/K3 work items.  Returns a tpc_status.
@@ -535,6 +545,10 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   LAUNCH_TRY(c, launch_k2_neighbours(L, n_items, c->d_items.as<Item>(), chunk, c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
                                      c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(),
                                      c->d_link_dn.as<int>(), P), launches);
+  if (c->T.link_skip)   // S2': links that may skip a row, for the hits S2 left unlinked (its time counts as neighbour finding)
+    LAUNCH_TRY(c, launch_k2_skip_links(L, n_items, c->d_items.as<Item>(), chunk, c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(),
+                                       c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(), c->d_link_up.as<int>(),
+                                       c->d_link_dn.as<int>(), P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[3], st));
   if (c->T.debug_keep && N > 0) {
     CUDA_TRY(c, c->d_raw_up.ensure((size_t)N * 4)); CUDA_TRY(c, c->d_raw_dn.ensure((size_t)N * 4));
@@ -551,7 +565,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, cudaEventRecord(c->ev[4], st));
   typedef unsigned long long u64;
   unsigned long long* d_k5cnt = (unsigned long long*)(c->d_counters.as<char>() + 128);
-  const bool variant = c->T.bridge_rows > 0;
+  const bool variant = c->T.bridge_rows > 0 && !c->T.link_skip;   // (seed bridging is not combined with S2')
   // Default path: NO device -> host read between K3 and the end of the call.  The number of start hits M stays in device memory
   // (d_nstart); the per-tracklet buffers are sized for a capacity M_cap guessed from the frame size and from the previous call, the
   // kernels read M themselves, and the guess is checked when the counters are read at the end (a frame that exceeds it is
@@ -909,7 +923,23 @@ int tpc_debug_get_links(tpc_ctx* c, int sector, int row, int cleaned, const int3
     CUDA_TRY(c, cudaMemcpy(c->dbg_up.data(), su + d.off, (size_t)d.n * 4, cudaMemcpyDeviceToHost));
     CUDA_TRY(c, cudaMemcpy(c->dbg_dn.data(), sd + d.off, (size_t)d.n * 4, cudaMemcpyDeviceToHost));
   }
+  // row distance of every link: 1, or what the S2' entries (position << 1 | k - 1) carry; 0 = no link
+  c->dbg_up_k.assign(std::max(d.n, 1), 0); c->dbg_dn_k.assign(std::max(d.n, 1), 0);
+  for (int i = 0; i < d.n; i++) {
+    int32_t& a = c->dbg_up[i]; int32_t& b = c->dbg_dn[i];
+    if (c->T.link_skip) {
+      if (a >= 0) { c->dbg_up_k[i] = (int8_t)((a & 1) + 1); a >>= 1; }
+      if (b >= 0) { c->dbg_dn_k[i] = (int8_t)((b & 1) + 1); b >>= 1; }
+    } else { c->dbg_up_k[i] = a >= 0; c->dbg_dn_k[i] = b >= 0; }
+  }
   *up = c->dbg_up.data(); *dn = c->dbg_dn.data(); *n = d.n;
+  return TPC_OK;
+}
+
+int tpc_debug_get_link_rows(tpc_ctx* c, const int8_t** up_k, const int8_t** dn_k, int32_t* n) {
+  if (!c || !up_k || !dn_k || !n) return fail(c, TPC_E_ARG, "tpc_debug_get_link_rows: null argument");
+  if (c->dbg_up_k.empty()) return fail(c, TPC_E_STATE, "tpc_debug_get_link_rows: call tpc_debug_get_links first");
+  *up_k = c->dbg_up_k.data(); *dn_k = c->dbg_dn_k.data(); *n = (int32_t)c->dbg_up.size();
   return TPC_OK;
 }
 

@@ -14,8 +14,12 @@ struct RowConst {
   float thr;     // cut2 * 0.5 * (a^2+b^2)
   float wzu, wzd;// continuous-mode z half-widths up / down
   float yedge;   // x_r * tan(dphi/2)
-  float pad[3];
+  // S2' (link_skip, reading A45): the same constants for a row distance of 2, and the acceptance limits of the pairs
+  // (k_u, k_d) = (2,1), (1,2), (2,2): cut2 * 0.5 * (a_ku^2 + b_kd^2)
+  float tu2, td2, a2, b2, wzu2, wzd2, thr21, thr12, thr22;
+  float pad[6];
 };
+static_assert(sizeof(RowConst) == 96, "RowConst layout");
 
 // One (sector,row) unit: where its clusters come from, where its sorted copy lives, and its S1 grid.
 struct UnitDesc {
@@ -41,6 +45,7 @@ struct Params {
   int max_gap, min_hits;
   int bridge_rows, bridge_min;    // NEXT-2 seed bridging (reading A39); bridge_rows = 0: off
   float bridge_wy, bridge_wz;
+  int link_skip;                  // NEXT-2 as SURVEY 8(f).2 wrote it (reading A45): 1 = links may skip one row; link tables then hold (position << 1 | k - 1)
 };
 
 // S9 (NEXT-3) matching parameters (reading A41), rounded to float once on the host
@@ -98,6 +103,10 @@ int launch_k1_grid(const Launch& L, int U, const UnitDesc* d_units, const float*
 int launch_k2_neighbours(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units,
                          const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up,
                          int* d_link_dn, const Params& P);
+
+// S2' (link_skip = 1): re-encodes the S2 links as (position << 1 | 0) and gives the hits S2 left unlinked a link that may skip a row
+int launch_k2_skip_links(const Launch& L, int n_items, const Item* d_items, int chunk, const UnitDesc* d_units, const RowConst* d_rows,
+                         const float2* d_yz, const int* d_perm, const int* d_bin_start, int* d_link_up, int* d_link_dn, const Params& P);
 
 int launch_k3_bridge(const Launch& L, int M, const int* d_start_unit, const int* d_start_pos, const UnitDesc* d_units,
                      const RowConst* d_rows, const float2* d_yz, const int* d_bin_start, const int* d_link_up, const int* d_link_dn,

@@ -48,23 +48,27 @@ def compare_grid(w, o, trk, units=None) -> int:
     return k
 
 
-def gather_links(w, trk, cleaned):
+def gather_links(w, trk, cleaned, with_rows=False):
     up = np.full(w.n_clusters, -2, np.int32)
     dn = np.full(w.n_clusters, -2, np.int32)
+    uk = np.full(w.n_clusters, -2, np.int32); dk = np.full(w.n_clusters, -2, np.int32)
     R = w.n_rows
     for u in range(w.n_sectors * R):
         a, b = int(w.unit_off[u]), int(w.unit_off[u + 1])
         if b > a:
-            up[a:b], dn[a:b] = trk.links(u // R, u % R, cleaned)
-    return up, dn
+            if with_rows:
+                up[a:b], dn[a:b], uk[a:b], dk[a:b] = trk.link_rows(u // R, u % R, cleaned)
+            else:
+                up[a:b], dn[a:b] = trk.links(u // R, u % R, cleaned)
+    return (up, dn, uk, dk) if with_rows else (up, dn)
 
 
 def compare_links(w, o, trk) -> dict:
     """Raw (S2) and cleaned (S3) link tables and the S4 start list; returns the differing-hit counts (bar: 0)."""
     out = {}
     for cleaned, (nu, nd) in ((False, ("link_up", "link_dn")), (True, ("clean_up", "clean_dn"))):
-        up, dn = gather_links(w, trk, cleaned)
-        diff = (up != o.get(nu)) | (dn != o.get(nd))
+        up, dn, uk, dk = gather_links(w, trk, cleaned, with_rows=True)
+        diff = (up != o.get(nu)) | (dn != o.get(nd)) | (uk != o.get(nu + "_k")) | (dk != o.get(nd + "_k"))   # positions and row distances
         out["cleaned" if cleaned else "raw"] = int(diff.sum())
     su, sp = trk.start_hits()
     out["start_equal"] = bool(np.array_equal(su, o.get("start_unit")) and np.array_equal(sp, o.get("start_pos")))

@@ -245,6 +245,21 @@ def test_seed_bridging_variant_parity():
         assert m1["eff"] >= m0["eff"] - 0.003, (m0["eff"], m1["eff"])
 
 
+def test_skip_link_variant_parity():
+    """NEXT-2 as SURVEY.md section 8(f).2 wrote it (S2', reading A45; link_skip = 1 on both sides): raw and cleaned link tables
+    with their row distances and the start list bit-exact, tracks and tracklets bit-identical; about half the tracklets of the
+    default path at an efficiency within 0.2 % of it."""
+    for w in (W.config(1), W.config(2), W.config(3, scale=0.1), W.config(4)):
+        rng = np.random.default_rng(8)
+        o, otr, gtr, res = _full_parity(w, grid_units=rng.choice(w.n_sectors * w.n_rows, min(60, w.n_sectors * w.n_rows), replace=False),
+                                        tracklets=True, link_skip=1)
+        assert (o.get("clean_up_k") == 2).sum() > 0.01 * w.n_clusters
+        base = P.make_oracle(w).run("s6")
+        assert len(o.get("start_unit")) <= 0.75 * len(base.get("start_unit"))
+        m0, m1 = H.truth_metrics(w, base.tracks()), H.truth_metrics(w, gtr)
+        assert m1["eff"] >= m0["eff"] - 0.002, (m0["eff"], m1["eff"])
+
+
 def test_large_units_take_the_partly_shared_k1_path():
     """Units of about 5 k clusters: K1 keeps cursors + sorted indices in shared memory but gathers (y, z) from global memory
     (the plan between the all-shared one of C3-sized units and the global-cursor one).  S0-S4 tables bit-exact."""
