@@ -16,7 +16,7 @@ _SO = os.path.join(_HERE, "libtpc_oracle.so")
 _SRC = os.path.join(_HERE, "tpc_oracle.cpp")
 _KINDS = {0: (C.c_int32, np.int32), 1: (C.c_int64, np.int64), 2: (C.c_double, np.float64), 3: (C.c_float, np.float32)}
 
-STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6, "s7": 7, "s8": 8, "s9": 9}
+STAGES = {"s0": 0, "s1": 1, "s2": 2, "s3": 3, "s4": 4, "s5": 5, "s6": 6, "s7": 7, "s8": 8, "s9": 9, "s10": 10}
 
 
 _SO_PLAIN = os.path.join(_HERE, "libtpc_oracle_plain.so")
@@ -196,6 +196,11 @@ class Oracle:
         """S9 (NEXT-3): next / prev segment of every track across a sector boundary (-1 none), leaver flag, outer state (run("s9") first)."""
         return {"next": self.get("mg_next"), "prev": self.get("mg_prev"), "leaver": self.get("mg_leaver"),
                 "outer": self.get("mg_outer").reshape(-1, 4)}
+
+    def loopers(self):
+        """S10 (NEXT-3, second half): per track the previous turn of the same looping particle (-1 none), the first turn of its group
+        (itself if it follows nobody) and the number of turns after it (run("s10") first)."""
+        return {"prev": self.get("lp_prev"), "root": self.get("lp_root"), "turn": self.get("lp_turn")}
 
     def tracklets(self):
         d = {k: self.get("tl_" + k) for k in ("n", "first", "last", "rowhit", "sector", "chi2", "x", "par", "cov", "zref")}

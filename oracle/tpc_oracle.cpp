@@ -62,6 +62,8 @@ struct Tunables {            // DESIGN.md table T (all are readings; the paper i
   double tube = 1.5;            // NEXT-4: radius of the tube around a track, cm
   // NEXT-3 (reading A41): cross-sector segment matching
   double merge_edge = 3.0; int merge_rows = 8; double merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05;
+  // NEXT-3, second half (reading A46): legs / turns of one looping particle
+  double loop_qmin = 5.0, loop_dy = 1.0, loop_ds = 0.1, loop_dt = 0.1, loop_dq = 0.5, loop_pmin = 2.0, loop_frac = 0.35; int loop_nmax = 20;
 };
 
 struct OracleBase {
@@ -113,6 +115,8 @@ struct Oracle : OracleBase {
   std::vector<int32_t> start_wave;   // 1 = first wave, 2 = bridged start hit kept for the rescue wave (bridge_rescue)
   // S9 (NEXT-3): cross-sector segment matching
   std::vector<int32_t> mg_next, mg_prev, mg_leaver; std::vector<double> mg_outer;   // outer: x, y, z, sinphi per track
+  // S10 (NEXT-3, second half): turns of one looping particle
+  std::vector<int32_t> lp_prev, lp_root, lp_turn;
   std::vector<double> z_d, ys_d, zs_d;   // export copies
 
   Oracle(int ns, int nr, const float* rx, double dphi_, double zmax, double tframe, double sy, double sz, double bz_, double vd)
@@ -820,6 +824,58 @@ struct Oracle : OracleBase {
     for (int64_t b = 0; b < NT; b++) if (bestA[b] >= 0) { mg_next[bestA[b]] = (int32_t)b; mg_prev[b] = bestA[b]; }
   }
 
+  // ---- S10 (NEXT-3, second half, SURVEY.md section 8(f).3 "recognise returning legs / extra turns"; "looping tracks",
+  //      PAPER.md:104 "secondary legs of looping tracks below 200 MeV/c"; reading A46).  In a uniform field every turn of a looping
+  //      particle runs over the SAME circle in the pad plane and is displaced along z by one pitch = (2 pi / |k|) * dz/ds, so the
+  //      later turns appear in the same sector as separate S6 tracks with the same (y, sin phi, dz/ds, q/pT) at the same x.
+  //      For tracks A, B of one sector, both with |q/pT| >= loop_qmin (pT <= 200 MeV/c): B's state is transported (parameters only)
+  //      to x_A; B follows A iff |dy| <= loop_dy, |d sin phi| <= loop_ds, |d dz/ds| <= loop_dt, |dq| <= loop_dq |q_A|, the pitch
+  //      p = (2 pi / |cB q_A|) * (t_A + t_B)/2 has |p| >= loop_pmin, and the number of turns tau = (z_B - z_A) / p is within
+  //      loop_frac of an integer n, 1 <= n <= loop_nmax.  B takes as predecessor the A with the smallest n, then the smallest score
+  //      (dy/loop_dy)^2 + (ds/loop_ds)^2 + (dt/loop_dt)^2, then the lowest index.  root = first turn of the group, turn = turns
+  //      after the root (0 for a track that follows nobody).
+  void s10_loopers() {
+    const int64_t NT = (int64_t)trk_sector.size();
+    lp_prev.assign(NT, -1); lp_root.assign(NT, 0); lp_turn.assign(NT, 0);
+    std::vector<int32_t> lp_n(NT, 0);
+    const Real qmin = (Real)T.loop_qmin, wy = (Real)T.loop_dy, ws = (Real)T.loop_ds, wt = (Real)T.loop_dt, wq = (Real)T.loop_dq;
+    const Real pmin = (Real)T.loop_pmin, frac = (Real)T.loop_frac, twopi = (Real)6.283185307179586;
+    for (int64_t b = 0; b < NT; b++) {
+      const Real qb = (Real)trk_par[b * 5 + 4];
+      if (!(std::fabs(qb) >= qmin)) continue;
+      bool have = false; int32_t best = -1, bestn = 0; Real bests = 0;
+      for (int64_t a = 0; a < NT; a++) {
+        if (a == b || trk_sector[a] != trk_sector[b]) continue;
+        const Real qa = (Real)trk_par[a * 5 + 4];
+        if (!(std::fabs(qa) >= qmin)) continue;
+        State st; for (int u = 0; u < 5; u++) for (int v = 0; v < 5; v++) st.C[u][v] = 0;
+        for (int k = 0; k < 5; k++) st.p[k] = (Real)trk_par[b * 5 + k];
+        const Real dx = (Real)trk_x[a] - (Real)trk_x[b];
+        if (dx != (Real)0 && !propagate_state(st, dx)) continue;
+        const Real dy = st.p[0] - (Real)trk_par[a * 5 + 0], ds = st.p[2] - (Real)trk_par[a * 5 + 2];
+        const Real dt = st.p[3] - (Real)trk_par[a * 5 + 3], dq = st.p[4] - qa;
+        if (!(std::fabs(dy) <= wy && std::fabs(ds) <= ws && std::fabs(dt) <= wt && std::fabs(dq) <= wq * std::fabs(qa))) continue;
+        const Real k = cB * qa;
+        const Real tav = (Real)0.5 * ((Real)trk_par[a * 5 + 3] + st.p[3]);
+        const Real pitch = (twopi / std::fabs(k)) * tav;
+        if (!(std::fabs(pitch) >= pmin)) continue;
+        const Real tau = (st.p[1] - (Real)trk_par[a * 5 + 1]) / pitch;
+        const Real nr = std::nearbyint(tau);
+        if (!(nr >= (Real)1 && std::fabs(tau - nr) <= frac && nr <= (Real)T.loop_nmax)) continue;
+        const int32_t n = (int32_t)nr;
+        const Real ey = dy / wy, es = ds / ws, et = dt / wt;
+        const Real score = (ey * ey + es * es) + et * et;
+        if (!have || n < bestn || (n == bestn && score < bests)) { have = true; best = (int32_t)a; bestn = n; bests = score; }
+      }
+      if (have) { lp_prev[b] = best; lp_n[b] = bestn; }
+    }
+    for (int64_t i = 0; i < NT; i++) {     // the predecessor lies n >= 1 turns earlier: following it ends at the first turn
+      int32_t r = (int32_t)i, t = 0;
+      for (int it = 0; it < 64 && lp_prev[r] >= 0; it++) { t += lp_n[r]; r = lp_prev[r]; }
+      lp_root[i] = r; lp_turn[i] = t;
+    }
+  }
+
   int run(int upto, int brute) override { return run_range(0, upto, brute); }
   // stages from..upto (the earlier ones must have run, or been set by hand: set_links); test hook for hand-built cases
   int run_range(int from, int upto, int brute) override {
@@ -836,6 +892,7 @@ struct Oracle : OracleBase {
         case 7: s7_refit(); break;
         case 8: s8_adjacent((brute & 2) != 0); break;
         case 9: s9_merge(); break;
+        case 10: s10_loopers(); break;
         default: break;
       }
     }
@@ -921,6 +978,9 @@ struct Oracle : OracleBase {
     if (s == "trk_cov") RET(trk_cov, 2)
     if (s == "trk_chi2") RET(trk_chi2, 2)
     if (s == "start_wave") RET(start_wave, 0)
+    if (s == "lp_prev") RET(lp_prev, 0)
+    if (s == "lp_root") RET(lp_root, 0)
+    if (s == "lp_turn") RET(lp_turn, 0)
     if (s == "mg_next") RET(mg_next, 0)
     if (s == "mg_prev") RET(mg_prev, 0)
     if (s == "mg_leaver") RET(mg_leaver, 0)
@@ -961,6 +1021,8 @@ int orc_set_param(void* h, const char* name, double v) {
   else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "bridge_rescue") T.bridge_rescue = (int)v; else if (s == "tube") T.tube = v; else if (s == "link_skip") T.link_skip = (int)v;
   else if (s == "merge_edge") T.merge_edge = v; else if (s == "merge_rows") T.merge_rows = (int)v; else if (s == "merge_dy") T.merge_dy = v;
   else if (s == "merge_dz") T.merge_dz = v; else if (s == "merge_ds") T.merge_ds = v; else if (s == "merge_dt") T.merge_dt = v;
+  else if (s == "loop_qmin") T.loop_qmin = v; else if (s == "loop_dy") T.loop_dy = v; else if (s == "loop_ds") T.loop_ds = v; else if (s == "loop_dt") T.loop_dt = v;
+  else if (s == "loop_dq") T.loop_dq = v; else if (s == "loop_pmin") T.loop_pmin = v; else if (s == "loop_frac") T.loop_frac = v; else if (s == "loop_nmax") T.loop_nmax = (int)v;
   else return -1;
   return 0;
 }
