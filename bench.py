@@ -205,6 +205,10 @@ def run_gpu(args, rank, world, local_rank):
     mg = [trk.merge_tracks(device_result=True) for _ in range(3)]
     merges = {"ms": float(np.mean([m["ms_merge"] for m in mg[1:]])), "matched_pairs": int((mg[-1]["next"] >= 0).sum().item()),
               "note": "S9 cross-sector segment matching (SURVEY 8(f).3), outside the timed step"}
+    # S10 (NEXT-3, second half, not part of the timed step): turns of one looping particle
+    lo = [trk.find_loopers(device_result=True) for _ in range(3)]
+    loopers = {"ms": float(np.mean([m["ms_loopers"] for m in lo[1:]])), "linked_tracks": int((lo[-1]["prev"] >= 0).sum().item()),
+               "note": "S10 looper turns (SURVEY 8(f).3), outside the timed step"}
     # NEXT-2 variant (seed bridging, reading A39), measured beside the default path, never mixed into `value`
     variant = None
     if args.variant and rank == 0:
@@ -346,7 +350,7 @@ def run_gpu(args, rank, world, local_rank):
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu, "cpu_baseline_parallel": cpu_par,
-           "variant_seed_bridging": variant, "cluster_marks": marks, "sector_merges": merges,
+           "variant_seed_bridging": variant, "cluster_marks": marks, "sector_merges": merges, "looper_turns": loopers,
            "refit": {"ms": refit_ms, "tracks_per_s": n_tracks / (refit_ms * 1e-3), "note": "S7 refit + collision time (SURVEY 8(f).1), outside the timed step"},
            "clocks": clocks}
     print(json.dumps(out))

@@ -106,6 +106,18 @@ typedef struct {
   float ms_merge;           /* device time of K9 (CUDA events on the context's stream), ms */
 } tpc_merges;
 
+/* Result of tpc_find_loopers: S10 of DESIGN.md section 4 (SURVEY.md section 8(f).3 "recognise returning legs / extra turns"
+ * "looping tracks", "secondary legs of looping tracks below 200 MeV/c"; reading A46 -- the paper prints no rule): the tracks
+ * of one sector that are successive turns of one looping particle (same circle in the pad plane, displaced along z by whole pitches).
+ * One entry per track of the last tpc_find_tracks* call.  Library-owned, host (device_result = 0) or device memory. */
+typedef struct {
+  int64_t n_tracks;
+  const int32_t* prev;      /* [n_tracks] the track that is an earlier turn of the same particle (the nearest one found), -1 = none */
+  const int32_t* root;      /* [n_tracks] first turn of the group (the track itself if it follows nobody) */
+  const int32_t* turn;      /* [n_tracks] number of turns after the root (0 for a root) */
+  float ms_loopers;         /* device time of K10 (CUDA events on the context's stream), ms */
+} tpc_loopers;
+
 /* Per-step device times of the last tpc_find_tracks* call (CUDA events on the context's stream), ms. */
 typedef struct {
   float ms_upload;          /* host staging -> device (0 if the clusters were already device-resident) */
@@ -184,6 +196,11 @@ int tpc_mark_clusters(tpc_ctx*, float tube_cm, int device_result, tpc_cluster_ma
 /* S9: match track segments across sector boundaries (tunables merge_edge, merge_rows, merge_dy, merge_dz, merge_ds, merge_dt).
  * Errors: TPC_E_ARG (null), TPC_E_STATE (no completed tpc_find_tracks* call), TPC_E_NOMEM, TPC_E_CUDA. */
 int tpc_merge_tracks(tpc_ctx*, int device_result, tpc_merges* out);
+
+/* S10: group the tracks of the last tpc_find_tracks* call that are turns of one looping particle (tunables loop_qmin [c/GeV, 5 = 200
+ * MeV/c], loop_dy, loop_ds, loop_dt, loop_dq, loop_pmin, loop_frac, loop_nmax).
+ * Errors: TPC_E_ARG (null), TPC_E_STATE (no completed tpc_find_tracks* call), TPC_E_NOMEM, TPC_E_CUDA. */
+int tpc_find_loopers(tpc_ctx*, int device_result, tpc_loopers* out);
 
 /* Forget the clusters and results, keep geometry, parameters and buffers (one call per event / time frame). */
 int tpc_clear(tpc_ctx*);

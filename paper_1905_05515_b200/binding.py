@@ -17,7 +17,7 @@ _SO = os.path.join(_HERE, "libtpc_b200.so")
 
 ABI_SYMBOLS = [
     "tpc_abi_version", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
-    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
+    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_find_loopers", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
     "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_link_rows", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
 
@@ -52,6 +52,10 @@ class _Marks(C.Structure):
 
 class _Merges(C.Structure):
     _fields_ = [("n_tracks", C.c_int64), ("next", C.c_void_p), ("prev", C.c_void_p), ("ms_merge", C.c_float)]
+
+
+class _Loopers(C.Structure):
+    _fields_ = [("n_tracks", C.c_int64), ("prev", C.c_void_p), ("root", C.c_void_p), ("turn", C.c_void_p), ("ms_loopers", C.c_float)]
 
 
 class _Timings(C.Structure):
@@ -102,6 +106,7 @@ def load_library():
     lib.tpc_refit_tracks.argtypes = [vp, C.c_int, C.POINTER(_Refit)]
     lib.tpc_mark_clusters.argtypes = [vp, C.c_float, C.c_int, C.POINTER(_Marks)]
     lib.tpc_merge_tracks.argtypes = [vp, C.c_int, C.POINTER(_Merges)]
+    lib.tpc_find_loopers.argtypes = [vp, C.c_int, C.POINTER(_Loopers)]
     lib.tpc_clear.argtypes = [vp]
     lib.tpc_destroy.argtypes = [vp]
     lib.tpc_destroy.restype = None
@@ -300,6 +305,16 @@ def tpc_merge_tracks(h, device_result=False) -> dict:
     return {"n_tracks": n, "ms_merge": float(t.ms_merge), "next": make(t.next, n, np.int32), "prev": make(t.prev, n, np.int32)}
 
 
+def tpc_find_loopers(h, device_result=False) -> dict:
+    """S10: previous turn / first turn / turn number of every track (turns of one looping particle), zero-copy views."""
+    t = _Loopers()
+    _check(h, load_library().tpc_find_loopers(h, 1 if device_result else 0, C.byref(t)))
+    make = _dev_tensor if device_result else _host_array
+    n = int(t.n_tracks)
+    return {"n_tracks": n, "ms_loopers": float(t.ms_loopers), "prev": make(t.prev, n, np.int32), "root": make(t.root, n, np.int32),
+            "turn": make(t.turn, n, np.int32)}
+
+
 class Tracker:
     """Context manager around one tpc_ctx, for the tests and bench.py."""
 
@@ -363,6 +378,9 @@ class Tracker:
 
     def merge_tracks(self, device_result=False) -> dict:
         return tpc_merge_tracks(self.h, device_result)
+
+    def find_loopers(self, device_result=False) -> dict:
+        return tpc_find_loopers(self.h, device_result)
 
     def clear(self):
         self._keep = []

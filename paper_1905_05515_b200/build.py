@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libtpc_b200.so")
-SOURCES = ["tpc_abi.cu", "scan.cu", "k1_grid.cu", "k2_neighbours.cu", "k3_clean_start.cu", "k5_tracklets.cu", "k6_selector.cu", "k7_refit.cu", "k8_tube.cu", "k9_merge.cu"]
+SOURCES = ["tpc_abi.cu", "scan.cu", "k1_grid.cu", "k2_neighbours.cu", "k3_clean_start.cu", "k5_tracklets.cu", "k6_selector.cu", "k7_refit.cu", "k8_tube.cu", "k9_merge.cu", "k10_loopers.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "shared"] + os.environ.get("TPC_NVCC_EXTRA", "").split()
 

@@ -92,6 +92,7 @@ struct Tunables {   // DESIGN.md table T
   int bridge_rescue = 0;                     // 1: dropped start hits are fitted in a second wave when the first left their chain unused (A39c)
   double bridge_wy = 1.0, bridge_wz = 1.5;
   double merge_edge = 3.0, merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05; int merge_rows = 8;   // NEXT-3 (reading A41)
+  double loop_qmin = 5.0, loop_dy = 1.0, loop_ds = 0.1, loop_dt = 0.1, loop_dq = 0.5, loop_pmin = 2.0, loop_frac = 0.35; int loop_nmax = 20;   // NEXT-3, second half (reading A46)
 };
 
 struct UnitSrc { long long src = 0; int n = 0; };
@@ -145,6 +146,7 @@ struct tpc_ctx {
   PinVec<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; PinVec<float> ho_x, ho_par, ho_cov, ho_chi2;
   PinVec<int64_t> ho_cl_begin;
   // S9 merges (device + host)
+  DevBuf l_prev, l_prev_n, l_root, l_turn; PinVec<int32_t> hl_prev, hl_root, hl_turn;   // S10 looper turns (device + host)
   DevBuf g_outer, g_row_in, g_row_out, g_leaver, g_sec_begin, g_cand, g_next, g_prev; PinVec<int32_t> hg_next, hg_prev;
   // S8 cluster marks (device + host)
   DevBuf m_att, m_adj, m_status, m_track; PinVec<int32_t> hm_status, hm_track;
@@ -254,13 +256,14 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
                     &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
                     &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->d_flag2, &c->d_used, &c->m_att, &c->m_adj, &c->m_status, &c->m_track,
-                    &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_cand, &c->g_next, &c->g_prev};
+                    &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_cand, &c->g_next, &c->g_prev,
+                    &c->l_prev, &c->l_prev_n, &c->l_root, &c->l_turn};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
   c->ho_sector.release(); c->ho_ndf.release(); c->ho_tracklet.release(); c->ho_cl_row.release(); c->ho_cl_index.release();
   c->ho_x.release(); c->ho_par.release(); c->ho_cov.release(); c->ho_chi2.release(); c->ho_cl_begin.release();
   c->hr_n.release(); c->hr_ndf.release(); c->hr_x.release(); c->hr_par.release(); c->hr_cov.release(); c->hr_chi2.release();
-  c->hr_z0.release(); c->hr_t0.release(); c->hm_status.release(); c->hm_track.release(); c->hg_next.release(); c->hg_prev.release();
+  c->hr_z0.release(); c->hr_t0.release(); c->hm_status.release(); c->hm_track.release(); c->hg_next.release(); c->hg_prev.release(); c->hl_prev.release(); c->hl_root.release(); c->hl_turn.release();
   for (auto& ev : c->ev) if (ev) cudaEventDestroy(ev);
   if (c->ev_load) cudaEventDestroy(c->ev_load);
   if (c->ev_tables) cudaEventDestroy(c->ev_tables);
@@ -303,6 +306,10 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "link_skip") { if (v != 0 && v != 1) return fail(c, TPC_E_ARG, "link_skip must be 0 or 1"); T.link_skip = (int)v; }
   else if (s == "merge_edge") rc = nonneg(T.merge_edge); else if (s == "merge_dy") rc = pos(T.merge_dy); else if (s == "merge_dz") rc = pos(T.merge_dz);
   else if (s == "merge_ds") rc = pos(T.merge_ds); else if (s == "merge_dt") rc = pos(T.merge_dt);
+  else if (s == "loop_qmin") rc = nonneg(T.loop_qmin); else if (s == "loop_dy") rc = pos(T.loop_dy); else if (s == "loop_ds") rc = pos(T.loop_ds);
+  else if (s == "loop_dt") rc = pos(T.loop_dt); else if (s == "loop_dq") rc = pos(T.loop_dq); else if (s == "loop_pmin") rc = pos(T.loop_pmin);
+  else if (s == "loop_frac") { if (!(v > 0 && v < 0.5)) return fail(c, TPC_E_ARG, "loop_frac must be in (0, 0.5)"); T.loop_frac = v; }
+  else if (s == "loop_nmax") { if (v < 1 || v > 1000) return fail(c, TPC_E_ARG, "loop_nmax must be in 1..1000"); T.loop_nmax = (int)v; }
   else if (s == "merge_rows") { if (v < 0 || v > 255) return fail(c, TPC_E_ARG, "merge_rows must be in 0..255"); T.merge_rows = (int)v; }
   else return fail(c, TPC_E_ARG, "tpc_set_param: unknown parameter '%s'", name);
   if (rc == TPC_OK) { c->rows_valid = false; c->tables_ready = false; }
@@ -878,6 +885,40 @@ int tpc_merge_tracks(tpc_ctx* c, int device_result, tpc_merges* out) {
   }
   CUDA_TRY(c, cudaStreamSynchronize(st));
   CUDA_TRY(c, cudaEventElapsedTime(&out->ms_merge, c->ev[8], c->ev[9]));
+  return TPC_OK;
+}
+// S10 (NEXT-3, second half): K10 over the tracks of the last call.
+int tpc_find_loopers(tpc_ctx* c, int device_result, tpc_loopers* out) {
+  if (!c || !out) return fail(c, TPC_E_ARG, "tpc_find_loopers: null argument");
+  memset(out, 0, sizeof(*out));
+  if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_find_loopers: call tpc_find_tracks first");
+  cudaStream_t st = c->stream;
+  Launch L{st, c->sm_count, c->T.k2_threads};
+  const long long nt = c->n_tracks; const size_t ntz = (size_t)std::max(nt, 1LL);
+  CUDA_TRY(c, c->l_prev.ensure(ntz * 4)); CUDA_TRY(c, c->l_prev_n.ensure(ntz * 4)); CUDA_TRY(c, c->l_root.ensure(ntz * 4));
+  CUDA_TRY(c, c->l_turn.ensure(ntz * 4)); CUDA_TRY(c, c->g_sec_begin.ensure((size_t)(c->NS + 2) * 4));
+  const Tunables& T = c->T;
+  K10Params K{(float)T.loop_qmin, (float)T.loop_dy, (float)T.loop_ds, (float)T.loop_dt, (float)T.loop_dq, (float)T.loop_pmin,
+              (float)T.loop_frac, (float)6.283185307179586, T.loop_nmax};
+  long long launches = 0;
+  CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
+  LAUNCH_TRY(c, launch_k10_loopers(L, nt, c->NS, c->o_sector.as<int>(), c->o_x.as<float>(), c->o_par.as<float>(), c->g_sec_begin.as<int>(),
+                                   c->l_prev.as<int>(), c->l_prev_n.as<int>(), c->l_root.as<int>(), c->l_turn.as<int>(), K, c->P), launches);
+  CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
+  out->n_tracks = nt;
+  if (!device_result) {
+    CUDA_TRY(c, c->hl_prev.resize(ntz)); CUDA_TRY(c, c->hl_root.resize(ntz)); CUDA_TRY(c, c->hl_turn.resize(ntz));
+    if (nt > 0) {
+      CUDA_TRY(c, cudaMemcpyAsync(c->hl_prev.data(), c->l_prev.p, (size_t)nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hl_root.data(), c->l_root.p, (size_t)nt * 4, cudaMemcpyDeviceToHost, st));
+      CUDA_TRY(c, cudaMemcpyAsync(c->hl_turn.data(), c->l_turn.p, (size_t)nt * 4, cudaMemcpyDeviceToHost, st));
+    }
+    out->prev = c->hl_prev.data(); out->root = c->hl_root.data(); out->turn = c->hl_turn.data();
+  } else {
+    out->prev = c->l_prev.as<int32_t>(); out->root = c->l_root.as<int32_t>(); out->turn = c->l_turn.as<int32_t>();
+  }
+  CUDA_TRY(c, cudaStreamSynchronize(st));
+  CUDA_TRY(c, cudaEventElapsedTime(&out->ms_loopers, c->ev[8], c->ev[9]));
   return TPC_OK;
 }
 int tpc_get_timings(tpc_ctx* c, tpc_timings* out) {

@@ -52,6 +52,9 @@ struct Params {
 struct K9Params { float edge, dy, dz, ds, dt, cd, sd; int rows;
                   int per_side; };   // sectors per closed ring in phi (18 for 20 degree sectors); 0 = the sectors do not close a ring: nothing to merge
 
+// S10 (NEXT-3, second half) parameters (reading A46), rounded to float once on the host
+struct K10Params { float qmin, dy, ds, dt, dq, pmin, frac, twopi; int nmax; };
+
 // Work item of K2/K3: a chunk of consecutive sorted hits of one unit.
 struct Item { int unit; int start; };
 
@@ -161,6 +164,9 @@ int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_se
                     const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first, const RowConst* d_rows, float* d_outer,
                     int* d_row_in, int* d_row_out, int* d_leaver, int* d_sec_begin, unsigned long long* d_cand, int* d_next,
                     int* d_prev, const K9Params& M, const Params& P);
+
+int launch_k10_loopers(const Launch& L, long long n_tracks, int NS, const int* o_sector, const float* o_x, const float* o_par,
+                       int* d_sec_begin, int* d_prev, int* d_prev_n, int* d_root, int* d_turn, const K10Params& K, const Params& P);
 
 // device-wide exclusive scans (own kernels; three launches each)
 int launch_scan_i32(const Launch& L, const int* d_in, int* d_out, int n, int* d_tmp, int* d_total);

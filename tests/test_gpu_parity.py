@@ -221,6 +221,34 @@ def test_cross_sector_merges_parity_c2_and_c3_scaled():
         assert np.all(np.array(trk.merge_tracks()["next"]) == -1)
 
 
+def test_looper_turns_parity_c4_and_c3_scaled():
+    """S10 (NEXT-3, second half): prev / root / turn arrays identical to the oracle's (identical track lists, the same fp32 transport on
+    both sides: no window edge can flip); linked tracks carry one particle label; host = device result."""
+    for w in (W.config(4), W.config(3, scale=0.1)):
+        o = P.make_oracle(w).run("s6"); o.run_range("s10", "s10")
+        otr, ol = o.tracks(), o.loopers()
+        with _tracker(w) as trk:
+            trk.load_workload(w)
+            gtr = trk.find_tracks().copy().as_dict()
+            m = trk.find_loopers()
+            pv, rt, tn = np.array(m["prev"]), np.array(m["root"]), np.array(m["turn"])
+            dev = trk.find_loopers(device_result=True)
+            assert np.array_equal(dev["prev"].cpu().numpy(), pv) and np.array_equal(dev["root"].cpu().numpy(), rt) and np.array_equal(dev["turn"].cpu().numpy(), tn)
+            assert m["ms_loopers"] > 0 and m["n_tracks"] == len(gtr["sector"])
+        assert np.array_equal(otr["cl_begin"], gtr["cl_begin"]) and np.array_equal(otr["cl_index"], gtr["cl_index"])
+        assert np.array_equal(pv, ol["prev"]) and np.array_equal(rt, ol["root"]) and np.array_equal(tn, ol["turn"])
+        if w.name == "C4":
+            assert (pv >= 0).sum() > 1000
+            labs = H.track_labels(w, gtr)
+            bad = sum(1 for i in np.nonzero(pv >= 0)[0] if labs[i][0] != labs[pv[i]][0])
+            assert bad <= 0.02 * (pv >= 0).sum()
+    w1 = W.config(1, scale=0.1)
+    with _tracker(w1) as trk:
+        with pytest.raises(Exception) as e:
+            trk.find_loopers()
+        assert e.value.code == -2
+
+
 def test_refit_before_find_tracks_is_a_state_error():
     import paper_1905_05515_b200 as T
     w = W.config(1, scale=0.1)
@@ -283,7 +311,7 @@ def test_next_rows_on_an_empty_result():
         y = np.array([1.0, 2.0, -3.0], np.float32); t = np.array([10.0, 20.0, 30.0], np.float32)
         trk.load(0, 5, y, t)
         assert trk.find_tracks().n_tracks == 0
-        assert trk.refit_tracks()["n_tracks"] == 0 and trk.merge_tracks()["n_tracks"] == 0
+        assert trk.refit_tracks()["n_tracks"] == 0 and trk.merge_tracks()["n_tracks"] == 0 and trk.find_loopers()["n_tracks"] == 0
         m = trk.mark_clusters()
         assert m["n_clusters"] == 3 and np.all(m["status"] == 0) and np.all(m["track"] == -1)
 
@@ -499,7 +527,7 @@ def test_abi_state_and_argument_errors_on_device():
             trk.links(0, 5, cleaned=False)                   # raw links need debug_keep
         assert e.value.code == -2
         trk.clear()
-        for call in (trk.refit_tracks, trk.mark_clusters, trk.merge_tracks):   # results are gone after tpc_clear
+        for call in (trk.refit_tracks, trk.mark_clusters, trk.merge_tracks, trk.find_loopers):   # results are gone after tpc_clear
             with pytest.raises(T.TpcError) as e:
                 call()
             assert e.value.code == -2
