@@ -98,18 +98,29 @@ def oracle_run(w, sectors):
 
 
 def oracle_run_parallel(w, n_threads):
-    """The same oracle, one independent instance per sector on n_threads host threads (sectors are independent; the paper's CPU
-    tracking scales linearly with cores).  Returns (seconds, clusters, threads)."""
-    import threading
+    """The same oracle over ALL sectors of the workload, one independent instance per sector, the instances shared out over
+    n_threads host threads (sectors are independent; the paper's CPU tracking scales linearly with cores).
+    Returns (seconds, clusters, threads)."""
+    import queue
     from tests import parity as P
     n_threads = max(1, min(n_threads, w.n_sectors))
-    orcs = [P.make_oracle(w.sector_slice([s])) for s in range(n_threads)]      # ctypes calls release the GIL
-    n = sum(int(w.unit_off[(s + 1) * w.n_rows] - w.unit_off[s * w.n_rows]) for s in range(n_threads))
-    th = [threading.Thread(target=o.run, args=("s6",)) for o in orcs]
+    orcs = [P.make_oracle(w.sector_slice([s])) for s in range(w.n_sectors)]      # ctypes calls release the GIL
+    todo = queue.SimpleQueue()
+    for o in orcs:
+        todo.put(o)
+
+    def work():
+        while True:
+            try:
+                o = todo.get_nowait()
+            except Exception:      # noqa: BLE001  (queue.Empty)
+                return
+            o.run("s6")
+    th = [threading.Thread(target=work) for _ in range(n_threads)]
     t0 = time.perf_counter()
     [t.start() for t in th]
     [t.join() for t in th]
-    return time.perf_counter() - t0, n, n_threads
+    return time.perf_counter() - t0, w.n_clusters, n_threads
 
 
 def run_reference(args, rank, world):
@@ -195,6 +206,8 @@ def run_gpu(args, rank, world, local_rank):
     value = total_clusters / (ms * 1e-3)
     kern = {k: acc[k] / args.steps for k in keys}
     n_tracks, n_refs = res.n_tracks, res.n_cluster_refs
+    # fp32 FMA-loop peak of this box at the clocks of this run (untimed part): the roofline denominator of S5
+    fma_peak = trk.measure_fp32_peak() if rank == 0 else None
     # S8 (NEXT-4, not part of the timed step): attachment status of every cluster (Fig. 7's attached / adjacent)
     mk = [trk.mark_clusters(1.5, device_result=True) for _ in range(3)]
     mark_ms = float(np.mean([m["ms_mark"] for m in mk[1:]]))
@@ -290,6 +303,42 @@ def run_gpu(args, rank, world, local_rank):
     h2d = 2 * 4 * N
     d2h = hres.n_tracks * (4 + 4 + 20 + 60 + 4 + 4 + 4) + (hres.n_tracks + 1) * 8 + hres.n_cluster_refs * 8
     trk.close()
+    # ---- linearity check (PAPER.md:41 / Fig. 1 "almost linear" run time versus event size): ns per cluster of the same
+    #      device-resident step on C2 (one event), the benched workload and C5 (10 ms frame), outside the timed region of `value`
+    linearity = None
+    if rank == 0 and world == 1 and not args.no_linearity:
+        linearity = {f"C{args.config}": {"clusters": N, "ms_per_step": ms, "ns_per_cluster": ms * 1e6 / N}}
+        for k in (2, 5):
+            if k == args.config:
+                continue
+            wk = W.config(k, seed=k)
+            with T.Tracker(**wk.geometry()) as tk:
+                tk.set_stream(stream.cuda_stream)
+                yk, tk_d = torch.from_numpy(wk.y).cuda(), torch.from_numpy(wk.t).cuda()
+                tk.load_batch(wk.unit_off, yk, tk_d)
+                for _ in range(3):
+                    rk = tk.find_tracks_device()
+                torch.cuda.synchronize()
+                e0.record(stream)
+                nst = 5
+                for _ in range(nst):
+                    rk = tk.find_tracks_device()
+                e1.record(stream)
+                torch.cuda.synchronize()
+                msk = e0.elapsed_time(e1) / nst
+                linearity[f"C{k}"] = {"clusters": wk.n_clusters, "ms_per_step": msk, "ns_per_cluster": msk * 1e6 / wk.n_clusters,
+                                      "tracks_per_step": int(rk.n_tracks), "collisions": wk.n_collisions,
+                                      "kernel_ms": {kk: tk.timings()[kk] for kk in keys}}
+                del yk, tk_d
+            if k == 2 and not args.no_cpu_baseline:      # the oracle on all 36 sectors of C2 as well (one core, and all cores)
+                dt1, n1, _ = oracle_run(wk, list(range(wk.n_sectors)))
+                dtp, np_, nth = oracle_run_parallel(wk, min(36, len(os.sched_getaffinity(0))))
+                linearity["C2"]["cpu_baseline"] = {"value": n1 / dt1, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt1,
+                                                   "sample": f"all 36 sectors of C2 ({n1} clusters)"}
+                linearity["C2"]["cpu_baseline_parallel"] = {"value": np_ / dtp, "unit": UNIT, "cores": nth, "seconds": dtp,
+                                                            "sample": f"all 36 sectors of C2 ({np_} clusters), one oracle instance per sector"}
+            del wk
+        torch.cuda.empty_cache()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -297,14 +346,17 @@ def run_gpu(args, rank, world, local_rank):
 
     # ---- roofline of every kernel; the dominant one goes into "roofline"
     hbm_peak, peak_src, sm_max = _peaks()
-    issue_peak = 148 * 128 * sm_max * 1e6 / 1e12    # T fp32 instructions/s: one per lane per clock
-    alu_peak = 2.0 * issue_peak                     # TFLOP/s: the FMA peak (two flops per lane per clock)
-    traffic = {}
+    nominal_issue = 148 * 128 * sm_max * 1e6 / 1e12  # T fp32 instructions/s: one per lane per clock (B200_PROFILING.md unit counts)
+    alu_peak = fma_peak if fma_peak else 2.0 * nominal_issue   # TFLOP/s: the FMA-loop throughput measured above (two flops per FMA)
+    issue_peak = 0.5 * alu_peak                      # T fp32 instructions/s
+    traffic, traffic_source = {}, None
     tp = os.path.join(ROOT, "profiles", f"traffic_c{args.config}.csv")   # DRAM bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
         for line in open(tp):
             f = line.strip().split(",")
-            if len(f) == 2 and f[1].isdigit():
+            if line.startswith("#"):
+                traffic_source = f"profiles/traffic_c{args.config}.csv: " + line[1:].strip()
+            elif len(f) == 2 and f[1].isdigit():
                 traffic[f[0]] = int(f[1])
     roofs = {}
     for name, key in (("grid", "ms_grid"), ("neighbours", "ms_neighbours"), ("clean_start", "ms_clean_start")):
@@ -315,13 +367,15 @@ def run_gpu(args, rank, world, local_rank):
     a = flops / (kern["ms_tracklets"] * 1e-3) / 1e12
     insts = INST_PROPAGATE * tm["n_propagations"] + INST_UPDATE * tm["n_updates"] + INST_PICKUP * tm["n_pickups"]
     roofs["tracklets"] = {"bound": "alu", "achieved": a, "peak": alu_peak, "unit": "TFLOP/s", "frac": a / alu_peak,
-                          "peak_source": "148 SM x 128 fp32 lanes x 2 flop (FMA) x sm_max_mhz (DESIGN.md section 8)", "ms": kern["ms_tracklets"],
+                          "peak_source": "measured: FMA loop of tpc_measure_fp32_peak in this run" if fma_peak else "nominal",
+                          "peak_nominal": 2.0 * nominal_issue, "ms": kern["ms_tracklets"],
                           "fp32_inst_frac": insts / (kern["ms_tracklets"] * 1e-3) / 1e12 / issue_peak,
                           "traffic": traffic.get("tracklets")}
     roofs["selector"] = {"bound": "hbm", "achieved": None, "peak": hbm_peak, "unit": "GB/s", "frac": None, "ms": kern["ms_selector"],
                          "traffic": traffic.get("selector")}
     dominant = max(("grid", "neighbours", "clean_start", "tracklets"), key=lambda k: roofs[k]["ms"])
     roofline = dict(roofs[dominant]); roofline["kernel"] = dominant
+    roofline["traffic_source"] = traffic_source
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -336,7 +390,7 @@ def run_gpu(args, rank, world, local_rank):
             cores = os.cpu_count() or 1
         dt, n, nth = oracle_run_parallel(w, min(36, cores))
         cpu_par = {"value": n / dt, "unit": UNIT, "cores": nth, "kind": "oracle, one instance per sector", "seconds": dt,
-                   "sample": f"sectors 0..{nth - 1} of C{args.config} ({n} clusters), one thread each, full S0..S6",
+                   "sample": f"all {w.n_sectors} sectors of C{args.config} ({n} clusters), one oracle instance per sector over {nth} threads, full S0..S6",
                    "host_cores": cores}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -350,7 +404,7 @@ def run_gpu(args, rank, world, local_rank):
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu, "cpu_baseline_parallel": cpu_par,
-           "variant_seed_bridging": variant, "cluster_marks": marks, "sector_merges": merges, "looper_turns": loopers,
+           "linearity": linearity, "variant_seed_bridging": variant, "cluster_marks": marks, "sector_merges": merges, "looper_turns": loopers,
            "refit": {"ms": refit_ms, "tracks_per_s": n_tracks / (refit_ms * 1e-3), "note": "S7 refit + collision time (SURVEY 8(f).1), outside the timed step"},
            "clocks": clocks}
     print(json.dumps(out))
@@ -365,8 +419,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="workload preset C1..C5 (default C3, the 50 kHz time frame)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-sectors", type=int, default=4, help="sectors of the workload the CPU oracle is timed on")
+    ap.add_argument("--ref-sectors", type=int, default=8, help="sectors of the workload the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-linearity", action="store_true", help="skip the C2 / C5 runs of the linearity check")
     ap.add_argument("--frames-in-flight", type=int, default=2, help="contexts / streams of the pipelined end-to-end arm")
     ap.add_argument("--variant", action="store_true", help="also time the NEXT-2 seed-bridging variant (extra field, not `value`)")
     ap.add_argument("--param", action="append", default=[], help="library tunable name=value (tpc_set_param), e.g. chunk=1024")

@@ -209,6 +209,11 @@ const char* tpc_last_error(const tpc_ctx*);   /* never NULL; ctx may be NULL (me
 
 int tpc_get_timings(tpc_ctx*, tpc_timings* out);
 
+/* Measurement utility for bench.py ("builder measures an FMA-loop peak"): fp32 fused-multiply-add throughput of
+ * the device at the clocks of the moment, in TFLOP/s (2 flops per FMA; 8 independent chains per thread, 2048 threads per SM).  It is
+ * the denominator of the roofline of the ALU-bound kernels; not part of the tracking path. */
+int tpc_measure_fp32_peak(tpc_ctx*, float* tflops);
+
 /* Parity / debug exports of the last tpc_find_tracks* call (host copies, library-owned, valid until the next call on the context). */
 int tpc_debug_get_grid(tpc_ctx*, int sector, int row, tpc_grid_view* out);
 /* cleaned = 0: S2 tables (needs debug_keep = 1), 1: after S3.  up/dn: [n] positions in the sorted order of row+1 / row-1, -1 = none. */

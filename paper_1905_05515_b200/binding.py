@@ -17,7 +17,7 @@ _SO = os.path.join(_HERE, "libtpc_b200.so")
 
 ABI_SYMBOLS = [
     "tpc_abi_version", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
-    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_find_loopers", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings",
+    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_find_loopers", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings", "tpc_measure_fp32_peak",
     "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_link_rows", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
 
@@ -113,6 +113,7 @@ def load_library():
     lib.tpc_last_error.argtypes = [vp]
     lib.tpc_last_error.restype = C.c_char_p
     lib.tpc_get_timings.argtypes = [vp, C.POINTER(_Timings)]
+    lib.tpc_measure_fp32_peak.argtypes = [vp, C.POINTER(C.c_float)]
     lib.tpc_debug_get_grid.argtypes = [vp, C.c_int, C.c_int, C.POINTER(_GridView)]
     lib.tpc_debug_get_links.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(_PI), C.POINTER(_PI), C.POINTER(C.c_int32)]
     lib.tpc_debug_get_link_rows.argtypes = [vp, C.POINTER(C.POINTER(C.c_int8)), C.POINTER(C.POINTER(C.c_int8)), C.POINTER(C.c_int32)]
@@ -388,6 +389,12 @@ class Tracker:
 
     def timings(self) -> dict:
         return tpc_get_timings(self.h)
+
+    def measure_fp32_peak(self) -> float:
+        """fp32 FMA-loop throughput of the device now, TFLOP/s (measurement utility of the library, not part of the path)."""
+        v = C.c_float()
+        _check(self.h, load_library().tpc_measure_fp32_peak(self.h, C.byref(v)))
+        return float(v.value)
 
     # ---- parity / debug exports
     def grid(self, sector, row) -> dict:

@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
                                                               const int* __restrict__ start_unit, const int* __restrict__ start_pos,
                                                               const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
                                                               const float2* __restrict__ yz, const int* __restrict__ link_up,
-                                                              int* __restrict__ rowhit, TlRec* __restrict__ rec, int* __restrict__ list_b,
+                                                              rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec, int* __restrict__ list_b,
                                                               int* __restrict__ list_c, int* __restrict__ ctl,
                                                               unsigned long long* __restrict__ counters, const Params P) {
   K5_PROLOGUE();
@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
   float2 cl = make_float2(0.f, 0.f);
   State st = {};
   const UnitDesc* __restrict__ su = units;
-  int* __restrict__ rh = rowhit;
+  rowhit_t* __restrict__ rh = rowhit;
 
   for (;;) {
     if (flush_now(mode, drained)) {
@@ -273,7 +273,7 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
 __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5b_extend_out(const int* __restrict__ list_b, const UnitDesc* __restrict__ units,
                                                                 const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                                 const int* __restrict__ perm, const int* __restrict__ bin_start,
-                                                                int* __restrict__ rowhit, TlRec* __restrict__ rec,
+                                                                rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec,
                                                                 int* __restrict__ list_c, int* __restrict__ ctl,
                                                                 unsigned long long* __restrict__ counters, const Params P) {
   K5_PROLOGUE();
@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5b_extend_out(const int*
   float zref = 0.0f;
   State st = {};
   const UnitDesc* __restrict__ su = units;
-  int* __restrict__ rh = rowhit;
+  rowhit_t* __restrict__ rh = rowhit;
 
   for (;;) {
     if (flush_now(mode, drained)) {
@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5b_extend_out(const int*
 __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5c_refit_in(const int* __restrict__ list_c, const UnitDesc* __restrict__ units,
                                                               const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                               const int* __restrict__ perm, const int* __restrict__ bin_start,
-                                                              int* __restrict__ rowhit, TlRec* __restrict__ rec,
+                                                              rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec,
                                                               int* __restrict__ list_d, int* __restrict__ ctl,
                                                               int* __restrict__ tl_n, int* __restrict__ tl_first,
                                                               int* __restrict__ tl_last, float* __restrict__ tl_chi2,
@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5c_refit_in(const int* _
   float2 cl = make_float2(0.f, 0.f);
   State st = {};
   const UnitDesc* __restrict__ su = units;
-  int* __restrict__ rh = rowhit;
+  rowhit_t* __restrict__ rh = rowhit;
 
   for (;;) {
     if (flush_now(mode, drained)) {
@@ -470,7 +470,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5c_refit_in(const int* _
 __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5d_extend_in(const int* __restrict__ list_d, const UnitDesc* __restrict__ units,
                                                                const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                                const int* __restrict__ perm, const int* __restrict__ bin_start,
-                                                               int* __restrict__ rowhit, const TlRec* __restrict__ rec,
+                                                               rowhit_t* __restrict__ rowhit, const TlRec* __restrict__ rec,
                                                                int* __restrict__ ctl, int* __restrict__ tl_n,
                                                                int* __restrict__ tl_first, int* __restrict__ tl_last,
                                                                float* __restrict__ tl_chi2, float* __restrict__ tl_par,
@@ -484,7 +484,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5d_extend_in(const int* 
   float zref = 0.0f, chi2 = 0.0f;
   State st = {};
   const UnitDesc* __restrict__ su = units;
-  int* __restrict__ rh = rowhit;
+  rowhit_t* __restrict__ rh = rowhit;
 
   for (;;) {
     if (flush_now(mode, drained)) {
@@ -568,7 +568,7 @@ size_t k5_scratch_bytes(long long M) {   // TlRec array + three task lists + con
 // its upper bound.  M: capacity of the per-tracklet arrays / scratch.
 int launch_k5_tracklets(const Launch& L, int n_run, const int* d_n_run, int M, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
                         const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
-                        const int* d_link_up, int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2,
+                        const int* d_link_up, rowhit_t* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2,
                         float* d_tl_par, float* d_tl_cov, unsigned long long* d_counters, void* d_scratch, const Params& P) {
   if (n_run <= 0) return 0;
   if (P.R > K5_MAX_ROWS) return -(int)cudaErrorInvalidValue;   // tpc_create limits n_rows to 255 (selector key)

@@ -15,6 +15,8 @@ namespace tpc {
 namespace {
 
 constexpr int K6_THREADS = 128;
+constexpr int K6_PER_BLOCK = 32;   // consecutive tracklets per CTA: the CTAs are scheduled in launch order, so the tracklets in flight at any
+                                   // time are neighbours in (sector, row) order and their owner keys share a small, L2-resident region
 constexpr unsigned long long REF_MASK = (1ull << 40) - 1ull;
 
 __device__ __forceinline__ unsigned long long make_key(int n, float chi2, int idx) {
@@ -28,13 +30,15 @@ __device__ __forceinline__ unsigned long long make_key(int n, float chi2, int id
 // their owner-key atomics / owner reads in parallel.
 __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M_cap, const int* __restrict__ M_dev, const int* __restrict__ run_list, const int R, const int min_hits,
                                                        const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
-                                                       const int* __restrict__ rowhit, const int* __restrict__ tl_n,
+                                                       const rowhit_t* __restrict__ rowhit, const int* __restrict__ tl_n,
                                                        const int* __restrict__ tl_first, const int* __restrict__ tl_last,
                                                        const float* __restrict__ tl_chi2, unsigned long long* __restrict__ owner,
                                                        unsigned long long* __restrict__ tl_key) {
-  const int lane = threadIdx.x & 31, n_warps = (int)(((long long)gridDim.x * blockDim.x) >> 5);
+  const int lane = threadIdx.x & 31, n_warps = K6_THREADS >> 5;
   const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
-  for (int q = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); q < M; q += n_warps) {
+  const long long q1 = min((long long)M, ((long long)blockIdx.x + 1) * K6_PER_BLOCK);
+  for (long long qq = (long long)blockIdx.x * K6_PER_BLOCK + (threadIdx.x >> 5); qq < q1; qq += n_warps) {
+  const int q = (int)qq;
   const int i = run_list ? run_list[q] : q;   // M entries of a run list (rescue variant), or all tracklets
   const int n = tl_n[i];
   const float chi2 = tl_chi2[i];
@@ -44,7 +48,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M_cap, const in
   if (lane == 0) tl_key[i] = key;
   if (!kept) continue;
   const UnitDesc* __restrict__ su = units + (long long)(u0 / R) * R;
-  const int* __restrict__ rh = rowhit + (long long)i * R;
+  const rowhit_t* __restrict__ rh = rowhit + (long long)i * R;
   for (int r = r_lo + lane; r <= r1; r += 32) {
     const int p = rh[r];
     if (p >= 0) atomicMax(&owner[su[r].off + p], key);
@@ -54,20 +58,22 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M_cap, const in
 
 __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M_cap, const int* __restrict__ M_dev, const int R, const int min_hits,
                                                        const int* __restrict__ start_unit, const UnitDesc* __restrict__ units,
-                                                       const int* __restrict__ rowhit, const int* __restrict__ tl_first,
+                                                       const rowhit_t* __restrict__ rowhit, const int* __restrict__ tl_first,
                                                        const int* __restrict__ tl_last, const unsigned long long* __restrict__ owner,
                                                        const unsigned long long* __restrict__ tl_key,
                                                        unsigned long long* __restrict__ scan_in) {
-  const int lane = threadIdx.x & 31, n_warps = (int)(((long long)gridDim.x * blockDim.x) >> 5);
+  const int lane = threadIdx.x & 31, n_warps = K6_THREADS >> 5;
   const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
-  for (int i = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); i < M_cap; i += n_warps) {
+  const long long i1 = min((long long)M_cap, ((long long)blockIdx.x + 1) * K6_PER_BLOCK);
+  for (long long ii = (long long)blockIdx.x * K6_PER_BLOCK + (threadIdx.x >> 5); ii < i1; ii += n_warps) {
+  const int i = (int)ii;
   if (i >= M) { if (lane == 0) scan_in[i] = 0ull; continue; }   // the scan runs over the capacity: entries beyond the count are 0
   const unsigned long long key = tl_key[i];
   const int u0 = start_unit[i], r_lo = tl_first[i], r1 = tl_last[i];     // read with the key, not after the decision it feeds
   int owned = 0;
   if (key) {
     const UnitDesc* __restrict__ su = units + (long long)(u0 / R) * R;
-    const int* __restrict__ rh = rowhit + (long long)i * R;
+    const rowhit_t* __restrict__ rh = rowhit + (long long)i * R;
     for (int r = r_lo + lane; r <= r1; r += 32) {
       const int p = rh[r];
       if (p >= 0 && owner[su[r].off + p] == key) owned++;
@@ -80,7 +86,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M_cap, const in
 
 __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M_cap, const int* __restrict__ M_dev, const int R, const int* __restrict__ start_unit,
                                                       const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
-                                                      const int* __restrict__ perm, const int* __restrict__ rowhit,
+                                                      const int* __restrict__ perm, const rowhit_t* __restrict__ rowhit,
                                                       const int* __restrict__ tl_n, const int* __restrict__ tl_first,
                                                       const int* __restrict__ tl_last, const float* __restrict__ tl_chi2,
                                                       const float* __restrict__ tl_par, const float* __restrict__ tl_cov,
@@ -94,20 +100,22 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M_cap, const int
                                                       int* __restrict__ o_cl_index, const unsigned long long* __restrict__ total,
                                                       const long long cap_tracks, const long long cap_refs) {
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const int lane = threadIdx.x & 31, n_warps = (int)(((long long)gridDim.x * blockDim.x) >> 5);
+  const int lane = threadIdx.x & 31, n_warps = K6_THREADS >> 5;
   const unsigned long long tot = *total;                       // (tracks << 40 | cluster references) of the scan
   const long long n_tracks = (long long)(tot >> 40), n_refs = (long long)(tot & REF_MASK);
   if (n_tracks > cap_tracks || n_refs > cap_refs) return;      // the caller sees the totals and repeats the call with larger buffers
   if (gt == 0) o_cl_begin[n_tracks] = n_refs;
   const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
-  for (int i = (int)(gt >> 5); i < M; i += n_warps) {
+  const long long i1 = min((long long)M, ((long long)blockIdx.x + 1) * K6_PER_BLOCK);
+  for (long long ii = (long long)blockIdx.x * K6_PER_BLOCK + (threadIdx.x >> 5); ii < i1; ii += n_warps) {
+  const int i = (int)ii;
   if (scan_in[i] == 0ull) continue;
   const unsigned long long so = scan_out[i];
   const long long t = (long long)(so >> 40);
   long long k = (long long)(so & REF_MASK);
   const int sec = start_unit[i] / R;
   const UnitDesc* __restrict__ su = units + (long long)sec * R;
-  const int* __restrict__ rh = rowhit + (long long)i * R;
+  const rowhit_t* __restrict__ rh = rowhit + (long long)i * R;
   const unsigned long long key = tl_key[i];
   const int r0 = tl_first[i], r1 = tl_last[i];
   if (lane == 0) {
@@ -129,15 +137,16 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M_cap, const int
 
 }  // namespace
 
-// grid of the warp-per-tracklet kernels: enough warps to fill the GPU several times over, never more than one warp per tracklet
+// grid of the warp-per-tracklet kernels: one CTA per K6_PER_BLOCK consecutive tracklets of the capacity (CTAs beyond the count exit)
 static int k6_blocks(const Launch& L, long long M) {
-  const long long want = (M * 32 + K6_THREADS - 1) / K6_THREADS, cap = (long long)L.sm_count * 16 * 8;
-  return (int)(want < 1 ? 1 : (want < cap ? want : cap));
+  (void)L;
+  const long long want = (M + K6_PER_BLOCK - 1) / K6_PER_BLOCK;
+  return (int)(want < 1 ? 1 : want);
 }
 
 // d_M: tracklet count in device memory (or nullptr: M_cap is the count); M_cap: capacity of the per-tracklet arrays
 int launch_k6_select(const Launch& L, int M_cap, const int* d_M, long long N, const int* d_start_unit, const UnitDesc* d_units,
-                     const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
+                     const rowhit_t* d_rowhit, const int* d_tl_n, const int* d_tl_first,
                      const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
                      unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
                      unsigned long long* d_total, const Params& P, bool owner_done) {
@@ -162,7 +171,7 @@ int launch_k6_select(const Launch& L, int M_cap, const int* d_M, long long N, co
 }
 
 // owner keys of the n_run tracklets of a run list (rescue variant: one call per K5 wave; the caller zeroes d_owner and d_tl_key first)
-int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int* d_start_unit, const UnitDesc* d_units, const int* d_rowhit,
+int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int* d_start_unit, const UnitDesc* d_units, const rowhit_t* d_rowhit,
                     const int* d_tl_n, const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner,
                     unsigned long long* d_tl_key, const Params& P) {
   if (n_run <= 0) return 0;
@@ -174,7 +183,7 @@ int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int
 
 // d_total: (tracks << 40 | references) written by the scan; the output arrays hold cap_tracks tracks / cap_refs references
 int launch_k6_emit(const Launch& L, int M_cap, const int* d_M, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
-                   const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
+                   const int* d_perm, const rowhit_t* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
                    const float* d_tl_chi2, const float* d_tl_par, const float* d_tl_cov, const unsigned long long* d_owner,
                    const unsigned long long* d_tl_key, const unsigned long long* d_scan_in, const unsigned long long* d_scan_out,
                    int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,

@@ -20,7 +20,7 @@ __global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks,
                                                        const int* __restrict__ o_tracklet, const long long* __restrict__ cl_begin,
                                                        const int* __restrict__ cl_row, const UnitDesc* __restrict__ units,
                                                        const RowConst* __restrict__ rows, const float2* __restrict__ yz,
-                                                       const int* __restrict__ rowhit, int* __restrict__ rf_n, int* __restrict__ rf_ndf,
+                                                       const rowhit_t* __restrict__ rowhit, int* __restrict__ rf_n, int* __restrict__ rf_ndf,
                                                        float* __restrict__ rf_x, float* __restrict__ rf_par, float* __restrict__ rf_cov,
                                                        float* __restrict__ rf_chi2, float* __restrict__ rf_z0, float* __restrict__ rf_t0,
                                                        const Params P) {
@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks,
   const long long a = cl_begin[i];
   const int m = (int)(cl_begin[i + 1] - a);
   const UnitDesc* __restrict__ su = units + (long long)o_sector[i] * R;
-  const int* __restrict__ rh = rowhit + (long long)o_tracklet[i] * R;
+  const rowhit_t* __restrict__ rh = rowhit + (long long)o_tracklet[i] * R;
   const int* __restrict__ cr = cl_row + a;
   auto cluster = [&](const int row) { return yz[su[row].off + rh[row]]; };
 
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks,
 }  // namespace
 
 int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, const int* o_tracklet, const long long* o_cl_begin,
-                    const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_rowhit,
+                    const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const rowhit_t* d_rowhit,
                     int* rf_n, int* rf_ndf, float* rf_x, float* rf_par, float* rf_cov, float* rf_chi2, float* rf_z0, float* rf_t0,
                     const Params& P) {
   if (n_tracks <= 0) return 0;

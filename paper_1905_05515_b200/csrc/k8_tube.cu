@@ -20,12 +20,12 @@ constexpr unsigned long long K8_NONE = ~0ull;
 __global__ void __launch_bounds__(K8_THREADS) k8_attach(const long long n_tracks, const int R, const int* __restrict__ o_sector,
                                                         const int* __restrict__ o_tracklet, const long long* __restrict__ cl_begin,
                                                         const int* __restrict__ cl_row, const UnitDesc* __restrict__ units,
-                                                        const int* __restrict__ rowhit, int* __restrict__ att) {
+                                                        const rowhit_t* __restrict__ rowhit, int* __restrict__ att) {
   const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (i >= n_tracks) return;
   const UnitDesc* __restrict__ su = units + (long long)o_sector[i] * R;
-  const int* __restrict__ rh = rowhit + (long long)o_tracklet[i] * R;
+  const rowhit_t* __restrict__ rh = rowhit + (long long)o_tracklet[i] * R;
   const long long b = cl_begin[i + 1];
   for (long long k = cl_begin[i] + lane; k < b; k += 32) {
     const int r = cl_row[k];
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(256) k8_status(const int U, const UnitDesc* __
 int launch_k8_status(const Launch& L, long long n_tracks, long long N, int U, const int* o_sector, const int* o_tracklet,
                      const float* o_par, const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first,
                      const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
-                     const int* d_rowhit, int* d_att, unsigned long long* d_adj, int* cl_status, int* cl_track, float tube,
+                     const rowhit_t* d_rowhit, int* d_att, unsigned long long* d_adj, int* cl_status, int* cl_track, float tube,
                      const Params& P) {
   if (N <= 0 || U <= 0) return 0;
   cudaError_t e = cudaMemsetAsync(d_att, 0xff, (size_t)N * sizeof(int), L.stream);

@@ -98,4 +98,28 @@ int launch_scan_u64(const Launch& L, const unsigned long long* d_in, unsigned lo
   return scan_impl<unsigned long long>(L, d_in, d_out, n, d_tmp, d_total);
 }
 
+// ---- fp32 FMA-loop peak (measurement utility for bench.py: the roofline denominator of the ALU-bound kernels, measured on the
+//      box at the clocks of the run instead of taken from a data sheet).  8 independent chains per thread, explicit __fmaf_rn
+//      (the library is compiled with -fmad=false), 2048 resident threads per SM.
+namespace {
+__global__ void __launch_bounds__(256) fma_peak_kernel(float* __restrict__ out, const int iters, const float a, const float b) {
+  float x0 = threadIdx.x * 1e-3f, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f, x4 = x0 + 4.f, x5 = x0 + 5.f, x6 = x0 + 6.f, x7 = x0 + 7.f;
+#pragma unroll 4
+  for (int i = 0; i < iters; i++) {
+    x0 = __fmaf_rn(x0, a, b); x1 = __fmaf_rn(x1, a, b); x2 = __fmaf_rn(x2, a, b); x3 = __fmaf_rn(x3, a, b);
+    x4 = __fmaf_rn(x4, a, b); x5 = __fmaf_rn(x5, a, b); x6 = __fmaf_rn(x6, a, b); x7 = __fmaf_rn(x7, a, b);
+  }
+  const float s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == 123.456f) out[0] = s;   // keeps the chains alive
+}
+}  // namespace
+
+// returns fused multiply-adds per launch (each is 2 flops), or a negative cudaError
+long long launch_fma_peak(const Launch& L, float* d_out, int iters) {
+  const int blocks = L.sm_count * 8;
+  fma_peak_kernel<<<blocks, 256, 0, L.stream>>>(d_out, iters, 0.999999f, 1e-7f);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? (long long)blocks * 256 * 8 * (long long)iters : -(long long)e;
+}
+
 }  // namespace tpc

@@ -616,7 +616,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
 
     // ---- K5: S5
     const size_t Mz = (size_t)std::max(Mc, 1);
-    CUDA_TRY(c, c->d_rowhit.ensure((size_t)(Mz + 32) * R * 4));
+    CUDA_TRY(c, c->d_rowhit.ensure((size_t)(Mz + 32) * R * sizeof(rowhit_t)));
     CUDA_TRY(c, c->d_k5scratch.ensure(k5_scratch_bytes(Mc)));
     CUDA_TRY(c, c->d_tl_n.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_first.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_last.ensure(Mz * 4));
     CUDA_TRY(c, c->d_tl_chi2.ensure(Mz * 4)); CUDA_TRY(c, c->d_tl_par.ensure(Mz * 20)); CUDA_TRY(c, c->d_tl_cov.ensure(Mz * 60));
@@ -627,7 +627,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
     auto run_k5 = [&](int n_run, const int* d_n, const int* list) -> int {
       LAUNCH_TRY(c, launch_k5_tracklets(L, n_run, d_n, Mc, list, c->d_start_unit.as<int>(), c->d_start_pos.as<int>(), c->d_units.as<UnitDesc>(),
                                         c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
-                                        c->d_link_up.as<int>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
+                                        c->d_link_up.as<int>(), c->d_rowhit.as<rowhit_t>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(),
                                         c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), d_k5cnt,
                                         c->d_k5scratch.p, P), launches);
       return TPC_OK;
@@ -658,7 +658,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
       // first half of the selector over the first wave: its owner keys are the "used" marks of the rescue test
       CUDA_TRY(c, cudaMemsetAsync(c->d_owner.p, 0, (size_t)std::max(N, 1LL) * 8, st));
       CUDA_TRY(c, cudaMemsetAsync(c->d_tl_key.p, 0, Mz * 8, st));
-      LAUNCH_TRY(c, launch_k6_owner(L, M1, list1, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
+      LAUNCH_TRY(c, launch_k6_owner(L, M1, list1, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<rowhit_t>(), c->d_tl_n.as<int>(),
                                     c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned long long*)c->d_owner.p,
                                     (unsigned long long*)c->d_tl_key.p, P), launches);
       LAUNCH_TRY(c, launch_k3_rescue_list(L, M, c->d_keep.as<int>(), c->d_start_unit.as<int>(), c->d_start_pos.as<int>(),
@@ -671,7 +671,7 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
       if (M2 > 0) {
         rc = run_k5(M2, nullptr, list2);
         if (rc != TPC_OK) return rc;
-        LAUNCH_TRY(c, launch_k6_owner(L, M2, list2, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<int>(), c->d_tl_n.as<int>(),
+        LAUNCH_TRY(c, launch_k6_owner(L, M2, list2, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rowhit.as<rowhit_t>(), c->d_tl_n.as<int>(),
                                       c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(), (unsigned long long*)c->d_owner.p,
                                       (unsigned long long*)c->d_tl_key.p, P), launches);
       }
@@ -686,11 +686,11 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
     CUDA_TRY(c, c->o_tracklet.ensure(cap_tracks * 4)); CUDA_TRY(c, c->o_cl_begin.ensure((cap_tracks + 1) * 8));
     CUDA_TRY(c, c->o_cl_row.ensure(cap_refs * 4)); CUDA_TRY(c, c->o_cl_index.ensure(cap_refs * 4));
     LAUNCH_TRY(c, launch_k6_select(L, Mc, d_M, N, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(),
-                                   c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(),
+                                   c->d_rowhit.as<rowhit_t>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(),
                                    c->d_tl_chi2.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
                                    c->d_scan_out.as<u64>(), c->d_scan_tmp64.as<u64>(), d_total64, P, rescue), launches);
     LAUNCH_TRY(c, launch_k6_emit(L, Mc, d_M, c->d_start_unit.as<int>(), c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_perm.as<int>(),
-                                 c->d_rowhit.as<int>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(),
+                                 c->d_rowhit.as<rowhit_t>(), c->d_tl_n.as<int>(), c->d_tl_first.as<int>(), c->d_tl_last.as<int>(), c->d_tl_chi2.as<float>(),
                                  c->d_tl_par.as<float>(), c->d_tl_cov.as<float>(), c->d_owner.as<u64>(), c->d_tl_key.as<u64>(), c->d_scan_in.as<u64>(),
                                  c->d_scan_out.as<u64>(), c->o_sector.as<int>(), c->o_x.as<float>(), c->o_par.as<float>(), c->o_cov.as<float>(),
                                  c->o_chi2.as<float>(), c->o_ndf.as<int>(), c->o_tracklet.as<int>(), c->o_cl_begin.as<long long>(),
@@ -784,7 +784,7 @@ int tpc_refit_tracks(tpc_ctx* c, int device_result, tpc_refit* out) {
   long long launches = 0;
   CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
   LAUNCH_TRY(c, launch_k7_refit(L, nt, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_cl_begin.as<long long>(), c->o_cl_row.as<int>(),
-                                c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_rowhit.as<int>(),
+                                c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_rowhit.as<rowhit_t>(),
                                 c->r_n.as<int>(), c->r_ndf.as<int>(), c->r_x.as<float>(), c->r_par.as<float>(), c->r_cov.as<float>(),
                                 c->r_chi2.as<float>(), c->r_z0.as<float>(), c->r_t0.as<float>(), c->P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
@@ -828,7 +828,7 @@ int tpc_mark_clusters(tpc_ctx* c, float tube_cm, int device_result, tpc_cluster_
   LAUNCH_TRY(c, launch_k8_status(L, c->n_tracks, N, c->NS * c->R, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_par.as<float>(),
                                  c->o_cl_begin.as<long long>(), c->o_cl_row.as<int>(), c->d_tl_first.as<int>(), c->d_units.as<UnitDesc>(),
                                  c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
-                                 c->d_rowhit.as<int>(), c->m_att.as<int>(), (unsigned long long*)c->m_adj.p, c->m_status.as<int>(),
+                                 c->d_rowhit.as<rowhit_t>(), c->m_att.as<int>(), (unsigned long long*)c->m_adj.p, c->m_status.as<int>(),
                                  c->m_track.as<int>(), tube_cm, c->P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
   out->n_clusters = N;
@@ -921,6 +921,26 @@ int tpc_find_loopers(tpc_ctx* c, int device_result, tpc_loopers* out) {
   CUDA_TRY(c, cudaEventElapsedTime(&out->ms_loopers, c->ev[8], c->ev[9]));
   return TPC_OK;
 }
+// Measurement utility: fp32 fused-multiply-add throughput of the device at the clocks of the moment (TFLOP/s, 2 flops per FMA).
+int tpc_measure_fp32_peak(tpc_ctx* c, float* tflops) {
+  if (!c || !tflops) return fail(c, TPC_E_ARG, "tpc_measure_fp32_peak: null argument");
+  cudaStream_t st = c->stream;
+  Launch L{st, c->sm_count, 0};
+  CUDA_TRY(c, c->d_counters.ensure(256));
+  float best = 0.f;
+  for (int rep = 0; rep < 4; rep++) {           // first launch warms up; best of the next three
+    CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
+    const long long fmas = launch_fma_peak(L, c->d_counters.as<float>() + 60, 1 << 14);
+    if (fmas < 0) return fail(c, TPC_E_CUDA, "fma_peak_kernel: %s", cudaGetErrorString((cudaError_t)(-fmas)));
+    CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    float ms = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[8], c->ev[9]));
+    if (rep > 0 && ms > 0.f) best = std::max(best, (float)(2.0 * (double)fmas / (ms * 1e-3) / 1e12));
+  }
+  *tflops = best;
+  return TPC_OK;
+}
 int tpc_get_timings(tpc_ctx* c, tpc_timings* out) {
   if (!c || !out) return fail(c, TPC_E_ARG, "tpc_get_timings: null argument");
   if (!c->have_result) return fail(c, TPC_E_STATE, "tpc_get_timings: no tpc_find_tracks call has completed");
@@ -1005,7 +1025,7 @@ int tpc_debug_get_tracklets(tpc_ctx* c, tpc_tracklet_view* out) {
   c->dbg_tl_chi2.resize(Mz); c->dbg_tl_x.resize(Mz); c->dbg_tl_par.resize(Mz * 5); c->dbg_tl_cov.resize(Mz * 15); c->dbg_rowhit.assign(Mz * R, -1);
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   if (M) {
-    std::vector<int32_t> su(M), raw((size_t)c->Mpad * R);
+    std::vector<int32_t> su(M); std::vector<rowhit_t> raw((size_t)c->Mpad * R);
     CUDA_TRY(c, cudaMemcpy(su.data(), c->d_start_unit.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
     CUDA_TRY(c, cudaMemcpy(c->dbg_tl_n.data(), c->d_tl_n.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
     CUDA_TRY(c, cudaMemcpy(c->dbg_tl_first.data(), c->d_tl_first.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
@@ -1013,7 +1033,7 @@ int tpc_debug_get_tracklets(tpc_ctx* c, tpc_tracklet_view* out) {
     CUDA_TRY(c, cudaMemcpy(c->dbg_tl_chi2.data(), c->d_tl_chi2.p, (size_t)M * 4, cudaMemcpyDeviceToHost));
     CUDA_TRY(c, cudaMemcpy(c->dbg_tl_par.data(), c->d_tl_par.p, (size_t)M * 20, cudaMemcpyDeviceToHost));
     CUDA_TRY(c, cudaMemcpy(c->dbg_tl_cov.data(), c->d_tl_cov.p, (size_t)M * 60, cudaMemcpyDeviceToHost));
-    CUDA_TRY(c, cudaMemcpy(raw.data(), c->d_rowhit.p, raw.size() * 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(c, cudaMemcpy(raw.data(), c->d_rowhit.p, raw.size() * sizeof(rowhit_t), cudaMemcpyDeviceToHost));
     for (int i = 0; i < M; i++) {
       c->dbg_tl_sector[i] = su[i] / R; c->dbg_tl_row[i] = su[i] % R; const int f = c->dbg_tl_first[i];
       c->dbg_tl_x[i] = f >= 0 && f < R ? c->row_x[f] : 0.0f;   // tracklets the rescue variant did not fit carry first = last = -1

@@ -6,6 +6,13 @@
 
 namespace tpc {
 
+// entry of the rowhit table [tracklet][row]: sorted position of the tracklet's cluster on that row, -1 = none
+#ifdef TPC_ROWHIT16
+typedef short rowhit_t;
+#else
+typedef int rowhit_t;
+#endif
+
 // Per-row constants, computed on the host in double and rounded once to float ("per-row constants").
 struct RowConst {
   float x;       // local x of the row
@@ -129,20 +136,20 @@ int launch_k3_clean_start(const Launch& L, int n_items, const Item* d_items, int
 size_t k5_scratch_bytes(long long M);   // handoff records + task lists + control block of the K5 phase kernels
 int launch_k5_tracklets(const Launch& L, int n_run, const int* d_n_run, int M, const int* d_run_list, const int* d_start_unit, const int* d_start_pos,
                         const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
-                        const int* d_link_up, int* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2,
+                        const int* d_link_up, rowhit_t* d_rowhit, int* d_tl_n, int* d_tl_first, int* d_tl_last, float* d_tl_chi2,
                         float* d_tl_par, float* d_tl_cov, unsigned long long* d_counters, void* d_scratch, const Params& P);
 
 int launch_k6_select(const Launch& L, int M_cap, const int* d_M, long long N, const int* d_start_unit, const UnitDesc* d_units,
-                     const int* d_rowhit, const int* d_tl_n, const int* d_tl_first,
+                     const rowhit_t* d_rowhit, const int* d_tl_n, const int* d_tl_first,
                      const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner, unsigned long long* d_tl_key,
                      unsigned long long* d_scan_in, unsigned long long* d_scan_out, unsigned long long* d_scan_tmp,
                      unsigned long long* d_total, const Params& P, bool owner_done);
-int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int* d_start_unit, const UnitDesc* d_units, const int* d_rowhit,
+int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int* d_start_unit, const UnitDesc* d_units, const rowhit_t* d_rowhit,
                     const int* d_tl_n, const int* d_tl_first, const int* d_tl_last, const float* d_tl_chi2, unsigned long long* d_owner,
                     unsigned long long* d_tl_key, const Params& P);
 
 int launch_k6_emit(const Launch& L, int M_cap, const int* d_M, const int* d_start_unit, const UnitDesc* d_units, const RowConst* d_rows,
-                   const int* d_perm, const int* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
+                   const int* d_perm, const rowhit_t* d_rowhit, const int* d_tl_n, const int* d_tl_first, const int* d_tl_last,
                    const float* d_tl_chi2, const float* d_tl_par, const float* d_tl_cov, const unsigned long long* d_owner,
                    const unsigned long long* d_tl_key, const unsigned long long* d_scan_in, const unsigned long long* d_scan_out,
                    int* o_sector, float* o_x, float* o_par, float* o_cov, float* o_chi2, int* o_ndf, int* o_tracklet,
@@ -150,14 +157,14 @@ int launch_k6_emit(const Launch& L, int M_cap, const int* d_M, const int* d_star
                    long long cap_refs, const Params& P);
 
 int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, const int* o_tracklet, const long long* o_cl_begin,
-                    const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_rowhit,
+                    const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const rowhit_t* d_rowhit,
                     int* rf_n, int* rf_ndf, float* rf_x, float* rf_par, float* rf_cov, float* rf_chi2, float* rf_z0, float* rf_t0,
                     const Params& P);
 
 int launch_k8_status(const Launch& L, long long n_tracks, long long N, int U, const int* o_sector, const int* o_tracklet,
                      const float* o_par, const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first,
                      const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
-                     const int* d_rowhit, int* d_att, unsigned long long* d_adj, int* cl_status, int* cl_track, float tube,
+                     const rowhit_t* d_rowhit, int* d_att, unsigned long long* d_adj, int* cl_status, int* cl_track, float tube,
                      const Params& P);
 
 int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_sector, const int* o_tracklet, const float* o_par,
@@ -172,6 +179,7 @@ int launch_k10_loopers(const Launch& L, long long n_tracks, int NS, const int* o
 int launch_scan_i32(const Launch& L, const int* d_in, int* d_out, int n, int* d_tmp, int* d_total);
 int launch_scan_u64(const Launch& L, const unsigned long long* d_in, unsigned long long* d_out, int n, unsigned long long* d_tmp,
                     unsigned long long* d_total);
+long long launch_fma_peak(const Launch& L, float* d_out, int iters);   // measurement utility (scan.cu)
 constexpr int SCAN_TILE = 4096;   // elements per CTA in the scans; tmp needs ceil(n/SCAN_TILE)+1 entries
 
 }  // namespace tpc
