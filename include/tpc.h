@@ -227,6 +227,9 @@ int tpc_debug_get_tracklets(tpc_ctx*, tpc_tracklet_view* out);
 
 /* Version of the ABI (incremented on incompatible change). */
 int tpc_abi_version(void);
+/* 1 if this library was built with -DTPC_CHECKED (libtpc_b200_checked.so: every data-dependent gather / scatter index in the kernels is
+ * bounds-checked and a failure makes tpc_find_tracks* return TPC_E_CUDA), 0 for the product build. */
+int tpc_checked_build(void);
 
 #ifdef __cplusplus
 }

@@ -13,10 +13,11 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libtpc_b200.so")
+# TPC_B200_LIB selects another build of the same library (tests/test_gpu_checked.py: the bounds-checked build); default: the product
+_SO = os.environ.get("TPC_B200_LIB") or os.path.join(_HERE, "libtpc_b200.so")
 
 ABI_SYMBOLS = [
-    "tpc_abi_version", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
+    "tpc_abi_version", "tpc_checked_build", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
     "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_find_loopers", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings", "tpc_measure_fp32_peak",
     "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_link_rows", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
@@ -96,6 +97,7 @@ def load_library():
     lib = C.CDLL(_SO)
     vp = C.c_void_p
     lib.tpc_abi_version.restype = C.c_int
+    lib.tpc_checked_build.restype = C.c_int
     lib.tpc_create.argtypes = [C.POINTER(_Geometry), C.c_float, C.c_float, C.POINTER(vp)]
     lib.tpc_set_param.argtypes = [vp, C.c_char_p, C.c_double]
     lib.tpc_set_stream.argtypes = [vp, vp]

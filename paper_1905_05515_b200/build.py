@@ -14,6 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libtpc_b200.so")
+SO_CHECKED = os.path.join(HERE, "libtpc_b200_checked.so")   # same sources with -DTPC_CHECKED: bounds checks in the kernels (tests only)
 SOURCES = ["tpc_abi.cu", "scan.cu", "k1_grid.cu", "k2_neighbours.cu", "k3_clean_start.cu", "k5_tracklets.cu", "k6_selector.cu", "k7_refit.cu", "k8_tube.cu", "k9_merge.cu", "k10_loopers.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "shared"] + os.environ.get("TPC_NVCC_EXTRA", "").split()
@@ -26,23 +27,20 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def _stale() -> bool:
-    if not os.path.exists(SO):
+def _stale(so) -> bool:
+    if not os.path.exists(so):
         return True
-    t = os.path.getmtime(SO)
+    t = os.path.getmtime(so)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "tpc.h"), __file__]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
-        return SO
-    objdir = os.path.join(HERE, "build")
+def _build_one(so: str, extra: list, objdir: str, verbose: bool) -> None:
     os.makedirs(objdir, exist_ok=True)
     procs = []
     for s in SOURCES:
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o",
-                                                                                  os.path.join(objdir, s[:-3] + ".o")]
+        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, s), "-o",
+                                                                                          os.path.join(objdir, s[:-3] + ".o")]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for s, p in procs:
         out, _ = p.communicate()
@@ -50,9 +48,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(out)
         if p.returncode:
             raise RuntimeError(f"nvcc failed on {s}")
-    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "shared", "-o", SO] + [os.path.join(objdir, s[:-3] + ".o") for s in SOURCES] + \
-          ["-Xlinker", "-rpath=/usr/local/cuda/lib64"]
+    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "shared", "-o", so] + \
+          [os.path.join(objdir, s[:-3] + ".o") for s in SOURCES] + ["-Xlinker", "-rpath=/usr/local/cuda/lib64"]
     subprocess.check_call(cmd)
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """The product library, and beside it the checked build (same sources, -DTPC_CHECKED: bounds checks in the kernels) that
+    tests/test_gpu_checked.py runs; the product never loads the checked build."""
+    if force or _stale(SO):
+        _build_one(SO, [], os.path.join(HERE, "build"), verbose)
+    if force or _stale(SO_CHECKED):
+        _build_one(SO_CHECKED, ["-DTPC_CHECKED"], os.path.join(HERE, "build", "checked"), False)
     return SO
 
 

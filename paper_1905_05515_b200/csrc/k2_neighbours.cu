@@ -120,6 +120,7 @@ __device__ __forceinline__ void search_chunk(const float2* __restrict__ yzu, con
       const float ey = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.x, y)), __fmul_rn(rc.a, __fsub_rn(y, cd.x)));
       const float ez = __fsub_rn(__fmul_rn(rc.b, __fsub_rn(cu.y, z)), __fmul_rn(rc.a, __fsub_rn(z, cd.y)));
       const float D = __fadd_rn(__fmul_rn(ey, ey), __fmul_rn(ez, ez));
+      TPC_CHECK(P, p >= 0 && p < du.n && q >= 0 && q < dd.n, 21);
       bool better = !have || D < bestD;
       if (have && D == bestD) {   // tie: lower original index of the up cluster, then of the down cluster (rare: global reads)
         const int iu = permu[p], ib = permu[bu];

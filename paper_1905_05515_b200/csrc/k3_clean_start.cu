@@ -127,6 +127,7 @@ __global__ void __launch_bounds__(K3_THREADS) k3_clean_flag(const Item* __restri
       const long long g = d.off + h;
       const int up = link_up[g], dn = link_dn[g];
       int cu = -1, cd = -1;
+      TPC_CHECK(P, P.link_skip || ((up < 0 || (r + 1 < R && up < units[u + 1].n)) && (dn < 0 || (r > 0 && dn < units[u - 1].n))), 31);
       if (!P.link_skip) {
         if (up >= 0 && r + 1 < R && link_dn[units[u + 1].off + up] == h) cu = up;
         if (dn >= 0 && r > 0 && link_up[units[u - 1].off + dn] == h) cd = dn;

@@ -242,7 +242,10 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
     int nxt_up = -1;
     // link entry: the position in the next row; with S2' (link_skip) position << 1 | k - 1, k = row distance of the link
     const int kk = P.link_skip ? (nxt & 1) + 1 : 1, pos = P.link_skip ? nxt >> 1 : nxt;
-    if (run) { const long long o = su[r + kk].off + pos; c = yz[o]; nxt_up = link_up[o]; }   // linked cluster + its own up-link
+    if (run) {   // linked cluster + its own up-link
+      TPC_CHECK(P, r + kk < R && pos >= 0 && pos < su[r + kk < R ? r + kk : r].n, 51);
+      const long long o = su[r + kk].off + pos; c = yz[o]; nxt_up = link_up[o];
+    }
     bool prop_ok = true;
     __syncwarp();
     if (run) { work += 1u; prop_ok = propagate(st, s_rx[r + kk] - s_rx[r], P); }   // one transport over the whole link
@@ -335,7 +338,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5b_extend_out(const int*
     float2 c = make_float2(0.f, 0.f);
     int hit = -1;
     __syncwarp();
-    if (do_pick) { work += 1u << 22; hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c); }
+    if (do_pick) { TPC_CHECK(P, rn < R, 52); work += 1u << 22; hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c); TPC_CHECK(P, hit < su[rn].n, 53); }
     __syncwarp();
     const bool have = do_pick && hit >= 0;
     if (do_pick) {
@@ -435,6 +438,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5c_refit_in(const int* _
     const int rn = r - 1;
     const int a = a_next;                      // rowhit of row rn, read one step ahead
     float2 c = cl;
+    TPC_CHECK(P, !run || (rn >= 0 && rn >= r0 && a < su[rn].n), 54);
     if (run && a >= 0) c = yz[su[rn].off + a]; // assigned cluster: its load hides behind the transport
     if (run && a < 0 && snap_cur) { snap_store(s_snap, tx, st); snap_cur = false; }   // this step may leave the state without an update
     bool have = init, do_pick = false;
@@ -533,7 +537,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5d_extend_in(const int* 
     float2 c = make_float2(0.f, 0.f);
     int hit = -1;
     __syncwarp();
-    if (do_pick) { work += 1u << 22; hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c); }
+    if (do_pick) { TPC_CHECK(P, rn >= 0, 55); work += 1u << 22; hit = pickup(su[rn], yz, perm, bin_start, st, zref, P, &c); TPC_CHECK(P, hit < su[rn].n, 56); }
     __syncwarp();
     const bool have = do_pick && hit >= 0;
     if (do_pick) {

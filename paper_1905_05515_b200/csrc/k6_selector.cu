@@ -14,6 +14,8 @@
 namespace tpc {
 namespace {
 
+struct CheckOnly { int* check; };   // the K6 kernels take no Params: TPC_CHECK needs only the flag word
+
 constexpr int K6_THREADS = 128;
 constexpr int K6_PER_BLOCK = 32;   // consecutive tracklets per CTA: the CTAs are scheduled in launch order, so the tracklets in flight at any
                                    // time are neighbours in (sector, row) order and their owner keys share a small, L2-resident region
@@ -33,7 +35,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M_cap, const in
                                                        const rowhit_t* __restrict__ rowhit, const int* __restrict__ tl_n,
                                                        const int* __restrict__ tl_first, const int* __restrict__ tl_last,
                                                        const float* __restrict__ tl_chi2, unsigned long long* __restrict__ owner,
-                                                       unsigned long long* __restrict__ tl_key) {
+                                                       unsigned long long* __restrict__ tl_key, const CheckOnly C) {
   const int lane = threadIdx.x & 31, n_warps = K6_THREADS >> 5;
   const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
   const long long q1 = min((long long)M, ((long long)blockIdx.x + 1) * K6_PER_BLOCK);
@@ -51,6 +53,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_owner(const int M_cap, const in
   const rowhit_t* __restrict__ rh = rowhit + (long long)i * R;
   for (int r = r_lo + lane; r <= r1; r += 32) {
     const int p = rh[r];
+    TPC_CHECK(C, p < su[r].n && r < R, 61);
     if (p >= 0) atomicMax(&owner[su[r].off + p], key);
   }
   }
@@ -61,7 +64,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M_cap, const in
                                                        const rowhit_t* __restrict__ rowhit, const int* __restrict__ tl_first,
                                                        const int* __restrict__ tl_last, const unsigned long long* __restrict__ owner,
                                                        const unsigned long long* __restrict__ tl_key,
-                                                       unsigned long long* __restrict__ scan_in) {
+                                                       unsigned long long* __restrict__ scan_in, const CheckOnly C) {
   const int lane = threadIdx.x & 31, n_warps = K6_THREADS >> 5;
   const int M = M_dev ? min(*M_dev, M_cap) : M_cap;
   const long long i1 = min((long long)M_cap, ((long long)blockIdx.x + 1) * K6_PER_BLOCK);
@@ -76,6 +79,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_count(const int M_cap, const in
     const rowhit_t* __restrict__ rh = rowhit + (long long)i * R;
     for (int r = r_lo + lane; r <= r1; r += 32) {
       const int p = rh[r];
+      TPC_CHECK(C, p < su[r].n && r < R, 62);
       if (p >= 0 && owner[su[r].off + p] == key) owned++;
     }
   }
@@ -98,7 +102,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M_cap, const int
                                                       float* __restrict__ o_chi2, int* __restrict__ o_ndf, int* __restrict__ o_tracklet,
                                                       long long* __restrict__ o_cl_begin, int* __restrict__ o_cl_row,
                                                       int* __restrict__ o_cl_index, const unsigned long long* __restrict__ total,
-                                                      const long long cap_tracks, const long long cap_refs) {
+                                                      const long long cap_tracks, const long long cap_refs, const CheckOnly C) {
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int lane = threadIdx.x & 31, n_warps = K6_THREADS >> 5;
   const unsigned long long tot = *total;                       // (tracks << 40 | cluster references) of the scan
@@ -129,7 +133,7 @@ __global__ void __launch_bounds__(K6_THREADS) k6_emit(const int M_cap, const int
     bool own = false;
     if (r <= r1) { const int p = rh[r]; if (p >= 0) { g = su[r].off + p; own = owner[g] == key; } }
     const unsigned m = __ballot_sync(0xffffffffu, own);
-    if (own) { const long long o = k + __popc(m & ((1u << lane) - 1u)); o_cl_row[o] = r; o_cl_index[o] = perm[g]; }
+    if (own) { const long long o = k + __popc(m & ((1u << lane) - 1u)); TPC_CHECK(C, o >= 0 && o < n_refs && t < n_tracks, 63); o_cl_row[o] = r; o_cl_index[o] = perm[g]; }
     k += __popc(m);
   }
   }
@@ -160,10 +164,10 @@ int launch_k6_select(const Launch& L, int M_cap, const int* d_M, long long N, co
     e = cudaMemsetAsync(d_owner, 0, (size_t)N * sizeof(unsigned long long), L.stream);
     if (e != cudaSuccess) return -(int)e;
     k6_owner<<<blocks, K6_THREADS, 0, L.stream>>>(M_cap, d_M, nullptr, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n, d_tl_first,
-                                                   d_tl_last, d_tl_chi2, d_owner, d_tl_key);
+                                                   d_tl_last, d_tl_chi2, d_owner, d_tl_key, CheckOnly{P.check});
   }
   k6_count<<<blocks, K6_THREADS, 0, L.stream>>>(M_cap, d_M, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_first, d_tl_last, d_owner,
-                                                 d_tl_key, d_scan_in);
+                                                 d_tl_key, d_scan_in, CheckOnly{P.check});
   int rc = launch_scan_u64(L, d_scan_in, d_scan_out, M_cap, d_scan_tmp, d_total);
   if (rc < 0) return rc;
   e = cudaGetLastError();
@@ -176,7 +180,7 @@ int launch_k6_owner(const Launch& L, int n_run, const int* d_run_list, const int
                     unsigned long long* d_tl_key, const Params& P) {
   if (n_run <= 0) return 0;
   k6_owner<<<k6_blocks(L, n_run), K6_THREADS, 0, L.stream>>>(n_run, nullptr, d_run_list, P.R, P.min_hits, d_start_unit, d_units, d_rowhit, d_tl_n,
-                                                              d_tl_first, d_tl_last, d_tl_chi2, d_owner, d_tl_key);
+                                                              d_tl_first, d_tl_last, d_tl_chi2, d_owner, d_tl_key, CheckOnly{P.check});
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }
@@ -192,7 +196,7 @@ int launch_k6_emit(const Launch& L, int M_cap, const int* d_M, const int* d_star
   k6_emit<<<k6_blocks(L, M_cap), K6_THREADS, 0, L.stream>>>(M_cap, d_M, P.R, d_start_unit, d_units, d_rows, d_perm, d_rowhit, d_tl_n, d_tl_first,
                                                              d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov, d_owner, d_tl_key, d_scan_in, d_scan_out,
                                                              o_sector, o_x, o_par, o_cov, o_chi2, o_ndf, o_tracklet, o_cl_begin, o_cl_row,
-                                                             o_cl_index, d_total, cap_tracks, cap_refs);
+                                                             o_cl_index, d_total, cap_tracks, cap_refs, CheckOnly{P.check});
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 1 : -(int)e;
 }

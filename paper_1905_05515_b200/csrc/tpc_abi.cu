@@ -201,6 +201,15 @@ extern "C" {
 
 int tpc_abi_version(void) { return 1; }
 
+// 1 for the checked build (bounds checks in the kernels, -DTPC_CHECKED), 0 for the product build
+int tpc_checked_build(void) {
+#ifdef TPC_CHECKED
+  return 1;
+#else
+  return 0;
+#endif
+}
+
 const char* tpc_last_error(const tpc_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
 int tpc_create(const tpc_geometry* g, float bz, float vdrift, tpc_ctx** out) {
@@ -433,6 +442,7 @@ void make_params_and_rows(tpc_ctx* c, std::vector<RowConst>& rows) {
   P.max_gap = T.max_gap; P.min_hits = T.min_hits;
   P.bridge_rows = T.link_skip ? 0 : T.bridge_rows; P.bridge_min = T.bridge_min; P.bridge_wy = (float)T.bridge_wy; P.bridge_wz = (float)T.bridge_wz;
   P.link_skip = T.link_skip;
+  P.check = nullptr;
 }
 
 // S1 grid descriptor of every unit + CSR offsets + K2/K3 work items.  Returns a tpc_status.
@@ -543,6 +553,10 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
   CUDA_TRY(c, c->d_start_unit.ensure((size_t)start_cap * 4));
   CUDA_TRY(c, c->d_start_pos.ensure((size_t)start_cap * 4));
   CUDA_TRY(c, c->d_counters.ensure(256));
+#ifdef TPC_CHECKED
+  c->P.check = reinterpret_cast<int*>(c->d_counters.as<char>() + 200);
+  CUDA_TRY(c, cudaMemsetAsync(c->P.check, 0, sizeof(int), st));
+#endif
 
   // ---- K1: S0 + S1
   LAUNCH_TRY(c, launch_k1_grid(L, U, c->d_units.as<UnitDesc>(), c->d_in_y.as<float>(), c->d_in_t.as<float>(), c->d_yz.as<float2>(),
@@ -701,7 +715,13 @@ int find_tracks_impl(tpc_ctx* c, tpc_tracks* out, bool to_host) {
     if (!variant) CUDA_TRY(c, cudaMemcpyAsync(c->p_small.p, d_nstart, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 64, d_total64, 8, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 128, d_k5cnt, 24, cudaMemcpyDeviceToHost, st));
+#ifdef TPC_CHECKED
+    CUDA_TRY(c, cudaMemcpyAsync(c->p_small.as<char>() + 200, c->P.check, sizeof(int), cudaMemcpyDeviceToHost, st));
+#endif
     CUDA_TRY(c, cudaStreamSynchronize(st));
+#ifdef TPC_CHECKED
+    if (*(int*)(c->p_small.as<char>() + 200) != 0) return fail(c, TPC_E_CUDA, "bounds check %d failed in a kernel (checked build)", *(int*)(c->p_small.as<char>() + 200));
+#endif
     if (!variant) {
       M = *c->p_small.as<int>();
       if (M < 0 || M > start_cap) return fail(c, TPC_E_CUDA, "start-hit count %d out of range", M);

@@ -52,6 +52,7 @@ struct Params {
   int max_gap, min_hits;
   int bridge_rows, bridge_min;    // NEXT-2 seed bridging (reading A39); bridge_rows = 0: off
   float bridge_wy, bridge_wz;
+  int* check;                     // TPC_CHECKED builds: device word that receives the code of a failed bounds check (else unused)
   int link_skip;                  // NEXT-2 as SURVEY 8(f).2 wrote it (reading A45): 1 = links may skip one row; link tables then hold (position << 1 | k - 1)
 };
 
@@ -64,6 +65,15 @@ struct K10Params { float qmin, dy, ds, dt, dq, pmin, frac, twopi; int nmax; };
 
 // Work item of K2/K3: a chunk of consecutive sorted hits of one unit.
 struct Item { int unit; int start; };
+
+// Bounds checks of the checked build (libtpc_b200_checked.so, -DTPC_CHECKED; compute-sanitizer is closed on the GPU pool, so the
+// library carries its own): every gather / scatter index that is computed from data is tested against the size of its array; a
+// failed test leaves its code in *P.check, which tpc_find_tracks* turns into TPC_E_CUDA.  Compiled out of the product build.
+#ifdef TPC_CHECKED
+#define TPC_CHECK(P, cond, code) do { if (!(cond)) atomicMax((P).check, (code)); } while (0)
+#else
+#define TPC_CHECK(P, cond, code) ((void)0)
+#endif
 
 // ---- device helpers ------------------------------------------------------------------------------------------------
 // S1 bin of a coordinate: fp32 subtract, fp32 multiply (no FMA), negative / NaN -> 0, clamp to nb-1, truncate.
