@@ -32,6 +32,15 @@ constexpr int K5_MAX_ROWS = 256;   // rows held in the shared-memory copy of the
 #ifndef K5_CTAS
 #define K5_CTAS 6
 #endif
+#ifndef K5_CTAS_B
+#define K5_CTAS_B 7   // measured on C3: k5b 1.58 ms at 6 CTAs / SM (78 registers), 1.49 ms at 7 (72, no spill), 1.73 ms at 5
+#endif
+#ifndef K5_CTAS_C
+#define K5_CTAS_C K5_CTAS
+#endif
+#ifndef K5_CTAS_D
+#define K5_CTAS_D 7   // k5d 1.46 -> 1.41 ms; k5c spills at 72 registers and stays at 6
+#endif
 constexpr int K5_FLUSH = K5_FLUSH_N;        // finished lanes of a warp that trigger the write-out / refill code
 constexpr unsigned FULL = 0xffffffffu;
 
@@ -273,7 +282,7 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
 
 // ---------------------------------------------------------------------------------------------------------------------------
 // Phase B: outward extrapolation with pick-up.  Task = tracklet whose Phase A ended with a good state below the last row.
-__global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5b_extend_out(const int* __restrict__ list_b, const UnitDesc* __restrict__ units,
+__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const int* __restrict__ list_b, const UnitDesc* __restrict__ units,
                                                                 const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                                 const int* __restrict__ perm, const int* __restrict__ bin_start,
                                                                 rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec,
@@ -361,7 +370,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5b_extend_out(const int*
 // Phase C, part 1: inward refit from the outermost updated row r_out down to the start row r0 (rows that A / B visited).
 // Rows with an assigned cluster are updated without a search; rows B left empty are searched again (rare); no gap counting
 // here (first_assigned = r0).  A tracklet with r0 = 0, or whose transport fails, is final; the others continue in k5d.
-__global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5c_refit_in(const int* __restrict__ list_c, const UnitDesc* __restrict__ units,
+__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int* __restrict__ list_c, const UnitDesc* __restrict__ units,
                                                               const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                               const int* __restrict__ perm, const int* __restrict__ bin_start,
                                                               rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec,
@@ -471,7 +480,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5c_refit_in(const int* _
 
 // ---------------------------------------------------------------------------------------------------------------------------
 // Phase C, part 2: inward extrapolation below the start row with pick-up (every row is below first_assigned: gaps count).
-__global__ void __launch_bounds__(K5_THREADS, K5_CTAS) k5d_extend_in(const int* __restrict__ list_d, const UnitDesc* __restrict__ units,
+__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int* __restrict__ list_d, const UnitDesc* __restrict__ units,
                                                                const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                                const int* __restrict__ perm, const int* __restrict__ bin_start,
                                                                rowhit_t* __restrict__ rowhit, const TlRec* __restrict__ rec,
