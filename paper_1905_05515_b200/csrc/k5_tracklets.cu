@@ -51,13 +51,14 @@ constexpr unsigned FULL = 0xffffffffu;
 struct __align__(16) TlRec {
   float st[20];
   float yl, zl, zref, chi2;
-  int u0, r_out, n, pad0;
+  int u0, r_out, n, next;   // next: phase the tracklet is due for (NEXT_B / NEXT_C / NEXT_D / NEXT_NONE)
   int pad[4];
 };
 static_assert(sizeof(TlRec) == 128, "TlRec is one 128-byte line");
 
-// control block of the four kernels (ints, zeroed by the caller before k5a): queue heads and task-list lengths
-enum : int { CT_QA = 0, CT_QB, CT_QC, CT_QD, CT_NB, CT_NC, CT_ND, CT_WORDS = 8 };
+// control block of the four kernels (ints, zeroed by the caller before k5a): the queue heads
+enum : int { CT_QA = 0, CT_QB, CT_QC, CT_QD, CT_WORDS = 8 };
+enum : int { NEXT_NONE = 0, NEXT_B = 1, NEXT_C = 2, NEXT_D = 3 };
 
 enum : int { MD_FETCH = 0, MD_INIT, MD_RUN, MD_DONE, MD_EXIT };
 
@@ -193,8 +194,7 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
                                                               const int* __restrict__ start_unit, const int* __restrict__ start_pos,
                                                               const UnitDesc* __restrict__ units, const RowConst* __restrict__ rows,
                                                               const float2* __restrict__ yz, const int* __restrict__ link_up,
-                                                              rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec, int* __restrict__ list_b,
-                                                              int* __restrict__ list_c, int* __restrict__ ctl,
+                                                              rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec, int* __restrict__ ctl,
                                                               unsigned long long* __restrict__ counters, const Params P) {
   K5_PROLOGUE();
   const int M = M_dev ? min(*M_dev, M_host) : M_host;   // task count: in device memory (default path: no read-back after K3) or given
@@ -214,12 +214,9 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
         float4* __restrict__ p = reinterpret_cast<float4*>(rec + i);
         store_state(p, st);
         p[5] = make_float4(cl.x, cl.y, zref, 0.0f);
-        reinterpret_cast<int4*>(p)[6] = make_int4(u0, r, 0, 0);
+        reinterpret_cast<int4*>(p)[6] = make_int4(u0, r, 0, to_b ? NEXT_B : NEXT_C);
         work_flush(work, s_work);
       }
-      const unsigned mb = __ballot_sync(FULL, to_b), mc = __ballot_sync(FULL, fin && !to_b);
-      if (mb) { const int s = list_append(mb, ctl + CT_NB, lane); if (to_b) list_b[s] = i; }
-      if (mc) { const int s = list_append(mc, ctl + CT_NC, lane); if (fin && !to_b) list_c[s] = i; }
       if (fin) mode = drained ? MD_EXIT : MD_FETCH;
     }
     const unsigned need = __ballot_sync(FULL, mode == MD_FETCH);
@@ -282,15 +279,15 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
 
 // ---------------------------------------------------------------------------------------------------------------------------
 // Phase B: outward extrapolation with pick-up.  Task = tracklet whose Phase A ended with a good state below the last row.
-__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const int* __restrict__ list_b, const UnitDesc* __restrict__ units,
+__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const int M_host, const int* __restrict__ M_dev, const int* __restrict__ run_list,
+                                                                const UnitDesc* __restrict__ units,
                                                                 const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                                 const int* __restrict__ perm, const int* __restrict__ bin_start,
-                                                                rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec,
-                                                                int* __restrict__ list_c, int* __restrict__ ctl,
+                                                                rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec, int* __restrict__ ctl,
                                                                 unsigned long long* __restrict__ counters, const Params P) {
   K5_PROLOGUE();
   __shared__ float s_sv[7][K5_THREADS];   // state after the outermost update (5 parameters) + that cluster (y, z)
-  const int n_tasks = ctl[CT_NB];
+  const int n_tasks = M_dev ? min(*M_dev, M_host) : M_host;
   int i = -1, r = 0, r_out = 0, gap = 0;
   bool extended = false;
   float zref = 0.0f;
@@ -309,8 +306,6 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const in
         }
         work_flush(work, s_work);
       }
-      const unsigned mc = __ballot_sync(FULL, fin);
-      if (mc) { const int s = list_append(mc, ctl + CT_NC, lane); if (fin) list_c[s] = i; }
       if (fin) mode = drained ? MD_EXIT : MD_FETCH;
     }
     const unsigned need = __ballot_sync(FULL, mode == MD_FETCH);
@@ -318,16 +313,18 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const in
       const int q = queue_fetch(need, ctl + CT_QB, lane);
       if (mode == MD_FETCH) {
         if (q < n_tasks) {
-          i = list_b[q];
+          i = run_list ? run_list[q] : q;
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
+          const int4 k = reinterpret_cast<const int4*>(p)[6];
+          if (k.w == NEXT_B) {           // (else: Phase A ended on the last row or with a failed transport; the lane fetches again)
           load_state(st, p);
           zref = p[5].z;
-          const int4 k = reinterpret_cast<const int4*>(p)[6];
           const int sec = k.x / R;
           r = r_out = k.y; gap = 0; extended = false;
           su = units + (long long)sec * R;
           rh = rowhit + (long long)i * R;
           mode = MD_RUN;
+          }
         } else mode = MD_EXIT;
       }
       drained = __any_sync(FULL, mode == MD_EXIT);
@@ -370,18 +367,18 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const in
 // Phase C, part 1: inward refit from the outermost updated row r_out down to the start row r0 (rows that A / B visited).
 // Rows with an assigned cluster are updated without a search; rows B left empty are searched again (rare); no gap counting
 // here (first_assigned = r0).  A tracklet with r0 = 0, or whose transport fails, is final; the others continue in k5d.
-__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int* __restrict__ list_c, const UnitDesc* __restrict__ units,
+__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int M_host, const int* __restrict__ M_dev, const int* __restrict__ run_list,
+                                                              const UnitDesc* __restrict__ units,
                                                               const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                               const int* __restrict__ perm, const int* __restrict__ bin_start,
-                                                              rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec,
-                                                              int* __restrict__ list_d, int* __restrict__ ctl,
+                                                              rowhit_t* __restrict__ rowhit, TlRec* __restrict__ rec, int* __restrict__ ctl,
                                                               int* __restrict__ tl_n, int* __restrict__ tl_first,
                                                               int* __restrict__ tl_last, float* __restrict__ tl_chi2,
                                                               float* __restrict__ tl_par, float* __restrict__ tl_cov,
                                                               unsigned long long* __restrict__ counters, const Params P) {
   K5_PROLOGUE();
   __shared__ float s_snap[20][K5_THREADS];   // state after the last update, saved only before a step that may not update
-  const int n_tasks = ctl[CT_NC];
+  const int n_tasks = M_dev ? min(*M_dev, M_host) : M_host;
   int i = -1, u0 = 0, r0 = 0, r = 0, r_out = 0, r_snap = 0, n = 0, a_next = -1, a_next2 = -1;
   bool snap_cur = true, final_ = false;
   float zref = 0.0f, chi2 = 0.0f;
@@ -405,16 +402,15 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int*
             for (int k = 0; k < 20; k++) v[k] = s_snap[k][tx];
           }
           write_tracklet(i, n, r_snap, r_out, chi2, zref, v, tl_n, tl_first, tl_last, tl_chi2, tl_par, tl_cov);
+          rec[i].next = NEXT_NONE;
         } else {   // the last step was the update with the start hit on row r0: the state is the snapshot
           float4* __restrict__ p = reinterpret_cast<float4*>(rec + i);
           store_state(p, st);
           p[5] = make_float4(cl.x, cl.y, zref, chi2);
-          reinterpret_cast<int4*>(p)[6] = make_int4(u0, r_out, n, 0);
+          reinterpret_cast<int4*>(p)[6] = make_int4(u0, r_out, n, NEXT_D);
         }
         work_flush(work, s_work);
       }
-      const unsigned md = __ballot_sync(FULL, to_d);
-      if (md) { const int s = list_append(md, ctl + CT_ND, lane); if (to_d) list_d[s] = i; }
       if (fin) mode = drained ? MD_EXIT : MD_FETCH;
     }
     const unsigned need = __ballot_sync(FULL, mode == MD_FETCH);
@@ -422,7 +418,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int*
       const int q = queue_fetch(need, ctl + CT_QC, lane);
       if (mode == MD_FETCH) {
         if (q < n_tasks) {
-          i = list_c[q];
+          i = run_list ? run_list[q] : q;   // every tracklet passes through this phase
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
           const float4 a = p[0], f = p[5];
           const int4 k = reinterpret_cast<const int4*>(p)[6];
@@ -480,7 +476,8 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int*
 
 // ---------------------------------------------------------------------------------------------------------------------------
 // Phase C, part 2: inward extrapolation below the start row with pick-up (every row is below first_assigned: gaps count).
-__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int* __restrict__ list_d, const UnitDesc* __restrict__ units,
+__global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int M_host, const int* __restrict__ M_dev, const int* __restrict__ run_list,
+                                                               const UnitDesc* __restrict__ units,
                                                                const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                                const int* __restrict__ perm, const int* __restrict__ bin_start,
                                                                rowhit_t* __restrict__ rowhit, const TlRec* __restrict__ rec,
@@ -491,7 +488,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int
                                                                const Params P) {
   K5_PROLOGUE();
   __shared__ float s_snap[20][K5_THREADS];   // state after the last update
-  const int n_tasks = ctl[CT_ND];
+  const int n_tasks = M_dev ? min(*M_dev, M_host) : M_host;
   int* const qd = ctl + CT_QD;
   int i = -1, r = 0, r_out = 0, r_snap = 0, n = 0, gap = 0;
   float zref = 0.0f, chi2 = 0.0f;
@@ -515,11 +512,12 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int
       const int q = queue_fetch(need, qd, lane);
       if (mode == MD_FETCH) {
         if (q < n_tasks) {
-          i = list_d[q];
+          i = run_list ? run_list[q] : q;
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
+          const int4 k = reinterpret_cast<const int4*>(p)[6];
+          if (k.w == NEXT_D) {           // (else: the tracklet ended in k5c; the lane fetches again)
           load_state(st, p);
           const float4 f = p[5];
-          const int4 k = reinterpret_cast<const int4*>(p)[6];
           zref = f.z; chi2 = f.w;
           const int sec = k.x / R;
           r = r_snap = k.x - sec * R; r_out = k.y; n = k.z; gap = 0;
@@ -527,6 +525,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int
           rh = rowhit + (long long)i * R;
           snap_store(s_snap, tx, st);
           mode = MD_RUN;
+          }
         } else mode = MD_EXIT;
       }
       drained = __any_sync(FULL, mode == MD_EXIT);
@@ -571,9 +570,9 @@ template <class K> int persistent_blocks(K kernel, int sm_count) {
 
 }  // namespace
 
-size_t k5_scratch_bytes(long long M) {   // TlRec array + three task lists + control block
+size_t k5_scratch_bytes(long long M) {   // TlRec array + control block
   const size_t m = (size_t)(M > 0 ? M : 1);
-  return m * sizeof(TlRec) + 3 * ((m * sizeof(int) + 127) & ~(size_t)127) + 128;
+  return m * sizeof(TlRec) + 128;
 }
 
 // d_scratch: k5_scratch_bytes(M) bytes, 128-byte aligned.  d_counters: three 64-bit work counters (accumulated).
@@ -585,13 +584,9 @@ int launch_k5_tracklets(const Launch& L, int n_run, const int* d_n_run, int M, c
                         float* d_tl_par, float* d_tl_cov, unsigned long long* d_counters, void* d_scratch, const Params& P) {
   if (n_run <= 0) return 0;
   if (P.R > K5_MAX_ROWS) return -(int)cudaErrorInvalidValue;   // tpc_create limits n_rows to 255 (selector key)
-  const size_t m = (size_t)M, lb = (m * sizeof(int) + 127) & ~(size_t)127;
   char* base = (char*)d_scratch;
   TlRec* rec = (TlRec*)base;
-  int* list_b = (int*)(base + m * sizeof(TlRec));
-  int* list_c = (int*)((char*)list_b + lb);
-  int* list_d = (int*)((char*)list_c + lb);
-  int* ctl = (int*)((char*)list_d + lb);
+  int* ctl = (int*)(base + (size_t)M * sizeof(TlRec));
   cudaError_t e = cudaMemsetAsync(ctl, 0, CT_WORDS * sizeof(int), L.stream);
   if (e != cudaSuccess) return -(int)e;
   static int nb_a = 0, nb_b = 0, nb_c = 0, nb_d = 0;
@@ -601,15 +596,15 @@ int launch_k5_tracklets(const Launch& L, int n_run, const int* d_n_run, int M, c
   }
   const int need = (n_run + K5_THREADS - 1) / K5_THREADS;
   k5a_seed_fit<<<nb_a < need ? nb_a : need, K5_THREADS, 0, L.stream>>>(n_run, d_n_run, d_run_list, d_start_unit, d_start_pos, d_units, d_rows, d_yz,
-                                                                      d_link_up, d_rowhit, rec, list_b, list_c, ctl, d_counters, P);
-  k5b_extend_out<<<nb_b < need ? nb_b : need, K5_THREADS, 0, L.stream>>>(list_b, d_units, d_rows, d_yz, d_perm, d_bin_start, d_rowhit, rec,
-                                                                        list_c, ctl, d_counters, P);
-  k5c_refit_in<<<nb_c < need ? nb_c : need, K5_THREADS, 0, L.stream>>>(list_c, d_units, d_rows, d_yz, d_perm, d_bin_start, d_rowhit, rec,
-                                                                      list_d, ctl, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par,
+                                                                      d_link_up, d_rowhit, rec, ctl, d_counters, P);
+  k5b_extend_out<<<nb_b < need ? nb_b : need, K5_THREADS, 0, L.stream>>>(n_run, d_n_run, d_run_list, d_units, d_rows, d_yz, d_perm, d_bin_start,
+                                                                        d_rowhit, rec, ctl, d_counters, P);
+  k5c_refit_in<<<nb_c < need ? nb_c : need, K5_THREADS, 0, L.stream>>>(n_run, d_n_run, d_run_list, d_units, d_rows, d_yz, d_perm, d_bin_start,
+                                                                      d_rowhit, rec, ctl, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par,
                                                                       d_tl_cov, d_counters, P);
-  k5d_extend_in<<<nb_d < need ? nb_d : need, K5_THREADS, 0, L.stream>>>(list_d, d_units, d_rows, d_yz, d_perm, d_bin_start, d_rowhit, rec,
-                                                                       ctl, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par, d_tl_cov,
-                                                                       d_counters, P);
+  k5d_extend_in<<<nb_d < need ? nb_d : need, K5_THREADS, 0, L.stream>>>(n_run, d_n_run, d_run_list, d_units, d_rows, d_yz, d_perm, d_bin_start,
+                                                                       d_rowhit, rec, ctl, d_tl_n, d_tl_first, d_tl_last, d_tl_chi2, d_tl_par,
+                                                                       d_tl_cov, d_counters, P);
   e = cudaGetLastError();
   return e == cudaSuccess ? 4 : -(int)e;
 }
