@@ -10,10 +10,12 @@
 //   k5d_extend_in  Phase C, rows below r0: inward extrapolation with pick-up
 // A phase kernel runs ONE kind of row step, so the lanes of a warp execute the same instruction stream at (nearly) full width:
 // the single state-machine kernel of round 1 ran its pick-up code at 8 of 32 lanes because only the lanes in an extrapolating
-// phase needed it (profiles/r1_ncu_k5_final.md).  Between the phases a tracklet is a 128-byte record in HBM (TlRec) and an entry
-// of the next kernel's task list (appended by the finishing lanes, warp-aggregated atomics; the order of a list does not enter
-// any result).  A lane that finishes waits until at least K5_FLUSH lanes of its warp have finished: the write-out + queue fetch
-// + task load code then runs for several lanes at once instead of for one lane in almost every iteration.
+// phase needed it (profiles/r1_ncu_k5_final.md).  Between the phases a tracklet is a 128-byte record in HBM (TlRec) whose `next`
+// field names the phase it is due for.  Every kernel walks the tracklets in START-LIST order (queue position = index in the run
+// list; a tracklet not due for this phase is skipped after one 16-byte read), so that neighbouring lanes work on neighbouring
+// tracks and share rowhit / grid lines in L1 / L2; completion-order task lists doubled the DRAM traffic.
+// The order does not enter any result.  A lane that finishes waits until at least K5_FLUSH lanes of its warp have finished: the
+// write-out + queue fetch + record load code then runs for several lanes at once instead of for one lane in almost every iteration.
 // z is carried relative to the start hit (z_rel = z - z_ref, formed in fp32 before use) so that long continuous time frames
 // (|z| up to 2.6e4 cm) keep full fp32 resolution.  Arithmetic is written term by term in the documented order and compiled
 // without FMA contraction (the fused multiply-adds of the transport / update are explicit, reading A43), so pick-up decisions
@@ -95,7 +97,7 @@ __device__ __forceinline__ void write_tracklet(const int i, const int n, const i
   for (int k = 0; k < 15; k++) oc[k] = v[5 + k];
 }
 
-// warp-aggregated append of the lanes in `m` to a task list; returns this lane's slot (valid for lanes in m)
+// warp-aggregated atomicAdd on a counter for the lanes in `m`; returns this lane's slot (valid for lanes in m)
 __device__ __forceinline__ int list_append(const unsigned m, int* __restrict__ count, const int lane) {
   int base = 0;
   const int leader = __ffs(m) - 1;
