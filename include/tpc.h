@@ -202,6 +202,28 @@ int tpc_merge_tracks(tpc_ctx*, int device_result, tpc_merges* out);
  * Errors: TPC_E_ARG (null), TPC_E_STATE (no completed tpc_find_tracks* call), TPC_E_NOMEM, TPC_E_CUDA. */
 int tpc_find_loopers(tpc_ctx*, int device_result, tpc_loopers* out);
 
+/* S10 for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): the
+ * same three kernels and the same result as tpc_find_loopers (reading A46; "secondary legs of looping tracks
+ * below 200 MeV/c"), but the call allocates NOTHING -- no cudaMalloc / cudaFree, no growth of a library buffer -- and does not
+ * synchronise: the three launches are queued on the context's stream and the call returns.
+ * Inputs (DEVICE memory, caller-owned, read on the stream): sector [n_tracks] in ascending order (as tpc_find_tracks* returns them,
+ * each in 0 .. n_sectors-1), x [n_tracks], par [n_tracks][5] (y, z, sin phi, dz/ds, q/pT) -- e.g. the arrays of tpc_find_tracks_device.
+ * Outputs (DEVICE memory, caller-owned, n_tracks int32 each): prev = previous turn of the same particle (-1 none), root = first turn
+ * of the group, turn = turns after the root.  Valid once the stream has reached the end of the call's work.
+ * Scratch: one file-scope static __device__ array of the library (1 MiB + 4 KiB; every GPU that loads the library holds it until the
+ * process exits), which bounds the size: n_tracks <= TPC_NOALLOC_MAX_TRACKS and n_sectors <= 1022.  ALL calls on a device share that
+ * array, whichever context or stream they use: calls whose work overlaps on the GPU (two streams, or two contexts on different
+ * streams) race on it and give undefined results -- keep them on one stream or order them with events.  The array keeps the previous
+ * call's contents; no word of it is read before the same call has written it, so nothing has to be cleared between calls.
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress, no allocation); make one call before a
+ * graph capture begins.  The current CUDA device must be the one the context was created on.
+ * Needs no preceding tpc_find_tracks*: field, s_max and the loop_* tunables are taken from the context.
+ * Errors: TPC_E_ARG (null context / array, negative n_tracks, an array that is not device memory), TPC_E_CAPACITY (n_tracks or
+ * n_sectors beyond the limit: nothing is launched), TPC_E_STATE (another device is current), TPC_E_CUDA.  n_tracks = 0 is a no-op. */
+#define TPC_NOALLOC_MAX_TRACKS 262144
+int tpc_find_loopers_noalloc(tpc_ctx*, int64_t n_tracks, const int32_t* d_sector, const float* d_x, const float* d_par,
+                             int32_t* d_prev, int32_t* d_root, int32_t* d_turn);
+
 /* Forget the clusters and results, keep geometry, parameters and buffers (one call per event / time frame). */
 int tpc_clear(tpc_ctx*);
 void tpc_destroy(tpc_ctx*);

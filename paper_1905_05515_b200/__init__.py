@@ -6,5 +6,5 @@ without a CUDA device the calls raise.
 """
 from .binding import (TpcError, Tracker, Tracks, abi_symbols, lib_path, load_library,  # noqa: F401
                       tpc_create, tpc_load_clusters, tpc_load_clusters_batch, tpc_find_tracks, tpc_find_tracks_device,
-                      tpc_refit_tracks, tpc_mark_clusters, tpc_merge_tracks, tpc_find_loopers, tpc_clear, tpc_destroy, tpc_set_param, tpc_set_stream, tpc_get_timings)
+                      tpc_refit_tracks, tpc_mark_clusters, tpc_merge_tracks, tpc_find_loopers, tpc_find_loopers_noalloc, tpc_clear, tpc_destroy, tpc_set_param, tpc_set_stream, tpc_get_timings)
 from .sharding import shard_units  # noqa: F401

@@ -18,7 +18,7 @@ _SO = os.environ.get("TPC_B200_LIB") or os.path.join(_HERE, "libtpc_b200.so")
 
 ABI_SYMBOLS = [
     "tpc_abi_version", "tpc_checked_build", "tpc_create", "tpc_set_param", "tpc_set_stream", "tpc_load_clusters", "tpc_load_clusters_batch",
-    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_find_loopers", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings", "tpc_measure_fp32_peak",
+    "tpc_find_tracks", "tpc_find_tracks_device", "tpc_refit_tracks", "tpc_mark_clusters", "tpc_merge_tracks", "tpc_find_loopers", "tpc_find_loopers_noalloc", "tpc_clear", "tpc_destroy", "tpc_last_error", "tpc_get_timings", "tpc_measure_fp32_peak",
     "tpc_debug_get_grid", "tpc_debug_get_links", "tpc_debug_get_link_rows", "tpc_debug_get_start_hits", "tpc_debug_get_tracklets",
 ]
 
@@ -109,6 +109,7 @@ def load_library():
     lib.tpc_mark_clusters.argtypes = [vp, C.c_float, C.c_int, C.POINTER(_Marks)]
     lib.tpc_merge_tracks.argtypes = [vp, C.c_int, C.POINTER(_Merges)]
     lib.tpc_find_loopers.argtypes = [vp, C.c_int, C.POINTER(_Loopers)]
+    lib.tpc_find_loopers_noalloc.argtypes = [vp, C.c_int64] + [C.c_void_p] * 6
     lib.tpc_clear.argtypes = [vp]
     lib.tpc_destroy.argtypes = [vp]
     lib.tpc_destroy.restype = None
@@ -318,6 +319,16 @@ def tpc_find_loopers(h, device_result=False) -> dict:
             "turn": make(t.turn, n, np.int32)}
 
 
+NOALLOC_MAX_TRACKS = 262144   # TPC_NOALLOC_MAX_TRACKS of include/tpc.h
+
+
+def tpc_find_loopers_noalloc(h, n_tracks, sector, x, par, prev, root, turn) -> None:
+    """S10 without any allocation: raw pointers (ints) or objects with data_ptr() to caller-owned DEVICE arrays; the work is queued on
+    the context's stream and the call returns without synchronising (include/tpc.h)."""
+    ptr = lambda a: C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else (int(a) if a is not None else 0))
+    _check(h, load_library().tpc_find_loopers_noalloc(h, int(n_tracks), ptr(sector), ptr(x), ptr(par), ptr(prev), ptr(root), ptr(turn)))
+
+
 class Tracker:
     """Context manager around one tpc_ctx, for the tests and bench.py."""
 
@@ -384,6 +395,9 @@ class Tracker:
 
     def find_loopers(self, device_result=False) -> dict:
         return tpc_find_loopers(self.h, device_result)
+
+    def find_loopers_noalloc(self, n_tracks, sector, x, par, prev, root, turn) -> None:
+        tpc_find_loopers_noalloc(self.h, n_tracks, sector, x, par, prev, root, turn)
 
     def clear(self):
         self._keep = []

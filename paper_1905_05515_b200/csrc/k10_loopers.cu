@@ -13,6 +13,14 @@
 // fp32, every operation spelled in the order of the definition (oracle S10; library built with -fmad=false).
 #include "kalman.cuh"
 
+#include <mutex>
+
+// Scratch of the allocation-free entry point tpc_find_loopers_noalloc (end of this file): sec_begin[K10_STATIC_MAX_SECTORS + 2],
+// padded to 1024 words, then prev_n[K10_STATIC_MAX_TRACKS].  1 MiB + 4 KiB, held by every GPU that loads the library until exit.
+// In HOST code this name is only a stand-in for the symbol, never a device address: the address comes from cudaGetSymbolAddress
+// (static_scratch() below), once per device.
+static __device__ __align__(256) int k10_static_scratch[1024 + tpc::K10_STATIC_MAX_TRACKS];
+
 namespace tpc {
 namespace {
 
@@ -84,6 +92,55 @@ int launch_k10_loopers(const Launch& L, long long n_tracks, int NS, const int* o
   k10_match<<<blocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_x, o_par, d_sec_begin, d_prev, d_prev_n, K, P);
   k10_roots<<<(int)((n_tracks + 255) / 256), 256, 0, L.stream>>>(n_tracks, d_prev, d_prev_n, d_root, d_turn);
   cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? 3 : -(int)e;
+}
+
+// ---- Allocation-free variant (tpc_find_loopers_noalloc): the same three kernels, their scratch (sec_begin, prev_n) in the
+// file-scope array k10_static_scratch instead of the context's grow-only cudaMalloc buffers.
+namespace {
+
+constexpr int K10_MAX_DEVICES = 64;
+static_assert(K10_STATIC_MAX_SECTORS + 2 <= 1024, "sec_begin has NS + 1 entries and lives in the first 1024 words of the scratch");
+std::mutex g_static_mu;
+int* g_static_ptr[K10_MAX_DEVICES] = {};   // device address of k10_static_scratch on each device, resolved once per device
+
+// Device address of the scratch on the CURRENT device (the symbol has one instance per device that loaded the library).
+cudaError_t static_scratch(int** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= K10_MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, k10_static_scratch);
+    if (e != cudaSuccess) return e;
+    g_static_ptr[dev] = static_cast<int*>(p);
+  }
+  *out = g_static_ptr[dev];
+  return cudaSuccess;
+}
+
+}  // namespace
+
+// Same result as launch_k10_loopers.  No cudaMalloc / cudaFree, no synchronisation.  Nothing in the scratch has to start at zero:
+// k10_ranges writes sec_begin[0..NS] and k10_match writes prev_n[0..n_tracks) before the kernels that follow read exactly those words,
+// so what an earlier call left behind (the array is shared by every call on the device) is never read.  Two calls that overlap on
+// the GPU (different streams) race on the array.  Returns the launches made, or -(cudaError_t).
+int launch_k10_loopers_static(const Launch& L, long long n_tracks, int NS, const int* o_sector, const float* o_x, const float* o_par,
+                              int* d_prev, int* d_root, int* d_turn, const K10Params& K, const Params& P) {
+  if (n_tracks <= 0) return 0;
+  if (n_tracks > K10_STATIC_MAX_TRACKS || NS > K10_STATIC_MAX_SECTORS) return -(int)cudaErrorInvalidValue;   // the ABI checks first
+  int* scratch = nullptr;
+  cudaError_t e = static_scratch(&scratch);
+  if (e != cudaSuccess) return -(int)e;
+  int* d_sec_begin = scratch;
+  int* d_prev_n = scratch + 1024;
+  k10_ranges<<<(NS + 1 + 63) / 64, 64, 0, L.stream>>>(n_tracks, NS, o_sector, d_sec_begin);
+  const int blocks = (int)((n_tracks + K10_THREADS - 1) / K10_THREADS);
+  k10_match<<<blocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_x, o_par, d_sec_begin, d_prev, d_prev_n, K, P);
+  k10_roots<<<(int)((n_tracks + 255) / 256), 256, 0, L.stream>>>(n_tracks, d_prev, d_prev_n, d_root, d_turn);
+  e = cudaGetLastError();
   return e == cudaSuccess ? 3 : -(int)e;
 }
 

@@ -941,6 +941,40 @@ int tpc_find_loopers(tpc_ctx* c, int device_result, tpc_loopers* out) {
   CUDA_TRY(c, cudaEventElapsedTime(&out->ms_loopers, c->ev[8], c->ev[9]));
   return TPC_OK;
 }
+// S10 without any allocation (include/tpc.h): caller-owned device inputs / outputs, scratch in a static __device__ array of
+// k10_loopers.cu, work queued on the context's stream, no synchronisation.  Needs no tpc_find_tracks* call: the constants it uses
+// (cB, s_max, the loop_* tunables) are formed here from the context's field and tunables by the formulas of make_params_and_rows.
+static_assert(TPC_NOALLOC_MAX_TRACKS == K10_STATIC_MAX_TRACKS, "tpc.h and tpc_internal.cuh state the same limit");
+int tpc_find_loopers_noalloc(tpc_ctx* c, int64_t n_tracks, const int32_t* d_sector, const float* d_x, const float* d_par,
+                             int32_t* d_prev, int32_t* d_root, int32_t* d_turn) {
+  if (!c) return fail(c, TPC_E_ARG, "tpc_find_loopers_noalloc: null context");
+  if (n_tracks < 0) return fail(c, TPC_E_ARG, "tpc_find_loopers_noalloc: n_tracks = %lld is negative", (long long)n_tracks);
+  if (n_tracks > TPC_NOALLOC_MAX_TRACKS)
+    return fail(c, TPC_E_CAPACITY, "tpc_find_loopers_noalloc: n_tracks = %lld exceeds TPC_NOALLOC_MAX_TRACKS = %d (the static scratch "
+                "array holds one word per track); use tpc_find_loopers", (long long)n_tracks, (int)TPC_NOALLOC_MAX_TRACKS);
+  if (c->NS > K10_STATIC_MAX_SECTORS)
+    return fail(c, TPC_E_CAPACITY, "tpc_find_loopers_noalloc: %d sectors exceed the %d the static scratch array holds", c->NS, K10_STATIC_MAX_SECTORS);
+  if (n_tracks == 0) return TPC_OK;
+  if (!d_sector || !d_x || !d_par || !d_prev || !d_root || !d_turn) return fail(c, TPC_E_ARG, "tpc_find_loopers_noalloc: null array");
+  if (pointer_kind(d_sector) != 2 || pointer_kind(d_x) != 2 || pointer_kind(d_par) != 2 || pointer_kind(d_prev) != 2 ||
+      pointer_kind(d_root) != 2 || pointer_kind(d_turn) != 2)
+    return fail(c, TPC_E_ARG, "tpc_find_loopers_noalloc: all six arrays must be device memory");
+  int dev = -1;
+  CUDA_TRY(c, cudaGetDevice(&dev));
+  if (dev != c->device) return fail(c, TPC_E_STATE, "tpc_find_loopers_noalloc: current device %d is not the context's device %d", dev, c->device);
+  const Tunables& T = c->T;
+  const K10Params K{(float)T.loop_qmin, (float)T.loop_dy, (float)T.loop_ds, (float)T.loop_dt, (float)T.loop_dq, (float)T.loop_pmin,
+                    (float)T.loop_frac, (float)6.283185307179586, T.loop_nmax};
+  Params P = c->P;
+  P.NS = c->NS; P.R = c->R;
+  P.cB = (float)(-0.00299792458 * (double)c->bz);
+  P.smax = (float)T.s_max;
+  P.check = nullptr;
+  const Launch L{c->stream, c->sm_count, c->T.k2_threads};
+  const int rc = launch_k10_loopers_static(L, (long long)n_tracks, c->NS, d_sector, d_x, d_par, d_prev, d_root, d_turn, K, P);
+  if (rc < 0) return fail(c, TPC_E_CUDA, "tpc_find_loopers_noalloc: %s", cudaGetErrorString((cudaError_t)(-rc)));
+  return TPC_OK;
+}
 // Measurement utility: fp32 fused-multiply-add throughput of the device at the clocks of the moment (TFLOP/s, 2 flops per FMA).
 int tpc_measure_fp32_peak(tpc_ctx* c, float* tflops) {
   if (!c || !tflops) return fail(c, TPC_E_ARG, "tpc_measure_fp32_peak: null argument");

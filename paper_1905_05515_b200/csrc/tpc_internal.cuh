@@ -62,6 +62,8 @@ struct K9Params { float edge, dy, dz, ds, dt, cd, sd; int rows;
 
 // S10 (NEXT-3, second half) parameters (reading A46), rounded to float once on the host
 struct K10Params { float qmin, dy, ds, dt, dq, pmin, frac, twopi; int nmax; };
+constexpr int K10_STATIC_MAX_TRACKS = 262144;   // limits of the allocation-free S10 entry point (= TPC_NOALLOC_MAX_TRACKS of tpc.h)
+constexpr int K10_STATIC_MAX_SECTORS = 1022;
 
 // Work item of K2/K3: a chunk of consecutive sorted hits of one unit.
 struct Item { int unit; int start; };
@@ -184,6 +186,9 @@ int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_se
 
 int launch_k10_loopers(const Launch& L, long long n_tracks, int NS, const int* o_sector, const float* o_x, const float* o_par,
                        int* d_sec_begin, int* d_prev, int* d_prev_n, int* d_root, int* d_turn, const K10Params& K, const Params& P);
+// allocation-free variant: scratch in a file-scope __device__ array of k10_loopers.cu, limits below (tpc_find_loopers_noalloc)
+int launch_k10_loopers_static(const Launch& L, long long n_tracks, int NS, const int* o_sector, const float* o_x, const float* o_par,
+                              int* d_prev, int* d_root, int* d_turn, const K10Params& K, const Params& P);
 
 // device-wide exclusive scans (own kernels; three launches each)
 int launch_scan_i32(const Launch& L, const int* d_in, int* d_out, int n, int* d_tmp, int* d_total);
