@@ -43,6 +43,21 @@ constexpr int K5_MAX_ROWS = 256;   // rows held in the shared-memory copy of the
 #ifndef K5_CTAS_D
 #define K5_CTAS_D 7   // k5d 1.46 -> 1.41 ms; k5c spills at 72 registers and stays at 6
 #endif
+// Two passes over the start list per phase kernel: the first takes the tracklets with at least K5_LONG_x rows ahead of them in this
+// phase (B: rows above the end of the chain; C: rows between the outermost cluster and the start hit; D: rows below the start hit),
+// the second the rest (0 = one pass).  When the queue runs dry every lane finishes the tracklet it holds and the warps run on with
+// ever fewer lanes (measured in k5b: 34 % of the warp iterations at 11 of 32 lanes); with the long tracklets taken first that tail
+// is made of short ones (19 % of the iterations).  C3: K5 4.63 -> 4.50 ms; a third class gained nothing more.  Each pass walks the
+// list in start-list order; the class of a tracklet does not change while a kernel runs, so exactly one pass takes it.
+#ifndef K5_LONG_B
+#define K5_LONG_B 64
+#endif
+#ifndef K5_LONG_C
+#define K5_LONG_C 40
+#endif
+#ifndef K5_LONG_D
+#define K5_LONG_D 30
+#endif
 constexpr int K5_FLUSH = K5_FLUSH_N;        // finished lanes of a warp that trigger the write-out / refill code
 constexpr unsigned FULL = 0xffffffffu;
 
@@ -105,6 +120,10 @@ __device__ __forceinline__ int list_append(const unsigned m, int* __restrict__ c
   base = __shfl_sync(FULL, base, leader);
   return base + __popc(m & ((1u << lane) - 1u));
 }
+
+// length class of a tracklet with `len` rows ahead of it in a phase: 0 = long (first pass), 1 = short (second pass)
+template <int LONG> __device__ __forceinline__ int len_class(const int len) { return LONG > 0 && len < LONG ? 1 : 0; }
+template <int LONG> __device__ __forceinline__ constexpr int len_passes() { return LONG > 0 ? 2 : 1; }
 
 // warp-aggregated fetch of queue positions for the lanes in `m`
 __device__ __forceinline__ int queue_fetch(const unsigned m, int* __restrict__ head, const int lane) { return list_append(m, head, lane); }
@@ -216,7 +235,7 @@ __global__ void __launch_bounds__(K5_THREADS, 8) k5a_seed_fit(const int M_host, 
         float4* __restrict__ p = reinterpret_cast<float4*>(rec + i);
         store_state(p, st);
         p[5] = make_float4(cl.x, cl.y, zref, 0.0f);
-        reinterpret_cast<int4*>(p)[6] = make_int4(u0, r, 0, to_b ? NEXT_B : NEXT_C);
+        reinterpret_cast<int4*>(p)[6] = make_int4(u0, r, r, to_b ? NEXT_B : NEXT_C);   // .z: row Phase B starts from (B moves .y, never .z)
         work_flush(work, s_work);
       }
       if (fin) mode = drained ? MD_EXIT : MD_FETCH;
@@ -314,11 +333,15 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const in
     if (need) {
       const int q = queue_fetch(need, ctl + CT_QB, lane);
       if (mode == MD_FETCH) {
-        if (q < n_tasks) {
-          i = run_list ? run_list[q] : q;
+        if (q < len_passes<K5_LONG_B>() * n_tasks) {
+          const int pass = len_passes<K5_LONG_B>() == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
+          i = run_list ? run_list[qq] : qq;
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
           const int4 k = reinterpret_cast<const int4*>(p)[6];
-          if (k.w == NEXT_B) {           // (else: Phase A ended on the last row or with a failed transport; the lane fetches again)
+          // (not NEXT_B: Phase A ended on the last row or with a failed transport; not this pass's class: another pass takes it; the
+          // lane fetches again.)  k.z, not k.y: B moves r_out while it runs, the class must not change under a concurrent pass.
+          const bool mine = k.w == NEXT_B && len_class<K5_LONG_B>(R - 1 - k.z) == pass;
+          if (mine) {
           load_state(st, p);
           zref = p[5].z;
           const int sec = k.x / R;
@@ -419,11 +442,13 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int 
     if (need) {
       const int q = queue_fetch(need, ctl + CT_QC, lane);
       if (mode == MD_FETCH) {
-        if (q < n_tasks) {
-          i = run_list ? run_list[q] : q;   // every tracklet passes through this phase
+        if (q < len_passes<K5_LONG_C>() * n_tasks) {
+          const int pass = len_passes<K5_LONG_C>() == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
+          i = run_list ? run_list[qq] : qq;   // every tracklet passes through this phase
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
-          const float4 a = p[0], f = p[5];
           const int4 k = reinterpret_cast<const int4*>(p)[6];
+          if (len_class<K5_LONG_C>(k.y - k.x % R) == pass) {   // (else: another pass takes it; the lane fetches again)
+          const float4 a = p[0], f = p[5];
           st.y = a.x; st.z = a.y; st.s = a.z; st.t = a.w; st.q = rec[i].st[4];
           cl = make_float2(f.x, f.y); zref = f.z;
           u0 = k.x; r_out = k.y;
@@ -435,6 +460,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int 
           a_next = r_out - 1 >= r0 ? rh[r_out - 1] : -1;
           a_next2 = r_out - 2 >= r0 ? rh[r_out - 2] : -1;
           mode = MD_INIT;
+          }
         } else mode = MD_EXIT;
       }
       drained = __any_sync(FULL, mode == MD_EXIT);
@@ -513,11 +539,14 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int
     if (need) {
       const int q = queue_fetch(need, qd, lane);
       if (mode == MD_FETCH) {
-        if (q < n_tasks) {
-          i = run_list ? run_list[q] : q;
+        if (q < len_passes<K5_LONG_D>() * n_tasks) {
+          const int pass = len_passes<K5_LONG_D>() == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
+          i = run_list ? run_list[qq] : qq;
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
           const int4 k = reinterpret_cast<const int4*>(p)[6];
-          if (k.w == NEXT_D) {           // (else: the tracklet ended in k5c; the lane fetches again)
+          // (not NEXT_D: the tracklet ended in k5c; not this pass's class: another pass takes it; the lane fetches again)
+          const bool mine = k.w == NEXT_D && len_class<K5_LONG_D>(k.x % R) == pass;
+          if (mine) {
           load_state(st, p);
           const float4 f = p[5];
           zref = f.z; chi2 = f.w;
