@@ -122,8 +122,15 @@ __device__ __forceinline__ int list_append(const unsigned m, int* __restrict__ c
 }
 
 // length class of a tracklet with `len` rows ahead of it in a phase: 0 = long (first pass), 1 = short (second pass)
-template <int LONG> __device__ __forceinline__ int len_class(const int len) { return LONG > 0 && len < LONG ? 1 : 0; }
-template <int LONG> __device__ __forceinline__ constexpr int len_passes() { return LONG > 0 ? 2 : 1; }
+template <int LONG> __device__ __forceinline__ int len_class(const int len, const int passes) { return passes == 2 && len < LONG ? 1 : 0; }
+// two passes only while the tail matters: with many tracklets per lane (C5: 32) the tail is a small part of the kernel and the second
+// walk over the list costs more than it saves (C5: K5 27.2 ms with one pass, 28.2 ms with two; C3, 4.8 per lane: 4.63 / 4.50 ms)
+#ifndef K5_TWO_PASS_MAX_PER_LANE
+#define K5_TWO_PASS_MAX_PER_LANE 12
+#endif
+template <int LONG> __device__ __forceinline__ int len_passes(const int n_tasks) {
+  return LONG > 0 && (long long)n_tasks < (long long)K5_TWO_PASS_MAX_PER_LANE * gridDim.x * K5_THREADS ? 2 : 1;
+}
 
 // warp-aggregated fetch of queue positions for the lanes in `m`
 __device__ __forceinline__ int queue_fetch(const unsigned m, int* __restrict__ head, const int lane) { return list_append(m, head, lane); }
@@ -309,6 +316,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const in
   K5_PROLOGUE();
   __shared__ float s_sv[7][K5_THREADS];   // state after the outermost update (5 parameters) + that cluster (y, z)
   const int n_tasks = M_dev ? min(*M_dev, M_host) : M_host;
+  const int passes = len_passes<K5_LONG_B>(n_tasks);
   int i = -1, r = 0, r_out = 0, gap = 0;
   bool extended = false;
   float zref = 0.0f;
@@ -333,14 +341,14 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_B) k5b_extend_out(const in
     if (need) {
       const int q = queue_fetch(need, ctl + CT_QB, lane);
       if (mode == MD_FETCH) {
-        if (q < len_passes<K5_LONG_B>() * n_tasks) {
-          const int pass = len_passes<K5_LONG_B>() == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
+        if (q < passes * n_tasks) {
+          const int pass = passes == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
           i = run_list ? run_list[qq] : qq;
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
           const int4 k = reinterpret_cast<const int4*>(p)[6];
           // (not NEXT_B: Phase A ended on the last row or with a failed transport; not this pass's class: another pass takes it; the
           // lane fetches again.)  k.z, not k.y: B moves r_out while it runs, the class must not change under a concurrent pass.
-          const bool mine = k.w == NEXT_B && len_class<K5_LONG_B>(R - 1 - k.z) == pass;
+          const bool mine = k.w == NEXT_B && len_class<K5_LONG_B>(R - 1 - k.z, passes) == pass;
           if (mine) {
           load_state(st, p);
           zref = p[5].z;
@@ -404,6 +412,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int 
   K5_PROLOGUE();
   __shared__ float s_snap[20][K5_THREADS];   // state after the last update, saved only before a step that may not update
   const int n_tasks = M_dev ? min(*M_dev, M_host) : M_host;
+  const int passes = len_passes<K5_LONG_C>(n_tasks);
   int i = -1, u0 = 0, r0 = 0, r = 0, r_out = 0, r_snap = 0, n = 0, a_next = -1, a_next2 = -1;
   bool snap_cur = true, final_ = false;
   float zref = 0.0f, chi2 = 0.0f;
@@ -442,12 +451,12 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_C) k5c_refit_in(const int 
     if (need) {
       const int q = queue_fetch(need, ctl + CT_QC, lane);
       if (mode == MD_FETCH) {
-        if (q < len_passes<K5_LONG_C>() * n_tasks) {
-          const int pass = len_passes<K5_LONG_C>() == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
+        if (q < passes * n_tasks) {
+          const int pass = passes == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
           i = run_list ? run_list[qq] : qq;   // every tracklet passes through this phase
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
           const int4 k = reinterpret_cast<const int4*>(p)[6];
-          if (len_class<K5_LONG_C>(k.y - k.x % R) == pass) {   // (else: another pass takes it; the lane fetches again)
+          if (len_class<K5_LONG_C>(k.y - k.x % R, passes) == pass) {   // (else: another pass takes it; the lane fetches again)
           const float4 a = p[0], f = p[5];
           st.y = a.x; st.z = a.y; st.s = a.z; st.t = a.w; st.q = rec[i].st[4];
           cl = make_float2(f.x, f.y); zref = f.z;
@@ -517,6 +526,7 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int
   K5_PROLOGUE();
   __shared__ float s_snap[20][K5_THREADS];   // state after the last update
   const int n_tasks = M_dev ? min(*M_dev, M_host) : M_host;
+  const int passes = len_passes<K5_LONG_D>(n_tasks);
   int* const qd = ctl + CT_QD;
   int i = -1, r = 0, r_out = 0, r_snap = 0, n = 0, gap = 0;
   float zref = 0.0f, chi2 = 0.0f;
@@ -539,13 +549,13 @@ __global__ void __launch_bounds__(K5_THREADS, K5_CTAS_D) k5d_extend_in(const int
     if (need) {
       const int q = queue_fetch(need, qd, lane);
       if (mode == MD_FETCH) {
-        if (q < len_passes<K5_LONG_D>() * n_tasks) {
-          const int pass = len_passes<K5_LONG_D>() == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
+        if (q < passes * n_tasks) {
+          const int pass = passes == 1 ? 0 : q / n_tasks, qq = q - pass * n_tasks;
           i = run_list ? run_list[qq] : qq;
           const float4* __restrict__ p = reinterpret_cast<const float4*>(rec + i);
           const int4 k = reinterpret_cast<const int4*>(p)[6];
           // (not NEXT_D: the tracklet ended in k5c; not this pass's class: another pass takes it; the lane fetches again)
-          const bool mine = k.w == NEXT_D && len_class<K5_LONG_D>(k.x % R) == pass;
+          const bool mine = k.w == NEXT_D && len_class<K5_LONG_D>(k.x % R, passes) == pass;
           if (mine) {
           load_state(st, p);
           const float4 f = p[5];
