@@ -203,18 +203,19 @@ int tpc_merge_tracks(tpc_ctx*, int device_result, tpc_merges* out);
 int tpc_find_loopers(tpc_ctx*, int device_result, tpc_loopers* out);
 
 /* S10 for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): the
- * same three kernels and the same result as tpc_find_loopers (reading A46; "secondary legs of looping tracks
+ * same kernels and the same result as tpc_find_loopers (reading A46; "secondary legs of looping tracks
  * below 200 MeV/c"), but the call allocates NOTHING -- no cudaMalloc / cudaFree, no growth of a library buffer -- and does not
- * synchronise: the three launches are queued on the context's stream and the call returns.
+ * synchronise: the four launches are queued on the context's stream and the call returns.
  * Inputs (DEVICE memory, caller-owned, read on the stream): sector [n_tracks] in ascending order (as tpc_find_tracks* returns them,
  * each in 0 .. n_sectors-1), x [n_tracks], par [n_tracks][5] (y, z, sin phi, dz/ds, q/pT) -- e.g. the arrays of tpc_find_tracks_device.
  * Outputs (DEVICE memory, caller-owned, n_tracks int32 each): prev = previous turn of the same particle (-1 none), root = first turn
  * of the group, turn = turns after the root.  Valid once the stream has reached the end of the call's work.
- * Scratch: one file-scope static __device__ array of the library (1 MiB + 4 KiB; every GPU that loads the library holds it until the
+ * Scratch: one file-scope static __device__ array of the library (2 MiB + 8 KiB; every GPU that loads the library holds it until the
  * process exits), which bounds the size: n_tracks <= TPC_NOALLOC_MAX_TRACKS and n_sectors <= 1022.  ALL calls on a device share that
  * array, whichever context or stream they use: calls whose work overlaps on the GPU (two streams, or two contexts on different
  * streams) race on it and give undefined results -- keep them on one stream or order them with events.  The array keeps the previous
- * call's contents; no word of it is read before the same call has written it, so nothing has to be cleared between calls.
+ * call's contents; the per-sector counters in it, the only words that must start at zero, are zeroed by the first kernel of every call,
+ * and no other word is read before the same call has written it.
  * The first call on a device resolves the array's device address (cudaGetSymbolAddress, no allocation); make one call before a
  * graph capture begins.  The current CUDA device must be the one the context was created on.
  * Needs no preceding tpc_find_tracks*: field, s_max and the loop_* tunables are taken from the context.

@@ -146,8 +146,8 @@ struct tpc_ctx {
   PinVec<int32_t> ho_sector, ho_ndf, ho_tracklet, ho_cl_row, ho_cl_index; PinVec<float> ho_x, ho_par, ho_cov, ho_chi2;
   PinVec<int64_t> ho_cl_begin;
   // S9 merges (device + host)
-  DevBuf l_prev, l_prev_n, l_root, l_turn; PinVec<int32_t> hl_prev, hl_root, hl_turn;   // S10 looper turns (device + host)
-  DevBuf g_outer, g_row_in, g_row_out, g_leaver, g_sec_begin, g_cand, g_next, g_prev; PinVec<int32_t> hg_next, hg_prev;
+  DevBuf l_prev, l_prev_n, l_root, l_turn, l_list, l_sec; PinVec<int32_t> hl_prev, hl_root, hl_turn;   // S10 looper turns (device + host)
+  DevBuf g_outer, g_row_in, g_row_out, g_leaver, g_sec_begin, g_list, g_blist, g_bucket, g_cand, g_next, g_prev; PinVec<int32_t> hg_next, hg_prev;
   // S8 cluster marks (device + host)
   DevBuf m_att, m_adj, m_status, m_track; PinVec<int32_t> hm_status, hm_track;
   // S7 refit (device + host)
@@ -265,8 +265,8 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
                     &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
                     &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->d_flag2, &c->d_used, &c->m_att, &c->m_adj, &c->m_status, &c->m_track,
-                    &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_cand, &c->g_next, &c->g_prev,
-                    &c->l_prev, &c->l_prev_n, &c->l_root, &c->l_turn};
+                    &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_list, &c->g_blist, &c->g_bucket, &c->g_cand, &c->g_next, &c->g_prev,
+                    &c->l_prev, &c->l_prev_n, &c->l_root, &c->l_turn, &c->l_list, &c->l_sec};
   for (DevBuf* b : bufs) b->release();
   c->h_y.release(); c->h_t.release(); c->p_units.release(); c->p_items.release(); c->p_small.release();
   c->ho_sector.release(); c->ho_ndf.release(); c->ho_tracklet.release(); c->ho_cl_row.release(); c->ho_cl_index.release();
@@ -875,7 +875,9 @@ int tpc_merge_tracks(tpc_ctx* c, int device_result, tpc_merges* out) {
   Launch L{st, c->sm_count, c->T.k2_threads};
   const long long nt = c->n_tracks; const size_t ntz = (size_t)std::max(nt, 1LL);
   CUDA_TRY(c, c->g_outer.ensure(ntz * 16)); CUDA_TRY(c, c->g_row_in.ensure(ntz * 4)); CUDA_TRY(c, c->g_row_out.ensure(ntz * 4));
-  CUDA_TRY(c, c->g_leaver.ensure(ntz * 4)); CUDA_TRY(c, c->g_sec_begin.ensure((size_t)(c->NS + 2) * 4)); CUDA_TRY(c, c->g_cand.ensure(ntz * 8));
+  CUDA_TRY(c, c->g_leaver.ensure(ntz * 4)); CUDA_TRY(c, c->g_list.ensure(ntz * 4)); CUDA_TRY(c, c->g_blist.ensure(ntz * 4));
+  { const size_t NB = (size_t)c->NS * c->R + 1; CUDA_TRY(c, c->g_bucket.ensure((3 * NB + NB / SCAN_TILE + 4) * 4)); }
+  CUDA_TRY(c, c->g_sec_begin.ensure((size_t)(c->NS + 2) * 4)); CUDA_TRY(c, c->g_cand.ensure(ntz * 8));
   CUDA_TRY(c, c->g_next.ensure(ntz * 4)); CUDA_TRY(c, c->g_prev.ensure(ntz * 4));
   const Tunables& T = c->T;
   // sectors per ring: 2 pi / dphi when that is an integer (to 1e-3 rad over the ring) and n_sectors is a whole number of rings
@@ -889,7 +891,7 @@ int tpc_merge_tracks(tpc_ctx* c, int device_result, tpc_merges* out) {
   CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
   LAUNCH_TRY(c, launch_k9_merge(L, nt, c->NS, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_par.as<float>(), c->o_cl_begin.as<long long>(),
                                 c->o_cl_row.as<int>(), c->d_tl_first.as<int>(), c->d_rows.as<RowConst>(), c->g_outer.as<float>(),
-                                c->g_row_in.as<int>(), c->g_row_out.as<int>(), c->g_leaver.as<int>(), c->g_sec_begin.as<int>(),
+                                c->g_row_in.as<int>(), c->g_row_out.as<int>(), c->g_leaver.as<int>(), c->g_sec_begin.as<int>(), c->g_list.as<int>(), c->g_blist.as<int>(), c->g_bucket.as<int>(),
                                 (unsigned long long*)c->g_cand.p, c->g_next.as<int>(), c->g_prev.as<int>(), M, c->P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
   out->n_tracks = nt;
@@ -916,13 +918,13 @@ int tpc_find_loopers(tpc_ctx* c, int device_result, tpc_loopers* out) {
   Launch L{st, c->sm_count, c->T.k2_threads};
   const long long nt = c->n_tracks; const size_t ntz = (size_t)std::max(nt, 1LL);
   CUDA_TRY(c, c->l_prev.ensure(ntz * 4)); CUDA_TRY(c, c->l_prev_n.ensure(ntz * 4)); CUDA_TRY(c, c->l_root.ensure(ntz * 4));
-  CUDA_TRY(c, c->l_turn.ensure(ntz * 4)); CUDA_TRY(c, c->g_sec_begin.ensure((size_t)(c->NS + 2) * 4));
+  CUDA_TRY(c, c->l_turn.ensure(ntz * 4)); CUDA_TRY(c, c->l_list.ensure(ntz * 4)); CUDA_TRY(c, c->l_sec.ensure((size_t)(c->NS + 1) * 2 * 4));
   const Tunables& T = c->T;
   K10Params K{(float)T.loop_qmin, (float)T.loop_dy, (float)T.loop_ds, (float)T.loop_dt, (float)T.loop_dq, (float)T.loop_pmin,
               (float)T.loop_frac, (float)6.283185307179586, T.loop_nmax};
   long long launches = 0;
   CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
-  LAUNCH_TRY(c, launch_k10_loopers(L, nt, c->NS, c->o_sector.as<int>(), c->o_x.as<float>(), c->o_par.as<float>(), c->g_sec_begin.as<int>(),
+  LAUNCH_TRY(c, launch_k10_loopers(L, nt, c->NS, c->o_sector.as<int>(), c->o_x.as<float>(), c->o_par.as<float>(), c->l_sec.as<int>(), c->l_list.as<int>(),
                                    c->l_prev.as<int>(), c->l_prev_n.as<int>(), c->l_root.as<int>(), c->l_turn.as<int>(), K, c->P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
   out->n_tracks = nt;

@@ -181,11 +181,11 @@ int launch_k8_status(const Launch& L, long long n_tracks, long long N, int U, co
 
 int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_sector, const int* o_tracklet, const float* o_par,
                     const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first, const RowConst* d_rows, float* d_outer,
-                    int* d_row_in, int* d_row_out, int* d_leaver, int* d_sec_begin, unsigned long long* d_cand, int* d_next,
-                    int* d_prev, const K9Params& M, const Params& P);
+                    int* d_row_in, int* d_row_out, int* d_leaver, int* d_sec_begin, int* d_list, int* d_blist, int* d_bucket,
+                    unsigned long long* d_cand, int* d_next, int* d_prev, const K9Params& M, const Params& P);
 
 int launch_k10_loopers(const Launch& L, long long n_tracks, int NS, const int* o_sector, const float* o_x, const float* o_par,
-                       int* d_sec_begin, int* d_prev, int* d_prev_n, int* d_root, int* d_turn, const K10Params& K, const Params& P);
+                       int* d_sec, int* d_list, int* d_prev, int* d_prev_n, int* d_root, int* d_turn, const K10Params& K, const Params& P);
 // allocation-free variant: scratch in a file-scope __device__ array of k10_loopers.cu, limits below (tpc_find_loopers_noalloc)
 int launch_k10_loopers_static(const Launch& L, long long n_tracks, int NS, const int* o_sector, const float* o_x, const float* o_par,
                               int* d_prev, int* d_root, int* d_turn, const K10Params& K, const Params& P);
