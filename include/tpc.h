@@ -198,7 +198,7 @@ int tpc_mark_clusters(tpc_ctx*, float tube_cm, int device_result, tpc_cluster_ma
 int tpc_merge_tracks(tpc_ctx*, int device_result, tpc_merges* out);
 
 /* S10: group the tracks of the last tpc_find_tracks* call that are turns of one looping particle (tunables loop_qmin [c/GeV, 5 = 200
- * MeV/c], loop_dy, loop_ds, loop_dt, loop_dq, loop_pmin, loop_frac, loop_nmax).
+ * MeV/c], loop_dy, loop_ds, loop_dt, loop_dq, loop_pmin, loop_frac, loop_nmax [1..255]).
  * Errors: TPC_E_ARG (null), TPC_E_STATE (no completed tpc_find_tracks* call), TPC_E_NOMEM, TPC_E_CUDA. */
 int tpc_find_loopers(tpc_ctx*, int device_result, tpc_loopers* out);
 

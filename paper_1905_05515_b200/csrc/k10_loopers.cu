@@ -9,7 +9,7 @@
 //   k10_compact : the tracks with |q/pT| >= loop_qmin (pT <= 200 MeV/c: about one track in ten) are gathered at the front of their
 //                 sector's index range (slot = sec_begin + atomic counter; the order inside a sector is arbitrary and enters no
 //                 result); the others get prev = -1 here
-//   k10_match   : one lane per gathered track B: its state is transported (parameters only) to the x of every gathered track A of
+//   k10_match   : one warp per gathered track B, one lane per candidate: B's state is transported (parameters only) to the x of every gathered track A of
 //                 its sector and compared inside the four windows; the number of turns tau = dz / pitch must be within loop_frac of
 //                 an integer n in 1..loop_nmax; predecessor = smallest n, then smallest score, then lowest index (the tie on the
 //                 index is explicit, so the arbitrary gathering order does not matter)
@@ -53,30 +53,34 @@ __global__ void __launch_bounds__(K10_THREADS) k10_compact(const long long n_tra
   } else { prev[i] = -1; prev_n[i] = 0; }
 }
 
+// One WARP per gathered track B; the lanes take the gathered tracks A of its sector in turn (32 pairs in flight per warp instead of a
+// serial loop of several hundred dependent reads per lane) and the warp reduces the minimum of the key
+// (n : 8 bits | score bits : 32 | index : 24; loop_nmax <= 255, at most 2^24 tracks as in K6), which is the order "smallest n, then smallest score, then lowest index".
 __global__ void __launch_bounds__(K10_THREADS) k10_match(const long long n_tracks, const int* __restrict__ o_sector,
                                                          const float* __restrict__ o_x, const float* __restrict__ o_par,
                                                          const int* __restrict__ sec_begin, const int* __restrict__ sec_count,
                                                          const int* __restrict__ list, int* __restrict__ prev,
                                                          int* __restrict__ prev_n, const K10Params L, const Params P) {
-  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // slot of the gathered list (same sector ranges as the tracks)
+  const long long j = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // slot of the gathered list (same sector ranges as the tracks)
+  const int lane = threadIdx.x & 31;
   if (j >= n_tracks) return;
   const int sec = o_sector[j], a0 = sec_begin[sec], a1 = a0 + sec_count[sec];
-  if (j >= a1) return;                                                     // beyond the gathered tracks of this sector
+  if (j >= a1) return;                                                           // beyond the gathered tracks of this sector (whole warp)
   const int b = list[j];
-  int best = -1, bestn = 0; float bests = 0.0f;
   const float* __restrict__ pb = o_par + (long long)b * 5;
-  const float qb = pb[4], xb = o_x[b];
-  for (int ja = a0; ja < a1; ja++) {
+  const float yb = pb[0], zb = pb[1], sb = pb[2], tb = pb[3], qb = pb[4], xb = o_x[b];
+  unsigned long long best = ~0ull;
+  for (int ja = a0 + lane; ja < a1; ja += 32) {
     const int a = list[ja];
     if (a == b) continue;
     const float* __restrict__ pa = o_par + (long long)a * 5;
     const float qa = pa[4];
     // dz/ds and q/pT are not changed by the transport: their two windows are tested first (same values, same outcome as testing
     // all four after it) and spare most pairs the transport
-    const float dt = pb[3] - pa[3], dq = qb - qa;
+    const float dt = tb - pa[3], dq = qb - qa;
     if (!(fabsf(dt) <= L.dt && fabsf(dq) <= L.dq * fabsf(qa))) continue;
     State st = {};
-    st.y = pb[0]; st.z = pb[1]; st.s = pb[2]; st.t = pb[3]; st.q = qb;
+    st.y = yb; st.z = zb; st.s = sb; st.t = tb; st.q = qb;
     const float dx = o_x[a] - xb;
     if (dx != 0.0f && !propagate(st, dx, P)) continue;
     const float dy = st.y - pa[0], ds = st.s - pa[2];
@@ -88,12 +92,18 @@ __global__ void __launch_bounds__(K10_THREADS) k10_match(const long long n_track
     const float tau = (st.z - pa[1]) / pitch;
     const float nr = rintf(tau);
     if (!(nr >= 1.0f && fabsf(tau - nr) <= L.frac && nr <= (float)L.nmax)) continue;
-    const int n = (int)nr;
     const float ey = dy / L.dy, es = ds / L.ds, et = dt / L.dt;
-    const float score = (ey * ey + es * es) + et * et;
-    if (best < 0 || n < bestn || (n == bestn && (score < bests || (score == bests && a < best)))) { best = a; bestn = n; bests = score; }
+    const float score = (ey * ey + es * es) + et * et;          // >= 0: its bit pattern orders like its value
+    const unsigned long long key = ((unsigned long long)(unsigned)(int)nr << 56) | ((unsigned long long)__float_as_uint(score) << 24) |
+                                   (unsigned long long)(unsigned)a;
+    if (key < best) best = key;
   }
-  prev[b] = best; prev_n[b] = bestn;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { const unsigned long long v = __shfl_xor_sync(0xffffffffu, best, o); if (v < best) best = v; }
+  if (lane == 0) {
+    prev[b] = best == ~0ull ? -1 : (int)(best & 0xFFFFFFull);
+    prev_n[b] = best == ~0ull ? 0 : (int)(best >> 56);
+  }
 }
 
 __global__ void __launch_bounds__(256) k10_roots(const long long n_tracks, const int* __restrict__ prev, const int* __restrict__ prev_n,
@@ -114,7 +124,8 @@ int k10_launch_all(const Launch& L, long long n_tracks, int NS, const int* o_sec
   k10_ranges<<<(NS + 1 + 63) / 64, 64, 0, L.stream>>>(n_tracks, NS, o_sector, d_sec_begin, d_sec_count);
   const int blocks = (int)((n_tracks + K10_THREADS - 1) / K10_THREADS);
   k10_compact<<<blocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_par, d_sec_begin, d_sec_count, d_list, d_prev, d_prev_n, K);
-  k10_match<<<blocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_x, o_par, d_sec_begin, d_sec_count, d_list, d_prev, d_prev_n, K, P);
+  const int wblocks = (int)((n_tracks * 32 + K10_THREADS - 1) / K10_THREADS);   // one warp per slot of the gathered list
+  k10_match<<<wblocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_x, o_par, d_sec_begin, d_sec_count, d_list, d_prev, d_prev_n, K, P);
   k10_roots<<<(int)((n_tracks + 255) / 256), 256, 0, L.stream>>>(n_tracks, d_prev, d_prev_n, d_root, d_turn);
   const cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? 4 : -(int)e;

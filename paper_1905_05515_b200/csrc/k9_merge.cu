@@ -8,7 +8,7 @@
 //                sector in phi
 //   scan, k9_fill : index of the tracks by (sector, first row): k9_outer counts, an exclusive scan gives the bucket starts, k9_fill
 //                writes the track indices (arbitrary order inside a bucket; the tie on the index in k9_propose is explicit)
-//   k9_propose : one lane per leaver A (the leavers are gathered into a list by k9_outer): outer state rotated into the neighbour's frame, transported to the first row of every
+//   k9_propose : one warp per leaver A (the leavers are gathered into a list by k9_outer), one lane per candidate: outer state rotated into the neighbour's frame, transported to the first row of every
 //                track B of that sector that starts within merge_rows rows of A's end (one contiguous range of the index),
 //                compared inside the four windows; the
 //                best B (score, then index) receives atomicMin of (score bits, A)
@@ -68,6 +68,8 @@ __global__ void __launch_bounds__(256) k9_fill(const long long n_tracks, const i
   blist[bucket_start[u] + atomicAdd(&bucket_fill[u], 1)] = (int)i;
 }
 
+// One WARP per leaver; the lanes take the candidates of the bucket range in turn and the warp reduces the minimum of
+// (score bits : 32 | index : 32) = "smallest score, then lowest index" (score >= 0: its bit pattern orders like its value).
 __global__ void __launch_bounds__(K9_THREADS) k9_propose(const long long n_tracks, const int* __restrict__ o_sector,
                                                          const float* __restrict__ o_par, const RowConst* __restrict__ rows,
                                                          const float* __restrict__ outer, const int* __restrict__ row_in,
@@ -76,7 +78,8 @@ __global__ void __launch_bounds__(K9_THREADS) k9_propose(const long long n_track
                                                          const int* __restrict__ list, const int* __restrict__ bucket_start,
                                                          const int* __restrict__ blist, unsigned long long* __restrict__ cand,
                                                          const K9Params M, const Params P) {
-  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long j = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
   if (j >= n_tracks || j >= *n_leavers) return;
   const long long a = list[j];
   const int lv = leaver[a];
@@ -91,11 +94,11 @@ __global__ void __launch_bounds__(K9_THREADS) k9_propose(const long long n_track
   const float xr = x * M.cd + y * ss;
   rot.y = y * M.cd - x * ss; rot.z = o[2]; rot.s = s * M.cd - c * ss; rot.t = o_par[a * 5 + 3]; rot.q = o_par[a * 5 + 4];
   const int ra = row_out[a];
-  int best = -1; float bests = 0.0f;
+  unsigned long long best = K9_NONE;
   // the tracks of sector nb that start within merge_rows rows of ra: buckets (nb, ra - rows) .. (nb, ra + rows), one contiguous range
   const int r_lo = max(0, ra - M.rows), r_hi = min(P.R - 1, ra + M.rows);
   const int j1 = bucket_start[nb * P.R + r_hi + 1];
-  for (int jb = bucket_start[nb * P.R + r_lo]; jb < j1; jb++) {
+  for (int jb = bucket_start[nb * P.R + r_lo] + lane; jb < j1; jb += 32) {
     const int b = blist[jb];
     const int rb = row_in[b];
     const float* __restrict__ pb = o_par + (long long)b * 5;
@@ -107,9 +110,13 @@ __global__ void __launch_bounds__(K9_THREADS) k9_propose(const long long n_track
     if (!(fabsf(dy) <= M.dy && fabsf(dz) <= M.dz && fabsf(ds) <= M.ds)) continue;
     const float ey = dy / M.dy, ez = dz / M.dz, es = ds / M.ds, et = dt / M.dt;
     const float score = ((ey * ey + ez * ez) + es * es) + et * et;
-    if (best < 0 || score < bests || (score == bests && b < best)) { best = b; bests = score; }
+    const unsigned long long key = ((unsigned long long)__float_as_uint(score) << 32) | (unsigned long long)(unsigned)b;
+    if (key < best) best = key;
   }
-  if (best >= 0) atomicMin(&cand[best], ((unsigned long long)__float_as_uint(bests) << 32) | (unsigned long long)(unsigned)a);
+#pragma unroll
+  for (int o2 = 16; o2 > 0; o2 >>= 1) { const unsigned long long v = __shfl_xor_sync(0xffffffffu, best, o2); if (v < best) best = v; }
+  if (lane == 0 && best != K9_NONE)
+    atomicMin(&cand[(unsigned)(best & 0xffffffffull)], (best & 0xffffffff00000000ull) | (unsigned long long)(unsigned)a);
 }
 
 __global__ void __launch_bounds__(256) k9_accept(const long long n_tracks, const unsigned long long* __restrict__ cand,
@@ -146,7 +153,8 @@ int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_se
   const int rc = launch_scan_i32(L, d_bcount, d_bstart, NB, d_btmp + 1, d_btmp);   // d_bstart[NB - 1] = number of tracks
   if (rc < 0) return rc;
   k9_fill<<<(int)((n_tracks + 255) / 256), 256, 0, L.stream>>>(n_tracks, P.R, o_sector, d_row_in, d_bstart, d_bfill, d_blist);
-  k9_propose<<<blocks, K9_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_par, d_rows, d_outer, d_row_in, d_row_out, d_leaver, d_sec_begin,
+  const int wblocks = (int)((n_tracks * 32 + K9_THREADS - 1) / K9_THREADS);   // one warp per slot of the leaver list
+  k9_propose<<<wblocks, K9_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_par, d_rows, d_outer, d_row_in, d_row_out, d_leaver, d_sec_begin,
                                                  d_sec_begin + NS + 1, d_list, d_bstart, d_blist, d_cand, M, P);
   k9_accept<<<(int)((n_tracks + 255) / 256), 256, 0, L.stream>>>(n_tracks, d_cand, d_next, d_prev);
   e = cudaGetLastError();

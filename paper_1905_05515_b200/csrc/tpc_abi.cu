@@ -318,7 +318,7 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "loop_qmin") rc = nonneg(T.loop_qmin); else if (s == "loop_dy") rc = pos(T.loop_dy); else if (s == "loop_ds") rc = pos(T.loop_ds);
   else if (s == "loop_dt") rc = pos(T.loop_dt); else if (s == "loop_dq") rc = pos(T.loop_dq); else if (s == "loop_pmin") rc = pos(T.loop_pmin);
   else if (s == "loop_frac") { if (!(v > 0 && v < 0.5)) return fail(c, TPC_E_ARG, "loop_frac must be in (0, 0.5)"); T.loop_frac = v; }
-  else if (s == "loop_nmax") { if (v < 1 || v > 1000) return fail(c, TPC_E_ARG, "loop_nmax must be in 1..1000"); T.loop_nmax = (int)v; }
+  else if (s == "loop_nmax") { if (v < 1 || v > 255) return fail(c, TPC_E_ARG, "loop_nmax must be in 1..255"); T.loop_nmax = (int)v; }
   else if (s == "merge_rows") { if (v < 0 || v > 255) return fail(c, TPC_E_ARG, "merge_rows must be in 0..255"); T.merge_rows = (int)v; }
   else return fail(c, TPC_E_ARG, "tpc_set_param: unknown parameter '%s'", name);
   if (rc == TPC_OK) { c->rows_valid = false; c->tables_ready = false; }
