@@ -149,7 +149,7 @@ struct tpc_ctx {
   DevBuf l_prev, l_prev_n, l_root, l_turn, l_list, l_sec; PinVec<int32_t> hl_prev, hl_root, hl_turn;   // S10 looper turns (device + host)
   DevBuf g_outer, g_row_in, g_row_out, g_leaver, g_sec_begin, g_list, g_blist, g_bucket, g_cand, g_next, g_prev; PinVec<int32_t> hg_next, hg_prev;
   // S8 cluster marks (device + host)
-  DevBuf m_att, m_adj, m_status, m_track; PinVec<int32_t> hm_status, hm_track;
+  DevBuf m_att, m_adj, m_status, m_track, m_path, m_path_end; PinVec<int32_t> hm_status, hm_track;
   // S7 refit (device + host)
   DevBuf r_n, r_ndf, r_x, r_par, r_cov, r_chi2, r_z0, r_t0;
   PinVec<int32_t> hr_n, hr_ndf; PinVec<float> hr_x, hr_par, hr_cov, hr_chi2, hr_z0, hr_t0;
@@ -264,7 +264,7 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
                     &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
-                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->d_flag2, &c->d_used, &c->m_att, &c->m_adj, &c->m_status, &c->m_track,
+                    &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->d_flag2, &c->d_used, &c->m_att, &c->m_adj, &c->m_status, &c->m_track, &c->m_path, &c->m_path_end,
                     &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_list, &c->g_blist, &c->g_bucket, &c->g_cand, &c->g_next, &c->g_prev,
                     &c->l_prev, &c->l_prev_n, &c->l_root, &c->l_turn, &c->l_list, &c->l_sec};
   for (DevBuf* b : bufs) b->release();
@@ -843,12 +843,13 @@ int tpc_mark_clusters(tpc_ctx* c, float tube_cm, int device_result, tpc_cluster_
   const long long N = c->N; const size_t Nz = (size_t)std::max(N, 1LL);
   CUDA_TRY(c, c->m_att.ensure(Nz * 4)); CUDA_TRY(c, c->m_adj.ensure(Nz * 8)); CUDA_TRY(c, c->m_status.ensure(Nz * 4));
   CUDA_TRY(c, c->m_track.ensure(Nz * 4));
+  { const size_t ntz = (size_t)std::max(c->n_tracks, 1LL); CUDA_TRY(c, c->m_path.ensure(ntz * c->R * 8)); CUDA_TRY(c, c->m_path_end.ensure(ntz * 4)); }
   long long launches = 0;
   CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
   LAUNCH_TRY(c, launch_k8_status(L, c->n_tracks, N, c->NS * c->R, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_par.as<float>(),
                                  c->o_cl_begin.as<long long>(), c->o_cl_row.as<int>(), c->d_tl_first.as<int>(), c->d_units.as<UnitDesc>(),
                                  c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_perm.as<int>(), c->d_bin_start.as<int>(),
-                                 c->d_rowhit.as<rowhit_t>(), c->m_att.as<int>(), (unsigned long long*)c->m_adj.p, c->m_status.as<int>(),
+                                 c->d_rowhit.as<rowhit_t>(), c->m_att.as<int>(), (unsigned long long*)c->m_adj.p, c->m_path.as<float2>(), c->m_path_end.as<int>(), c->m_status.as<int>(),
                                  c->m_track.as<int>(), tube_cm, c->P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
   out->n_clusters = N;

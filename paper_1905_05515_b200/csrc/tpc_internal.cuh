@@ -176,7 +176,7 @@ int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, co
 int launch_k8_status(const Launch& L, long long n_tracks, long long N, int U, const int* o_sector, const int* o_tracklet,
                      const float* o_par, const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first,
                      const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const int* d_perm, const int* d_bin_start,
-                     const rowhit_t* d_rowhit, int* d_att, unsigned long long* d_adj, int* cl_status, int* cl_track, float tube,
+                     const rowhit_t* d_rowhit, int* d_att, unsigned long long* d_adj, float2* d_path, int* d_path_end, int* cl_status, int* cl_track, float tube,
                      const Params& P);
 
 int launch_k9_merge(const Launch& L, long long n_tracks, int NS, const int* o_sector, const int* o_tracklet, const float* o_par,
