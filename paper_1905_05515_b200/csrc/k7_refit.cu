@@ -6,7 +6,7 @@
 // outermost cluster reached with a fresh C0 -> state, covariance, chi2, n, ndf = 2n - 5 at the innermost cluster used.  The
 // collision time follows from the extrapolation of that state to the beam line: z0 = z - (dz/ds) * arc, t0 = -z0 / vdrift.
 //
-// One lane per track; the fp32 state lives in registers (same transport / update code as K5, kalman.cuh).  The cluster
+// One lane per track, the tracks taken in the order of their length (longest first); the fp32 state lives in registers (same transport / update code as K5, kalman.cuh).  The cluster
 // coordinates are fetched through the tracklet's rowhit line and the sorted (y, z) array: the next cluster's row and position
 // are read one step ahead of the transport that needs them.
 #include "kalman.cuh"
@@ -15,8 +15,29 @@ namespace tpc {
 namespace {
 
 constexpr int K7_THREADS = 128;
+constexpr int K7_CLASSES = 256;   // length classes of the ordering: clusters of a track (at most one per row, n_rows <= 255)
 
-__global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks, const int* __restrict__ o_sector,
+// Tracks ordered by their number of clusters, longest first (counting sort: k7_count, k7_starts, k7_fill): k7_refit runs one
+// track per lane from start to end, so a warp takes as long as its longest track; with equally long tracks side by side the lanes
+// of a warp finish together.  The order inside a length class is arbitrary and enters no result.
+__global__ void __launch_bounds__(256) k7_count(const long long n_tracks, const long long* __restrict__ cl_begin, int* __restrict__ count) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_tracks) return;
+  atomicAdd(&count[min((int)(cl_begin[i + 1] - cl_begin[i]), K7_CLASSES - 1)], 1);
+}
+__global__ void k7_starts(const int* __restrict__ count, int* __restrict__ start) {   // one thread: K7_CLASSES entries, longest class first
+  int acc = 0;
+  for (int m = K7_CLASSES - 1; m >= 0; m--) { start[m] = acc; acc += count[m]; }
+}
+__global__ void __launch_bounds__(256) k7_fill(const long long n_tracks, const long long* __restrict__ cl_begin, const int* __restrict__ start,
+                                               int* __restrict__ fill, int* __restrict__ order) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_tracks) return;
+  const int m = min((int)(cl_begin[i + 1] - cl_begin[i]), K7_CLASSES - 1);
+  order[start[m] + atomicAdd(&fill[m], 1)] = (int)i;
+}
+
+__global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks, const int* __restrict__ order, const int* __restrict__ o_sector,
                                                        const int* __restrict__ o_tracklet, const long long* __restrict__ cl_begin,
                                                        const int* __restrict__ cl_row, const UnitDesc* __restrict__ units,
                                                        const RowConst* __restrict__ rows, const float2* __restrict__ yz,
@@ -24,8 +45,9 @@ __global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks,
                                                        float* __restrict__ rf_x, float* __restrict__ rf_par, float* __restrict__ rf_cov,
                                                        float* __restrict__ rf_chi2, float* __restrict__ rf_z0, float* __restrict__ rf_t0,
                                                        const Params P) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_tracks) return;
+  const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_tracks) return;
+  const long long i = order[j];
   const int R = P.R;
   const long long a = cl_begin[i];
   const int m = (int)(cl_begin[i + 1] - a);
@@ -99,13 +121,20 @@ __global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks,
 int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, const int* o_tracklet, const long long* o_cl_begin,
                     const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const rowhit_t* d_rowhit,
                     int* rf_n, int* rf_ndf, float* rf_x, float* rf_par, float* rf_cov, float* rf_chi2, float* rf_z0, float* rf_t0,
-                    const Params& P) {
+                    int* d_order /* n_tracks ints */, int* d_classes /* 3 * K7_CLASSES ints */, const Params& P) {
   if (n_tracks <= 0) return 0;
+  int* d_count = d_classes; int* d_fill = d_classes + K7_CLASSES; int* d_start = d_classes + 2 * K7_CLASSES;
+  cudaError_t e0 = cudaMemsetAsync(d_count, 0, (size_t)2 * K7_CLASSES * sizeof(int), L.stream);
+  if (e0 != cudaSuccess) return -(int)e0;
+  const int b256 = (int)((n_tracks + 255) / 256);
+  k7_count<<<b256, 256, 0, L.stream>>>(n_tracks, o_cl_begin, d_count);
+  k7_starts<<<1, 1, 0, L.stream>>>(d_count, d_start);
+  k7_fill<<<b256, 256, 0, L.stream>>>(n_tracks, o_cl_begin, d_start, d_fill, d_order);
   const int blocks = (int)((n_tracks + K7_THREADS - 1) / K7_THREADS);
-  k7_refit<<<blocks, K7_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_tracklet, o_cl_begin, o_cl_row, d_units, d_rows, d_yz, d_rowhit,
+  k7_refit<<<blocks, K7_THREADS, 0, L.stream>>>(n_tracks, d_order, o_sector, o_tracklet, o_cl_begin, o_cl_row, d_units, d_rows, d_yz, d_rowhit,
                                                 rf_n, rf_ndf, rf_x, rf_par, rf_cov, rf_chi2, rf_z0, rf_t0, P);
   cudaError_t e = cudaGetLastError();
-  return e == cudaSuccess ? 1 : -(int)e;
+  return e == cudaSuccess ? 4 : -(int)e;
 }
 
 }  // namespace tpc

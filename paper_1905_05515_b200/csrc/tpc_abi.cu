@@ -151,7 +151,7 @@ struct tpc_ctx {
   // S8 cluster marks (device + host)
   DevBuf m_att, m_adj, m_status, m_track, m_path, m_path_end; PinVec<int32_t> hm_status, hm_track;
   // S7 refit (device + host)
-  DevBuf r_n, r_ndf, r_x, r_par, r_cov, r_chi2, r_z0, r_t0;
+  DevBuf r_n, r_ndf, r_x, r_par, r_cov, r_chi2, r_z0, r_t0, r_order, r_classes;
   PinVec<int32_t> hr_n, hr_ndf; PinVec<float> hr_x, hr_par, hr_cov, hr_chi2, hr_z0, hr_t0;
   std::vector<int8_t> dbg_up_k, dbg_dn_k;
   std::vector<float> dbg_yz; std::vector<int32_t> dbg_perm, dbg_bins, dbg_up, dbg_dn, dbg_su, dbg_sp;
@@ -263,7 +263,7 @@ void tpc_destroy(tpc_ctx* c) {
                     &c->d_start_unit, &c->d_start_pos, &c->d_counters, &c->d_k5scratch, &c->d_rowhit, &c->d_tl_n, &c->d_tl_first, &c->d_tl_last, &c->d_tl_chi2,
                     &c->d_tl_par, &c->d_tl_cov, &c->d_owner, &c->d_tl_key, &c->d_scan_in, &c->d_scan_out, &c->d_scan_tmp64, &c->o_sector,
                     &c->o_x, &c->o_par, &c->o_cov, &c->o_chi2, &c->o_ndf, &c->o_tracklet, &c->o_cl_begin, &c->o_cl_row, &c->o_cl_index,
-                    &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0,
+                    &c->r_n, &c->r_ndf, &c->r_x, &c->r_par, &c->r_cov, &c->r_chi2, &c->r_z0, &c->r_t0, &c->r_order, &c->r_classes,
                     &c->d_keep, &c->d_keep_pos, &c->d_start_unit2, &c->d_start_pos2, &c->d_flag2, &c->d_used, &c->m_att, &c->m_adj, &c->m_status, &c->m_track, &c->m_path, &c->m_path_end,
                     &c->g_outer, &c->g_row_in, &c->g_row_out, &c->g_leaver, &c->g_sec_begin, &c->g_list, &c->g_blist, &c->g_bucket, &c->g_cand, &c->g_next, &c->g_prev,
                     &c->l_prev, &c->l_prev_n, &c->l_root, &c->l_turn, &c->l_list, &c->l_sec};
@@ -801,12 +801,13 @@ int tpc_refit_tracks(tpc_ctx* c, int device_result, tpc_refit* out) {
   CUDA_TRY(c, c->r_n.ensure(ntz * 4)); CUDA_TRY(c, c->r_ndf.ensure(ntz * 4)); CUDA_TRY(c, c->r_x.ensure(ntz * 4));
   CUDA_TRY(c, c->r_par.ensure(ntz * 20)); CUDA_TRY(c, c->r_cov.ensure(ntz * 60)); CUDA_TRY(c, c->r_chi2.ensure(ntz * 4));
   CUDA_TRY(c, c->r_z0.ensure(ntz * 4)); CUDA_TRY(c, c->r_t0.ensure(ntz * 4));
+  CUDA_TRY(c, c->r_order.ensure(ntz * 4)); CUDA_TRY(c, c->r_classes.ensure(768 * 4));
   long long launches = 0;
   CUDA_TRY(c, cudaEventRecord(c->ev[8], st));
   LAUNCH_TRY(c, launch_k7_refit(L, nt, c->o_sector.as<int>(), c->o_tracklet.as<int>(), c->o_cl_begin.as<long long>(), c->o_cl_row.as<int>(),
                                 c->d_units.as<UnitDesc>(), c->d_rows.as<RowConst>(), c->d_yz.as<float2>(), c->d_rowhit.as<rowhit_t>(),
                                 c->r_n.as<int>(), c->r_ndf.as<int>(), c->r_x.as<float>(), c->r_par.as<float>(), c->r_cov.as<float>(),
-                                c->r_chi2.as<float>(), c->r_z0.as<float>(), c->r_t0.as<float>(), c->P), launches);
+                                c->r_chi2.as<float>(), c->r_z0.as<float>(), c->r_t0.as<float>(), c->r_order.as<int>(), c->r_classes.as<int>(), c->P), launches);
   CUDA_TRY(c, cudaEventRecord(c->ev[9], st));
   out->n_tracks = nt;
   if (!device_result) {

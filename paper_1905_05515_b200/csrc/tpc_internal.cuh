@@ -171,7 +171,7 @@ int launch_k6_emit(const Launch& L, int M_cap, const int* d_M, const int* d_star
 int launch_k7_refit(const Launch& L, long long n_tracks, const int* o_sector, const int* o_tracklet, const long long* o_cl_begin,
                     const int* o_cl_row, const UnitDesc* d_units, const RowConst* d_rows, const float2* d_yz, const rowhit_t* d_rowhit,
                     int* rf_n, int* rf_ndf, float* rf_x, float* rf_par, float* rf_cov, float* rf_chi2, float* rf_z0, float* rf_t0,
-                    const Params& P);
+                    int* d_order, int* d_classes /* 768 ints */, const Params& P);
 
 int launch_k8_status(const Launch& L, long long n_tracks, long long N, int U, const int* o_sector, const int* o_tracklet,
                      const float* o_par, const long long* o_cl_begin, const int* o_cl_row, const int* d_tl_first,
