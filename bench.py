@@ -227,6 +227,7 @@ def run_gpu(args, rank, world, local_rank):
     if args.variant and rank == 0:
         variant = {}
         for vname, vp in (("skip_links", dict(link_skip=1.0)),
+                          ("skip_links_strict", dict(link_skip=1.0, skip_cut2=0.4375)),
                           ("drop_bridged", dict(bridge_rows=4.0, bridge_min=8.0)),
                           ("rescue_wave", dict(bridge_rows=4.0, bridge_min=3.0, bridge_rescue=1.0))):
             with T.Tracker(**w.geometry(), **vp) as tv:
@@ -247,7 +248,8 @@ def run_gpu(args, rank, world, local_rank):
                                   "tracks_per_step": int(rv.n_tracks), "cluster_refs_per_step": int(rv.n_cluster_refs),
                                   "kernel_ms": {k: vt[k] for k in keys}}
         variant["note"] = ("NEXT-2 variants (SURVEY 8(f).2), all off by default because they change the result: skip_links = S2', links "
-                           "that may skip one pad row (reading A45); seed bridging (readings A39 / A39c): drop_bridged drops the start hits "
+                           "that may skip one pad row (reading A45), skip_links_strict = the same with a quarter of cut2 for the pairs that skip a row "
+                           "(the setting that keeps the efficiency of the default path); seed bridging (readings A39 / A39c): drop_bridged drops the start hits "
                            "that continue a lower chain, rescue_wave fits them in a second K5 wave when the first left their chain unused; "
                            "efficiency versus generator truth in DESIGN.md section 11")
     # S7 (NEXT-1, not part of the timed S0..S6 step): refit over the owned clusters + collision time, device-resident result

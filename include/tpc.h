@@ -158,7 +158,8 @@ int tpc_create(const tpc_geometry* geometry, float bz_tesla, float vdrift_cm_per
 /* Tunables of DESIGN.md table T by name: wy wz dzdx_max wz0 cut2 min_seed c0_y c0_z c0_sinphi c0_dzds c0_qpt s_max n_sigma
  * w_max max_gap edge_margin min_hits grid_scale, plus debug_keep (1 = keep pre-cleaning link tables for tpc_debug_get_links) and
  * link_skip (default 0; 1 = S2', the gap-tolerant seeding variant of SURVEY.md section 8(f).2: a cluster without an accepted pair on
- * the adjacent rows may link over one missing row; changes the result), bridge_rows / bridge_min /
+ * the adjacent rows may link over one missing row; changes the result; skip_cut2 = cut2 of the pairs that
+ * skip a row, default 1.75 = cut2, 0.4375 keeps the efficiency of the default path), bridge_rows / bridge_min /
  * bridge_rescue (seed-bridging variants, readings A39 / A39c; ignored with link_skip), and
  * pinned_async (default 0; 1 = a PINNED host source of tpc_load_clusters* is read by DMA on the context's stream AFTER the load call
  * has returned: the caller then keeps those buffers untouched until the next tpc_find_tracks* on the context returns.  With 0 the

@@ -59,6 +59,7 @@ struct Tunables {            // DESIGN.md table T (all are readings; the paper i
   int bridge_min = 3;           // clusters the lower chain must have
   int bridge_rescue = 0;        // 1: dropped start hits get their tracklet after all when the first wave left their chain unused
   int link_skip = 0;            // NEXT-2 as SURVEY 8(f).2 wrote it (reading A45): 1 = a link may skip one pad row
+  double skip_cut2 = 1.75;      // cut2 of the pairs that skip a row (S2'; = cut2 by default, smaller = stricter: DESIGN.md section 11.1)
   double tube = 1.5;            // NEXT-4: radius of the tube around a track, cm
   // NEXT-3 (reading A41): cross-sector segment matching
   double merge_edge = 3.0; int merge_rows = 8; double merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05;
@@ -136,7 +137,7 @@ struct Oracle : OracleBase {
       wzu[r] = (Real)(T.dzdx_max * a + T.wz0); wzd[r] = (Real)(T.dzdx_max * b + T.wz0);
       yedge[r] = (Real)(x * std::tan(0.5 * dphi));
     }
-    // S2' (reading A45): row distance 2 upwards (index "2" first) / downwards; thr_{ku kd} = cut2 * 0.5 * (a_ku^2 + b_kd^2)
+    // S2' (reading A45): row distance 2 upwards (index "2" first) / downwards; thr_{ku kd} = skip_cut2 * 0.5 * (a_ku^2 + b_kd^2)
     tu2.assign(R, 1); td2.assign(R, 1); ar2.assign(R, 0); br2.assign(R, 0); wzu2.assign(R, 0); wzd2.assign(R, 0);
     thr21.assign(R, 0); thr12.assign(R, 0); thr22.assign(R, 0);
     for (int r = 0; r < R; r++) {
@@ -145,8 +146,8 @@ struct Oracle : OracleBase {
       double a = xu - x, b = x - xd, a2 = xu2 - x, b2 = x - xd2;
       tu2[r] = (Real)(xu2 / x); td2[r] = (Real)(xd2 / x); ar2[r] = (Real)a2; br2[r] = (Real)b2;
       wzu2[r] = (Real)(T.dzdx_max * a2 + T.wz0); wzd2[r] = (Real)(T.dzdx_max * b2 + T.wz0);
-      thr21[r] = (Real)(T.cut2 * 0.5 * (a2 * a2 + b * b)); thr12[r] = (Real)(T.cut2 * 0.5 * (a * a + b2 * b2));
-      thr22[r] = (Real)(T.cut2 * 0.5 * (a2 * a2 + b2 * b2));
+      thr21[r] = (Real)(T.skip_cut2 * 0.5 * (a2 * a2 + b * b)); thr12[r] = (Real)(T.skip_cut2 * 0.5 * (a * a + b2 * b2));
+      thr22[r] = (Real)(T.skip_cut2 * 0.5 * (a2 * a2 + b2 * b2));
     }
     cB = (Real)(-0.00299792458 * bz);
   }
@@ -262,7 +263,8 @@ struct Oracle : OracleBase {
   //      further: candidates on rows r+1, r+2 / r-1, r-2 in the windows of S2 scaled to the row distance k (centre y * x_{r+-k}/x_r;
   //      half-width k*wy; z: centre z * x_{r+-k}/x_r with half-width k*wz in triggered mode, centre z with half-width
   //      dzdx_max*|dx| + wz0 in continuous mode).  Pair residual as in S2 with the actual distances a = x_u - x_r, b = x_r - x_d:
-  //      ey = b (y_u - y) - a (y - y_d), ez likewise, D = ey^2 + ez^2, accepted iff D < cut2 * 0.5 * (a^2 + b^2).
+  //      ey = b (y_u - y) - a (y - y_d), ez likewise, D = ey^2 + ez^2, accepted iff D < skip_cut2 * 0.5 * (a^2 + b^2)
+  //      (skip_cut2 = cut2 unless set: a stricter cut for the longer lever arm keeps the efficiency of the r+-1 path).
   //      Level 3: pairs that skip one row on one side, (k_u, k_d) = (2,1) and (1,2); if none is accepted, level 4: (2,2).
   //      Within a level the accepted pair with the minimum key (D, k_u, original index of up, original index of down) wins.
   void s2_skip_links(bool brute) {
@@ -1018,7 +1020,7 @@ int orc_set_param(void* h, const char* name, double v) {
   else if (s == "c0_y") T.c0[0] = v; else if (s == "c0_z") T.c0[1] = v; else if (s == "c0_sinphi") T.c0[2] = v;
   else if (s == "c0_dzds") T.c0[3] = v; else if (s == "c0_qpt") T.c0[4] = v;
   else if (s == "grid_scale") T.grid_scale = v;
-  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "bridge_rescue") T.bridge_rescue = (int)v; else if (s == "tube") T.tube = v; else if (s == "link_skip") T.link_skip = (int)v;
+  else if (s == "bridge_rows") T.bridge_rows = (int)v; else if (s == "bridge_wy") T.bridge_wy = v; else if (s == "bridge_wz") T.bridge_wz = v; else if (s == "bridge_min") T.bridge_min = (int)v; else if (s == "bridge_rescue") T.bridge_rescue = (int)v; else if (s == "tube") T.tube = v; else if (s == "link_skip") T.link_skip = (int)v; else if (s == "skip_cut2") T.skip_cut2 = v;
   else if (s == "merge_edge") T.merge_edge = v; else if (s == "merge_rows") T.merge_rows = (int)v; else if (s == "merge_dy") T.merge_dy = v;
   else if (s == "merge_dz") T.merge_dz = v; else if (s == "merge_ds") T.merge_ds = v; else if (s == "merge_dt") T.merge_dt = v;
   else if (s == "loop_qmin") T.loop_qmin = v; else if (s == "loop_dy") T.loop_dy = v; else if (s == "loop_ds") T.loop_ds = v; else if (s == "loop_dt") T.loop_dt = v;

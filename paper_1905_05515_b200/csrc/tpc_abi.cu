@@ -89,6 +89,7 @@ struct Tunables {   // DESIGN.md table T
   int k2_threads = 0;         // K2 block size (0 = default 256); tuning knob
   int bridge_rows = 0, bridge_min = 3;       // NEXT-2 seed bridging (reading A39): 0 = off
   int link_skip = 0;                         // NEXT-2 (reading A45): 1 = links may skip one pad row (S2')
+  double skip_cut2 = 1.75;                   // cut2 of the pairs that skip a row (= cut2 by default; smaller = stricter)
   int bridge_rescue = 0;                     // 1: dropped start hits are fitted in a second wave when the first left their chain unused (A39c)
   double bridge_wy = 1.0, bridge_wz = 1.5;
   double merge_edge = 3.0, merge_dy = 1.5, merge_dz = 2.0, merge_ds = 0.05, merge_dt = 0.05; int merge_rows = 8;   // NEXT-3 (reading A41)
@@ -313,6 +314,7 @@ int tpc_set_param(tpc_ctx* c, const char* name, double v) {
   else if (s == "bridge_wy") rc = pos(T.bridge_wy); else if (s == "bridge_wz") rc = pos(T.bridge_wz);
   else if (s == "bridge_rescue") T.bridge_rescue = v != 0;
   else if (s == "link_skip") { if (v != 0 && v != 1) return fail(c, TPC_E_ARG, "link_skip must be 0 or 1"); T.link_skip = (int)v; }
+  else if (s == "skip_cut2") { if (!(v > 0)) return fail(c, TPC_E_ARG, "skip_cut2 must be > 0"); T.skip_cut2 = v; }
   else if (s == "merge_edge") rc = nonneg(T.merge_edge); else if (s == "merge_dy") rc = pos(T.merge_dy); else if (s == "merge_dz") rc = pos(T.merge_dz);
   else if (s == "merge_ds") rc = pos(T.merge_ds); else if (s == "merge_dt") rc = pos(T.merge_dt);
   else if (s == "loop_qmin") rc = nonneg(T.loop_qmin); else if (s == "loop_dy") rc = pos(T.loop_dy); else if (s == "loop_ds") rc = pos(T.loop_ds);
@@ -427,8 +429,8 @@ void make_params_and_rows(tpc_ctx* c, std::vector<RowConst>& rows) {
     const double a2 = xu2 - x, b2 = x - xd2;
     k.tu2 = (float)(xu2 / x); k.td2 = (float)(xd2 / x); k.a2 = (float)a2; k.b2 = (float)b2;
     k.wzu2 = (float)(T.dzdx_max * a2 + T.wz0); k.wzd2 = (float)(T.dzdx_max * b2 + T.wz0);
-    k.thr21 = (float)(T.cut2 * 0.5 * (a2 * a2 + b * b)); k.thr12 = (float)(T.cut2 * 0.5 * (a * a + b2 * b2));
-    k.thr22 = (float)(T.cut2 * 0.5 * (a2 * a2 + b2 * b2));
+    k.thr21 = (float)(T.skip_cut2 * 0.5 * (a2 * a2 + b * b)); k.thr12 = (float)(T.skip_cut2 * 0.5 * (a * a + b2 * b2));
+    k.thr22 = (float)(T.skip_cut2 * 0.5 * (a2 * a2 + b2 * b2));
     for (float& f : k.pad) f = 0.f;
   }
   Params& P = c->P;

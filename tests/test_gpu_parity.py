@@ -286,6 +286,13 @@ def test_skip_link_variant_parity():
         assert len(o.get("start_unit")) <= 0.75 * len(base.get("start_unit"))
         m0, m1 = H.truth_metrics(w, base.tracks()), H.truth_metrics(w, gtr)
         assert m1["eff"] >= m0["eff"] - 0.002, (m0["eff"], m1["eff"])
+    # the operating point DESIGN.md section 11.1 proposes: a stricter cut for the pairs that skip a row (skip_cut2, both sides)
+    for w in (W.config(2), W.config(3, scale=0.1)):
+        o, otr, gtr, res = _full_parity(w, tracklets=True, link_skip=1, skip_cut2=0.4375)
+        base = P.make_oracle(w).run("s6")
+        assert len(o.get("start_unit")) <= 0.7 * len(base.get("start_unit"))
+        m0, m1 = H.truth_metrics(w, base.tracks()), H.truth_metrics(w, gtr)
+        assert m1["eff"] >= m0["eff"] - 0.0005, (m0["eff"], m1["eff"])
 
 
 def test_large_units_take_the_partly_shared_k1_path():

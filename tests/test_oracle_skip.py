@@ -139,11 +139,13 @@ def test_mutual_links_carry_the_row_distance():
     assert heads == _starts(o)
 
 
-def _restate(w, row_x, cut2, wy=1.5, wz=1.5, **oracle_params):
+def _restate(w, row_x, cut2, wy=1.5, wz=1.5, skip_cut2=None, **oracle_params):
     """O(N^2) restatement of S2' in numpy fp32 for the hits S2 left without a link, from the definition (reading A45).
-    Returns the number of hits that got a skipping link."""
+    Returns the number of hits that got a skipping link.  skip_cut2: cut of the pairs that skip a row (default: the oracle's 1.75,
+    which the callers that pass another cut2 set explicitly)."""
     base = Oracle.for_workload(w, cut2=cut2, **oracle_params).run("s2")
-    o = Oracle.for_workload(w, link_skip=1, cut2=cut2, **oracle_params).run("s2")
+    skip_cut2 = cut2 if skip_cut2 is None else skip_cut2
+    o = Oracle.for_workload(w, link_skip=1, cut2=cut2, skip_cut2=skip_cut2, **oracle_params).run("s2")
     got = _links_orig(w, o, RAW)
     base_up = _links_orig(w, base, RAW)[:, 0]
     f = np.float32
@@ -174,7 +176,7 @@ def _restate(w, row_x, cut2, wy=1.5, wz=1.5, **oracle_params):
                     if r + ku > R - 1 or r - kd < 0:
                         continue
                     A64, B64 = X[r + ku] - X[r], X[r] - X[r - kd]
-                    A, B, lim = f(A64), f(B64), f(cut2 * 0.5 * (A64 * A64 + B64 * B64))
+                    A, B, lim = f(A64), f(B64), f(skip_cut2 * 0.5 * (A64 * A64 + B64 * B64))
                     for i in cand[(+1, ku)]:
                         for j in cand[(-1, kd)]:
                             ey = f(f(B * f(w.y[i] - y)) - f(A * f(y - w.y[j])))
@@ -219,6 +221,9 @@ def test_numpy_restatement_on_a_dense_cloud():
                    np.ones(len(ys), np.float32), -np.ones(len(ys), np.int32), np.zeros(len(ys), np.uint8), base.particles, base.coll_t0, base.coll_mult)
     n_new, n_wide = _restate(w, base.row_x, cut2=25.0)
     assert n_new > 30 and n_wide > 5
+    # the pairs that skip a row have their own cut (skip_cut2): a stricter one links fewer hits, S2 itself (cut2) is untouched
+    n_strict, _ = _restate(w, base.row_x, cut2=25.0, skip_cut2=6.0)
+    assert 5 < n_strict < n_new
 
 
 def test_exact_tie_between_the_two_one_sided_levels_goes_to_the_shorter_up_link():
@@ -259,6 +264,42 @@ def test_every_level_has_its_own_threshold():
         o.load(off, np.array(ys, np.float32), np.array(ts, np.float32)); o.run("s2")
         h = int(off[50])
         assert (o.get("link_up")[h] >= 0) == linked and (o.get("link_up_k")[h], o.get("link_dn_k")[h]) == ((1, 2) if linked else (0, 0))
+
+
+def test_skip_cut2_is_the_cut_of_the_skipping_pairs_only():
+    """Same hand-made case as above with d2 = -0.5: D = 4 against thr_12 = skip_cut2 * 0.5 * (1 + 4): linked at 1.75 (4.375) and at
+    1.61 (4.025), not at 1.59 (3.975); cut2 (the adjacent pairs) does not enter: cut2 = 0.1 / 100 change nothing here.  And the other
+    way: an adjacent pair with D = 0.25 (u1 = +0.25, d1 = +0.25: ey = 0.5) is accepted by cut2 = 1.75 (thr = 1.75) whatever skip_cut2 is.
+    Fails under: skip_cut2 ignored; skip_cut2 applied to the adjacent level."""
+    R = 152
+    X = (100.0 + np.arange(R)).astype(np.float32)
+    def run(rows, **params):
+        off = np.zeros(R + 1, np.int64); ys, ts = [], []
+        for r in range(R):
+            cl = rows.get(r, [])
+            off[r + 1] = off[r] + len(cl); ys += [c[0] for c in cl]; ts += [(250.0 - c[1]) / 2.0 for c in cl]
+        o = Oracle(n_sectors=1, n_rows=R, row_x=X, sector_dphi=2 * math.pi / 18, z_max=250.0, t_frame=0.0, sigma_y=0.1, sigma_z=0.15,
+                   bz=0.5, vdrift=2.0, link_skip=1, **params)
+        o.load(off, np.array(ys, np.float32), np.array(ts, np.float32)); o.run("s2")
+        h = int(off[50])
+        return int(o.get("link_up_k")[h]), int(o.get("link_dn_k")[h])
+    skipping = {51: [(1.25, 0.0)], 50: [(0.0, 0.0)], 48: [(-0.5, 0.0)]}
+    assert run(skipping) == (1, 2) and run(skipping, skip_cut2=1.61) == (1, 2) and run(skipping, skip_cut2=1.59) == (0, 0)
+    assert run(skipping, cut2=0.1) == (1, 2) and run(skipping, cut2=100.0, skip_cut2=1.59) == (0, 0)
+    adjacent = {51: [(0.25, 0.0)], 50: [(0.0, 0.0)], 49: [(0.25, 0.0)]}
+    assert run(adjacent) == (1, 1) and run(adjacent, skip_cut2=1e-6) == (1, 1) and run(adjacent, cut2=0.1) == (0, 0)
+
+
+def test_a_stricter_cut_for_skipping_pairs_keeps_the_efficiency():
+    """Operating point DESIGN.md section 11.1 proposes: skip_cut2 = 0.4375 (a quarter of cut2).  Generator truth: efficiency not
+    below the r+-1 path by more than 0.05 %, fewer fakes than with skip_cut2 = cut2, still at most 0.7 of the start hits."""
+    for w in (W.config(1), W.config(3, scale=0.1)):
+        b = Oracle.for_workload(w).run("s6")
+        loose = Oracle.for_workload(w, link_skip=1).run("s6")
+        tight = Oracle.for_workload(w, link_skip=1, skip_cut2=0.4375).run("s6")
+        mb, ml, mt = (H.truth_metrics(w, o.tracks()) for o in (b, loose, tight))
+        assert mt["eff"] >= mb["eff"] - 0.0005, (mb["eff"], mt["eff"])
+        assert mt["fakes"] <= ml["fakes"] and len(_starts(loose)) <= len(_starts(tight)) <= 0.7 * len(_starts(b))
 
 
 def test_fewer_tracklets_at_the_documented_efficiency():
