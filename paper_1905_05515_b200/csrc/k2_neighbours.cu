@@ -316,8 +316,9 @@ __device__ __forceinline__ void skip_level(SkipBest& best, const int ku, const i
 // fast path of S2': like k2_neighbours, the candidates of the (at most two) bin rows of a window are scanned once into a bit mask
 struct SkipMask { Win w; unsigned m; bool ok; };   // ok = false: more than two bin rows or more than 32 candidates (generic path)
 
-__device__ __forceinline__ SkipMask skip_scan(const SkipWin& sw, const UnitDesc& g, const float2* __restrict__ yz,
-                                              const int* __restrict__ bin_start) {
+// first half: the candidate range(s) of the window from the bin table (up to four reads; the four windows of a hit are done
+// together so that their 16 reads are in flight at once)
+__device__ __forceinline__ SkipMask skip_ranges(const SkipWin& sw, const UnitDesc& g, const int* __restrict__ bin_start) {
   SkipMask r; r.m = 0u; r.ok = true;
   r.w.ylo = sw.ylo; r.w.yhi = sw.yhi; r.w.zlo = sw.zlo; r.w.zhi = sw.zhi; r.w.wide = false; r.w.a0 = r.w.n0 = r.w.a1m = r.w.n = 0;
   if (!sw.any) return r;
@@ -326,11 +327,15 @@ __device__ __forceinline__ SkipMask skip_scan(const SkipWin& sw, const UnitDesc&
   const int ra = sw.bz0 * g.ny;
   r.w.a0 = bs[ra + sw.by0]; r.w.n0 = bs[ra + sw.by1 + 1] - r.w.a0; r.w.n = r.w.n0;
   if (sw.bz1 > sw.bz0) { const int rb = ra + g.ny; const int a1 = bs[rb + sw.by0]; r.w.n += bs[rb + sw.by1 + 1] - a1; r.w.a1m = a1 - r.w.n0; }
-  if (r.w.n > 32) { r.ok = false; return r; }
+  if (r.w.n > 32) r.ok = false;
+  return r;
+}
+// second half: the candidates inside the window as a bit mask
+__device__ __forceinline__ void skip_fill(SkipMask& r, const UnitDesc& g, const float2* __restrict__ yz) {
+  if (!r.ok) return;
   const float2* __restrict__ hits = yz + g.off;
 #pragma unroll 1
   for (int j = 0; j < r.w.n; j++) { if (in_win(hits[win_pos(r.w, j)], r.w)) r.m |= 1u << j; }
-  return r;
 }
 
 __device__ __forceinline__ void skip_level_masks(SkipBest& best, const int ku, const int kd, const SkipMask& mu, const SkipMask& md,
@@ -363,7 +368,10 @@ __device__ __forceinline__ void skip_level_masks(SkipBest& best, const int ku, c
   }
 }
 
-__global__ void __launch_bounds__(256) k2_skip_links(const Item* __restrict__ items, const int chunk, const UnitDesc* __restrict__ units,
+#ifndef K2S_CTAS
+#define K2S_CTAS 6   // measured on C3 (K2 + K2'): 0.96 ms at 3 CTAs / SM (the compiler's choice at 80 registers), 0.79 at 4, 0.72 at 5, 0.71 at 6, 0.70 at 8: latency-bound, occupancy pays more than the spills cost
+#endif
+__global__ void __launch_bounds__(256, K2S_CTAS) k2_skip_links(const Item* __restrict__ items, const int chunk, const UnitDesc* __restrict__ units,
                                                      const RowConst* __restrict__ rows, const float2* __restrict__ yz,
                                                      const int* __restrict__ perm, const int* __restrict__ bin_start,
                                                      int* __restrict__ link_up, int* __restrict__ link_dn, const Params P) {
@@ -390,8 +398,14 @@ __global__ void __launch_bounds__(256) k2_skip_links(const Item* __restrict__ it
   if (n_open == 0) return;
   const bool cont = P.continuous != 0;
   const bool up2 = r + 2 <= R - 1, dn2 = r - 2 >= 0;
-  const UnitDesc gu1 = units[u + 1], gd1 = units[u - 1];
-  const UnitDesc gu2 = up2 ? units[u + 2] : gu1, gd2 = dn2 ? units[u - 2] : gd1;
+  // the four neighbour descriptors are the same for every thread: shared memory instead of 4 x 16 registers per thread
+  __shared__ UnitDesc s_g[4];
+  if (threadIdx.x < 4) {
+    const int k = threadIdx.x;   // 0: r+1, 1: r-1, 2: r+2 (or r+1), 3: r-2 (or r-1)
+    s_g[k] = units[k == 0 ? u + 1 : k == 1 ? u - 1 : k == 2 ? (up2 ? u + 2 : u + 1) : (dn2 ? u - 2 : u - 1)];
+  }
+  __syncthreads();
+  const UnitDesc& gu1 = s_g[0]; const UnitDesc& gd1 = s_g[1]; const UnitDesc& gu2 = s_g[2]; const UnitDesc& gd2 = s_g[3];
   const float wy1 = __fmul_rn(1.0f, P.wy), wy2 = __fmul_rn(2.0f, P.wy), wz1 = __fmul_rn(1.0f, P.wz), wz2 = __fmul_rn(2.0f, P.wz);
   for (int j = threadIdx.x; j < n_open; j += blockDim.x) {
     const int k = s_list[j];
@@ -404,8 +418,9 @@ __global__ void __launch_bounds__(256) k2_skip_links(const Item* __restrict__ it
     SkipWin wu2 = wu1, wd2 = wd1; wu2.any = wd2.any = false;
     if (dn2) wd2 = skip_window(y, z, rc.td2, wy2, cont ? rc.wzd2 : wz2, cont, gd2);
     if (up2) wu2 = skip_window(y, z, rc.tu2, wy2, cont ? rc.wzu2 : wz2, cont, gu2);
-    const SkipMask mu1 = skip_scan(wu1, gu1, yz, bin_start), md1 = skip_scan(wd1, gd1, yz, bin_start);
-    const SkipMask mu2 = skip_scan(wu2, gu2, yz, bin_start), md2 = skip_scan(wd2, gd2, yz, bin_start);
+    SkipMask mu1 = skip_ranges(wu1, gu1, bin_start), md1 = skip_ranges(wd1, gd1, bin_start);
+    SkipMask mu2 = skip_ranges(wu2, gu2, bin_start), md2 = skip_ranges(wd2, gd2, bin_start);
+    skip_fill(mu1, gu1, yz); skip_fill(md1, gd1, yz); skip_fill(mu2, gu2, yz); skip_fill(md2, gd2, yz);
     if (mu1.ok && md1.ok && mu2.ok && md2.ok) {
       skip_level_masks(best, 1, 2, mu1, md2, gu1, gd2, rc.a, rc.b2, rc.thr12, y, z, yz, perm);
       skip_level_masks(best, 2, 1, mu2, md1, gu2, gd1, rc.a2, rc.b, rc.thr21, y, z, yz, perm);
