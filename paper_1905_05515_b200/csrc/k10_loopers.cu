@@ -8,7 +8,7 @@
 //                 counters of k10_compact
 //   k10_compact : the tracks with |q/pT| >= loop_qmin (pT <= 200 MeV/c: about one track in ten) are gathered at the front of their
 //                 sector's index range (slot = sec_begin + atomic counter; the order inside a sector is arbitrary and enters no
-//                 result); the others get prev = -1 here
+//                 result); every track gets prev = -1 here
 //   k10_match   : one warp per gathered track B, one lane per candidate: B's state is transported (parameters only) to the x of every gathered track A of
 //                 its sector and compared inside the four windows; the number of turns tau = dz / pitch must be within loop_frac of
 //                 an integer n in 1..loop_nmax; predecessor = smallest n, then smallest score, then lowest index (the tie on the
@@ -44,13 +44,16 @@ __global__ void k10_ranges(const long long n_tracks, const int NS, const int* __
 __global__ void __launch_bounds__(K10_THREADS) k10_compact(const long long n_tracks, const int* __restrict__ o_sector,
                                                            const float* __restrict__ o_par, const int* __restrict__ sec_begin,
                                                            int* __restrict__ sec_count, int* __restrict__ list, int* __restrict__ prev,
-                                                           int* __restrict__ prev_n, const K10Params L) {
+                                                           int* __restrict__ prev_n, const int NS, const K10Params L) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_tracks) return;
-  if (fabsf(o_par[i * 5 + 4]) >= L.qmin) {
-    const int sec = o_sector[i];
-    list[sec_begin[sec] + atomicAdd(&sec_count[sec], 1)] = (int)i;
-  } else { prev[i] = -1; prev_n[i] = 0; }
+  const int sec = o_sector[i];
+  // (sector out of range, or a slot beyond the array: only with caller-made arrays that are not in ascending sector order --
+  // tpc_find_loopers_noalloc; such a track takes no part, nothing is written out of bounds)
+  long long slot = -1;
+  if (fabsf(o_par[i * 5 + 4]) >= L.qmin && (unsigned)sec < (unsigned)NS) slot = (long long)sec_begin[sec] + atomicAdd(&sec_count[sec], 1);
+  if (slot >= 0 && slot < n_tracks) list[slot] = (int)i;
+  prev[i] = -1; prev_n[i] = 0;   // every track starts without a predecessor; k10_match overwrites the gathered ones
 }
 
 // One WARP per gathered track B; the lanes take the gathered tracks A of its sector in turn (32 pairs in flight per warp instead of a
@@ -64,15 +67,18 @@ __global__ void __launch_bounds__(K10_THREADS) k10_match(const long long n_track
   const long long j = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // slot of the gathered list (same sector ranges as the tracks)
   const int lane = threadIdx.x & 31;
   if (j >= n_tracks) return;
-  const int sec = o_sector[j], a0 = sec_begin[sec], a1 = a0 + sec_count[sec];
-  if (j >= a1) return;                                                           // beyond the gathered tracks of this sector (whole warp)
+  const int sec = o_sector[j];
+  if ((unsigned)sec >= (unsigned)P.NS) return;
+  const int a0 = sec_begin[sec], a1 = (int)min((long long)a0 + sec_count[sec], n_tracks);
+  if (j < a0 || j >= a1) return;                                                 // beyond the gathered tracks of this sector (whole warp)
   const int b = list[j];
+  if ((unsigned)b >= (unsigned long long)n_tracks) return;                       // (stale slot: arrays not in ascending sector order)
   const float* __restrict__ pb = o_par + (long long)b * 5;
   const float yb = pb[0], zb = pb[1], sb = pb[2], tb = pb[3], qb = pb[4], xb = o_x[b];
   unsigned long long best = ~0ull;
   for (int ja = a0 + lane; ja < a1; ja += 32) {
     const int a = list[ja];
-    if (a == b) continue;
+    if (a == b || (unsigned)a >= (unsigned long long)n_tracks) continue;
     const float* __restrict__ pa = o_par + (long long)a * 5;
     const float qa = pa[4];
     // dz/ds and q/pT are not changed by the transport: their two windows are tested first (same values, same outcome as testing
@@ -123,7 +129,7 @@ int k10_launch_all(const Launch& L, long long n_tracks, int NS, const int* o_sec
                    int* d_sec_count, int* d_list, int* d_prev, int* d_prev_n, int* d_root, int* d_turn, const K10Params& K, const Params& P) {
   k10_ranges<<<(NS + 1 + 63) / 64, 64, 0, L.stream>>>(n_tracks, NS, o_sector, d_sec_begin, d_sec_count);
   const int blocks = (int)((n_tracks + K10_THREADS - 1) / K10_THREADS);
-  k10_compact<<<blocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_par, d_sec_begin, d_sec_count, d_list, d_prev, d_prev_n, K);
+  k10_compact<<<blocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_par, d_sec_begin, d_sec_count, d_list, d_prev, d_prev_n, NS, K);
   const int wblocks = (int)((n_tracks * 32 + K10_THREADS - 1) / K10_THREADS);   // one warp per slot of the gathered list
   k10_match<<<wblocks, K10_THREADS, 0, L.stream>>>(n_tracks, o_sector, o_x, o_par, d_sec_begin, d_sec_count, d_list, d_prev, d_prev_n, K, P);
   k10_roots<<<(int)((n_tracks + 255) / 256), 256, 0, L.stream>>>(n_tracks, d_prev, d_prev_n, d_root, d_turn);

@@ -73,6 +73,18 @@ def test_noalloc_loopers_equal_the_allocating_path_on_two_calls_in_a_row():
         assert e.value.code == -5 and "TPC_NOALLOC_MAX_TRACKS" in str(e.value) and str(B.NOALLOC_MAX_TRACKS) in str(e.value)
         torch.cuda.synchronize()
         assert all(bool((o[k] == -7).all()) for k in o)
+        # arrays that break the contract (sectors shuffled, some out of range) give a meaningless grouping but no fault, and the next
+        # correct call is right again (the scratch keeps nothing that matters from the bad call)
+        g = torch.Generator(device="cuda"); g.manual_seed(5)
+        bad = sector0[torch.randperm(n0, device="cuda", generator=g)].clone()
+        bad[::7] = 1000
+        bad[1::11] = -3
+        trk0.find_loopers_noalloc(n0, bad, x0, par0, o["prev"], o["root"], o["turn"])
+        torch.cuda.synchronize()
+        assert bool(((o["prev"] >= -1) & (o["prev"] < n0)).all())
+        trk0.find_loopers_noalloc(n0, sector0, x0, par0, o["prev"], o["root"], o["turn"])
+        torch.cuda.synchronize()
+        assert all(torch.equal(o[k], ref0[k]) for k in o)
         # host memory is not accepted; n_tracks = 0 is a no-op; negative n_tracks is an argument error
         host = np.zeros(n0, np.int32)
         with pytest.raises(T.TpcError) as e:
