@@ -51,7 +51,15 @@ __global__ void __launch_bounds__(K10_THREADS) k10_compact(const long long n_tra
   // (sector out of range, or a slot beyond the array: only with caller-made arrays that are not in ascending sector order --
   // tpc_find_loopers_noalloc; such a track takes no part, nothing is written out of bounds)
   long long slot = -1;
-  if (fabsf(o_par[i * 5 + 4]) >= L.qmin && (unsigned)sec < (unsigned)NS) slot = (long long)sec_begin[sec] + atomicAdd(&sec_count[sec], 1);
+  const bool take = fabsf(o_par[i * 5 + 4]) >= L.qmin && (unsigned)sec < (unsigned)NS;
+  if (take) {   // one atomic per sector and warp (the tracks are in sector order: nearly always one group)
+    const unsigned peers = __match_any_sync(__activemask(), sec);
+    const int leader = __ffs(peers) - 1, lane = threadIdx.x & 31;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(&sec_count[sec], __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    slot = (long long)sec_begin[sec] + base + __popc(peers & ((1u << lane) - 1u));
+  }
   if (slot >= 0 && slot < n_tracks) list[slot] = (int)i;
   prev[i] = -1; prev_n[i] = 0;   // every track starts without a predecessor; k10_match overwrites the gathered ones
 }

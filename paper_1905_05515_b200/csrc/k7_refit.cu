@@ -21,9 +21,13 @@ constexpr int K7_CLASSES = 256;   // length classes of the ordering: clusters of
 // track per lane from start to end, so a warp takes as long as its longest track; with equally long tracks side by side the lanes
 // of a warp finish together.  The order inside a length class is arbitrary and enters no result.
 __global__ void __launch_bounds__(256) k7_count(const long long n_tracks, const long long* __restrict__ cl_begin, int* __restrict__ count) {
+  __shared__ int s_cnt[K7_CLASSES];   // histogram of the CTA first: most tracks fall into a few classes, global atomics on them would serialise
+  s_cnt[threadIdx.x] = 0;
+  __syncthreads();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_tracks) return;
-  atomicAdd(&count[min((int)(cl_begin[i + 1] - cl_begin[i]), K7_CLASSES - 1)], 1);
+  if (i < n_tracks) atomicAdd(&s_cnt[min((int)(cl_begin[i + 1] - cl_begin[i]), K7_CLASSES - 1)], 1);
+  __syncthreads();
+  if (s_cnt[threadIdx.x]) atomicAdd(&count[threadIdx.x], s_cnt[threadIdx.x]);
 }
 __global__ void k7_starts(const int* __restrict__ count, int* __restrict__ start) {   // one thread: K7_CLASSES entries, longest class first
   int acc = 0;
@@ -31,10 +35,16 @@ __global__ void k7_starts(const int* __restrict__ count, int* __restrict__ start
 }
 __global__ void __launch_bounds__(256) k7_fill(const long long n_tracks, const long long* __restrict__ cl_begin, const int* __restrict__ start,
                                                int* __restrict__ fill, int* __restrict__ order) {
+  __shared__ int s_cnt[K7_CLASSES], s_base[K7_CLASSES];
+  s_cnt[threadIdx.x] = 0;
+  __syncthreads();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_tracks) return;
-  const int m = min((int)(cl_begin[i + 1] - cl_begin[i]), K7_CLASSES - 1);
-  order[start[m] + atomicAdd(&fill[m], 1)] = (int)i;
+  int m = 0, rank = 0;
+  if (i < n_tracks) { m = min((int)(cl_begin[i + 1] - cl_begin[i]), K7_CLASSES - 1); rank = atomicAdd(&s_cnt[m], 1); }
+  __syncthreads();
+  if (s_cnt[threadIdx.x]) s_base[threadIdx.x] = start[threadIdx.x] + atomicAdd(&fill[threadIdx.x], s_cnt[threadIdx.x]);   // one range per class and CTA
+  __syncthreads();
+  if (i < n_tracks) order[s_base[m] + rank] = (int)i;
 }
 
 __global__ void __launch_bounds__(K7_THREADS) k7_refit(const long long n_tracks, const int* __restrict__ order, const int* __restrict__ o_sector,

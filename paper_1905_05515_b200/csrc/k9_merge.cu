@@ -57,7 +57,14 @@ __global__ void __launch_bounds__(K9_THREADS) k9_outer(const long long n_tracks,
     o[0] = o[1] = o[2] = o[3] = 0.0f;
   }
   leaver[i] = lv;
-  if (lv) list[atomicAdd(n_leavers, 1)] = (int)i;   // leavers gathered in arbitrary order (no result depends on it): full warps in k9_propose
+  if (lv) {   // leavers gathered in arbitrary order (no result depends on it): full warps in k9_propose; one atomic per warp
+    const unsigned peers = __activemask();
+    const int leader = __ffs(peers) - 1, lane = threadIdx.x & 31;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(n_leavers, __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    list[base + __popc(peers & ((1u << lane) - 1u))] = (int)i;
+  }
 }
 
 __global__ void __launch_bounds__(256) k9_fill(const long long n_tracks, const int R, const int* __restrict__ o_sector, const int* __restrict__ row_in,
