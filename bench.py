@@ -300,6 +300,33 @@ def run_gpu(args, rank, world, local_rank):
     if errs:
         raise errs[0]
     ms_e2e = max_over_ranks(e0.elapsed_time(e1) / args.steps)
+    # the same NF contexts / streams on the frame they hold (device-resident: no load, results stay in HBM): what a stream of frames
+    # gains when the kernel chains of two frames run side by side and fill each other's tails (extra key, not `value`)
+
+    def worker_dev(j):
+        try:
+            torch.cuda.set_device(local_rank)
+            for _ in steps_of[j]:
+                trks[j].find_tracks_device()
+        except Exception as ex:      # noqa: BLE001
+            errs.append(ex)
+
+    for t_ in trks:
+        t_.find_tracks_device()
+    barrier()
+    e0.record(stream)
+    for s_ in streams:
+        s_.wait_event(e0)
+    th = [threading.Thread(target=worker_dev, args=(j,)) for j in range(NF)]
+    [t_.start() for t_ in th]
+    [t_.join() for t_ in th]
+    for s_ in streams:
+        stream.wait_stream(s_)
+    e1.record(stream)
+    barrier()
+    if errs:
+        raise errs[0]
+    ms_dev_pipe = max_over_ranks(e0.elapsed_time(e1) / args.steps)
     for t_ in trks:
         t_.close()
     h2d = 2 * 4 * N
@@ -404,6 +431,9 @@ def run_gpu(args, rank, world, local_rank):
            "e2e": {"value": total_clusters / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h, "mode": f"{NF} frames in flight ({NF} contexts, {NF} streams, one host thread each, pinned_async=1: the pinned input is read by DMA after the load call returns): copies overlap kernels",
                    "serial_ms_per_step": ms_e2e_serial, "serial_value": total_clusters / (ms_e2e_serial * 1e-3)},
+           "device_resident_in_flight": {"value": total_clusters / (ms_dev_pipe * 1e-3), "unit": UNIT, "ms_per_step": ms_dev_pipe, "frames_in_flight": NF,
+                                         "note": "the same step with the kernel chains of several frames side by side (one context and stream per frame in flight, "
+                                                 "inputs and results in HBM): they fill each other's tails; `value` is one frame at a time"},
            "gpu_launches": int(launches), "kernel_ms": kern,
            "s5_work": {k: int(tm[k]) for k in ("n_start_hits", "n_propagations", "n_updates", "n_pickups")}, "roofline": roofline, "roofline_all": roofs, "cpu_baseline": cpu, "cpu_baseline_parallel": cpu_par,
            "linearity": linearity, "variant_seed_bridging": variant, "cluster_marks": marks, "sector_merges": merges, "looper_turns": loopers,
